@@ -1,0 +1,259 @@
+"""CPU ORACLE bindings -- TEST INFRASTRUCTURE, NOT THE PRODUCT (see gc_oracle.h).
+
+ctypes wrapper around ``oracle/libgc_oracle.so`` (plain C, built by :func:`build`).  Only ``tests/``,
+``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs may import
+this package.  It shares nothing with ``paper_2605_16734_b200/csrc``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libgc_oracle.so")
+_SRC = os.path.join(_HERE, "gc_oracle.c")
+_HDR = os.path.join(_HERE, "gc_oracle.h")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -fopenmp, no fast-math, no FMA contraction."""
+    if (not force and os.path.exists(_SO)
+            and os.path.getmtime(_SO) >= max(os.path.getmtime(_SRC), os.path.getmtime(_HDR))):
+        return _SO
+    cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c11", "-ffp-contract=off",
+           "-Wall", "-Wextra", _SRC, "-o", _SO, "-lm"]
+    subprocess.run(cmd, check=True)
+    return _SO
+
+
+class _Desc(C.Structure):
+    _fields_ = [("ns", C.c_int32), ("nfp", C.c_int32), ("nh", C.c_int32),
+                ("xm", C.c_void_p), ("xn", C.c_void_p), ("bmnc", C.c_void_p),
+                ("G", C.c_void_p), ("I", C.c_void_p), ("iota", C.c_void_p),
+                ("psi0", C.c_double), ("nk", C.c_int32),
+                ("mode_m", C.c_void_p), ("mode_n", C.c_void_p),
+                ("mode_omega", C.c_void_p), ("mode_phase", C.c_void_p), ("phihat", C.c_void_p)]
+
+
+class _Params(C.Structure):
+    _fields_ = [("mass", C.c_double), ("charge", C.c_double), ("t0", C.c_double), ("t_max", C.c_double),
+                ("rtol", C.c_double), ("atol", C.c_double), ("v_ref", C.c_double),
+                ("h0", C.c_double), ("h_min", C.c_double), ("s_loss", C.c_double), ("s_min", C.c_double),
+                ("max_steps", C.c_int64), ("poincare_capacity", C.c_int64), ("traj_capacity", C.c_int64)]
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        L = C.CDLL(_SO)
+        L.oracle_field_create.restype = C.c_void_p
+        L.oracle_field_create.argtypes = [C.POINTER(_Desc)]
+        L.oracle_field_destroy.argtypes = [C.c_void_p]
+        L.oracle_scale_accept.restype = C.c_double
+        L.oracle_scale_accept.argtypes = [C.c_double]
+        L.oracle_scale_reject.restype = C.c_double
+        L.oracle_scale_reject.argtypes = [C.c_double]
+        L.oracle_err_norm.restype = C.c_double
+        L.oracle_num_threads.restype = C.c_int
+        L.oracle_trace.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def lagrange(ns: int, s: float):
+    i0 = C.c_int32(0)
+    w = np.zeros(4)
+    dw = np.zeros(4)
+    _load().oracle_lagrange(C.c_int32(ns), C.c_double(s), C.byref(i0), _p(w), _p(dw))
+    return int(i0.value), w, dw
+
+
+def scale_accept(err: float) -> float:
+    return float(_load().oracle_scale_accept(err))
+
+
+def scale_reject(err: float) -> float:
+    return float(_load().oracle_scale_reject(err))
+
+
+def err_norm(y, y_new, delta, rtol, atol) -> float:
+    y, y_new, delta = _f64(y), _f64(y_new), _f64(delta)
+    return float(_load().oracle_err_norm(_p(y), _p(y_new), _p(delta), C.c_double(rtol), C.c_double(atol)))
+
+
+def dp5_dense(y, y_new, k, h, tau):
+    y, y_new, k = _f64(y), _f64(y_new), _f64(k)
+    assert k.shape == (7, 4)
+    out = np.zeros(4)
+    _load().oracle_dp5_dense(_p(y), _p(y_new), _p(k), C.c_double(h), C.c_double(tau), _p(out))
+    return out
+
+
+@dataclass
+class TraceResult:
+    y: np.ndarray          # [4][n]: s, theta, zeta, v_par (m/s)
+    t: np.ndarray          # [n]
+    status: np.ndarray     # [n] int32
+    n_acc: np.ndarray
+    n_rej: np.ndarray
+    n_forced: np.ndarray
+    h: np.ndarray          # [n] next step proposal
+    poincare: np.ndarray | None = None      # [count][4]
+    poincare_count: int = 0
+    traj: np.ndarray | None = None          # [n][cap][5]
+    traj_count: np.ndarray | None = None
+
+
+class OracleField:
+    """Host tables copied into the C oracle (oracle_field_create)."""
+
+    def __init__(self, fld):
+        L = _load()
+        self._keep = dict(
+            xm=_i32(fld.xm), xn=_i32(fld.xn), bmnc=_f64(fld.bmnc), G=_f64(fld.G), I=_f64(fld.I),
+            iota=_f64(fld.iota), mode_m=_i32(fld.mode_m), mode_n=_i32(fld.mode_n),
+            mode_omega=_f64(fld.mode_omega), mode_phase=_f64(fld.mode_phase), phihat=_f64(fld.phihat))
+        k = self._keep
+        self.ns, self.nh, self.nk = int(fld.ns), int(k["xm"].shape[0]), int(k["mode_m"].shape[0])
+        assert k["bmnc"].shape == (self.ns, self.nh)
+        if self.nk:
+            assert k["phihat"].shape == (self.ns, self.nk)
+        d = _Desc(self.ns, int(fld.nfp), self.nh, _p(k["xm"]), _p(k["xn"]), _p(k["bmnc"]),
+                  _p(k["G"]), _p(k["I"]), _p(k["iota"]), float(fld.psi0), self.nk,
+                  _p(k["mode_m"]), _p(k["mode_n"]), _p(k["mode_omega"]), _p(k["mode_phase"]),
+                  _p(k["phihat"]))
+        self._h = C.c_void_p(L.oracle_field_create(C.byref(d)))
+        if not self._h.value:
+            raise ValueError("oracle_field_create rejected the description")
+        self.psi0 = float(fld.psi0)
+
+    def __del__(self):
+        try:
+            if self._h.value:
+                _load().oracle_field_destroy(self._h)
+                self._h = C.c_void_p(None)
+        except Exception:
+            pass
+
+    # ---- point evaluations ---------------------------------------------------------------------------
+    def eval_B(self, s, th, ze):
+        out = np.zeros(4)
+        _load().oracle_eval_B(self._h, C.c_double(s), C.c_double(th), C.c_double(ze), _p(out))
+        return out
+
+    def eval_B_many(self, s, th, ze):
+        s, th, ze = np.broadcast_arrays(_f64(s), _f64(th), _f64(ze))
+        out = np.zeros((s.size, 4))
+        for i, (a, b, c) in enumerate(zip(s.ravel(), th.ravel(), ze.ravel())):
+            out[i] = self.eval_B(a, b, c)
+        return out
+
+    def eval_profiles(self, s):
+        out = np.zeros(6)
+        _load().oracle_eval_profiles(self._h, C.c_double(s), _p(out))
+        return out
+
+    def eval_pert(self, s, th, ze, t):
+        out = np.zeros(9)
+        _load().oracle_eval_pert(self._h, C.c_double(s), C.c_double(th), C.c_double(ze), C.c_double(t),
+                                 _p(out))
+        return out
+
+    def rhs(self, mass, charge, mu, v_ref, t, y):
+        y = _f64(y)
+        out = np.zeros(4)
+        _load().oracle_rhs(self._h, C.c_double(mass), C.c_double(charge), C.c_double(mu),
+                           C.c_double(v_ref), C.c_double(t), _p(y), _p(out))
+        return out
+
+    def dp5_attempt(self, mass, charge, mu, v_ref, t, y, k1, h):
+        y, k1 = _f64(y), _f64(k1)
+        y_new, k, delta = np.zeros(4), np.zeros((7, 4)), np.zeros(4)
+        _load().oracle_dp5_attempt(self._h, C.c_double(mass), C.c_double(charge), C.c_double(mu),
+                                   C.c_double(v_ref), C.c_double(t), _p(y), _p(k1), C.c_double(h),
+                                   _p(y_new), _p(k), _p(delta))
+        return y_new, k, delta
+
+    # ---- ensembles -----------------------------------------------------------------------------------
+    def trace(self, spec, s0, th0, ze0, vpar0, mu, h_in=None, poincare_capacity=0, traj_capacity=0,
+              t0=None, t_max=None) -> TraceResult:
+        s0, th0, ze0, vpar0, mu = map(_f64, (s0, th0, ze0, vpar0, mu))
+        n = s0.shape[0]
+        p = _Params(spec.mass, spec.charge, spec.t0 if t0 is None else t0,
+                    spec.t_max if t_max is None else t_max, spec.rtol, spec.atol, spec.v_ref,
+                    spec.h0, spec.h_min, spec.s_loss, spec.s_min, int(spec.max_steps),
+                    int(poincare_capacity), int(traj_capacity))
+        h = np.zeros(n) if h_in is None else _f64(h_in).copy()
+        y = np.zeros((4, n))
+        t = np.zeros(n)
+        status = np.zeros(n, np.int32)
+        n_acc, n_rej, n_forced = (np.zeros(n, np.int32) for _ in range(3))
+        pc = np.zeros((max(poincare_capacity, 1), 4)) if poincare_capacity else None
+        pcount = C.c_int64(0)
+        traj = np.zeros((n, traj_capacity, 5)) if traj_capacity else None
+        tcount = np.zeros(n, np.int64) if traj_capacity else None
+        rc = _load().oracle_trace(self._h, C.byref(p), C.c_int64(n), _p(s0), _p(th0), _p(ze0), _p(vpar0),
+                                  _p(mu), _p(h), _p(y), _p(t), _p(status), _p(n_acc), _p(n_rej),
+                                  _p(n_forced), _p(pc), C.byref(pcount) if poincare_capacity else None,
+                                  _p(traj), _p(tcount))
+        if rc != 0:
+            raise ValueError("oracle_trace: bad arguments")
+        res = TraceResult(y, t, status, n_acc, n_rej, n_forced, h)
+        if poincare_capacity:
+            res.poincare_count = int(pcount.value)
+            res.poincare = pc[:min(res.poincare_count, poincare_capacity)]
+        if traj_capacity:
+            res.traj, res.traj_count = traj, tcount
+        return res
+
+    def rk4(self, mass, charge, v_ref, s0, th0, ze0, vpar0, mu, t0, h, nsteps):
+        s0, th0, ze0, vpar0, mu = map(_f64, (s0, th0, ze0, vpar0, mu))
+        n = s0.shape[0]
+        y = np.zeros((4, n))
+        _load().oracle_rk4(self._h, C.c_double(mass), C.c_double(charge), C.c_double(v_ref), C.c_int64(n),
+                           _p(s0), _p(th0), _p(ze0), _p(vpar0), _p(mu), C.c_double(t0), C.c_double(h),
+                           C.c_int64(nsteps), _p(y))
+        return y
+
+
+_RHS_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double))
+
+
+def dp5_attempt_fn(fun, t, y, h, k1=None):
+    """One Dormand-Prince attempt on an arbitrary Python right-hand side ``fun(t, y[4]) -> dydt[4]``
+    (tableau pins only)."""
+    y = _f64(y)
+
+    def _cb(_ctx, tt, yp, dp):
+        out = fun(tt, np.array([yp[i] for i in range(4)]))
+        for i in range(4):
+            dp[i] = float(out[i])
+
+    cb = _RHS_FN(_cb)
+    k1 = _f64(fun(t, y.copy())) if k1 is None else _f64(k1)
+    y_new, k, delta = np.zeros(4), np.zeros((7, 4)), np.zeros(4)
+    _load().oracle_dp5_attempt_fn(cb, None, C.c_double(t), _p(y), _p(k1), C.c_double(h),
+                                  _p(y_new), _p(k), _p(delta))
+    return y_new, k, delta

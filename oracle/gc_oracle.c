@@ -1,0 +1,462 @@
+/* gc_oracle.c -- CPU ORACLE (test infrastructure, not the product).  See gc_oracle.h.
+ *
+ * Plain C, FP64, one libm sin + cos per harmonic, sequential sums in index order, no blocking, no
+ * fusion, no reordering: written so that each function can be checked against the cited passage by
+ * eye.  OpenMP is used over particles only ("trajectories are independent").
+ */
+#include "gc_oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+struct oracle_field {
+  int32_t ns, nfp, nh, nk;
+  int32_t *xm, *xn, *mode_m, *mode_n;
+  double *bmnc, *G, *I, *iota, *mode_omega, *mode_phase, *phihat;
+  double psi0;
+};
+
+static void *dup_mem(const void *src, size_t bytes) {
+  void *p = malloc(bytes ? bytes : 1);
+  if (p && bytes) memcpy(p, src, bytes);
+  return p;
+}
+
+oracle_field *oracle_field_create(const oracle_field_desc *d) {
+  if (!d || d->ns < 4 || d->nh < 1 || d->nk < 0) return NULL;
+  oracle_field *f = (oracle_field *)calloc(1, sizeof(*f));
+  f->ns = d->ns; f->nfp = d->nfp; f->nh = d->nh; f->nk = d->nk; f->psi0 = d->psi0;
+  f->xm = (int32_t *)dup_mem(d->xm, sizeof(int32_t) * d->nh);
+  f->xn = (int32_t *)dup_mem(d->xn, sizeof(int32_t) * d->nh);
+  f->bmnc = (double *)dup_mem(d->bmnc, sizeof(double) * (size_t)d->ns * d->nh);
+  f->G = (double *)dup_mem(d->G, sizeof(double) * d->ns);
+  f->I = (double *)dup_mem(d->I, sizeof(double) * d->ns);
+  f->iota = (double *)dup_mem(d->iota, sizeof(double) * d->ns);
+  if (d->nk > 0) {
+    f->mode_m = (int32_t *)dup_mem(d->mode_m, sizeof(int32_t) * d->nk);
+    f->mode_n = (int32_t *)dup_mem(d->mode_n, sizeof(int32_t) * d->nk);
+    f->mode_omega = (double *)dup_mem(d->mode_omega, sizeof(double) * d->nk);
+    f->mode_phase = (double *)dup_mem(d->mode_phase, sizeof(double) * d->nk);
+    f->phihat = (double *)dup_mem(d->phihat, sizeof(double) * (size_t)d->ns * d->nk);
+  }
+  return f;
+}
+
+void oracle_field_destroy(oracle_field *f) {
+  if (!f) return;
+  free(f->xm); free(f->xn); free(f->bmnc); free(f->G); free(f->I); free(f->iota);
+  free(f->mode_m); free(f->mode_n); free(f->mode_omega); free(f->mode_phase); free(f->phihat);
+  free(f);
+}
+
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+/* ---- O1: radial cubic Lagrange interpolation on the uniform grid -------------------- */
+void oracle_lagrange(int32_t ns, double s, int32_t *i0_out, double w[4], double dw[4]) {
+  double u = s * (double)(ns - 1);
+  double c = floor(u);
+  int32_t i0;
+  if (!(c >= 1.0)) i0 = 0;                         /* also catches NaN */
+  else if (c - 1.0 >= (double)(ns - 4)) i0 = ns - 4;
+  else i0 = (int32_t)c - 1;
+  double x = u - (double)i0;                       /* nodes of the stencil sit at x = 0,1,2,3 */
+  w[0] = -(x - 1.0) * (x - 2.0) * (x - 3.0) / 6.0;
+  w[1] = x * (x - 2.0) * (x - 3.0) / 2.0;
+  w[2] = -x * (x - 1.0) * (x - 3.0) / 2.0;
+  w[3] = x * (x - 1.0) * (x - 2.0) / 6.0;
+  double scale = (double)(ns - 1);                 /* d/ds = (ns-1) d/dx */
+  dw[0] = -((x - 2.0) * (x - 3.0) + (x - 1.0) * (x - 3.0) + (x - 1.0) * (x - 2.0)) / 6.0 * scale;
+  dw[1] = ((x - 2.0) * (x - 3.0) + x * (x - 3.0) + x * (x - 2.0)) / 2.0 * scale;
+  dw[2] = -((x - 1.0) * (x - 3.0) + x * (x - 3.0) + x * (x - 1.0)) / 2.0 * scale;
+  dw[3] = ((x - 1.0) * (x - 2.0) + x * (x - 2.0) + x * (x - 1.0)) / 6.0 * scale;
+  *i0_out = i0;
+}
+
+/* value and d/ds of one tabulated quantity with row stride `stride` */
+static void interp(const double *tab, int32_t stride, int32_t i0, const double w[4], const double dw[4],
+                   double *val, double *dval) {
+  double v = 0.0, d = 0.0;
+  for (int j = 0; j < 4; ++j) {
+    double t = tab[(size_t)(i0 + j) * stride];
+    v += w[j] * t;
+    d += dw[j] * t;
+  }
+  *val = v; *dval = d;
+}
+
+/* ---- O2: equilibrium field strength and its derivatives ------------------------------------------- */
+void oracle_eval_B(const oracle_field *f, double s, double th, double ze, double out[4]) {
+  int32_t i0; double w[4], dw[4];
+  oracle_lagrange(f->ns, s, &i0, w, dw);
+  double B = 0.0, Bs = 0.0, Bth = 0.0, Bze = 0.0;
+  for (int k = 0; k < f->nh; ++k) {
+    double b, bs;
+    interp(f->bmnc + k, f->nh, i0, w, dw, &b, &bs);
+    double m = (double)f->xm[k], nn = (double)f->xn[k] * (double)f->nfp;
+    double ang = m * th - nn * ze;
+    double c = cos(ang), sn = sin(ang);
+    B += b * c;
+    Bs += bs * c;
+    Bth += -m * b * sn;
+    Bze += nn * b * sn;
+  }
+  out[0] = B; out[1] = Bs; out[2] = Bth; out[3] = Bze;
+}
+
+void oracle_eval_profiles(const oracle_field *f, double s, double out[6]) {
+  int32_t i0; double w[4], dw[4];
+  oracle_lagrange(f->ns, s, &i0, w, dw);
+  interp(f->G, 1, i0, w, dw, &out[0], &out[1]);
+  interp(f->I, 1, i0, w, dw, &out[2], &out[3]);
+  interp(f->iota, 1, i0, w, dw, &out[4], &out[5]);
+}
+
+/* ---- O3: shear-Alfven perturbation, Phi and alpha with E_par = 0 (A14) ----------------- */
+void oracle_eval_pert(const oracle_field *f, double s, double th, double ze, double t, double out[9]) {
+  for (int i = 0; i < 9; ++i) out[i] = 0.0;
+  if (f->nk == 0) return;
+  int32_t i0; double w[4], dw[4];
+  oracle_lagrange(f->ns, s, &i0, w, dw);
+  double G, Gs, I, Is, io, ios;
+  interp(f->G, 1, i0, w, dw, &G, &Gs);
+  interp(f->I, 1, i0, w, dw, &I, &Is);
+  interp(f->iota, 1, i0, w, dw, &io, &ios);
+  double Phi = 0, Phi_s = 0, Phi_th = 0, Phi_ze = 0, al = 0, al_s = 0, al_th = 0, al_ze = 0, al_t = 0;
+  for (int k = 0; k < f->nk; ++k) {
+    double ph, ph_s;
+    interp(f->phihat + k, f->nk, i0, w, dw, &ph, &ph_s);
+    double m = (double)f->mode_m[k], n = (double)f->mode_n[k], om = f->mode_omega[k];
+    double ang = m * th - n * ze + om * t + f->mode_phase[k];
+    double sn = sin(ang), c = cos(ang);
+    /* alpha_hat = -Phi_hat (iota m - n) / (omega (G + iota I)) */
+    double N = io * m - n, N_s = ios * m;
+    double Dn = om * (G + io * I), Dn_s = om * (Gs + ios * I + io * Is);
+    double ah = -ph * N / Dn;
+    double ah_s = -(ph_s * N / Dn + ph * N_s / Dn - ph * N * Dn_s / (Dn * Dn));
+    Phi += ph * sn;
+    Phi_s += ph_s * sn;
+    Phi_th += m * ph * c;
+    Phi_ze += -n * ph * c;
+    al += ah * sn;
+    al_s += ah_s * sn;
+    al_th += m * ah * c;
+    al_ze += -n * ah * c;
+    al_t += om * ah * c;
+  }
+  out[0] = Phi; out[1] = Phi_s / f->psi0; out[2] = Phi_th; out[3] = Phi_ze;
+  out[4] = al; out[5] = al_s / f->psi0; out[6] = al_th; out[7] = al_ze; out[8] = al_t;
+}
+
+/* ---- O4: guiding-centre equations in Boozer coordinates (A4) ------------------------
+ * Euler-Lagrange equations of L = q(psi + rho_c I) thdot + q(rho_c G - chi) zedot - H,
+ * rho_c = m v/(q B) + alpha, H = m v^2/2 + mu B + q Phi, chi' = iota, covariant radial component dropped. */
+void oracle_rhs(const oracle_field *f, double mass, double charge, double mu, double v_ref,
+                double t, const double y[4], double dydt[4]) {
+  double s = y[0], th = y[1], ze = y[2], v = y[3] * v_ref;
+  double fb[4], pr[6], pt[9];
+  oracle_eval_B(f, s, th, ze, fb);
+  oracle_eval_profiles(f, s, pr);
+  oracle_eval_pert(f, s, th, ze, t, pt);
+  double psi0 = f->psi0;
+  double B = fb[0], B_psi = fb[1] / psi0, B_th = fb[2], B_ze = fb[3];
+  double G = pr[0], Gp = pr[1] / psi0, I = pr[2], Ip = pr[3] / psi0, iota = pr[4];
+  double Phi_psi = pt[1], Phi_th = pt[2], Phi_ze = pt[3];
+  double al = pt[4], al_psi = pt[5], al_th = pt[6], al_ze = pt[7], al_t = pt[8];
+
+  double rho = mass * v / (charge * B);
+  double rho_c = rho + al;
+  double F = mass * v * v / B + mu;
+  double a = 1.0 + rho_c * Ip + al_psi * I;
+  double b = iota - rho_c * Gp - al_psi * G;
+  double D = a * G + b * I;
+  double C = al_th * G - al_ze * I;
+  double h_psi = F / charge * B_psi + Phi_psi;
+  double h_th = F / charge * B_th + Phi_th;
+  double h_ze = F / charge * B_ze + Phi_ze;
+  double psidot = (I * h_ze - G * h_th + C * v * B) / D;
+  double thdot = (b * v * B + G * h_psi) / D;
+  double zedot = (a * v * B - I * h_psi) / D;
+  double Lam = a * B_ze + b * B_th + C * B_psi;
+  double mvdot = (-mu * B * Lam - charge * B * (a * Phi_ze + b * Phi_th + C * Phi_psi)
+                  + (mass * v / B) * (B_psi * (I * Phi_ze - G * Phi_th) + Phi_psi * (G * B_th - I * B_ze))) / D
+                 - charge * B * al_t;
+  dydt[0] = psidot / psi0;
+  dydt[1] = thdot;
+  dydt[2] = zedot;
+  dydt[3] = mvdot / mass / v_ref;
+}
+
+/* ---- O5: Dormand-Prince 5(4), FSAL ---------------------------------------------------- */
+static const double DP_C[7] = {0.0, 1.0 / 5.0, 3.0 / 10.0, 4.0 / 5.0, 8.0 / 9.0, 1.0, 1.0};
+static const double DP_A[7][6] = {
+    {0, 0, 0, 0, 0, 0},
+    {1.0 / 5.0, 0, 0, 0, 0, 0},
+    {3.0 / 40.0, 9.0 / 40.0, 0, 0, 0, 0},
+    {44.0 / 45.0, -56.0 / 15.0, 32.0 / 9.0, 0, 0, 0},
+    {19372.0 / 6561.0, -25360.0 / 2187.0, 64448.0 / 6561.0, -212.0 / 729.0, 0, 0},
+    {9017.0 / 3168.0, -355.0 / 33.0, 46732.0 / 5247.0, 49.0 / 176.0, -5103.0 / 18656.0, 0},
+    {35.0 / 384.0, 0.0, 500.0 / 1113.0, 125.0 / 192.0, -2187.0 / 6784.0, 11.0 / 84.0}};
+static const double DP_E[7] = {71.0 / 57600.0, 0.0, -71.0 / 16695.0, 71.0 / 1920.0,
+                               -17253.0 / 339200.0, 22.0 / 525.0, -1.0 / 40.0};
+static const double DP_D[7] = {-12715105075.0 / 11282082432.0, 0.0, 87487479700.0 / 32700410799.0,
+                               -10690763975.0 / 1880347072.0, 701980252875.0 / 199316789632.0,
+                               -1453857185.0 / 822651844.0, 69997945.0 / 29380423.0};
+
+void oracle_dp5_attempt_fn(oracle_rhs_fn fn, void *ctx, double t, const double y[4], const double k1[4],
+                           double h, double y_new[4], double k[7][4], double delta[4]) {
+  for (int c = 0; c < 4; ++c) k[0][c] = k1[c];
+  double ys[4];
+  for (int i = 1; i < 7; ++i) {                      /* stages 2..7; stage 7 is evaluated at y_new */
+    for (int c = 0; c < 4; ++c) {
+      double acc = 0.0;
+      for (int j = 0; j < i; ++j) acc += DP_A[i][j] * k[j][c];
+      ys[c] = y[c] + h * acc;
+    }
+    fn(ctx, t + DP_C[i] * h, ys, k[i]);
+  }
+  for (int c = 0; c < 4; ++c) {
+    y_new[c] = ys[c];                                /* row 7 of A is the 5th-order weights */
+    double e = 0.0;
+    for (int j = 0; j < 7; ++j) e += DP_E[j] * k[j][c];
+    delta[c] = h * e;
+  }
+}
+
+typedef struct { const oracle_field *f; double mass, charge, mu, v_ref; } gc_ctx;
+
+static void gc_rhs_fn(void *ctx, double t, const double y[4], double dydt[4]) {
+  const gc_ctx *g = (const gc_ctx *)ctx;
+  oracle_rhs(g->f, g->mass, g->charge, g->mu, g->v_ref, t, y, dydt);
+}
+
+void oracle_dp5_attempt(const oracle_field *f, double mass, double charge, double mu, double v_ref,
+                        double t, const double y[4], const double k1[4], double h,
+                        double y_new[4], double k[7][4], double delta[4]) {
+  gc_ctx g = {f, mass, charge, mu, v_ref};
+  oracle_dp5_attempt_fn(gc_rhs_fn, &g, t, y, k1, h, y_new, k, delta);
+}
+
+/* ---- O8: continuous extension of the step --------------------------------------------------------- */
+static void dense_and_slope(const double y[4], const double y_new[4], const double k[7][4], double h,
+                            double tau, double y_tau[4], double dy_dtau[4]) {
+  double sg = 1.0 - tau;
+  for (int c = 0; c < 4; ++c) {
+    double r1 = y[c], r2 = y_new[c] - y[c];
+    double r3 = h * k[0][c] - r2;
+    double r4 = r2 - h * k[6][c] - r3;
+    double r5 = 0.0;
+    for (int j = 0; j < 7; ++j) r5 += DP_D[j] * k[j][c];
+    r5 *= h;
+    double P4 = r4 + sg * r5, dP4 = -r5;
+    double P3 = r3 + tau * P4, dP3 = P4 + tau * dP4;
+    double P2 = r2 + sg * P3, dP2 = -P3 + sg * dP3;
+    y_tau[c] = r1 + tau * P2;
+    dy_dtau[c] = P2 + tau * dP2;
+  }
+}
+
+void oracle_dp5_dense(const double y[4], const double y_new[4], const double k[7][4], double h,
+                      double tau, double y_tau[4]) {
+  double d[4];
+  dense_and_slope(y, y_new, k, h, tau, y_tau, d);
+}
+
+/* ---- O6: error norm and step-size factors (Press 2007 style; A10) ---------------------------------- */
+double oracle_err_norm(const double y[4], const double y_new[4], const double delta[4],
+                       double rtol, double atol) {
+  double acc = 0.0;
+  for (int c = 0; c < 4; ++c) {
+    double sk = atol + rtol * fmax(fabs(y[c]), fabs(y_new[c]));
+    double r = delta[c] / sk;
+    acc += r * r;
+  }
+  return sqrt(acc / 4.0);
+}
+
+#define CTRL_SAFETY 0.9
+#define CTRL_MINSCALE 0.2
+#define CTRL_MAXSCALE 10.0
+#define CTRL_ALPHA 0.2          /* beta = 0: alpha = 0.2 - 0.75 beta */
+
+double oracle_scale_accept(double err) {
+  if (err == 0.0) return CTRL_MAXSCALE;
+  double sc = CTRL_SAFETY * pow(err, -CTRL_ALPHA);
+  if (sc < CTRL_MINSCALE) sc = CTRL_MINSCALE;
+  if (sc > CTRL_MAXSCALE) sc = CTRL_MAXSCALE;
+  return sc;
+}
+
+double oracle_scale_reject(double err) {
+  if (!isfinite(err)) return CTRL_MINSCALE;
+  double sc = CTRL_SAFETY * pow(err, -CTRL_ALPHA);
+  return sc > CTRL_MINSCALE ? sc : CTRL_MINSCALE;
+}
+
+static int all_finite4(const double v[4]) {
+  return isfinite(v[0]) && isfinite(v[1]) && isfinite(v[2]) && isfinite(v[3]);
+}
+
+/* O8: record every crossing of zeta = 2 pi k inside the accepted step (t, y) -> (t+h, y_new). */
+static void poincare_step(int64_t id, double t, double h, const double y[4], const double y_new[4],
+                          const double k[7][4], double *buf, int64_t cap, int64_t *count) {
+  const double TWO_PI = 6.283185307179586476925286766559;
+  double k0 = floor(y[2] / TWO_PI), k1 = floor(y_new[2] / TWO_PI);
+  if (k0 == k1) return;
+  double kfirst, klast, kstep;
+  if (k1 > k0) { kfirst = k0 + 1.0; klast = k1; kstep = 1.0; }        /* planes crossed going up   */
+  else { kfirst = k0; klast = k1 + 1.0; kstep = -1.0; }               /* planes crossed going down */
+  for (double kp = kfirst; kstep > 0 ? kp <= klast : kp >= klast; kp += kstep) {
+    double target = TWO_PI * kp;
+    double lo = 0.0, hi = 1.0, yt[4], dy[4];
+    double glo = y[2] - target;
+    for (int it = 0; it < 8; ++it) {                                  /* bisection to bracket */
+      double mid = 0.5 * (lo + hi);
+      dense_and_slope(y, y_new, k, h, mid, yt, dy);
+      double g = yt[2] - target;
+      if ((g < 0.0) == (glo < 0.0) && g != 0.0) { lo = mid; glo = g; } else { hi = mid; }
+    }
+    double tau = 0.5 * (lo + hi);
+    double tol = 1e-12 * fmax(1.0, fabs(target));
+    for (int it = 0; it < 20; ++it) {                                 /* Newton polish */
+      dense_and_slope(y, y_new, k, h, tau, yt, dy);
+      double g = yt[2] - target;
+      if (fabs(g) < tol || dy[2] == 0.0) break;
+      double tn = tau - g / dy[2];
+      if (tn < lo) tn = lo;
+      if (tn > hi) tn = hi;
+      tau = tn;
+    }
+    dense_and_slope(y, y_new, k, h, tau, yt, dy);
+    int64_t slot;
+#pragma omp atomic capture
+    slot = (*count)++;
+    if (slot < cap) {
+      double thm = fmod(yt[1], TWO_PI);
+      if (thm < 0.0) thm += TWO_PI;
+      buf[slot * 4 + 0] = (double)id;
+      buf[slot * 4 + 1] = t + tau * h;
+      buf[slot * 4 + 2] = yt[0];
+      buf[slot * 4 + 3] = thm;
+    }
+  }
+}
+
+/* ---- O5-O8: the trace -------------------------------------------------------------------------------- */
+int oracle_trace(const oracle_field *f, const oracle_trace_params *p, int64_t n,
+                 const double *s0, const double *th0, const double *ze0, const double *vpar0,
+                 const double *mu, double *h_inout,
+                 double *y_out, double *t_out, int32_t *status,
+                 int32_t *n_acc_out, int32_t *n_rej_out, int32_t *n_forced_out,
+                 double *poincare, int64_t *poincare_count,
+                 double *traj, int64_t *traj_count) {
+  if (!f || !p || n < 0 || !(p->v_ref > 0.0) || !(p->h0 > 0.0) || p->h_min < 0.0) return -1;
+  if (poincare_count) *poincare_count = 0;
+  int64_t pcap = (poincare && poincare_count) ? p->poincare_capacity : 0;
+  int64_t tcap = (traj && traj_count) ? p->traj_capacity : 0;
+
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int64_t i = 0; i < n; ++i) {
+    double y[4] = {s0[i], th0[i], ze0[i], vpar0[i] / p->v_ref};
+    double t = p->t0, h = (h_inout && h_inout[i] > 0.0) ? h_inout[i] : p->h0;
+    if (h < p->h_min) h = p->h_min;
+    double k[7][4], k1[4], y_new[4], delta[4];
+    int64_t attempts = 0;
+    int32_t n_acc = 0, n_rej = 0, n_forced = 0, st = -1;
+    int prev_rejected = 0;
+    int64_t ntraj = 0;
+    oracle_rhs(f, p->mass, p->charge, mu[i], p->v_ref, t, y, k1);
+    if (!all_finite4(y) || !all_finite4(k1)) st = 4;
+    else if (!(t < p->t_max)) st = 0;
+    while (st < 0) {
+      double h_try = h;
+      int clipped = 0;
+      if (t + h_try >= p->t_max) { h_try = p->t_max - t; clipped = 1; }       /* end clip */
+      if (!(t + h_try > t)) { st = 4; break; }                                /* step underflow */
+      int forced = prev_rejected && p->h_min > 0.0 && h == p->h_min;
+      oracle_dp5_attempt(f, p->mass, p->charge, mu[i], p->v_ref, t, y, k1, h_try, y_new, k, delta);
+      ++attempts;
+      double err = oracle_err_norm(y, y_new, delta, p->rtol, p->atol);
+      int finite = all_finite4(y_new) && all_finite4(k[6]) && isfinite(err);
+      int accept;
+      if (forced) {
+        if (!finite) { st = 4; break; }
+        accept = 1;
+      } else {
+        accept = finite && err <= 1.0;
+      }
+      if (accept) {
+        double sc = oracle_scale_accept(err);
+        double h_next = prev_rejected ? h_try * fmin(sc, 1.0) : h_try * sc;
+        if (pcap > 0) poincare_step(i, t, h_try, y, y_new, (const double(*)[4])k, poincare, pcap, poincare_count);
+        t = clipped ? p->t_max : t + h_try;
+        for (int c = 0; c < 4; ++c) { y[c] = y_new[c]; k1[c] = k[6][c]; }
+        ++n_acc;
+        if (forced) ++n_forced;
+        prev_rejected = 0;
+        if (!clipped) h = h_next;              /* a clipped last step keeps the unclipped proposal */
+        if (h < p->h_min) h = p->h_min;
+        if (ntraj < tcap) {
+          double *r = traj + ((size_t)i * tcap + ntraj) * 5;
+          r[0] = t; r[1] = y[0]; r[2] = y[1]; r[3] = y[2]; r[4] = y[3];
+        }
+        ++ntraj;
+        /* O7 stop rules, in this order */
+        if (y[0] >= p->s_loss) st = 1;
+        else if (y[0] <= p->s_min) st = 2;
+        else if (clipped) st = 0;
+        else if (attempts >= p->max_steps) st = 3;
+      } else {
+        ++n_rej;
+        h = h_try * oracle_scale_reject(err);
+        if (h < p->h_min) h = p->h_min;
+        prev_rejected = 1;
+        if (attempts >= p->max_steps) st = 3;
+      }
+    }
+    y_out[0 * n + i] = y[0];
+    y_out[1 * n + i] = y[1];
+    y_out[2 * n + i] = y[2];
+    y_out[3 * n + i] = y[3] * p->v_ref;        /* v_par back in m/s */
+    t_out[i] = t;
+    status[i] = st;
+    if (h_inout) h_inout[i] = h;
+    if (n_acc_out) n_acc_out[i] = n_acc;
+    if (n_rej_out) n_rej_out[i] = n_rej;
+    if (n_forced_out) n_forced_out[i] = n_forced;
+    if (traj_count) traj_count[i] = ntraj;
+  }
+  return 0;
+}
+
+/* ---- check (d): classical RK4 at fixed step -------------------------------------------------------- */
+void oracle_rk4(const oracle_field *f, double mass, double charge, double v_ref, int64_t n,
+                const double *s0, const double *th0, const double *ze0, const double *vpar0,
+                const double *mu, double t0, double h, int64_t nsteps, double *y_out) {
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int64_t i = 0; i < n; ++i) {
+    double y[4] = {s0[i], th0[i], ze0[i], vpar0[i] / v_ref}, k1[4], k2[4], k3[4], k4[4], yt[4];
+    for (int64_t st = 0; st < nsteps; ++st) {
+      double t = t0 + (double)st * h;
+      oracle_rhs(f, mass, charge, mu[i], v_ref, t, y, k1);
+      for (int c = 0; c < 4; ++c) yt[c] = y[c] + 0.5 * h * k1[c];
+      oracle_rhs(f, mass, charge, mu[i], v_ref, t + 0.5 * h, yt, k2);
+      for (int c = 0; c < 4; ++c) yt[c] = y[c] + 0.5 * h * k2[c];
+      oracle_rhs(f, mass, charge, mu[i], v_ref, t + 0.5 * h, yt, k3);
+      for (int c = 0; c < 4; ++c) yt[c] = y[c] + h * k3[c];
+      oracle_rhs(f, mass, charge, mu[i], v_ref, t + h, yt, k4);
+      for (int c = 0; c < 4; ++c) y[c] += h / 6.0 * (k1[c] + 2.0 * k2[c] + 2.0 * k3[c] + k4[c]);
+    }
+    y_out[0 * n + i] = y[0]; y_out[1 * n + i] = y[1]; y_out[2 * n + i] = y[2];
+    y_out[3 * n + i] = y[3] * v_ref;
+  }
+}

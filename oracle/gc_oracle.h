@@ -1,0 +1,111 @@
+/* gc_oracle.h -- CPU ORACLE for the guiding-centre hot path.  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, double-precision restatement of what the path computes, written from the paper
+ * (/root/reference/PAPER.md at survey time; cited below as PAPER.md:<line>) and, where the paper prints
+ * no mathematics, from the readings O1-O8 / A1-A22 recorded in SURVEY.md section 8(c) and DESIGN.md.
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may load
+ * this library.  It shares no code, header, table or constant generator with the CUDA path under
+ * paper_2605_16734_b200/csrc/ and include/.
+ *
+ * Pins (tests/test_oracle_*.py): Lagrange weights vs polynomial exactness and scipy; harmonic sums vs
+ * finite differences and an independent numpy series; DP5 tableau vs exact-rational order conditions
+ * and scipy's RK45 step; the RHS vs the Euler-Lagrange equations of the guiding-centre Lagrangian
+ * solved numerically; energy, P_zeta, helical momentum, n*H - omega*P_zeta invariants; closed-form
+ * orbits; brute-force RK4.  FIRM3D-level agreement (same numbers as the reference code on its own
+ * equilibria) is PARITY UNPINNED: no code, equilibrium file or printed equation exists to pin it to.
+ */
+#ifndef GC_ORACLE_H
+#define GC_ORACLE_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Field description: harmonics on a uniform radial grid s_j = j/(ns-1). Host pointers,
+ * copied by oracle_field_create. */
+typedef struct {
+  int32_t ns, nfp, nh;
+  const int32_t *xm, *xn;      /* [nh]; phase m*theta - n*nfp*zeta                         */
+  const double *bmnc;          /* [ns][nh] node-major                                      */
+  const double *G, *I, *iota;  /* [ns]                                                     */
+  double psi0;                 /* psi = psi0 * s                                           */
+  int32_t nk;                  /* perturbation harmonics, 0 = static                       */
+  const int32_t *mode_m, *mode_n;          /* [nk]; phase m*theta - n*zeta + omega*t + phase */
+  const double *mode_omega, *mode_phase;   /* [nk]                                          */
+  const double *phihat;        /* [ns][nk] node-major, volts                               */
+} oracle_field_desc;
+
+typedef struct oracle_field oracle_field;
+
+typedef struct {
+  double mass, charge;
+  double t0, t_max;
+  double rtol, atol;
+  double v_ref;
+  double h0, h_min;
+  double s_loss, s_min;
+  int64_t max_steps;
+  int64_t poincare_capacity;   /* records in the shared buffer; 0 disables O8 */
+  int64_t traj_capacity;       /* per-particle accepted-step records; 0 disables (oracle-only) */
+} oracle_trace_params;
+
+oracle_field *oracle_field_create(const oracle_field_desc *d);
+void oracle_field_destroy(oracle_field *f);
+
+/* O1: stencil start i0, x = s*(ns-1) - i0, cubic Lagrange weights w[4] and d/ds weights dw[4]. */
+void oracle_lagrange(int32_t ns, double s, int32_t *i0, double w[4], double dw[4]);
+
+/* O2: out = {B, dB/ds, dB/dtheta, dB/dzeta}. */
+void oracle_eval_B(const oracle_field *f, double s, double th, double ze, double out[4]);
+/* O1 on profiles: out = {G, dG/ds, I, dI/ds, iota, diota/ds}. */
+void oracle_eval_profiles(const oracle_field *f, double s, double out[6]);
+/* O3: out = {Phi, Phi_psi, Phi_theta, Phi_zeta, alpha, alpha_psi, alpha_theta, alpha_zeta, alpha_t}. */
+void oracle_eval_pert(const oracle_field *f, double s, double th, double ze, double t, double out[9]);
+
+/* O4: y = (s, theta, zeta, u = v_par/v_ref); dydt likewise. */
+void oracle_rhs(const oracle_field *f, double mass, double charge, double mu, double v_ref,
+                double t, const double y[4], double dydt[4]);
+
+/* O5: one Dormand-Prince attempt of size h from (t, y) with k1 = f(t, y) given.
+ * Outputs y_new (5th order), k[7][4] (k[0] = k1 copied, k[6] = f(t+h, y_new)), delta[4] (embedded error). */
+void oracle_dp5_attempt(const oracle_field *f, double mass, double charge, double mu, double v_ref,
+                        double t, const double y[4], const double k1[4], double h,
+                        double y_new[4], double k[7][4], double delta[4]);
+/* The same attempt on an arbitrary 4-component right-hand side (used by the tableau pins). */
+typedef void (*oracle_rhs_fn)(void *ctx, double t, const double y[4], double dydt[4]);
+void oracle_dp5_attempt_fn(oracle_rhs_fn fn, void *ctx, double t, const double y[4], const double k1[4],
+                           double h, double y_new[4], double k[7][4], double delta[4]);
+/* O8: continuous extension at t + tau*h, tau in [0,1]. */
+void oracle_dp5_dense(const double y[4], const double y_new[4], const double k[7][4], double h,
+                      double tau, double y_tau[4]);
+/* O6: error norm and the two step-size factors. */
+double oracle_err_norm(const double y[4], const double y_new[4], const double delta[4],
+                       double rtol, double atol);
+double oracle_scale_accept(double err);   /* factor applied to h after an accepted attempt */
+double oracle_scale_reject(double err);   /* factor applied to h after a rejected attempt  */
+
+/* O5-O8: trace n particles (OpenMP over particles only).  All arrays host memory.
+ * y_out [4][n]; status 0 t_max, 1 lost, 2 axis, 3 max_steps, 4 non-finite/stalled.
+ * traj [n][traj_capacity][5] = (t, s, theta, zeta, u) after each accepted step (oracle-only diagnostic).
+ * poincare [cap][4] = (id, t, s, theta mod 2pi); *poincare_count counts all hits (may exceed cap).
+ * Returns 0, or -1 on bad arguments. */
+int oracle_trace(const oracle_field *f, const oracle_trace_params *p, int64_t n,
+                 const double *s0, const double *th0, const double *ze0, const double *vpar0,
+                 const double *mu, double *h_inout,
+                 double *y_out, double *t_out, int32_t *status,
+                 int32_t *n_acc, int32_t *n_rej, int32_t *n_forced,
+                 double *poincare, int64_t *poincare_count,
+                 double *traj, int64_t *traj_count);
+
+/* Check (d): classical fixed-step RK4, nsteps steps of size h from t0; y_out [4][n]. */
+void oracle_rk4(const oracle_field *f, double mass, double charge, double v_ref, int64_t n,
+                const double *s0, const double *th0, const double *ze0, const double *vpar0,
+                const double *mu, double t0, double h, int64_t nsteps, double *y_out);
+
+int oracle_num_threads(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

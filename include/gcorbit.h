@@ -1,0 +1,144 @@
+/* gcorbit.h -- C ABI of the B200 guiding-centre orbit tracer (libgcorbit.so, sm_100a, FP64).
+ *
+ * The boundary follows the paper's statement of the problem: "Integration of guiding center trajectories
+ * is performed given the magnetic field, particle initial conditions, and integrator specification"
+ * (section "Structure and capabilities").  The field is a set of Fourier harmonics on a
+ * uniform radial grid evaluated by Lagrange interpolation, optionally with a superimposed MHD-mode
+ * perturbation stored as a radial grid of Fourier harmonics; the integrator is a
+ * Dormand-Prince 5 scheme with minimum-step control; particles are independent
+ * (PAPER.md:48).  Where the paper prints no mathematics the operations are those of DESIGN.md section 2
+ * (readings O1-O8, A1-A22 of SURVEY.md section 8(c)).
+ *
+ * Conventions.  Every function returns GC_OK (0) or a negative gc_status; the text of the last failure
+ * on the calling thread is available from gc_last_error().  No C++ exception crosses the boundary.
+ * The library never frees or retains caller buffers.  There is no CPU fallback: every entry point that
+ * computes needs a CUDA device and fails with GC_ECUDA otherwise.
+ */
+#ifndef GCORBIT_H
+#define GCORBIT_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  GC_OK = 0,
+  GC_EINVAL = -1,   /* bad shape, NULL where data is required, NaN in a table, ns < 4, omega == 0 ... */
+  GC_ENOMEM = -2,   /* host or device allocation failed                                               */
+  GC_ECUDA = -3     /* CUDA runtime error; gc_last_error() carries cudaGetErrorString                 */
+} gc_status;
+
+typedef struct gc_field gc_field;   /* opaque; owns the device copies of all tables */
+
+/* Field description.  ALL POINTERS ARE HOST MEMORY and are copied by gc_field_create.
+ *   B(s,th,ze) = sum_k bmnc[.][k](s) cos(xm[k] th - xn[k] nfp ze)          stellarator-symmetric
+ *   radial grid s_j = j/(ns-1), j = 0..ns-1; cubic (4-point) Lagrange interpolation in s (O1)
+ *   perturbation  Phi = sum_k phihat[.][k](s) sin(mode_m th - mode_n ze + mode_omega t + mode_phase),
+ *   alpha from Phi by the ideal-MHD constraint E_par = 0 (O3).
+ * Harmonic lists may come in any order; duplicate (m, n) pairs add.  Requires xm >= 0. */
+typedef struct {
+  int32_t ns;                 /* radial nodes, >= 4                                             */
+  int32_t nfp;                /* field periods, >= 1                                            */
+  int32_t nh;                 /* equilibrium harmonics, >= 1                                    */
+  const int32_t* xm;          /* [nh] poloidal mode numbers, >= 0                               */
+  const int32_t* xn;          /* [nh] toroidal mode numbers in units of nfp                     */
+  const double* bmnc;         /* [ns][nh] node-major, tesla                                     */
+  const double* G;            /* [ns] T m  (covariant toroidal component)                       */
+  const double* I;            /* [ns] T m  (covariant poloidal component)                       */
+  const double* iota;         /* [ns] rotational transform                                      */
+  double psi0;                /* psi = psi0 * s: toroidal flux / 2 pi at s = 1, T m^2, != 0     */
+  int32_t nk;                 /* perturbation harmonics; 0 = static field                       */
+  const int32_t* mode_m;      /* [nk]                                                           */
+  const int32_t* mode_n;      /* [nk] actual toroidal numbers                                   */
+  const double* mode_omega;   /* [nk] rad/s, nonzero                                            */
+  const double* mode_phase;   /* [nk] rad                                                       */
+  const double* phihat;       /* [ns][nk] node-major, volts                                     */
+} gc_field_desc;
+
+/* Integrator specification (O5-O8).  The state integrated is (s, theta, zeta, v_par/v_ref). */
+typedef struct {
+  double mass, charge;        /* kg, C                                                          */
+  double t0, t_max;           /* s                                                              */
+  double rtol, atol;          /* RMS error norm, sk_i = atol + rtol max(|y_i|, |y_new_i|)       */
+  double v_ref;               /* m/s, > 0: scale of v_par in the error norm (A11)               */
+  double h0, h_min;           /* s; h0 > 0 first trial step; h_min >= 0 (0 disables the rule)   */
+  double s_loss, s_min;       /* stop when s >= s_loss (lost) or s <= s_min (axis)              */
+  int64_t max_steps;          /* attempted steps per particle before status 3                   */
+  int64_t poincare_capacity;  /* records available in `poincare`; 0 disables recording (O8)     */
+} gc_trace_params;
+
+/* Per-particle exit status written by gc_trace. */
+enum { GC_ST_TMAX = 0, GC_ST_LOST = 1, GC_ST_AXIS = 2, GC_ST_MAXSTEPS = 3, GC_ST_NONFINITE = 4 };
+
+/* Kernel selection for gc_trace (gc_set_kernel).  AUTO takes the warp-cooperative kernel when the field
+ * fits its layout (max |xn| <= 16, max xm <= 31) and the generic one otherwise. */
+enum { GC_KERNEL_AUTO = 0, GC_KERNEL_GENERIC = 1, GC_KERNEL_WARP = 2 };
+
+/* Copies the tables to the device, checks them (finite values, xm >= 0, omega != 0) and builds the
+ * packed by-node layout of the warp kernel.  *out is NULL on failure. */
+int gc_field_create(const gc_field_desc* desc, gc_field** out);
+int gc_field_destroy(gc_field* f);
+
+/* O2 at n points.  DEVICE pointers.  B [n]; dB [3][n] = dB/ds, dB/dtheta, dB/dzeta, or NULL.
+ * Asynchronous on `stream` (a cudaStream_t, NULL = default stream).  Used to compute mu and by tests. */
+int gc_field_eval(const gc_field* f, int64_t n, const double* s, const double* th, const double* ze,
+                  double* B, double* dB, void* stream);
+
+/* O3 at n points and time t.  DEVICE pointers.  out [9][n] = Phi, Phi_psi, Phi_theta, Phi_zeta, alpha,
+ * alpha_psi, alpha_theta, alpha_zeta, alpha_t.  All zero for a static field. */
+int gc_pert_eval(const gc_field* f, int64_t n, const double* s, const double* th, const double* ze,
+                 double t, double* out, void* stream);
+
+/* O4 at n states.  DEVICE pointers.  y [4][n] = s, theta, zeta, v_par (m/s); dydt [4][n] = ds/dt,
+ * dtheta/dt, dzeta/dt, dv_par/dt (m/s^2).  Evaluated by the same device code path as the selected trace
+ * kernel, so tests can pin the right-hand side alone. */
+int gc_rhs_eval(const gc_field* f, double mass, double charge, double t, int64_t n, const double* y,
+                const double* mu, double* dydt, void* stream);
+
+/* O5-O8: trace n independent particles.  ALL ARRAY POINTERS ARE DEVICE MEMORY owned by the caller and
+ * must stay valid until `stream` is synchronised; the call is asynchronous on `stream`.
+ *   in : s0, th0, ze0, vpar0 (m/s), mu (J/T)         [n] each, never modified
+ *   io : h_inout [n] or NULL: first trial step if > 0 (else params->h0); next proposal on return
+ *   out: y_out [4][n] = s, theta, zeta, v_par (m/s);  t_out [n] end time (loss time when status == 1);
+ *        status [n] (GC_ST_*);  n_acc, n_rej, n_forced [n] each or NULL (attempt counters);
+ *        poincare [capacity][4] = particle id, t, s, theta mod 2 pi, or NULL;
+ *        poincare_count: one int64 on the device, total crossings found (> capacity means the excess
+ *        was dropped).  Record order is unspecified.
+ * Per-particle failures are reported in `status`, never as a call failure. */
+int gc_trace(const gc_field* f, const gc_trace_params* params, int64_t n,
+             const double* s0, const double* th0, const double* ze0, const double* vpar0,
+             const double* mu, double* h_inout,
+             double* y_out, double* t_out, int32_t* status,
+             int32_t* n_acc, int32_t* n_rej, int32_t* n_forced,
+             double* poincare, int64_t* poincare_count, void* stream);
+
+/* The same trace with HOST buffers: allocates device scratch, copies the inputs in, runs gc_trace,
+ * copies every non-NULL output back and synchronises.  `poincare_count` is a host int64 here. */
+int gc_trace_host(const gc_field* f, const gc_trace_params* params, int64_t n,
+                  const double* s0, const double* th0, const double* ze0, const double* vpar0,
+                  const double* mu, double* h_inout,
+                  double* y_out, double* t_out, int32_t* status,
+                  int32_t* n_acc, int32_t* n_rej, int32_t* n_forced,
+                  double* poincare, int64_t* poincare_count);
+
+/* Kernel choice (GC_KERNEL_*) for later gc_trace / gc_rhs_eval calls on this field; GC_EINVAL if the
+ * field does not fit the requested kernel. */
+int gc_set_kernel(gc_field* f, int32_t kernel);
+/* Which kernel gc_trace will launch for this field (GC_KERNEL_GENERIC or GC_KERNEL_WARP), and its launch
+ * geometry; any pointer may be NULL. */
+int gc_kernel_info(const gc_field* f, int32_t* kernel, int32_t* blocks, int32_t* threads_per_block,
+                   int32_t* smem_bytes, int32_t* regs_per_thread);
+
+/* Register-only DFMA loop on every SM: measures the FP64 pipe's sustained rate that the roofline of
+ * DESIGN.md section 6 is quoted against.  Writes achieved FLOP/s (2 per DFMA) to *flops_per_s (host).
+ * Synchronous. */
+int gc_fp64_peak_probe(double* flops_per_s, double* elapsed_ms);
+
+/* Thread-local text of the last nonzero return ("" if none). */
+const char* gc_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

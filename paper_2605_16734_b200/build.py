@@ -1,0 +1,43 @@
+"""Build libgcorbit.so in-tree with nvcc for sm_100a (no JIT cache: the .so travels with the repo snapshot)."""
+from __future__ import annotations
+
+import os
+import subprocess
+import sys
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(_HERE, "csrc")
+SO = os.path.join(_HERE, "libgcorbit.so")
+SOURCES = ["gcorbit_api.cu"]
+HEADERS = ["device_math.cuh", "field.cuh", "kernels_generic.cuh", "kernels_warp.cuh",
+           os.path.join("..", "..", "include", "gcorbit.h")]
+
+
+def nvcc_cmd(extra=()):
+    return ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
+            "-shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v", *extra,
+            *[os.path.join(CSRC, s) for s in SOURCES], "-o", SO]
+
+
+def needs_build() -> bool:
+    if not os.path.exists(SO):
+        return True
+    t = os.path.getmtime(SO)
+    deps = [os.path.join(CSRC, s) for s in SOURCES + HEADERS] + [os.path.abspath(__file__)]
+    return any(os.path.getmtime(d) > t for d in deps)
+
+
+def build(force: bool = False, verbose: bool = False, extra=()) -> str:
+    if force or needs_build():
+        r = subprocess.run(nvcc_cmd(extra), capture_output=True, text=True)
+        if verbose or r.returncode != 0:
+            sys.stderr.write(r.stdout + r.stderr)
+        if r.returncode != 0:
+            raise RuntimeError("nvcc failed building libgcorbit.so")
+        with open(os.path.join(_HERE, "build_ptxas.log"), "w") as fh:
+            fh.write(" ".join(nvcc_cmd(extra)) + "\n" + r.stdout + r.stderr)
+    return SO
+
+
+if __name__ == "__main__":
+    build(force=True, verbose=True, extra=tuple(sys.argv[1:]))

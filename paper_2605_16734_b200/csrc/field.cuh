@@ -1,0 +1,45 @@
+// field.cuh -- device-side view of a gc_field and the launch parameter blocks.
+#pragma once
+#include <stdint.h>
+
+namespace gc {
+
+// Device pointers into the tables owned by gc_field.  Passed to kernels by value.
+struct FieldDev {
+  int ns, nfp, nh, nk;
+  double psi0, inv_psi0;
+  // as given by the caller (generic kernel, gc_field_eval)
+  const int* xm;         // [nh]
+  const int* xn;         // [nh]
+  const double* bmnc;    // [ns][nh]
+  const double* G;       // [ns]
+  const double* I;       // [ns]
+  const double* iota;    // [ns]
+  const int* mode_m;     // [nk]
+  const int* mode_n;     // [nk]
+  const double* omega;   // [nk]
+  const double* phase;   // [nk]
+  const double* phihat;  // [ns][nk]
+  // packed by-node layout of the warp kernel (kernels_warp.cuh): rows[node][it][lane]
+  const double* rows;
+  int M, N;              // max xm, max |xn|
+  int cl_log;            // log2(lanes per m-group)
+  int nit_main, nx, nit; // main iterations, extra iterations, total
+};
+
+// Integrator parameters as the kernels see them (gc_trace_params + derived values).
+struct TraceDev {
+  double mass, charge, t0, t_max, rtol, atol, v_ref, inv_v_ref, h0, h_min, s_loss, s_min;
+  long long max_steps, poincare_capacity;
+  long long n;
+  const double *s0, *th0, *ze0, *vpar0, *mu;
+  double* h_inout;
+  double *y_out, *t_out;
+  int* status;
+  int *n_acc, *n_rej, *n_forced;
+  double* poincare;
+  unsigned long long* poincare_count;
+  unsigned long long* work_counter;   // persistent-kernel particle queue head
+};
+
+}  // namespace gc

@@ -1,0 +1,497 @@
+// gcorbit_api.cu -- C ABI of libgcorbit.so (include/gcorbit.h): table upload and packing, kernel dispatch.
+// Build: nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -shared -Xcompiler -fPIC
+#include "../../include/gcorbit.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+namespace gc { constexpr int GC_ST_NONFINITE_ = 4; }
+#include "kernels_generic.cuh"
+#include "kernels_warp.cuh"
+
+namespace {
+
+thread_local std::string g_last_error;
+
+int fail(int code, const std::string& msg) {
+  g_last_error = msg;
+  return code;
+}
+
+#define GC_CUDA(expr)                                                                          \
+  do {                                                                                         \
+    cudaError_t e_ = (expr);                                                                   \
+    if (e_ != cudaSuccess)                                                                     \
+      return fail(e_ == cudaErrorMemoryAllocation ? GC_ENOMEM : GC_ECUDA,                      \
+                  std::string(#expr) + ": " + cudaGetErrorString(e_));                         \
+  } while (0)
+
+template <typename T>
+int upload(const T* host, size_t count, T** dev) {
+  *dev = nullptr;
+  if (count == 0) return GC_OK;
+  GC_CUDA(cudaMalloc((void**)dev, count * sizeof(T)));
+  GC_CUDA(cudaMemcpy(*dev, host, count * sizeof(T), cudaMemcpyHostToDevice));
+  return GC_OK;
+}
+
+bool all_finite(const double* p, size_t n) {
+  for (size_t i = 0; i < n; ++i)
+    if (!std::isfinite(p[i])) return false;
+  return true;
+}
+
+}  // namespace
+
+struct gc_field {
+  gc::FieldDev dev{};
+  std::vector<void*> allocs;
+  int kernel = GC_KERNEL_GENERIC;   // resolved choice
+  bool warp_ok = false;
+  int nit_main_inst = 0;            // instantiated (padded) main iteration count
+  int sm_count = 0;
+};
+
+namespace {
+
+// ---- warp-kernel instantiations -------------------------------------------------------------------------------
+// NIT_MAIN is padded up to the next compiled size; NX in {1, 2}; NREG = iterations kept in registers.
+struct WarpInst {
+  int nit_main, nx;
+  bool modes;
+  const void* trace_fn;
+  const void* rhs_fn;
+  int smem_bytes;
+};
+
+template <int NIT_MAIN, int NX, bool MODES, int NREG>
+WarpInst make_inst() {
+  constexpr int NSM = NIT_MAIN + NX - NREG;
+  return WarpInst{NIT_MAIN, NX, MODES,
+                  (const void*)gc::trace_warp_kernel<NIT_MAIN, NX, MODES, NREG>,
+                  (const void*)gc::rhs_eval_warp_kernel<NIT_MAIN, NX, MODES, NREG>,
+                  (int)(sizeof(gc::WarpScratch) * gc::kWarpsPerBlock +
+                        (size_t)gc::kWarpsPerBlock * NSM * 4 * 32 * sizeof(double))};
+}
+
+#ifndef GC_NREG_LARGE
+#define GC_NREG_LARGE 18
+#endif
+
+const std::vector<WarpInst>& warp_instances() {
+  static const std::vector<WarpInst> v = {
+      make_inst<5, 1, false, 6>(),  make_inst<5, 1, true, 6>(),  make_inst<5, 2, true, 7>(),
+      make_inst<9, 1, false, 10>(), make_inst<9, 1, true, 10>(), make_inst<9, 2, true, 11>(),
+      make_inst<17, 1, false, (GC_NREG_LARGE < 18 ? GC_NREG_LARGE : 18)>(),
+      make_inst<17, 1, true, (GC_NREG_LARGE < 18 ? GC_NREG_LARGE : 18)>(),
+      make_inst<17, 2, true, (GC_NREG_LARGE < 19 ? GC_NREG_LARGE : 19)>(),
+  };
+  return v;
+}
+
+const WarpInst* find_inst(const gc_field* f) {
+  if (!f->warp_ok) return nullptr;
+  for (const WarpInst& w : warp_instances())
+    if (w.nit_main == f->nit_main_inst && w.nx == f->dev.nx && w.modes == (f->dev.nk > 0)) return &w;
+  return nullptr;
+}
+
+int ensure_smem(const void* fn, int bytes) {
+  GC_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  return GC_OK;
+}
+
+// Packed rows[node][it][lane] of the warp kernel (kernels_warp.cuh header comment).
+int pack_rows(gc_field* f, const gc_field_desc* d) {
+  gc::FieldDev& v = f->dev;
+  const int M = v.M, N = v.N;
+  f->warp_ok = false;
+  if (N > gc::kMaxN || M > 28) return GC_OK;
+  int cl_log = 5;
+  if (N > 0) {
+    cl_log = 1;
+    while ((1 << cl_log) < 2 * N) ++cl_log;
+  }
+  const int groups = 32 >> cl_log;
+  const int nit_main = N > 0 ? (M + 1 + groups - 1) / groups : 0;
+  const int nx = (M + 4 + d->nk + 31) / 32;
+  int inst = -1;
+  for (const WarpInst& w : warp_instances())
+    if (w.nit_main >= nit_main && w.nit_main * groups <= gc::kMaxRowsM && w.nx == nx &&
+        w.modes == (d->nk > 0) && (inst < 0 || w.nit_main < inst))
+      inst = w.nit_main;
+  if (inst < 0) return GC_OK;
+  const int nit = inst + nx;
+  std::vector<double> rows((size_t)d->ns * nit * 32, 0.0);
+  const int cl = 1 << cl_log;
+  for (int node = 0; node < d->ns; ++node) {
+    double* row = rows.data() + (size_t)node * nit * 32;
+    for (int k = 0; k < d->nh; ++k) {
+      const int m = d->xm[k], n = d->xn[k];
+      const double b = d->bmnc[(size_t)node * d->nh + k];
+      if (n == 0) {
+        row[(size_t)inst * 32 + m] += b;                      // n = 0 column: extra index m
+        continue;
+      }
+      const int an = n > 0 ? n : -n;
+      const int g = m % groups, it = m / groups;
+      const int laneP = g * cl + 2 * (an - 1), laneQ = laneP + 1;
+      row[(size_t)it * 32 + laneP] += b;                      // P = b(m,n) + b(m,-n)
+      row[(size_t)it * 32 + laneQ] += n > 0 ? b : -b;         // Q = b(m,n) - b(m,-n)
+    }
+    auto extra = [&](int e) -> double& { return row[(size_t)(inst + e / 32) * 32 + (e % 32)]; };
+    extra(M + 1) = d->G[node];
+    extra(M + 2) = d->I[node];
+    extra(M + 3) = d->iota[node];
+    for (int k = 0; k < d->nk; ++k) extra(M + 4 + k) = d->phihat[(size_t)node * d->nk + k];
+  }
+  double* dev_rows = nullptr;
+  int rc = upload(rows.data(), rows.size(), &dev_rows);
+  if (rc != GC_OK) return rc;
+  f->allocs.push_back(dev_rows);
+  v.rows = dev_rows;
+  v.cl_log = cl_log;
+  v.nit_main = inst;
+  v.nx = nx;
+  v.nit = nit;
+  f->nit_main_inst = inst;
+  f->warp_ok = true;
+  return GC_OK;
+}
+
+int build_trace_dev(const gc_field* f, const gc_trace_params* p, int64_t n, gc::TraceDev* t) {
+  if (!f || !p) return fail(GC_EINVAL, "gc_trace: NULL field or params");
+  if (n < 0) return fail(GC_EINVAL, "gc_trace: n < 0");
+  if (!(p->v_ref > 0.0) || !(p->h0 > 0.0) || !(p->h_min >= 0.0) || !(p->mass > 0.0) || p->charge == 0.0 ||
+      !(p->rtol >= 0.0) || !(p->atol >= 0.0) || !(p->rtol + p->atol > 0.0) || p->max_steps < 1 ||
+      p->poincare_capacity < 0 || !std::isfinite(p->t0) || !std::isfinite(p->t_max))
+    return fail(GC_EINVAL, "gc_trace: invalid integrator specification");
+  t->mass = p->mass; t->charge = p->charge; t->t0 = p->t0; t->t_max = p->t_max;
+  t->rtol = p->rtol; t->atol = p->atol; t->v_ref = p->v_ref; t->inv_v_ref = 1.0 / p->v_ref;
+  t->h0 = p->h0; t->h_min = p->h_min; t->s_loss = p->s_loss; t->s_min = p->s_min;
+  t->max_steps = p->max_steps; t->poincare_capacity = p->poincare_capacity; t->n = n;
+  return GC_OK;
+}
+
+__global__ void dfma_probe_kernel(double* out, int iters) {
+  double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6,
+         a7 = a0 + 7;
+  const double x = 0.999999999, y = 1e-12;
+  for (int i = 0; i < iters; ++i) {
+    a0 = fma(a0, x, y); a1 = fma(a1, x, y); a2 = fma(a2, x, y); a3 = fma(a3, x, y);
+    a4 = fma(a4, x, y); a5 = fma(a5, x, y); a6 = fma(a6, x, y); a7 = fma(a7, x, y);
+  }
+  if (a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7 == 12345.678) out[0] = a0;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* gc_last_error(void) { return g_last_error.c_str(); }
+
+int gc_field_destroy(gc_field* f) {
+  if (!f) return GC_OK;
+  for (void* p : f->allocs) cudaFree(p);
+  delete f;
+  return GC_OK;
+}
+
+int gc_field_create(const gc_field_desc* d, gc_field** out) {
+  if (!out) return fail(GC_EINVAL, "gc_field_create: out is NULL");
+  *out = nullptr;
+  if (!d) return fail(GC_EINVAL, "gc_field_create: desc is NULL");
+  if (d->ns < 4) return fail(GC_EINVAL, "gc_field_create: ns < 4");
+  if (d->nfp < 1) return fail(GC_EINVAL, "gc_field_create: nfp < 1");
+  if (d->nh < 1 || d->nk < 0) return fail(GC_EINVAL, "gc_field_create: nh < 1 or nk < 0");
+  if (!d->xm || !d->xn || !d->bmnc || !d->G || !d->I || !d->iota)
+    return fail(GC_EINVAL, "gc_field_create: NULL table pointer");
+  if (d->nk > 0 && (!d->mode_m || !d->mode_n || !d->mode_omega || !d->mode_phase || !d->phihat))
+    return fail(GC_EINVAL, "gc_field_create: NULL mode table pointer");
+  if (!(d->psi0 != 0.0) || !std::isfinite(d->psi0)) return fail(GC_EINVAL, "gc_field_create: psi0 must be finite, nonzero");
+  if (!all_finite(d->bmnc, (size_t)d->ns * d->nh) || !all_finite(d->G, d->ns) || !all_finite(d->I, d->ns) ||
+      !all_finite(d->iota, d->ns))
+    return fail(GC_EINVAL, "gc_field_create: non-finite value in an equilibrium table");
+  int M = 0, N = 0;
+  for (int k = 0; k < d->nh; ++k) {
+    if (d->xm[k] < 0) return fail(GC_EINVAL, "gc_field_create: xm < 0");
+    M = d->xm[k] > M ? d->xm[k] : M;
+    const int an = d->xn[k] < 0 ? -d->xn[k] : d->xn[k];
+    N = an > N ? an : N;
+  }
+  for (int k = 0; k < d->nk; ++k) {
+    if (!(d->mode_omega[k] != 0.0) || !std::isfinite(d->mode_omega[k]))
+      return fail(GC_EINVAL, "gc_field_create: mode_omega must be finite, nonzero");
+    if (!std::isfinite(d->mode_phase[k])) return fail(GC_EINVAL, "gc_field_create: non-finite mode_phase");
+  }
+  if (d->nk > 0 && !all_finite(d->phihat, (size_t)d->ns * d->nk))
+    return fail(GC_EINVAL, "gc_field_create: non-finite value in phihat");
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1)
+    return fail(GC_ECUDA, "gc_field_create: no CUDA device (this library has no CPU fallback)");
+  gc_field* f = new (std::nothrow) gc_field;
+  if (!f) return fail(GC_ENOMEM, "gc_field_create: host allocation failed");
+  gc::FieldDev& v = f->dev;
+  v.ns = d->ns; v.nfp = d->nfp; v.nh = d->nh; v.nk = d->nk; v.psi0 = d->psi0; v.inv_psi0 = 1.0 / d->psi0;
+  v.M = M; v.N = N;
+  int rc = GC_OK;
+  auto up = [&](auto host, size_t count, auto** devp) {
+    if (rc != GC_OK) return;
+    rc = upload(host, count, devp);
+    if (rc == GC_OK && *devp) f->allocs.push_back((void*)*devp);
+  };
+  int *xm, *xn, *mm, *mn;
+  double *bmnc, *G, *I, *iota, *om, *ph, *phihat;
+  up(d->xm, d->nh, &xm); up(d->xn, d->nh, &xn); up(d->bmnc, (size_t)d->ns * d->nh, &bmnc);
+  up(d->G, d->ns, &G); up(d->I, d->ns, &I); up(d->iota, d->ns, &iota);
+  up(d->mode_m, d->nk, &mm); up(d->mode_n, d->nk, &mn); up(d->mode_omega, d->nk, &om);
+  up(d->mode_phase, d->nk, &ph); up(d->phihat, (size_t)d->ns * d->nk, &phihat);
+  if (rc == GC_OK) {
+    v.xm = xm; v.xn = xn; v.bmnc = bmnc; v.G = G; v.I = I; v.iota = iota;
+    v.mode_m = mm; v.mode_n = mn; v.omega = om; v.phase = ph; v.phihat = phihat;
+    rc = pack_rows(f, d);
+  }
+  if (rc == GC_OK) {
+    int devid = 0;
+    cudaGetDevice(&devid);
+    cudaDeviceGetAttribute(&f->sm_count, cudaDevAttrMultiProcessorCount, devid);
+    f->kernel = f->warp_ok ? GC_KERNEL_WARP : GC_KERNEL_GENERIC;
+    if (f->warp_ok) {
+      const WarpInst* w = find_inst(f);
+      rc = ensure_smem(w->trace_fn, w->smem_bytes);
+      if (rc == GC_OK) rc = ensure_smem(w->rhs_fn, w->smem_bytes);
+    }
+  }
+  if (rc != GC_OK) {
+    const std::string keep = g_last_error;
+    gc_field_destroy(f);
+    g_last_error = keep;
+    return rc;
+  }
+  *out = f;
+  return GC_OK;
+}
+
+int gc_set_kernel(gc_field* f, int32_t kernel) {
+  if (!f) return fail(GC_EINVAL, "gc_set_kernel: NULL field");
+  if (kernel == GC_KERNEL_AUTO) kernel = f->warp_ok ? GC_KERNEL_WARP : GC_KERNEL_GENERIC;
+  if (kernel == GC_KERNEL_WARP && !f->warp_ok)
+    return fail(GC_EINVAL, "gc_set_kernel: field does not fit the warp kernel (max|xn| <= 16, max xm <= 28)");
+  if (kernel != GC_KERNEL_WARP && kernel != GC_KERNEL_GENERIC) return fail(GC_EINVAL, "gc_set_kernel: unknown kernel");
+  f->kernel = kernel;
+  return GC_OK;
+}
+
+int gc_kernel_info(const gc_field* f, int32_t* kernel, int32_t* blocks, int32_t* threads, int32_t* smem,
+                   int32_t* regs) {
+  if (!f) return fail(GC_EINVAL, "gc_kernel_info: NULL field");
+  cudaFuncAttributes at{};
+  int b, t, s;
+  if (f->kernel == GC_KERNEL_WARP) {
+    const WarpInst* w = find_inst(f);
+    GC_CUDA(cudaFuncGetAttributes(&at, w->trace_fn));
+    b = f->sm_count; t = gc::kWarpsPerBlock * 32; s = w->smem_bytes;
+  } else {
+    GC_CUDA(cudaFuncGetAttributes(&at, (const void*)gc::trace_generic_kernel));
+    b = f->sm_count * 4; t = 128; s = 0;
+  }
+  if (kernel) *kernel = f->kernel;
+  if (blocks) *blocks = b;
+  if (threads) *threads = t;
+  if (smem) *smem = s;
+  if (regs) *regs = at.numRegs;
+  return GC_OK;
+}
+
+int gc_field_eval(const gc_field* f, int64_t n, const double* s, const double* th, const double* ze, double* B,
+                  double* dB, void* stream) {
+  if (!f || n < 0) return fail(GC_EINVAL, "gc_field_eval: NULL field or n < 0");
+  if (n == 0) return GC_OK;
+  if (!s || !th || !ze || !B) return fail(GC_EINVAL, "gc_field_eval: NULL array");
+  const int tb = 128;
+  gc::field_eval_kernel<<<(unsigned)((n + tb - 1) / tb), tb, 0, (cudaStream_t)stream>>>(f->dev, n, s, th, ze, B, dB);
+  GC_CUDA(cudaGetLastError());
+  return GC_OK;
+}
+
+int gc_pert_eval(const gc_field* f, int64_t n, const double* s, const double* th, const double* ze, double t,
+                 double* out, void* stream) {
+  if (!f || n < 0) return fail(GC_EINVAL, "gc_pert_eval: NULL field or n < 0");
+  if (n == 0) return GC_OK;
+  if (!s || !th || !ze || !out) return fail(GC_EINVAL, "gc_pert_eval: NULL array");
+  const int tb = 128;
+  gc::pert_eval_kernel<<<(unsigned)((n + tb - 1) / tb), tb, 0, (cudaStream_t)stream>>>(f->dev, n, s, th, ze, t, out);
+  GC_CUDA(cudaGetLastError());
+  return GC_OK;
+}
+
+int gc_rhs_eval(const gc_field* f, double mass, double charge, double t, int64_t n, const double* y,
+                const double* mu, double* dydt, void* stream) {
+  if (!f || n < 0) return fail(GC_EINVAL, "gc_rhs_eval: NULL field or n < 0");
+  if (n == 0) return GC_OK;
+  if (!y || !mu || !dydt) return fail(GC_EINVAL, "gc_rhs_eval: NULL array");
+  if (f->kernel == GC_KERNEL_WARP) {
+    const WarpInst* w = find_inst(f);
+    long long nn = n;
+    void* args[] = {(void*)&f->dev, &mass, &charge, &t, &nn, (void*)&y, (void*)&mu, (void*)&dydt};
+    long long blocks = (n + gc::kWarpsPerBlock - 1) / gc::kWarpsPerBlock;
+    if (blocks > f->sm_count) blocks = f->sm_count;
+    GC_CUDA(cudaLaunchKernel(w->rhs_fn, dim3((unsigned)blocks), dim3(gc::kWarpsPerBlock * 32), args,
+                             (size_t)w->smem_bytes, (cudaStream_t)stream));
+  } else {
+    const int tb = 128;
+    gc::rhs_eval_generic_kernel<<<(unsigned)((n + tb - 1) / tb), tb, 0, (cudaStream_t)stream>>>(
+        f->dev, mass, charge, t, n, y, mu, dydt);
+    GC_CUDA(cudaGetLastError());
+  }
+  return GC_OK;
+}
+
+int gc_trace(const gc_field* f, const gc_trace_params* params, int64_t n, const double* s0, const double* th0,
+             const double* ze0, const double* vpar0, const double* mu, double* h_inout, double* y_out,
+             double* t_out, int32_t* status, int32_t* n_acc, int32_t* n_rej, int32_t* n_forced, double* poincare,
+             int64_t* poincare_count, void* stream) {
+  gc::TraceDev t{};
+  int rc = build_trace_dev(f, params, n, &t);
+  if (rc != GC_OK) return rc;
+  if (n == 0) return GC_OK;
+  if (!s0 || !th0 || !ze0 || !vpar0 || !mu || !y_out || !t_out || !status)
+    return fail(GC_EINVAL, "gc_trace: NULL particle array");
+  if (params->poincare_capacity > 0 && (!poincare || !poincare_count))
+    return fail(GC_EINVAL, "gc_trace: poincare_capacity > 0 needs poincare and poincare_count");
+  cudaStream_t st = (cudaStream_t)stream;
+  t.s0 = s0; t.th0 = th0; t.ze0 = ze0; t.vpar0 = vpar0; t.mu = mu; t.h_inout = h_inout;
+  t.y_out = y_out; t.t_out = t_out; t.status = status; t.n_acc = n_acc; t.n_rej = n_rej; t.n_forced = n_forced;
+  t.poincare = poincare;
+  t.poincare_count = reinterpret_cast<unsigned long long*>(poincare_count);
+  if (!poincare || !poincare_count) t.poincare_capacity = 0;
+  if (poincare_count) GC_CUDA(cudaMemsetAsync(poincare_count, 0, sizeof(int64_t), st));
+  if (f->kernel == GC_KERNEL_WARP) {
+    const WarpInst* w = find_inst(f);
+    unsigned long long* counter = nullptr;
+    GC_CUDA(cudaMallocAsync((void**)&counter, sizeof(unsigned long long), st));
+    GC_CUDA(cudaMemsetAsync(counter, 0, sizeof(unsigned long long), st));
+    t.work_counter = counter;
+    void* args[] = {(void*)&f->dev, (void*)&t};
+    long long blocks = (n + gc::kWarpsPerBlock - 1) / gc::kWarpsPerBlock;
+    if (blocks > f->sm_count) blocks = f->sm_count;
+    GC_CUDA(cudaLaunchKernel(w->trace_fn, dim3((unsigned)blocks), dim3(gc::kWarpsPerBlock * 32), args,
+                             (size_t)w->smem_bytes, st));
+    GC_CUDA(cudaFreeAsync(counter, st));
+  } else {
+    long long blocks = (n + 127) / 128;
+    if (blocks > (long long)f->sm_count * 16) blocks = (long long)f->sm_count * 16;
+    gc::trace_generic_kernel<<<(unsigned)blocks, 128, 0, st>>>(f->dev, t);
+    GC_CUDA(cudaGetLastError());
+  }
+  return GC_OK;
+}
+
+int gc_trace_host(const gc_field* f, const gc_trace_params* params, int64_t n, const double* s0,
+                  const double* th0, const double* ze0, const double* vpar0, const double* mu, double* h_inout,
+                  double* y_out, double* t_out, int32_t* status, int32_t* n_acc, int32_t* n_rej,
+                  int32_t* n_forced, double* poincare, int64_t* poincare_count) {
+  if (!f || !params || n < 0) return fail(GC_EINVAL, "gc_trace_host: NULL field/params or n < 0");
+  if (n == 0) return GC_OK;
+  if (!s0 || !th0 || !ze0 || !vpar0 || !mu || !y_out || !t_out || !status)
+    return fail(GC_EINVAL, "gc_trace_host: NULL particle array");
+  const size_t nd = (size_t)n;
+  const int64_t cap = (poincare && poincare_count) ? params->poincare_capacity : 0;
+  // one device slab: 5 inputs, h, y_out[4], t_out (doubles) | status + 3 counters (int32) | poincare
+  const size_t n_dbl = nd * 11 + (size_t)cap * 4 + 1;
+  double* dbl = nullptr;
+  int32_t* i32 = nullptr;
+  cudaStream_t st = nullptr;
+  int rc = GC_OK;
+  auto cleanup = [&]() {
+    if (dbl) cudaFree(dbl);
+    if (i32) cudaFree(i32);
+    if (st) cudaStreamDestroy(st);
+  };
+#define GC_H(expr)                                                                 \
+  do {                                                                             \
+    cudaError_t e_ = (expr);                                                       \
+    if (e_ != cudaSuccess) {                                                       \
+      rc = fail(e_ == cudaErrorMemoryAllocation ? GC_ENOMEM : GC_ECUDA,            \
+                std::string(#expr) + ": " + cudaGetErrorString(e_));               \
+      cleanup();                                                                   \
+      return rc;                                                                   \
+    }                                                                              \
+  } while (0)
+  GC_H(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
+  GC_H(cudaMalloc((void**)&dbl, n_dbl * sizeof(double)));
+  GC_H(cudaMalloc((void**)&i32, nd * 4 * sizeof(int32_t)));
+  double *d_s = dbl, *d_th = dbl + nd, *d_ze = dbl + 2 * nd, *d_v = dbl + 3 * nd, *d_mu = dbl + 4 * nd,
+         *d_h = dbl + 5 * nd, *d_y = dbl + 6 * nd, *d_t = dbl + 10 * nd, *d_pc = dbl + 11 * nd;
+  int64_t* d_cnt = reinterpret_cast<int64_t*>(dbl + 11 * nd + (size_t)cap * 4);
+  const size_t bytes = nd * sizeof(double);
+  GC_H(cudaMemcpyAsync(d_s, s0, bytes, cudaMemcpyHostToDevice, st));
+  GC_H(cudaMemcpyAsync(d_th, th0, bytes, cudaMemcpyHostToDevice, st));
+  GC_H(cudaMemcpyAsync(d_ze, ze0, bytes, cudaMemcpyHostToDevice, st));
+  GC_H(cudaMemcpyAsync(d_v, vpar0, bytes, cudaMemcpyHostToDevice, st));
+  GC_H(cudaMemcpyAsync(d_mu, mu, bytes, cudaMemcpyHostToDevice, st));
+  if (h_inout) GC_H(cudaMemcpyAsync(d_h, h_inout, bytes, cudaMemcpyHostToDevice, st));
+  rc = gc_trace(f, params, n, d_s, d_th, d_ze, d_v, d_mu, h_inout ? d_h : nullptr, d_y, d_t, i32,
+                n_acc ? i32 + nd : nullptr, n_rej ? i32 + 2 * nd : nullptr, n_forced ? i32 + 3 * nd : nullptr,
+                cap > 0 ? d_pc : nullptr, cap > 0 ? d_cnt : nullptr, st);
+  if (rc != GC_OK) { cleanup(); return rc; }
+  GC_H(cudaMemcpyAsync(y_out, d_y, 4 * bytes, cudaMemcpyDeviceToHost, st));
+  GC_H(cudaMemcpyAsync(t_out, d_t, bytes, cudaMemcpyDeviceToHost, st));
+  GC_H(cudaMemcpyAsync(status, i32, nd * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  if (h_inout) GC_H(cudaMemcpyAsync(h_inout, d_h, bytes, cudaMemcpyDeviceToHost, st));
+  if (n_acc) GC_H(cudaMemcpyAsync(n_acc, i32 + nd, nd * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  if (n_rej) GC_H(cudaMemcpyAsync(n_rej, i32 + 2 * nd, nd * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  if (n_forced) GC_H(cudaMemcpyAsync(n_forced, i32 + 3 * nd, nd * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  if (cap > 0) {
+    GC_H(cudaMemcpyAsync(poincare_count, d_cnt, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+    GC_H(cudaStreamSynchronize(st));
+    const int64_t got = *poincare_count < cap ? *poincare_count : cap;
+    if (got > 0) GC_H(cudaMemcpyAsync(poincare, d_pc, (size_t)got * 4 * sizeof(double), cudaMemcpyDeviceToHost, st));
+  } else if (poincare_count) {
+    *poincare_count = 0;
+  }
+  GC_H(cudaStreamSynchronize(st));
+#undef GC_H
+  cleanup();
+  return GC_OK;
+}
+
+int gc_fp64_peak_probe(double* flops_per_s, double* elapsed_ms) {
+  int devid = 0, sms = 0;
+  GC_CUDA(cudaGetDevice(&devid));
+  GC_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, devid));
+  double* out = nullptr;
+  GC_CUDA(cudaMalloc((void**)&out, sizeof(double)));
+  const int iters = 200000, blocks = sms * 2, threads = 512;
+  cudaEvent_t a, b;
+  GC_CUDA(cudaEventCreate(&a));
+  GC_CUDA(cudaEventCreate(&b));
+  dfma_probe_kernel<<<blocks, threads>>>(out, 1000);
+  GC_CUDA(cudaDeviceSynchronize());
+  float best = 1e30f;
+  for (int rep = 0; rep < 3; ++rep) {
+    GC_CUDA(cudaEventRecord(a));
+    dfma_probe_kernel<<<blocks, threads>>>(out, iters);
+    GC_CUDA(cudaEventRecord(b));
+    GC_CUDA(cudaEventSynchronize(b));
+    float ms = 0;
+    GC_CUDA(cudaEventElapsedTime(&ms, a, b));
+    best = ms < best ? ms : best;
+  }
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  cudaFree(out);
+  const double flops = 2.0 * 8.0 * (double)iters * (double)blocks * (double)threads;
+  if (flops_per_s) *flops_per_s = flops / (best * 1e-3);
+  if (elapsed_ms) *elapsed_ms = best;
+  return GC_OK;
+}
+
+}  // extern "C"

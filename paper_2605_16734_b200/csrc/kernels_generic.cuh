@@ -1,0 +1,334 @@
+// kernels_generic.cuh -- shape-agnostic kernels: one thread per point / particle, tables read from global
+// memory in the caller's layout, one sincos per harmonic.  This is the path for fields that do not fit the
+// warp kernel's packed layout, the engine of gc_field_eval / gc_pert_eval, and the kernel that the warp
+// kernel was first validated against.  Same equations and controller as kernels_warp.cuh.
+#pragma once
+#include "device_math.cuh"
+#include "field.cuh"
+
+namespace gc {
+
+// ---- O2 / O3 point evaluations -------------------------------------------------------------------------
+struct Profiles { double G, Gs, I, Is, io, ios; };
+
+__device__ __forceinline__ void interp4(const double* tab, int stride, int i0, const double w[4],
+                                        const double dw[4], double& v, double& d) {
+  const double t0 = __ldg(tab + (size_t)(i0 + 0) * stride), t1 = __ldg(tab + (size_t)(i0 + 1) * stride);
+  const double t2 = __ldg(tab + (size_t)(i0 + 2) * stride), t3 = __ldg(tab + (size_t)(i0 + 3) * stride);
+  v = fma(w[3], t3, fma(w[2], t2, fma(w[1], t1, w[0] * t0)));
+  d = fma(dw[3], t3, fma(dw[2], t2, fma(dw[1], t1, dw[0] * t0)));
+}
+
+__device__ inline void eval_B_generic(const FieldDev& f, int i0, const double w[4], const double dw[4],
+                                      double th, double ze, double out[4]) {
+  const double thr = reduce_2pi(th);
+  const double phr = reduce_2pi((double)f.nfp * ze);
+  double B = 0.0, Bs = 0.0, Bth = 0.0, Bze = 0.0;
+  for (int k = 0; k < f.nh; ++k) {
+    double b, bs;
+    interp4(f.bmnc + k, f.nh, i0, w, dw, b, bs);
+    const double m = (double)__ldg(f.xm + k), n = (double)__ldg(f.xn + k);
+    double sn, cs;
+    sincos_poly(fma(m, thr, -n * phr), sn, cs);
+    B = fma(b, cs, B);
+    Bs = fma(bs, cs, Bs);
+    Bth = fma(-m * b, sn, Bth);
+    Bze = fma(n * (double)f.nfp * b, sn, Bze);
+  }
+  out[0] = B; out[1] = Bs; out[2] = Bth; out[3] = Bze;
+}
+
+// out = Phi, Phi_psi, Phi_th, Phi_ze, al, al_psi, al_th, al_ze, al_t
+__device__ inline void eval_pert_generic(const FieldDev& f, int i0, const double w[4], const double dw[4],
+                                         const Profiles& p, double th, double ze, double t, double out[9]) {
+  double Phi = 0, Phi_s = 0, Phi_th = 0, Phi_ze = 0, al = 0, al_s = 0, al_th = 0, al_ze = 0, al_t = 0;
+  const double thr = reduce_2pi(th), zer = reduce_2pi(ze);
+  const double GI = p.G + p.io * p.I, GI_s = p.Gs + p.ios * p.I + p.io * p.Is;
+  for (int k = 0; k < f.nk; ++k) {
+    double ph, ph_s;
+    interp4(f.phihat + k, f.nk, i0, w, dw, ph, ph_s);
+    const double m = (double)__ldg(f.mode_m + k), n = (double)__ldg(f.mode_n + k);
+    const double om = __ldg(f.omega + k);
+    const double wt = reduce_2pi(om * t);
+    double sn, cs;
+    sincos_poly(fma(m, thr, fma(-n, zer, wt + __ldg(f.phase + k))), sn, cs);
+    // alpha_hat = -Phi_hat (iota m - n) / (omega (G + iota I))    (O3)
+    const double inv = 1.0 / (om * GI);
+    const double N = fma(p.io, m, -n);
+    const double ah = -ph * N * inv;
+    const double ah_s = -(ph_s * N + ph * p.ios * m) * inv + ph * N * inv * (GI_s / GI);
+    Phi = fma(ph, sn, Phi);
+    Phi_s = fma(ph_s, sn, Phi_s);
+    Phi_th = fma(m * ph, cs, Phi_th);
+    Phi_ze = fma(-n * ph, cs, Phi_ze);
+    al = fma(ah, sn, al);
+    al_s = fma(ah_s, sn, al_s);
+    al_th = fma(m * ah, cs, al_th);
+    al_ze = fma(-n * ah, cs, al_ze);
+    al_t = fma(om * ah, cs, al_t);
+  }
+  out[0] = Phi; out[1] = Phi_s * f.inv_psi0; out[2] = Phi_th; out[3] = Phi_ze;
+  out[4] = al; out[5] = al_s * f.inv_psi0; out[6] = al_th; out[7] = al_ze; out[8] = al_t;
+}
+
+// ---- O4: guiding-centre algebra, shared by both kernels --------------------------------------------------
+// fb = B, B_s, B_th, B_ze; pt = perturbation block (all zero for a static field); v = v_par in m/s.
+// Returns ds/dt, dtheta/dt, dzeta/dt, d(v_par)/dt.
+__device__ __forceinline__ void gc_algebra(double mass, double charge, double mu, double inv_psi0,
+                                           double v, const double fb[4], const Profiles& p,
+                                           const double pt[9], double dy[4]) {
+  const double B = fb[0], B_psi = fb[1] * inv_psi0, B_th = fb[2], B_ze = fb[3];
+  const double G = p.G, Gp = p.Gs * inv_psi0, I = p.I, Ip = p.Is * inv_psi0;
+  const double Phi_psi = pt[1], Phi_th = pt[2], Phi_ze = pt[3];
+  const double al = pt[4], al_psi = pt[5], al_th = pt[6], al_ze = pt[7], al_t = pt[8];
+  const double invB = 1.0 / B;
+  const double rho_c = mass * v * invB / charge + al;
+  const double Fq = (mass * v * v * invB + mu) / charge;
+  const double a = 1.0 + rho_c * Ip + al_psi * I;
+  const double b = p.io - rho_c * Gp - al_psi * G;
+  const double invD = 1.0 / (a * G + b * I);
+  const double C = al_th * G - al_ze * I;
+  const double h_psi = fma(Fq, B_psi, Phi_psi), h_th = fma(Fq, B_th, Phi_th), h_ze = fma(Fq, B_ze, Phi_ze);
+  const double vB = v * B;
+  const double Lam = a * B_ze + b * B_th + C * B_psi;
+  dy[0] = (I * h_ze - G * h_th + C * vB) * invD * inv_psi0;
+  dy[1] = (b * vB + G * h_psi) * invD;
+  dy[2] = (a * vB - I * h_psi) * invD;
+  const double mvdot = (-mu * B * Lam - charge * B * (a * Phi_ze + b * Phi_th + C * Phi_psi)
+                        + mass * v * invB * (B_psi * (I * Phi_ze - G * Phi_th) + Phi_psi * (G * B_th - I * B_ze)))
+                           * invD - charge * B * al_t;
+  dy[3] = mvdot / mass;
+}
+
+// y = (s, theta, zeta, u = v_par / v_ref); dy in the same scaled variables.
+__device__ inline void rhs_generic(const FieldDev& f, double mass, double charge, double mu, double v_ref,
+                                   double inv_v_ref, double t, const double y[4], double dy[4]) {
+  int i0;
+  double w[4], dw[4], fb[4], pt[9];
+  lagrange_weights(f.ns, y[0], i0, w, dw);
+  Profiles p;
+  interp4(f.G, 1, i0, w, dw, p.G, p.Gs);
+  interp4(f.I, 1, i0, w, dw, p.I, p.Is);
+  interp4(f.iota, 1, i0, w, dw, p.io, p.ios);
+  eval_B_generic(f, i0, w, dw, y[1], y[2], fb);
+  if (f.nk > 0) {
+    eval_pert_generic(f, i0, w, dw, p, y[1], y[2], t, pt);
+  } else {
+#pragma unroll
+    for (int i = 0; i < 9; ++i) pt[i] = 0.0;
+  }
+  gc_algebra(mass, charge, mu, f.inv_psi0, y[3] * v_ref, fb, p, pt, dy);
+  dy[3] *= inv_v_ref;
+}
+
+// ---- O8: Poincare records from the continuous extension of an accepted step ------------------------------
+// r1..r5 are the dense-output coefficients of components s, theta, zeta (index 0..2).
+struct Dense3 { double r1[3], r2[3], r3[3], r4[3], r5[3]; };
+
+__device__ __forceinline__ void dense_eval(const Dense3& d, int c, double tau, double& y, double& dy) {
+  const double sg = 1.0 - tau;
+  const double P4 = fma(sg, d.r5[c], d.r4[c]), dP4 = -d.r5[c];
+  const double P3 = fma(tau, P4, d.r3[c]), dP3 = fma(tau, dP4, P4);
+  const double P2 = fma(sg, P3, d.r2[c]), dP2 = fma(sg, dP3, -P3);
+  y = fma(tau, P2, d.r1[c]);
+  dy = fma(tau, dP2, P2);
+}
+
+// Called by ONE thread per particle-step.  zeta0/zeta1 are the step's end values of zeta.
+__device__ inline void poincare_emit(const Dense3& d, long long id, double t, double h, double zeta0,
+                                     double zeta1, double* buf, long long cap, unsigned long long* count) {
+  constexpr double kTwoPi = 6.283185307179586476925286766559;
+  const double k0 = floor(zeta0 / kTwoPi), k1 = floor(zeta1 / kTwoPi);
+  if (k0 == k1) return;
+  const double kstep = k1 > k0 ? 1.0 : -1.0;
+  const double kfirst = k1 > k0 ? k0 + 1.0 : k0;
+  const double klast = k1 > k0 ? k1 : k1 + 1.0;
+  for (double kp = kfirst; kstep > 0 ? kp <= klast : kp >= klast; kp += kstep) {
+    const double target = kTwoPi * kp;
+    double lo = 0.0, hi = 1.0, glo = zeta0 - target, yv, dv;
+    for (int it = 0; it < 8; ++it) {
+      const double mid = 0.5 * (lo + hi);
+      dense_eval(d, 2, mid, yv, dv);
+      const double g = yv - target;
+      if ((g < 0.0) == (glo < 0.0) && g != 0.0) { lo = mid; glo = g; } else { hi = mid; }
+    }
+    double tau = 0.5 * (lo + hi);
+    const double tol = 1e-12 * fmax(1.0, fabs(target));
+    for (int it = 0; it < 20; ++it) {
+      dense_eval(d, 2, tau, yv, dv);
+      const double g = yv - target;
+      if (fabs(g) < tol || dv == 0.0) break;
+      tau = fmin(fmax(tau - g / dv, lo), hi);
+    }
+    const unsigned long long slot = atomicAdd(count, 1ULL);
+    if ((long long)slot < cap) {
+      double sv, thv;
+      dense_eval(d, 0, tau, sv, dv);
+      dense_eval(d, 1, tau, thv, dv);
+      double thm = fmod(thv, kTwoPi);
+      if (thm < 0.0) thm += kTwoPi;
+      double* r = buf + slot * 4;
+      r[0] = (double)id; r[1] = fma(tau, h, t); r[2] = sv; r[3] = thm;
+    }
+  }
+}
+
+// ---- generic trace: one thread per particle ----------------------------------------------------------------
+__global__ void __launch_bounds__(128) trace_generic_kernel(FieldDev f, TraceDev p) {
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < p.n;
+       i += (long long)gridDim.x * blockDim.x) {
+    const double mu = p.mu[i];
+    double y[4] = {p.s0[i], p.th0[i], p.ze0[i], p.vpar0[i] * p.inv_v_ref};
+    double t = p.t0;
+    double h = (p.h_inout && p.h_inout[i] > 0.0) ? p.h_inout[i] : p.h0;
+    if (h < p.h_min) h = p.h_min;
+    double k[7][4], yn[4], ys[4];
+    long long attempts = 0;
+    int n_acc = 0, n_rej = 0, n_forced = 0, st = -1;
+    bool prev_rejected = false;
+    rhs_generic(f, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, t, y, k[0]);
+    if (!finite4(y[0], y[1], y[2], y[3]) || !finite4(k[0][0], k[0][1], k[0][2], k[0][3])) st = GC_ST_NONFINITE_;
+    else if (!(t < p.t_max)) st = 0;
+    while (st < 0) {
+      double h_try = h;
+      bool clipped = false;
+      if (t + h_try >= p.t_max) { h_try = p.t_max - t; clipped = true; }
+      if (!(t + h_try > t)) { st = GC_ST_NONFINITE_; break; }
+      const bool forced = prev_rejected && p.h_min > 0.0 && h == p.h_min;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) ys[c] = fma(h_try * dp::a21, k[0][c], y[c]);
+      rhs_generic(f, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, fma(dp::c2, h_try, t), ys, k[1]);
+#pragma unroll
+      for (int c = 0; c < 4; ++c) ys[c] = fma(h_try, fma(dp::a32, k[1][c], dp::a31 * k[0][c]), y[c]);
+      rhs_generic(f, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, fma(dp::c3, h_try, t), ys, k[2]);
+#pragma unroll
+      for (int c = 0; c < 4; ++c)
+        ys[c] = fma(h_try, fma(dp::a43, k[2][c], fma(dp::a42, k[1][c], dp::a41 * k[0][c])), y[c]);
+      rhs_generic(f, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, fma(dp::c4, h_try, t), ys, k[3]);
+#pragma unroll
+      for (int c = 0; c < 4; ++c)
+        ys[c] = fma(h_try, fma(dp::a54, k[3][c], fma(dp::a53, k[2][c], fma(dp::a52, k[1][c], dp::a51 * k[0][c]))),
+                    y[c]);
+      rhs_generic(f, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, fma(dp::c5, h_try, t), ys, k[4]);
+#pragma unroll
+      for (int c = 0; c < 4; ++c)
+        ys[c] = fma(h_try, fma(dp::a65, k[4][c], fma(dp::a64, k[3][c], fma(dp::a63, k[2][c],
+                    fma(dp::a62, k[1][c], dp::a61 * k[0][c])))), y[c]);
+      rhs_generic(f, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, t + h_try, ys, k[5]);
+#pragma unroll
+      for (int c = 0; c < 4; ++c)
+        yn[c] = fma(h_try, fma(dp::a76, k[5][c], fma(dp::a75, k[4][c], fma(dp::a74, k[3][c],
+                    fma(dp::a73, k[2][c], dp::a71 * k[0][c])))), y[c]);
+      rhs_generic(f, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, t + h_try, yn, k[6]);
+      ++attempts;
+      double acc = 0.0;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const double delta = h_try * fma(dp::e7, k[6][c], fma(dp::e6, k[5][c], fma(dp::e5, k[4][c],
+                                 fma(dp::e4, k[3][c], fma(dp::e3, k[2][c], dp::e1 * k[0][c])))));
+        const double sk = fma(p.rtol, fmax(fabs(y[c]), fabs(yn[c])), p.atol);
+        const double r = delta / sk;
+        acc = fma(r, r, acc);
+      }
+      const double err = sqrt(acc * 0.25);
+      const bool finite = finite4(yn[0], yn[1], yn[2], yn[3]) &&
+                          finite4(k[6][0], k[6][1], k[6][2], k[6][3]) && isfinite(err);
+      bool accept;
+      if (forced) {
+        if (!finite) { st = GC_ST_NONFINITE_; break; }
+        accept = true;
+      } else {
+        accept = finite && err <= 1.0;
+      }
+      if (accept) {
+        const double sc = scale_after_accept(err);
+        const double h_next = prev_rejected ? h_try * fmin(sc, 1.0) : h_try * sc;
+        if (p.poincare_capacity > 0 && floor(y[2] / 6.283185307179586476925286766559) !=
+                                           floor(yn[2] / 6.283185307179586476925286766559)) {
+          Dense3 d;
+#pragma unroll
+          for (int c = 0; c < 3; ++c) {
+            d.r1[c] = y[c];
+            d.r2[c] = yn[c] - y[c];
+            d.r3[c] = h_try * k[0][c] - d.r2[c];
+            d.r4[c] = d.r2[c] - h_try * k[6][c] - d.r3[c];
+            d.r5[c] = h_try * fma(dp::d7, k[6][c], fma(dp::d6, k[5][c], fma(dp::d5, k[4][c],
+                                  fma(dp::d4, k[3][c], fma(dp::d3, k[2][c], dp::d1 * k[0][c])))));
+          }
+          poincare_emit(d, i, t, h_try, y[2], yn[2], p.poincare, p.poincare_capacity, p.poincare_count);
+        }
+        t = clipped ? p.t_max : t + h_try;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) { y[c] = yn[c]; k[0][c] = k[6][c]; }
+        ++n_acc;
+        if (forced) ++n_forced;
+        prev_rejected = false;
+        if (!clipped) h = h_next;
+        if (h < p.h_min) h = p.h_min;
+        if (y[0] >= p.s_loss) st = 1;
+        else if (y[0] <= p.s_min) st = 2;
+        else if (clipped) st = 0;
+        else if (attempts >= p.max_steps) st = 3;
+      } else {
+        ++n_rej;
+        h = h_try * scale_after_reject(err);
+        if (h < p.h_min) h = p.h_min;
+        prev_rejected = true;
+        if (attempts >= p.max_steps) st = 3;
+      }
+    }
+    p.y_out[0 * p.n + i] = y[0];
+    p.y_out[1 * p.n + i] = y[1];
+    p.y_out[2 * p.n + i] = y[2];
+    p.y_out[3 * p.n + i] = y[3] * p.v_ref;
+    p.t_out[i] = t;
+    p.status[i] = st;
+    if (p.h_inout) p.h_inout[i] = h;
+    if (p.n_acc) p.n_acc[i] = n_acc;
+    if (p.n_rej) p.n_rej[i] = n_rej;
+    if (p.n_forced) p.n_forced[i] = n_forced;
+  }
+}
+
+__global__ void field_eval_kernel(FieldDev f, long long n, const double* s, const double* th, const double* ze,
+                                  double* B, double* dB) {
+  const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int i0;
+  double w[4], dw[4], out[4];
+  lagrange_weights(f.ns, s[i], i0, w, dw);
+  eval_B_generic(f, i0, w, dw, th[i], ze[i], out);
+  B[i] = out[0];
+  if (dB) { dB[i] = out[1]; dB[n + i] = out[2]; dB[2 * n + i] = out[3]; }
+}
+
+__global__ void pert_eval_kernel(FieldDev f, long long n, const double* s, const double* th, const double* ze,
+                                 double t, double* out) {
+  const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int i0;
+  double w[4], dw[4], pt[9];
+  lagrange_weights(f.ns, s[i], i0, w, dw);
+  Profiles p;
+  interp4(f.G, 1, i0, w, dw, p.G, p.Gs);
+  interp4(f.I, 1, i0, w, dw, p.I, p.Is);
+  interp4(f.iota, 1, i0, w, dw, p.io, p.ios);
+  if (f.nk > 0) {
+    eval_pert_generic(f, i0, w, dw, p, th[i], ze[i], t, pt);
+  } else {
+    for (int j = 0; j < 9; ++j) pt[j] = 0.0;
+  }
+  for (int j = 0; j < 9; ++j) out[j * n + i] = pt[j];
+}
+
+__global__ void rhs_eval_generic_kernel(FieldDev f, double mass, double charge, double t, long long n,
+                                        const double* y, const double* mu, double* dydt) {
+  const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double yy[4] = {y[i], y[n + i], y[2 * n + i], y[3 * n + i]};
+  double dy[4];
+  rhs_generic(f, mass, charge, mu[i], 1.0, 1.0, t, yy, dy);
+  for (int c = 0; c < 4; ++c) dydt[c * n + i] = dy[c];
+}
+
+}  // namespace gc

@@ -1,0 +1,355 @@
+"""bench.py -- guiding-centre particle-steps/s (FP64) on B200, with roofline, end-to-end and CPU-oracle legs.
+
+    python bench.py --gpus N --steps K --warmup W            # this repo's CUDA path (one rank per GPU)
+    python bench.py --impl reference --gpus N --steps K --warmup W   # the CPU oracle, as it stands
+
+Workload: BASELINE.json configs[1] -- 100,000 alpha particles per GPU, static field with 545 harmonics on
+101 radial nodes, rtol = atol = 1e-9, h_min = 1e-12.  One "step" advances the whole
+ensemble by one segment of simulated time (default 2e-5 s, about 10^3 Dormand-Prince attempts per
+particle) with ONE gc_trace call that continues the previous step in place (GC_TRACE_RESUME), so K steps
+are the first (W + K) * segment seconds of the config-1 trace; lost particles drop out as they do there.
+A particle-step is one ATTEMPTED Dormand-Prince step (6 right-hand sides), accepted or rejected.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "guiding-center particle-steps/s (FP64)"
+UNIT = "particle-steps/s"
+# FP64 ALU peak used as the roofline denominator: 148 SMs x 64 FP64 lanes x 2 flop
+# x 1.965 GHz (clocks.max.sm in MEASURED_PEAKS.json) = 37.2 TFLOP/s; gc_fp64_peak_probe measures the
+# sustained DFMA rate of the same box in the same run and is reported beside it.
+FP64_LANES_PER_SM = 64
+
+
+def flops_per_step(nh: int, M: int, nk: int, n_omega: int) -> float:
+    """F_RHS = 28 nh + 18 (M + 1) + 350 (+ 75 K + 40 n_omega); F_step = 6 F_RHS + 250."""
+    f_rhs = 28.0 * nh + 18.0 * (M + 1) + 350.0 + 75.0 * nk + 40.0 * n_omega
+    return 6.0 * f_rhs + 250.0
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1)")
+    ap.add_argument("--particles", type=int, default=None, help="particles per GPU (default: the config's, "
+                    "capped at 100000 per step for configs 3-4 unless given)")
+    ap.add_argument("--segment", type=float, default=2e-5, help="simulated seconds per step")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "warp", "generic"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
+
+    def stop(self, t_start: float, t_end: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        rows = [r for (ts, r) in self.rows if t_start <= ts <= t_end + 0.2 and len(r) >= 7] or \
+               [r for (_, r) in self.rows if len(r) >= 7]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        num = lambda x: float(x) if x.replace(".", "", 1).isdigit() else float("nan")
+        sm = sorted(num(r[0]) for r in rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [nm for j, nm in enumerate(names) if any(r[3 + j].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": num(rows[0][1]),
+                "power_w_max": max(num(r[2]) for r in rows), "samples": len(rows), "reasons": reasons}
+
+
+def workload(args, rank: int):
+    from paper_2605_16734_b200 import workloads as W
+    cfg = args.config
+    fld, spec = W.make_field(cfg), W.make_spec(cfg)
+    full = {0: 512, 1: 100_000, 2: 100_000, 3: 1_000_000, 4: 1_000_000}[cfg]
+    n = args.particles if args.particles else full
+    P = W.make_particles(cfg, n, stream=rank)
+    M = int(fld.xm.max())
+    n_omega = len(set(np.asarray(fld.mode_omega).tolist()))
+    info = {"workload": f"BASELINE.json configs[{cfg}]: {n} alphas per GPU, nh={fld.nh}, ns={fld.ns}, "
+                        f"nk={fld.nk}, rtol={spec.rtol:g}, h_min={spec.h_min:g}; one step = one gc_trace call "
+                        f"advancing the ensemble by {args.segment:g} s of simulated time (GC_TRACE_RESUME)",
+            "particles_per_gpu": n, "segment_s": args.segment, "nh": fld.nh, "ns": fld.ns, "nk": fld.nk,
+            "rtol": spec.rtol,
+            "flop_per_particle_step": flops_per_step(fld.nh, M, fld.nk, n_omega)}
+    return fld, spec, P, info
+
+
+# ---- the CPU oracle legs -------------------------------------------------------------------------------------
+def oracle_sample(fld, spec, P, seg: float, target_s: float):
+    """Time the oracle, as it stands, on a bounded sample: the first n_s particles of the ensemble traced
+    over [0, seg].  A pilot on 2 particles per thread sizes n_s for about target_s of wall time."""
+    import oracle
+    from paper_2605_16734_b200 import workloads as W
+    OF = oracle.OracleField(fld)
+    cores = oracle.num_threads()
+
+    def run(k):
+        Q = P.head(k)
+        B = OF.eval_B_many(Q.s, Q.theta, Q.zeta)[:, 0]
+        mu = W.mu_from(Q, B)
+        t0 = time.perf_counter()
+        r = OF.trace(spec, Q.s, Q.theta, Q.zeta, Q.vpar, mu, t0=0.0, t_max=seg)
+        dt = time.perf_counter() - t0
+        return int(r.n_acc.sum() + r.n_rej.sum()), dt
+
+    k0 = min(P.n, 2 * cores)
+    a0, d0 = run(k0)
+    rate = a0 / max(d0, 1e-9)
+    per_particle = a0 / k0
+    k = int(min(P.n, max(k0, target_s * rate / max(per_particle, 1.0))))
+    k = max(cores, (k // cores) * cores)
+    a, d = run(k)
+    return {"value": a / d, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {k} particles of the ensemble over [0, {seg:g}] s: {a} attempted steps in {d:.2f} s "
+                      f"(oracle/gc_oracle.c, gcc -O2 -fopenmp, {cores} threads)"}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores; each step = one segment over a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    from paper_2605_16734_b200 import workloads as W
+    fld, spec, P, info = workload(args, 0)
+    OF = oracle.OracleField(fld)
+    cores = oracle.num_threads()
+    seg = args.segment
+    # pilot: size the sample so that one step takes about cpu_seconds / (steps + warmup), at least one
+    # particle per thread
+    Q = P.head(min(P.n, 2 * cores))
+    mu = W.mu_from(Q, OF.eval_B_many(Q.s, Q.theta, Q.zeta)[:, 0])
+    t0 = time.perf_counter()
+    r = OF.trace(spec, Q.s, Q.theta, Q.zeta, Q.vpar, mu, t0=0.0, t_max=seg)
+    d0 = time.perf_counter() - t0
+    per_step_budget = max(1.0, 4.0 * args.cpu_seconds / (args.steps + args.warmup))
+    k = int(min(P.n, max(cores, Q.n * per_step_budget / max(d0, 1e-9))))
+    k = min(P.n, max(cores, (k // cores) * cores))
+    Q = P.head(k)
+    mu = W.mu_from(Q, OF.eval_B_many(Q.s, Q.theta, Q.zeta)[:, 0])
+    y = np.stack([Q.s, Q.theta, Q.zeta, Q.vpar])
+    h = np.zeros(k)
+    alive = np.arange(k)
+    attempts, elapsed = 0, 0.0
+    for step in range(args.warmup + args.steps):
+        t_a, t_b = step * seg, (step + 1) * seg
+        t0 = time.perf_counter()
+        r = OF.trace(spec, y[0, alive], y[1, alive], y[2, alive], y[3, alive], mu[alive], h_in=h[alive],
+                     t0=t_a, t_max=t_b)
+        dt = time.perf_counter() - t0
+        y[:, alive] = r.y
+        h[alive] = r.h
+        if step >= args.warmup:
+            attempts += int(r.n_acc.sum() + r.n_rej.sum())
+            elapsed += dt
+        alive = alive[r.status == 0]
+    value = attempts / elapsed
+    sample = (f"first {k} particles of the ensemble, {args.steps} segments of {seg:g} s after {args.warmup} "
+              f"warm-up segments: {attempts} attempted steps in {elapsed:.2f} s")
+    info["particles_per_gpu"] = k
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * elapsed / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": info,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# ---- the CUDA arm ---------------------------------------------------------------------------------------------
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2605_16734_b200 import build as B, ensemble as E, gcorbit as G, workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA arm has no CPU fallback (use --impl reference)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    if rank == 0:
+        B.build()
+    if world > 1:
+        dist.barrier()
+
+    fld, spec, P, info = workload(args, rank)
+    n, seg, K, Wu = P.n, args.segment, args.steps, args.warmup
+    GF = G.Field(fld)
+    if args.kernel != "auto":
+        GF.set_kernel({"warp": G.GC_KERNEL_WARP, "generic": G.GC_KERNEL_GENERIC}[args.kernel])
+    kinfo = GF.kernel_info()
+    T = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device=dev)
+    s, th, ze, vpar = T(P.s), T(P.theta), T(P.zeta), T(P.vpar)
+    Bst, _ = GF.field_eval(s, th, ze, derivs=False)          # mu = m v_perp^2 / (2 B) needs B at the start (A5)
+    mu = T(0.5 * spec.mass * P.vperp2()) / Bst
+    h = torch.zeros(n, dtype=torch.float64, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)          # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def attempts_of(st):
+        return int((st.n_acc.sum(dtype=torch.int64) + st.n_rej.sum(dtype=torch.int64)).item())
+
+    # warm-up: the first W segments of the trace
+    state = GF.trace(spec, s, th, ze, vpar, mu, h_inout=h, t0=0.0, t_max=seg)
+    for w in range(1, max(Wu, 1)):
+        GF.trace_resume(spec, state, mu, t0=w * seg, t_max=(w + 1) * seg)
+    torch.cuda.synchronize()
+    first = max(Wu, 1)
+    a_before = attempts_of(state)
+    alive_before = int((state.status == 0).sum().item())
+
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local) if rank == 0 else None
+    t_wall0 = time.time()
+    for k in range(K):
+        flush.fill_(k & 0xFF)                                  # L2 flush between timed iterations (not timed)
+        ev[k][0].record(stream)
+        GF.trace_resume(spec, state, mu, t0=(first + k) * seg, t_max=(first + k + 1) * seg)
+        ev[k][1].record(stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t_wall1 = time.time()
+    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    kernel_ms = float(sum(step_ms))
+    attempts = attempts_of(state) - a_before
+    alive_after = int((state.status == 0).sum().item())
+    ms_max, attempts_all = E.reduce_timing(kernel_ms, attempts, dev)
+    value = attempts_all / (ms_max * 1e-3)
+
+    # ---- e2e: the same segments through gc_trace_host, pinned host buffers, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        Ke = min(K, 3)
+        pin = lambda t: t.detach().cpu().pin_memory()
+        hy, ht, hs, hh, hmu = pin(state.y), pin(state.t), pin(state.status), pin(state.h), pin(mu)
+        hna, hnr, hnf = pin(state.n_acc), pin(state.n_rej), pin(state.n_forced)
+        bufs = G.TraceResult(hy.numpy(), ht.numpy(), hs.numpy(), hna.numpy(), hnr.numpy(), hnf.numpy(), hh.numpy())
+        yv = bufs.y
+        a0 = int(bufs.n_acc.sum(dtype=np.int64) + bufs.n_rej.sum(dtype=np.int64))
+        if world > 1:
+            dist.barrier()
+        t0 = time.perf_counter()
+        for k in range(Ke):
+            GF.trace_host(spec, yv[0], yv[1], yv[2], yv[3], hmu.numpy(), t0=(first + K + k) * seg,
+                          t_max=(first + K + k + 1) * seg, bufs=bufs, flags=G.GC_TRACE_RESUME)
+        dt_ms = (time.perf_counter() - t0) * 1e3
+        a1 = int(bufs.n_acc.sum(dtype=np.int64) + bufs.n_rej.sum(dtype=np.int64))
+        ms_e, att_e = E.reduce_timing(dt_ms, a1 - a0, dev)
+        # bytes gc_trace_host copies per call under GC_TRACE_RESUME (gcorbit_api.cu): inputs 5 x 8n, h 8n,
+        # y 32n, t 8n, status 4n, counters 12n in; y 32n, t 8n, status 4n, h 8n, counters 12n out
+        e2e = {"value": att_e / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 104 * n,
+               "d2h_bytes_per_step": 64 * n, "steps": Ke, "ms_per_step": ms_e / Ke,
+               "api": "gc_trace_host (pinned host buffers; device scratch allocated inside the call)"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peak_nominal = 148 * FP64_LANES_PER_SM * 2 * 1.965e9 / 1e12
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            mp = json.load(fh)
+        peak_nominal = torch.cuda.get_device_properties(dev).multi_processor_count * FP64_LANES_PER_SM * 2 * \
+            float(mp["sm_max_mhz"]) * 1e6 / 1e12
+    except Exception:
+        pass
+    probe_flops, _ = G.fp64_peak_probe()
+    fstep = info["flop_per_particle_step"]
+    achieved = attempts * fstep / (kernel_ms * 1e-3) / 1e12         # this rank's kernel, TFLOP/s
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        try:
+            with open(tp) as fh:
+                traffic = json.load(fh).get(f"config{args.config}_dram_bytes_per_launch")
+        except Exception:
+            traffic = None
+    roofline = {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
+                "frac": achieved / peak_nominal, "traffic": traffic,
+                "kernel": f"trace_{kinfo['kernel']}_kernel", "launch_ms_avg": kernel_ms / K,
+                "peak_source": "148 SMs x 64 FP64 lanes x 2 flop x clocks.max.sm (DESIGN.md section 6)",
+                "peak_probe_tflops": probe_flops / 1e12,
+                "frac_of_probe": achieved / (probe_flops / 1e12),
+                "flop_per_particle_step": fstep,
+                "particle_steps_per_launch": attempts / K}
+    cpu = None
+    if not args.no_cpu_baseline:
+        cpu = oracle_sample(fld, spec, P, seg, args.cpu_seconds)
+    info.update({"kernel": kinfo, "l2": "flushed between timed steps (256 MiB write, outside each step's event pair)",
+                 "alive_before": alive_before, "alive_after": alive_after,
+                 "simulated_window_s": [first * seg, (first + K) * seg]})
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wu,
+           "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic", "config": info,
+           "rhs_evals_per_s": 6.0 * value, "accepted_fraction": None,
+           "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": K, "clocks": clocks,
+           "wall_s_timed_region": t_wall1 - t_wall0}
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

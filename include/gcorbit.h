@@ -66,7 +66,15 @@ typedef struct {
   double s_loss, s_min;       /* stop when s >= s_loss (lost) or s <= s_min (axis)              */
   int64_t max_steps;          /* attempted steps per particle before status 3                   */
   int64_t poincare_capacity;  /* records available in `poincare`; 0 disables recording (O8)     */
+  int64_t flags;              /* GC_TRACE_* bits, 0 = none                                      */
 } gc_trace_params;
+
+/* gc_trace_params.flags.  GC_TRACE_RESUME: `status` is read on entry and only particles whose status is
+ * GC_ST_TMAX (0) are traced, from (s0, th0, ze0, vpar0) at t0; every output of the others is left as it
+ * is, and n_acc, n_rej, n_forced are added to instead of overwritten (max_steps stays per call).  Together with h_inout, and with s0..vpar0 aliasing the rows of y_out (allowed: a particle is read
+ * once before anything of it is written), a long horizon runs as consecutive calls on the same buffers,
+ * each continuing where the last one stopped (checkpoint / resume). */
+enum { GC_TRACE_RESUME = 1 };
 
 /* Per-particle exit status written by gc_trace. */
 enum { GC_ST_TMAX = 0, GC_ST_LOST = 1, GC_ST_AXIS = 2, GC_ST_MAXSTEPS = 3, GC_ST_NONFINITE = 4 };
@@ -98,7 +106,8 @@ int gc_rhs_eval(const gc_field* f, double mass, double charge, double t, int64_t
 
 /* O5-O8: trace n independent particles.  ALL ARRAY POINTERS ARE DEVICE MEMORY owned by the caller and
  * must stay valid until `stream` is synchronised; the call is asynchronous on `stream`.
- *   in : s0, th0, ze0, vpar0 (m/s), mu (J/T)         [n] each, never modified
+ *   in : s0, th0, ze0, vpar0 (m/s), mu (J/T)         [n] each, never modified unless they alias y_out
+ *        (s0 = y_out, th0 = y_out + n, ze0 = y_out + 2n, vpar0 = y_out + 3n is allowed)
  *   io : h_inout [n] or NULL: first trial step if > 0 (else params->h0); next proposal on return
  *   out: y_out [4][n] = s, theta, zeta, v_par (m/s);  t_out [n] end time (loss time when status == 1);
  *        status [n] (GC_ST_*);  n_acc, n_rej, n_forced [n] each or NULL (attempt counters);
@@ -113,8 +122,10 @@ int gc_trace(const gc_field* f, const gc_trace_params* params, int64_t n,
              int32_t* n_acc, int32_t* n_rej, int32_t* n_forced,
              double* poincare, int64_t* poincare_count, void* stream);
 
-/* The same trace with HOST buffers: allocates device scratch, copies the inputs in, runs gc_trace,
- * copies every non-NULL output back and synchronises.  `poincare_count` is a host int64 here. */
+/* The same trace with HOST buffers: allocates device scratch, copies the inputs in (with GC_TRACE_RESUME
+ * also y_out, t_out, status and the counters, so that untouched particles keep their values), runs
+ * gc_trace, copies every non-NULL output back and synchronises.  `poincare_count` is a host int64 here.
+ * Pinned host buffers make the copies asynchronous; pageable ones work too. */
 int gc_trace_host(const gc_field* f, const gc_trace_params* params, int64_t n,
                   const double* s0, const double* th0, const double* ze0, const double* vpar0,
                   const double* mu, double* h_inout,

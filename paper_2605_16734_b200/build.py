@@ -19,12 +19,24 @@ def nvcc_cmd(extra=()):
             *[os.path.join(CSRC, s) for s in SOURCES], "-o", SO]
 
 
+STAMP = SO + ".srchash"
+
+
+def source_hash() -> str:
+    """Content hash of everything the library is built from (mtimes do not survive a repo snapshot)."""
+    import hashlib
+    h = hashlib.sha256()
+    for d in [os.path.join(CSRC, s) for s in SOURCES + HEADERS] + [os.path.abspath(__file__)]:
+        with open(d, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()
+
+
 def needs_build() -> bool:
-    if not os.path.exists(SO):
+    if not os.path.exists(SO) or not os.path.exists(STAMP):
         return True
-    t = os.path.getmtime(SO)
-    deps = [os.path.join(CSRC, s) for s in SOURCES + HEADERS] + [os.path.abspath(__file__)]
-    return any(os.path.getmtime(d) > t for d in deps)
+    with open(STAMP) as fh:
+        return fh.read().strip() != source_hash()
 
 
 def build(force: bool = False, verbose: bool = False, extra=()) -> str:
@@ -36,6 +48,8 @@ def build(force: bool = False, verbose: bool = False, extra=()) -> str:
             raise RuntimeError("nvcc failed building libgcorbit.so")
         with open(os.path.join(_HERE, "build_ptxas.log"), "w") as fh:
             fh.write(" ".join(nvcc_cmd(extra)) + "\n" + r.stdout + r.stderr)
+        with open(STAMP, "w") as fh:
+            fh.write(source_hash())
     return SO
 
 

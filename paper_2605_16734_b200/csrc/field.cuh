@@ -32,6 +32,7 @@ struct TraceDev {
   double mass, charge, t0, t_max, rtol, atol, v_ref, inv_v_ref, h0, h_min, s_loss, s_min;
   long long max_steps, poincare_capacity;
   long long n;
+  int resume;                         // GC_TRACE_RESUME: skip particles whose status is not 0 on entry
   const double *s0, *th0, *ze0, *vpar0, *mu;
   double* h_inout;
   double *y_out, *t_out;

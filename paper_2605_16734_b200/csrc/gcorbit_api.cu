@@ -170,12 +170,13 @@ int build_trace_dev(const gc_field* f, const gc_trace_params* p, int64_t n, gc::
   if (n < 0) return fail(GC_EINVAL, "gc_trace: n < 0");
   if (!(p->v_ref > 0.0) || !(p->h0 > 0.0) || !(p->h_min >= 0.0) || !(p->mass > 0.0) || p->charge == 0.0 ||
       !(p->rtol >= 0.0) || !(p->atol >= 0.0) || !(p->rtol + p->atol > 0.0) || p->max_steps < 1 ||
-      p->poincare_capacity < 0 || !std::isfinite(p->t0) || !std::isfinite(p->t_max))
+      p->poincare_capacity < 0 || (p->flags & ~(int64_t)GC_TRACE_RESUME) != 0 || !std::isfinite(p->t0) || !std::isfinite(p->t_max))
     return fail(GC_EINVAL, "gc_trace: invalid integrator specification");
   t->mass = p->mass; t->charge = p->charge; t->t0 = p->t0; t->t_max = p->t_max;
   t->rtol = p->rtol; t->atol = p->atol; t->v_ref = p->v_ref; t->inv_v_ref = 1.0 / p->v_ref;
   t->h0 = p->h0; t->h_min = p->h_min; t->s_loss = p->s_loss; t->s_min = p->s_min;
   t->max_steps = p->max_steps; t->poincare_capacity = p->poincare_capacity; t->n = n;
+  t->resume = (p->flags & GC_TRACE_RESUME) ? 1 : 0;
   return GC_OK;
 }
 
@@ -438,6 +439,14 @@ int gc_trace_host(const gc_field* f, const gc_trace_params* params, int64_t n, c
   GC_H(cudaMemcpyAsync(d_v, vpar0, bytes, cudaMemcpyHostToDevice, st));
   GC_H(cudaMemcpyAsync(d_mu, mu, bytes, cudaMemcpyHostToDevice, st));
   if (h_inout) GC_H(cudaMemcpyAsync(d_h, h_inout, bytes, cudaMemcpyHostToDevice, st));
+  if (params->flags & GC_TRACE_RESUME) {
+    GC_H(cudaMemcpyAsync(d_y, y_out, 4 * bytes, cudaMemcpyHostToDevice, st));
+    GC_H(cudaMemcpyAsync(d_t, t_out, bytes, cudaMemcpyHostToDevice, st));
+    GC_H(cudaMemcpyAsync(i32, status, nd * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    if (n_acc) GC_H(cudaMemcpyAsync(i32 + nd, n_acc, nd * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    if (n_rej) GC_H(cudaMemcpyAsync(i32 + 2 * nd, n_rej, nd * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    if (n_forced) GC_H(cudaMemcpyAsync(i32 + 3 * nd, n_forced, nd * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  }
   rc = gc_trace(f, params, n, d_s, d_th, d_ze, d_v, d_mu, h_inout ? d_h : nullptr, d_y, d_t, i32,
                 n_acc ? i32 + nd : nullptr, n_rej ? i32 + 2 * nd : nullptr, n_forced ? i32 + 3 * nd : nullptr,
                 cap > 0 ? d_pc : nullptr, cap > 0 ? d_cnt : nullptr, st);

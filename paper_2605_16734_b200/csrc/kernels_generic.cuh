@@ -177,6 +177,7 @@ __device__ inline void poincare_emit(const Dense3& d, long long id, double t, do
 __global__ void __launch_bounds__(128) trace_generic_kernel(FieldDev f, TraceDev p) {
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < p.n;
        i += (long long)gridDim.x * blockDim.x) {
+    if (p.resume && p.status[i] != 0) continue;            // finished in an earlier segment
     const double mu = p.mu[i];
     double y[4] = {p.s0[i], p.th0[i], p.ze0[i], p.vpar0[i] * p.inv_v_ref};
     double t = p.t0;
@@ -284,9 +285,9 @@ __global__ void __launch_bounds__(128) trace_generic_kernel(FieldDev f, TraceDev
     p.t_out[i] = t;
     p.status[i] = st;
     if (p.h_inout) p.h_inout[i] = h;
-    if (p.n_acc) p.n_acc[i] = n_acc;
-    if (p.n_rej) p.n_rej[i] = n_rej;
-    if (p.n_forced) p.n_forced[i] = n_forced;
+    if (p.n_acc) p.n_acc[i] = (p.resume ? p.n_acc[i] : 0) + n_acc;
+    if (p.n_rej) p.n_rej[i] = (p.resume ? p.n_rej[i] : 0) + n_rej;
+    if (p.n_forced) p.n_forced[i] = (p.resume ? p.n_forced[i] : 0) + n_forced;
   }
 }
 

@@ -335,6 +335,7 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, 1) trace_warp_kernel(Fiel
     idx = __shfl_sync(kFull, idx, 0);
     if ((long long)idx >= p.n) break;
     const long long i = (long long)idx;
+    if (p.resume && p.status[i] != 0) continue;            // finished in an earlier segment
     rhs.cur_i0 = -1000;                                    // forces a full window load
 
     const double mu = p.mu[i];
@@ -476,9 +477,10 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, 1) trace_warp_kernel(Fiel
       p.t_out[i] = t;
       p.status[i] = st;
       if (p.h_inout) p.h_inout[i] = h;
-      if (p.n_acc) p.n_acc[i] = n_acc;
-      if (p.n_rej) p.n_rej[i] = n_rej;
-      if (p.n_forced) p.n_forced[i] = n_forced;
+      // counters restart at 0 per call, except under GC_TRACE_RESUME where they add to what is there
+      if (p.n_acc) p.n_acc[i] = (p.resume ? p.n_acc[i] : 0) + n_acc;
+      if (p.n_rej) p.n_rej[i] = (p.resume ? p.n_rej[i] : 0) + n_rej;
+      if (p.n_forced) p.n_forced[i] = (p.resume ? p.n_forced[i] : 0) + n_forced;
     }
   }
 }

@@ -42,7 +42,7 @@ class gc_trace_params(C.Structure):
     _fields_ = [("mass", C.c_double), ("charge", C.c_double), ("t0", C.c_double), ("t_max", C.c_double),
                 ("rtol", C.c_double), ("atol", C.c_double), ("v_ref", C.c_double),
                 ("h0", C.c_double), ("h_min", C.c_double), ("s_loss", C.c_double), ("s_min", C.c_double),
-                ("max_steps", C.c_int64), ("poincare_capacity", C.c_int64)]
+                ("max_steps", C.c_int64), ("poincare_capacity", C.c_int64), ("flags", C.c_int64)]
 
 
 _lib = None
@@ -99,11 +99,14 @@ def _stream_ptr(torch):
     return C.c_void_p(torch.cuda.current_stream().cuda_stream)
 
 
-def make_params(spec, t0=None, t_max=None, poincare_capacity=0) -> gc_trace_params:
+GC_TRACE_RESUME = 1
+
+
+def make_params(spec, t0=None, t_max=None, poincare_capacity=0, flags=0) -> gc_trace_params:
     return gc_trace_params(spec.mass, spec.charge, spec.t0 if t0 is None else t0,
                            spec.t_max if t_max is None else t_max, spec.rtol, spec.atol, spec.v_ref,
                            spec.h0, spec.h_min, spec.s_loss, spec.s_min, int(spec.max_steps),
-                           int(poincare_capacity))
+                           int(poincare_capacity), int(flags))
 
 
 @dataclass
@@ -193,7 +196,7 @@ class Field:
 
     # ---- gc_trace (device tensors) ---------------------------------------------------------------------------
     def trace(self, spec, s0, th0, ze0, vpar0, mu, h_inout=None, poincare_capacity=0, t0=None, t_max=None,
-              counters=True, out=None) -> TraceResult:
+              counters=True, out=None, flags=0) -> TraceResult:
         """Asynchronous on torch's current stream.  ``out`` may carry a previous TraceResult whose buffers are
         reused (no allocation inside a timed region)."""
         torch = _torch()
@@ -201,7 +204,7 @@ class Field:
         dev = s0.device
         for x in (s0, th0, ze0, vpar0, mu):
             assert x.dtype == torch.float64 and x.is_cuda and x.is_contiguous() and x.numel() == n
-        p = make_params(spec, t0, t_max, poincare_capacity)
+        p = make_params(spec, t0, t_max, poincare_capacity, flags)
         if out is None:
             i32 = lambda: torch.empty(n, dtype=torch.int32, device=dev)
             out = TraceResult(torch.empty((4, n), dtype=torch.float64, device=dev),
@@ -220,17 +223,33 @@ class Field:
         out._count_tensor = cnt
         return out
 
+    def trace_resume(self, spec, state: TraceResult, mu, t0, t_max, poincare_capacity=0) -> TraceResult:
+        """Continue a previous ``trace`` result in place over [t0, t_max] (GC_TRACE_RESUME): the rows of
+        ``state.y`` are the initial conditions and receive the new states; ``state.h`` carries the step
+        proposals; particles whose status is not 0 are left untouched."""
+        if state.h is None:
+            raise ValueError("trace_resume needs the h_inout buffer of the first call")
+        y = state.y
+        return self.trace(spec, y[0], y[1], y[2], y[3], mu, h_inout=state.h,
+                          poincare_capacity=poincare_capacity, t0=t0, t_max=t_max, out=state,
+                          flags=GC_TRACE_RESUME)
+
     # ---- gc_trace_host (numpy in, numpy out; copies inside the call) --------------------------------------------
     def trace_host(self, spec, s0, th0, ze0, vpar0, mu, h_in=None, poincare_capacity=0, t0=None, t_max=None,
-                   bufs=None) -> TraceResult:
-        f64 = lambda a: np.ascontiguousarray(a, np.float64)
-        s0, th0, ze0, vpar0, mu = map(f64, (s0, th0, ze0, vpar0, mu))
+                   bufs=None, flags=0) -> TraceResult:
+        """Host numpy arrays in and out (views of pinned torch tensors make the copies asynchronous).  With
+        ``bufs`` given its arrays are the output buffers; under GC_TRACE_RESUME they are also read, ``bufs.h``
+        is the h_inout array and the inputs may be the rows of ``bufs.y``."""
+        chk = lambda a: a if (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.flags.c_contiguous) \
+            else np.ascontiguousarray(a, np.float64)
+        s0, th0, ze0, vpar0, mu = map(chk, (s0, th0, ze0, vpar0, mu))
         n = s0.shape[0]
-        p = make_params(spec, t0, t_max, poincare_capacity)
+        p = make_params(spec, t0, t_max, poincare_capacity, flags)
         if bufs is None:
-            bufs = TraceResult(np.empty((4, n)), np.empty(n), np.empty(n, np.int32), np.empty(n, np.int32),
-                               np.empty(n, np.int32), np.empty(n, np.int32), None)
-        bufs.h = np.zeros(n) if h_in is None else f64(h_in).copy()
+            bufs = TraceResult(np.empty((4, n)), np.empty(n), np.zeros(n, np.int32), np.zeros(n, np.int32),
+                               np.zeros(n, np.int32), np.zeros(n, np.int32), None)
+        if not (flags & GC_TRACE_RESUME) or bufs.h is None:
+            bufs.h = np.zeros(n) if h_in is None else chk(h_in).copy()
         pc = np.empty((max(poincare_capacity, 1), 4)) if poincare_capacity else None
         cnt = C.c_int64(0)
         _check(load_library().gc_trace_host(self._h, C.byref(p), n, _hp(s0), _hp(th0), _hp(ze0), _hp(vpar0),

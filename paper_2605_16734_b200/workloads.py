@@ -188,14 +188,16 @@ def add_random_aes(fld: Field, K: int = 16, seed: int = 2004) -> Field:
     return fld
 
 
-def make_particles(config: int, n: int | None = None) -> Particles:
+def make_particles(config: int, n: int | None = None, stream: int = 0) -> Particles:
     """Initial conditions of BASELINE.json:configs[config]; draw order s, theta, zeta, pitch, speed (A21).
     ``n`` overrides the ensemble size; the first k particles of a larger draw are NOT the same as a draw
     of k, so subsamples are always taken with ``Particles.head`` from the full-size draw or drawn at the
     size the test states."""
     full = {0: 512, 1: 100_000, 2: 100_000, 3: 1_000_000, 4: 1_000_000}[config]
     n = full if n is None else int(n)
-    rng = np.random.default_rng(1000 + config)
+    # stream 0 is the ensemble of the config; stream r > 0 is an independent draw of the same recipe (one
+    # per rank of a weak-scaling run)
+    rng = np.random.default_rng(1000 + config if stream == 0 else [1000 + config, int(stream)])
     if config == 0:
         s = np.full(n, 0.25)
     elif config in (1, 2):

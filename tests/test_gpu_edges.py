@@ -1,0 +1,234 @@
+"""-m gpu: edge cases of the boundary and of the controller (O6-O8), each against the oracle."""
+from __future__ import annotations
+
+import dataclasses
+
+import numpy as np
+import pytest
+
+from gpu_common import assert_trace_parity, gpu_trace, make_case, rel_diff, sort_poincare, to_dev
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def case0():
+    return make_case(0, 96)
+
+
+@pytest.fixture(scope="module")
+def case4():
+    return make_case(4, 64)
+
+
+def _kernels():
+    from paper_2605_16734_b200 import gcorbit as G
+    return [G.GC_KERNEL_GENERIC, G.GC_KERNEL_WARP]
+
+
+def test_empty_ensemble(case0):
+    import torch
+    fld, spec, P, OF, GF, mu = case0
+    e = torch.empty(0, dtype=torch.float64, device="cuda:0")
+    r = GF.trace(spec, e, e, e, e, e)
+    torch.cuda.synchronize()
+    assert r.y.shape == (4, 0) and r.status.numel() == 0
+    B, dB = GF.field_eval(e, e, e)
+    assert B.numel() == 0
+
+
+def test_t0_at_or_past_t_max_returns_inputs(case0):
+    fld, spec, P, OF, GF, mu = case0
+    for kern in _kernels():
+        GF.set_kernel(kern)
+        r = gpu_trace(GF, spec, P, mu, t0=1e-5, t_max=1e-5)
+        assert (r.status.cpu().numpy() == 0).all()
+        assert (r.n_acc.cpu().numpy() == 0).all() and (r.n_rej.cpu().numpy() == 0).all()
+        y = r.y.cpu().numpy()
+        assert np.array_equal(y[0], P.s) and np.array_equal(y[1], P.theta) and np.array_equal(y[2], P.zeta)
+        assert np.abs(y[3] - P.vpar).max() <= 4e-16 * spec.v_ref          # v_par round-trips through u = v/v_ref
+        assert (r.t.cpu().numpy() == 1e-5).all()
+
+
+def test_start_outside_and_nonfinite(case0):
+    """s0 >= s_loss is lost after its first accepted step; s0 <= s_min is an axis stop; NaN/inf inputs end
+    with status 4 (O6, O7) -- the same on both sides."""
+    fld, spec, P, OF, GF, mu = case0
+    Q = P.head(8)
+    Q.s[:] = [1.0, 1.05, 5e-4, 0.25, 0.25, 0.25, 0.25, 0.6]
+    Q.theta[3] = np.nan
+    Q.zeta[4] = np.inf
+    m = mu[:8].copy()
+    m[5] = np.nan
+    o = OF.trace(spec, Q.s, Q.theta, Q.zeta, Q.vpar, m, t_max=2e-6)
+    assert o.status[1] == 1 and o.status[2] == 2 and list(o.status[3:6]) == [4, 4, 4]
+    for kern in _kernels():
+        GF.set_kernel(kern)
+        r = gpu_trace(GF, spec, Q, m, t_max=2e-6)
+        assert np.array_equal(r.status.cpu().numpy(), o.status)
+        ok = o.status != 4
+        assert rel_diff(r.y.cpu().numpy()[:, ok], o.y[:, ok], spec.v_ref).max() < 1e-9
+        assert np.array_equal(r.n_acc.cpu().numpy()[ok], o.n_acc[ok])
+
+
+def test_max_steps_cap(case0):
+    fld, spec, P, OF, GF, mu = case0
+    sp = dataclasses.replace(spec, max_steps=7)
+    o = OF.trace(sp, P.s, P.theta, P.zeta, P.vpar, mu)
+    assert (o.status == 3).all()
+    for kern in _kernels():
+        GF.set_kernel(kern)
+        r = gpu_trace(GF, sp, P, mu)
+        assert (r.status.cpu().numpy() == 3).all()
+        assert np.array_equal(r.n_acc.cpu().numpy() + r.n_rej.cpu().numpy(), np.full(P.n, 7))
+        assert_trace_parity(r, o, sp, min_same=0.97, label="max_steps")
+
+
+def test_minimum_step_forces_acceptance(case0):
+    """A9: with h_min above the natural step every attempt after a rejection is made at h_min and accepted
+    whatever its error."""
+    fld, spec, P, OF, GF, mu = case0
+    sp = dataclasses.replace(spec, h_min=2e-7, h0=1e-6)
+    o = OF.trace(sp, P.s, P.theta, P.zeta, P.vpar, mu, t_max=2e-5)
+    assert o.n_forced.sum() > 0
+    for kern in _kernels():
+        GF.set_kernel(kern)
+        r = gpu_trace(GF, sp, P, mu, t_max=2e-5)
+        assert np.array_equal(r.status.cpu().numpy(), o.status)
+        same = (r.n_acc.cpu().numpy() == o.n_acc) & (r.n_rej.cpu().numpy() == o.n_rej)
+        assert same.mean() > 0.9
+        assert np.array_equal(r.n_forced.cpu().numpy()[same], o.n_forced[same])
+        # forced steps carry errors far above rtol: compare at the accuracy those steps have
+        assert rel_diff(r.y.cpu().numpy()[:, same], o.y[:, same], sp.v_ref).max() < 1e-7
+
+
+def test_h_inout_roundtrip_and_segments(case0):
+    """Two calls joined by h_inout and GC_TRACE_RESUME equal the oracle run with the same segmentation; lost
+    or stopped particles are not touched by the second call."""
+    import torch
+    fld, spec, P, OF, GF, mu = case0
+    Q = P.head(96)
+    Q.s[:6] = 0.97                                                   # some of these are lost in segment 1
+    t1, t2 = 1.5e-5, 3e-5
+    o1 = OF.trace(spec, Q.s, Q.theta, Q.zeta, Q.vpar, mu, t0=0.0, t_max=t1)
+    alive = o1.status == 0
+    o2 = OF.trace(spec, o1.y[0, alive], o1.y[1, alive], o1.y[2, alive], o1.y[3, alive], mu[alive],
+                  h_in=o1.h[alive], t0=t1, t_max=t2)
+    for kern in _kernels():
+        GF.set_kernel(kern)
+        h = torch.zeros(Q.n, dtype=torch.float64, device="cuda:0")
+        mu_d = to_dev(mu)
+        st = GF.trace(spec, to_dev(Q.s), to_dev(Q.theta), to_dev(Q.zeta), to_dev(Q.vpar), mu_d, h_inout=h,
+                      t0=0.0, t_max=t1)
+        torch.cuda.synchronize()
+        y1, s1 = st.y.cpu().numpy().copy(), st.status.cpu().numpy().copy()
+        assert np.array_equal(s1, o1.status)
+        assert np.abs(h.cpu().numpy() / o1.h - 1).max() < 1e-6
+        GF.trace_resume(spec, st, mu_d, t0=t1, t_max=t2)
+        torch.cuda.synchronize()
+        y2, s2 = st.y.cpu().numpy(), st.status.cpu().numpy()
+        assert np.array_equal(y2[:, ~alive], y1[:, ~alive]) and np.array_equal(s2[~alive], s1[~alive])
+        assert np.array_equal(s2[alive], o2.status)
+        assert rel_diff(y2[:, alive], o2.y, spec.v_ref).max() < 1e-6
+        assert np.median(rel_diff(y2[:, alive], o2.y, spec.v_ref)) < 1e-9
+        # counters accumulate over the two calls
+        tot = st.n_acc.cpu().numpy()[alive] + st.n_rej.cpu().numpy()[alive]
+        ref = o1.n_acc[alive] + o1.n_rej[alive] + o2.n_acc + o2.n_rej
+        assert (tot == ref).mean() > 0.97
+
+
+def test_trace_host_equals_device_trace(case4):
+    """gc_trace_host (host buffers, copies inside) returns bit-for-bit what gc_trace returns."""
+    fld, spec, P, OF, GF, mu = case4
+    r = gpu_trace(GF, spec, P, mu, t_max=1e-5, poincare_capacity=1024)
+    hres = GF.trace_host(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=1e-5, poincare_capacity=1024)
+    assert np.array_equal(hres.y, r.y.cpu().numpy())
+    assert np.array_equal(hres.t, r.t.cpu().numpy())
+    assert np.array_equal(hres.status, r.status.cpu().numpy())
+    assert np.array_equal(hres.n_acc, r.n_acc.cpu().numpy())
+    assert np.array_equal(hres.n_rej, r.n_rej.cpu().numpy())
+    assert hres.poincare_count == r.poincare_count
+    assert np.array_equal(sort_poincare(hres.poincare), sort_poincare(r.poincare.cpu().numpy()))
+
+
+def test_poincare_overflow_keeps_counting(case4):
+    fld, spec, P, OF, GF, mu = case4
+    full = gpu_trace(GF, spec, P, mu, t_max=1e-5, poincare_capacity=4096)
+    assert full.poincare_count > 8
+    small = gpu_trace(GF, spec, P, mu, t_max=1e-5, poincare_capacity=8)
+    assert small.poincare_count == full.poincare_count and small.poincare.shape[0] == 8
+    # every kept record is one of the full run's records
+    a = sort_poincare(full.poincare.cpu().numpy())
+    for rec in small.poincare.cpu().numpy():
+        assert (np.abs(a - rec).max(axis=1) == 0).any()
+
+
+def test_invalid_arguments_are_reported(case0):
+    import ctypes as C
+    from paper_2605_16734_b200 import gcorbit as G
+    fld, spec, P, OF, GF, mu = case0
+    for bad in (dict(v_ref=0.0), dict(h0=0.0), dict(h_min=-1.0), dict(rtol=0.0, atol=0.0), dict(max_steps=0),
+                dict(mass=0.0), dict(charge=0.0), dict(t_max=float("nan"))):
+        with pytest.raises(G.GcError) as ei:
+            gpu_trace(GF, dataclasses.replace(spec, **bad), P, mu)
+        assert ei.value.code == G.GC_EINVAL, bad
+    L = G.load_library()
+    p = G.make_params(spec)
+    assert L.gc_trace(GF._h, C.byref(p), 4, *([None] * 15)) == G.GC_EINVAL
+    assert b"NULL" in L.gc_last_error()
+    p.flags = 64
+    assert L.gc_trace(GF._h, C.byref(p), 0, *([None] * 15)) == G.GC_EINVAL
+    with pytest.raises(G.GcError):
+        GF.set_kernel(99)
+
+
+def test_field_create_rejects_bad_tables():
+    from paper_2605_16734_b200 import gcorbit as G, workloads as W
+    fld = W.make_field(0)
+    bad = dataclasses.replace(fld, bmnc=fld.bmnc.copy())
+    bad.bmnc[3, 5] = np.nan
+    with pytest.raises(G.GcError) as ei:
+        G.Field(bad)
+    assert ei.value.code == G.GC_EINVAL
+    bad = dataclasses.replace(fld, xm=-fld.xm)
+    with pytest.raises(G.GcError):
+        G.Field(bad)
+    modes = W.make_field(2)
+    bad = dataclasses.replace(modes, mode_omega=np.zeros_like(modes.mode_omega))
+    with pytest.raises(G.GcError):
+        G.Field(bad)
+    small = dataclasses.replace(fld, ns=3, bmnc=fld.bmnc[:3], G=fld.G[:3], I=fld.I[:3], iota=fld.iota[:3])
+    with pytest.raises(G.GcError):
+        G.Field(small)
+
+
+def test_fields_outside_the_warp_layout_use_the_generic_kernel():
+    """max |xn| > 16 does not fit the packed layout: AUTO falls back to the generic kernel, which still
+    matches the oracle; harmonics given in shuffled order with a duplicated (m, n) pair add up."""
+    import oracle
+    from paper_2605_16734_b200 import gcorbit as G, workloads as W
+    fld = W.make_equilibrium(4, 20, 31)
+    GF = G.Field(fld)
+    assert GF.kernel_info()["kernel"] == "generic"
+    with pytest.raises(G.GcError):
+        GF.set_kernel(G.GC_KERNEL_WARP)
+    spec = W.make_spec(0)
+    P = W.make_particles(0, 40)
+    OF = oracle.OracleField(fld)
+    mu = W.mu_from(P, OF.eval_B_many(P.s, P.theta, P.zeta)[:, 0])
+    r = gpu_trace(GF, spec, P, mu, t_max=5e-6)
+    o = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=5e-6)
+    assert_trace_parity(r, o, spec, min_same=0.95, label="generic N=20")
+
+    base = W.make_field(0)
+    perm = np.random.default_rng(3).permutation(base.nh)
+    xm = np.concatenate([base.xm[perm], base.xm[10:11]])
+    xn = np.concatenate([base.xn[perm], base.xn[10:11]])
+    bm = np.concatenate([base.bmnc[:, perm], 0.5 * base.bmnc[:, 10:11]], axis=1)
+    shuf = dataclasses.replace(base, xm=xm, xn=xn, bmnc=np.ascontiguousarray(bm))
+    GF2, OF2 = G.Field(shuf), oracle.OracleField(shuf)
+    assert GF2.kernel_info()["kernel"] == "warp"
+    mu2 = W.mu_from(P, OF2.eval_B_many(P.s, P.theta, P.zeta)[:, 0])
+    r = gpu_trace(GF2, spec, P, mu2, t_max=5e-6)
+    o = OF2.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu2, t_max=5e-6)
+    assert_trace_parity(r, o, spec, min_same=0.95, label="shuffled harmonics")

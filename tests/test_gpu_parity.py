@@ -1,0 +1,179 @@
+"""-m gpu: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the seeded
+synthetic inputs of BASELINE.json:configs (SURVEY.md section 8(c) "GPU-vs-oracle acceptance")."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+from gpu_common import (FLIP_RTOL, SAME_RTOL, assert_trace_parity, gpu_trace, make_case, rel_diff,
+                        sort_poincare, to_dev)
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = ["generic", "warp"]
+
+
+def _set_kernel(GF, name):
+    from paper_2605_16734_b200 import gcorbit as G
+    GF.set_kernel({"generic": G.GC_KERNEL_GENERIC, "warp": G.GC_KERNEL_WARP}[name])
+
+
+@pytest.fixture(scope="module")
+def cases():
+    cache = {}
+
+    def get(config, n):
+        if (config, n) not in cache:
+            cache[(config, n)] = make_case(config, n)
+        return cache[(config, n)]
+    return get
+
+
+# ---- O2 / O3: point evaluations ---------------------------------------------------------------------------------
+@pytest.mark.parametrize("config", [0, 1])
+def test_field_eval_matches_oracle(cases, config):
+    import torch
+    fld, spec, P, OF, GF, mu = cases(config, 300)
+    # include points outside [0, 1] (clamped stencil extrapolates, A6) and large unwrapped angles (A12)
+    s = P.s.copy(); th = P.theta.copy(); ze = P.zeta.copy()
+    s[:4] = [-0.01, 0.0, 1.0, 1.02]
+    th[4:8] += 5.0e3
+    ze[8:12] -= 2.0e4
+    B, dB = GF.field_eval(to_dev(s), to_dev(th), to_dev(ze))
+    torch.cuda.synchronize()
+    ref = OF.eval_B_many(s, th, ze)
+    B, dB = B.cpu().numpy(), dB.cpu().numpy()
+    assert np.abs(B / ref[:, 0] - 1.0).max() < 1e-12
+    for c in range(3):
+        # unwrapped angles of 1e4 rad carry 1e4 * eps of phase noise on BOTH sides
+        assert np.abs(dB[c] - ref[:, 1 + c]).max() <= 1e-10 * np.abs(ref[:, 1 + c]).max()
+
+
+@pytest.mark.parametrize("config", [2, 4])
+def test_pert_eval_matches_oracle(cases, config):
+    import torch
+    fld, spec, P, OF, GF, mu = cases(config, 200)
+    t = 3.7e-5
+    out = GF.pert_eval(to_dev(P.s), to_dev(P.theta), to_dev(P.zeta), t)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()
+    ref = np.array([OF.eval_pert(P.s[i], P.theta[i], P.zeta[i], t) for i in range(P.n)]).T
+    for q in range(9):
+        assert np.abs(out[q] - ref[q]).max() <= 1e-11 * np.abs(ref[q]).max(), q
+
+
+def test_pert_eval_static_field_is_zero(cases):
+    import torch
+    fld, spec, P, OF, GF, mu = cases(0, 64)
+    out = GF.pert_eval(to_dev(P.s), to_dev(P.theta), to_dev(P.zeta), 1e-5)
+    torch.cuda.synchronize()
+    assert float(out.abs().max()) == 0.0
+
+
+# ---- O4: the right-hand side alone, both kernels ------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("config", [0, 1, 2, 4])
+def test_rhs_matches_oracle(cases, config, kernel):
+    import torch
+    fld, spec, P, OF, GF, mu = cases(config, 256)
+    _set_kernel(GF, kernel)
+    t = 3.3e-5
+    y = np.stack([P.s, P.theta + 50.0, P.zeta - 30.0, P.vpar])
+    got = GF.rhs_eval(spec.mass, spec.charge, t, to_dev(y), to_dev(mu))
+    torch.cuda.synchronize()
+    got = got.cpu().numpy()
+    ref = np.array([OF.rhs(spec.mass, spec.charge, mu[i], 1.0, t, y[:, i]) for i in range(P.n)]).T
+    for c in range(4):
+        scale = np.maximum(np.abs(ref[c]), 1e-6 * np.abs(ref[c]).max())
+        assert (np.abs(got[c] - ref[c]) / scale).max() < 1e-9, (c, (np.abs(got[c] - ref[c]) / scale).max())
+    _set_kernel(GF, "warp")
+
+
+# ---- O5-O7: the trace ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_trace_config0_full(cases, kernel):
+    """BASELINE.json configs[0] in full: 512 alphas, t_max = 1e-4 s, rtol 1e-9."""
+    fld, spec, P, OF, GF, mu = cases(0, None)
+    assert P.n == 512 and spec.t_max == 1e-4
+    _set_kernel(GF, kernel)
+    r = gpu_trace(GF, spec, P, mu)
+    o = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu)
+    info = assert_trace_parity(r, o, spec, label=f"config 0 {kernel}")
+    print(f"config 0 {kernel}: {info}, attempts {int(o.n_acc.sum() + o.n_rej.sum())}")
+    _set_kernel(GF, "warp")
+
+
+@pytest.mark.parametrize("config,n,t_max", [(1, 296, 2e-5), (2, 256, 2e-5), (3, 301, 3e-5), (4, 256, 2e-5)])
+def test_trace_subsamples(cases, config, n, t_max):
+    """Short-horizon subsamples of configs 1-4 (n chosen ragged against 8 warps per block)."""
+    fld, spec, P, OF, GF, mu = cases(config, n)
+    cap = 4096 if config == 4 else 0
+    r = gpu_trace(GF, spec, P, mu, t_max=t_max, poincare_capacity=cap)
+    o = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=t_max, poincare_capacity=cap)
+    info = assert_trace_parity(r, o, spec, label=f"config {config}")
+    print(f"config {config}: {info}")
+    if cap:
+        # O8: same crossings (record order is unspecified: compare sorted by particle, time)
+        assert r.poincare_count == o.poincare_count > 0
+        a, b = sort_poincare(r.poincare.cpu().numpy()), sort_poincare(o.poincare)
+        assert np.array_equal(a[:, 0], b[:, 0])
+        assert np.abs(a[:, 1] - b[:, 1]).max() <= 1e-9 * t_max
+        assert np.abs(a[:, 2] - b[:, 2]).max() <= 1e-9
+        dth = np.abs(a[:, 3] - b[:, 3])
+        assert np.minimum(dth, 2 * np.pi - dth).max() <= 1e-8
+
+
+def test_trace_generic_kernel_with_modes(cases):
+    fld, spec, P, OF, GF, mu = cases(2, 256)
+    _set_kernel(GF, "generic")
+    r = gpu_trace(GF, spec, P.head(64), mu[:64], t_max=1e-5)
+    Q = P.head(64)
+    o = OF.trace(spec, Q.s, Q.theta, Q.zeta, Q.vpar, mu[:64], t_max=1e-5)
+    assert_trace_parity(r, o, spec, min_same=0.95, label="config 2 generic")
+    _set_kernel(GF, "warp")
+
+
+@pytest.mark.parametrize("n", [1, 7, 33, 148 * 8 + 3])
+def test_trace_ragged_sizes(cases, n):
+    """One particle, fewer particles than warps in a block, and one more wave than the persistent grid holds."""
+    fld, spec, P, OF, GF, mu = cases(0, 148 * 8 + 3)
+    Q = P.head(n)
+    r = gpu_trace(GF, spec, Q, mu[:n], t_max=3e-6)
+    o = OF.trace(spec, Q.s, Q.theta, Q.zeta, Q.vpar, mu[:n], t_max=3e-6)
+    assert_trace_parity(r, o, spec, min_same=0.0 if n < 100 else 0.99, label=f"n={n}")
+
+
+def test_full_size_launch_sampled(cases):
+    """BASELINE.json configs[1] at full size in the launch configuration bench.py times (100,000 particles,
+    one 2e-5 s segment, in-place resume of a second segment); 48 sampled particles checked one by one."""
+    import torch
+    from paper_2605_16734_b200 import gcorbit as G
+    fld, spec, P, OF, GF, _ = cases(1, 64)          # fields only; the full ensemble is drawn here
+    from paper_2605_16734_b200 import workloads as W
+    P = W.make_particles(1)
+    assert P.n == 100_000
+    s, th, ze, vp = (to_dev(x) for x in (P.s, P.theta, P.zeta, P.vpar))
+    B, _ = GF.field_eval(s, th, ze, derivs=False)
+    mu_d = to_dev(0.5 * spec.mass * P.vperp2()) / B
+    h = torch.zeros(P.n, dtype=torch.float64, device="cuda:0")
+    seg = 2e-5
+    st = GF.trace(spec, s, th, ze, vp, mu_d, h_inout=h, t0=0.0, t_max=seg)
+    GF.trace_resume(spec, st, mu_d, t0=seg, t_max=2 * seg)
+    torch.cuda.synchronize()
+    status = st.status.cpu().numpy()
+    assert set(np.unique(status)) <= {0, 1}
+    assert (st.t.cpu().numpy()[status == 0] == 2 * seg).all()
+    idx = np.random.default_rng(7).choice(P.n, 48, replace=False)
+    idx = np.union1d(idx, np.nonzero(status == 1)[0][:8])          # and a few lost ones if any
+    mu = mu_d.cpu().numpy()
+    Q = W.Particles(P.s[idx], P.theta[idx], P.zeta[idx], P.pitch[idx], P.speed[idx])
+    o1 = OF.trace(spec, Q.s, Q.theta, Q.zeta, Q.vpar, mu[idx], t0=0.0, t_max=seg)
+    alive = o1.status == 0
+    o2 = OF.trace(spec, o1.y[0, alive], o1.y[1, alive], o1.y[2, alive], o1.y[3, alive], mu[idx][alive],
+                  h_in=o1.h[alive], t0=seg, t_max=2 * seg)
+    y_ref, st_ref, t_ref = o1.y.copy(), o1.status.copy(), o1.t.copy()
+    y_ref[:, alive], st_ref[alive], t_ref[alive] = o2.y, o2.status, o2.t
+    assert np.array_equal(status[idx], st_ref)
+    rel = rel_diff(st.y.cpu().numpy()[:, idx], y_ref, spec.v_ref)
+    assert np.median(rel) < SAME_RTOL and rel.max() < FLIP_RTOL, rel.max()
+    assert (np.abs(st.t.cpu().numpy()[idx] - t_ref) <= 1e-12 * t_ref).all()

@@ -81,7 +81,21 @@ def test_max_steps_cap(case0):
         r = gpu_trace(GF, sp, P, mu)
         assert (r.status.cpu().numpy() == 3).all()
         assert np.array_equal(r.n_acc.cpu().numpy() + r.n_rej.cpu().numpy(), np.full(P.n, 7))
-        assert_trace_parity(r, o, sp, min_same=0.97, label="max_steps")
+        # A capped particle ends at ITS OWN time, not at a common t_max.  The first proposals h come from
+        # err**-0.2 while the embedded error (|delta| ~ 1e-12 at h = 1e-8 s) still carries the rounding noise
+        # of the harmonic sum at the 1e-6 level, so two correct implementations end ~1e-7 apart (relative)
+        # in t and ydot * dt apart in y.  Compare after removing ydot * dt.
+        same = (r.n_acc.cpu().numpy() == o.n_acc) & (r.n_rej.cpu().numpy() == o.n_rej)
+        assert same.mean() >= 0.97
+        yg, tg = r.y.cpu().numpy(), r.t.cpu().numpy()
+        dt = tg - o.t
+        assert (np.abs(dt) <= 1e-5 * o.t).all()
+        floor = np.array([1.0, 1.0, 1.0, sp.v_ref])
+        for i in np.nonzero(same)[0]:
+            yo = o.y[:, i] / np.array([1.0, 1.0, 1.0, sp.v_ref])
+            ydot = OF.rhs(sp.mass, sp.charge, mu[i], sp.v_ref, o.t[i], yo) * np.array([1.0, 1.0, 1.0, sp.v_ref])
+            resid = np.abs(yg[:, i] - o.y[:, i] - ydot * dt[i]) / np.maximum(np.abs(o.y[:, i]), floor)
+            assert resid.max() <= 1e-9, (i, resid)
 
 
 def test_minimum_step_forces_acceptance(case0):
@@ -123,7 +137,9 @@ def test_h_inout_roundtrip_and_segments(case0):
         torch.cuda.synchronize()
         y1, s1 = st.y.cpu().numpy().copy(), st.status.cpu().numpy().copy()
         assert np.array_equal(s1, o1.status)
-        assert np.abs(h.cpu().numpy() / o1.h - 1).max() < 1e-6
+        # the proposal is h * 0.9 * err**-0.2 and err carries the rounding noise of the embedded error estimate
+        dh = np.abs(h.cpu().numpy() / o1.h - 1)
+        assert dh.max() < 1e-5 and np.median(dh) < 1e-8
         GF.trace_resume(spec, st, mu_d, t0=t1, t_max=t2)
         torch.cuda.synchronize()
         y2, s2 = st.y.cpu().numpy(), st.status.cpu().numpy()

@@ -5,8 +5,8 @@ from __future__ import annotations
 import numpy as np
 import pytest
 
-from gpu_common import (FLIP_RTOL, SAME_RTOL, assert_trace_parity, gpu_trace, make_case, rel_diff,
-                        sort_poincare, to_dev)
+from gpu_common import (COND_FACTOR, FLIP_RTOL, SAME_RTOL, assert_trace_parity, gpu_trace, make_case,
+                        oracle_conditioning, rel_diff, sort_poincare, to_dev)
 
 pytestmark = pytest.mark.gpu
 
@@ -90,6 +90,18 @@ def test_rhs_matches_oracle(cases, config, kernel):
 
 
 # ---- O5-O7: the trace ---------------------------------------------------------------------------------------------
+_FULL = {}
+
+
+def _oracle_full(cases):
+    """Config 0 oracle run and its conditioning, computed once for both kernels."""
+    if not _FULL:
+        fld, spec, P, OF, GF, mu = cases(0, None)
+        o = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu)
+        _FULL["o"], _FULL["cond"] = o, oracle_conditioning(OF, spec, P, mu, o)
+    return _FULL["o"], _FULL["cond"]
+
+
 @pytest.mark.parametrize("kernel", KERNELS)
 def test_trace_config0_full(cases, kernel):
     """BASELINE.json configs[0] in full: 512 alphas, t_max = 1e-4 s, rtol 1e-9."""
@@ -97,8 +109,9 @@ def test_trace_config0_full(cases, kernel):
     assert P.n == 512 and spec.t_max == 1e-4
     _set_kernel(GF, kernel)
     r = gpu_trace(GF, spec, P, mu)
-    o = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu)
-    info = assert_trace_parity(r, o, spec, label=f"config 0 {kernel}")
+    o, cond = _oracle_full(cases)
+    # 1e-4 s is ~3000 steps: ~1-2 % of the particles are ill-conditioned in the oracle itself (gpu_common)
+    info = assert_trace_parity(r, o, spec, label=f"config 0 {kernel}", cond=cond, min_within=0.95)
     print(f"config 0 {kernel}: {info}, attempts {int(o.n_acc.sum() + o.n_rej.sum())}")
     _set_kernel(GF, "warp")
 
@@ -110,7 +123,8 @@ def test_trace_subsamples(cases, config, n, t_max):
     cap = 4096 if config == 4 else 0
     r = gpu_trace(GF, spec, P, mu, t_max=t_max, poincare_capacity=cap)
     o = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=t_max, poincare_capacity=cap)
-    info = assert_trace_parity(r, o, spec, label=f"config {config}")
+    cond = oracle_conditioning(OF, spec, P, mu, o, t_max=t_max)
+    info = assert_trace_parity(r, o, spec, label=f"config {config}", cond=cond, min_within=0.99)
     print(f"config {config}: {info}")
     if cap:
         # O8: same crossings (record order is unspecified: compare sorted by particle, time)
@@ -129,7 +143,8 @@ def test_trace_generic_kernel_with_modes(cases):
     r = gpu_trace(GF, spec, P.head(64), mu[:64], t_max=1e-5)
     Q = P.head(64)
     o = OF.trace(spec, Q.s, Q.theta, Q.zeta, Q.vpar, mu[:64], t_max=1e-5)
-    assert_trace_parity(r, o, spec, min_same=0.95, label="config 2 generic")
+    cond = oracle_conditioning(OF, spec, Q, mu[:64], o, t_max=1e-5)
+    assert_trace_parity(r, o, spec, min_same=0.95, label="config 2 generic", cond=cond, min_within=0.98)
     _set_kernel(GF, "warp")
 
 
@@ -140,7 +155,8 @@ def test_trace_ragged_sizes(cases, n):
     Q = P.head(n)
     r = gpu_trace(GF, spec, Q, mu[:n], t_max=3e-6)
     o = OF.trace(spec, Q.s, Q.theta, Q.zeta, Q.vpar, mu[:n], t_max=3e-6)
-    assert_trace_parity(r, o, spec, min_same=0.0 if n < 100 else 0.99, label=f"n={n}")
+    cond = oracle_conditioning(OF, spec, Q, mu[:n], o, t_max=3e-6)
+    assert_trace_parity(r, o, spec, min_same=0.0 if n < 100 else 0.99, label=f"n={n}", cond=cond)
 
 
 def test_full_size_launch_sampled(cases):
@@ -167,13 +183,27 @@ def test_full_size_launch_sampled(cases):
     idx = np.union1d(idx, np.nonzero(status == 1)[0][:8])          # and a few lost ones if any
     mu = mu_d.cpu().numpy()
     Q = W.Particles(P.s[idx], P.theta[idx], P.zeta[idx], P.pitch[idx], P.speed[idx])
-    o1 = OF.trace(spec, Q.s, Q.theta, Q.zeta, Q.vpar, mu[idx], t0=0.0, t_max=seg)
-    alive = o1.status == 0
-    o2 = OF.trace(spec, o1.y[0, alive], o1.y[1, alive], o1.y[2, alive], o1.y[3, alive], mu[idx][alive],
-                  h_in=o1.h[alive], t0=seg, t_max=2 * seg)
-    y_ref, st_ref, t_ref = o1.y.copy(), o1.status.copy(), o1.t.copy()
-    y_ref[:, alive], st_ref[alive], t_ref[alive] = o2.y, o2.status, o2.t
+
+    def two_segments(Qp):
+        o1 = OF.trace(spec, Qp.s, Qp.theta, Qp.zeta, Qp.vpar, mu[idx], t0=0.0, t_max=seg)
+        alive = o1.status == 0
+        o2 = OF.trace(spec, o1.y[0, alive], o1.y[1, alive], o1.y[2, alive], o1.y[3, alive], mu[idx][alive],
+                      h_in=o1.h[alive], t0=seg, t_max=2 * seg)
+        y_ref, st_ref, t_ref = o1.y.copy(), o1.status.copy(), o1.t.copy()
+        y_ref[:, alive], st_ref[alive], t_ref[alive] = o2.y, o2.status, o2.t
+        return y_ref, st_ref, t_ref
+
+    y_ref, st_ref, t_ref = two_segments(Q)
+    # the oracle's own conditioning on these particles (gpu_common): theta0 moved by ~1 ulp
+    spread, tspread = np.zeros(len(idx)), np.zeros(len(idx))
+    for eps in (1e-15, -1e-15):
+        Qp = W.Particles(Q.s, Q.theta * (1.0 + eps), Q.zeta, Q.pitch, Q.speed)
+        y2, st2, t2 = two_segments(Qp)
+        assert np.array_equal(st2, st_ref)
+        spread = np.maximum(spread, rel_diff(y2, y_ref, spec.v_ref))
+        tspread = np.maximum(tspread, np.abs(t2 - t_ref) / t_ref)
     assert np.array_equal(status[idx], st_ref)
     rel = rel_diff(st.y.cpu().numpy()[:, idx], y_ref, spec.v_ref)
-    assert np.median(rel) < SAME_RTOL and rel.max() < FLIP_RTOL, rel.max()
-    assert (np.abs(st.t.cpu().numpy()[idx] - t_ref) <= 1e-12 * t_ref).all()
+    assert np.median(rel) < 1e-11 and (rel <= np.maximum(SAME_RTOL, COND_FACTOR * spread)).all(), rel.max()
+    relt = np.abs(st.t.cpu().numpy()[idx] - t_ref) / t_ref
+    assert (relt <= np.maximum(SAME_RTOL, COND_FACTOR * tspread)).all(), relt.max()

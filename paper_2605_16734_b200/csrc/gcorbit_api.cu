@@ -14,6 +14,7 @@
 namespace gc { constexpr int GC_ST_NONFINITE_ = 4; }
 #include "kernels_generic.cuh"
 #include "kernels_warp.cuh"
+#include "kernels_tile.cuh"
 
 namespace {
 
@@ -52,10 +53,13 @@ bool all_finite(const double* p, size_t n) {
 struct gc_field {
   gc::FieldDev dev{};
   std::vector<void*> allocs;
-  int kernel = GC_KERNEL_GENERIC;   // resolved choice
+  int kernel = GC_KERNEL_AUTO;      // requested choice; resolved per call by resolve_kernel()
   bool warp_ok = false;
+  bool tile_ok = false;
   int nit_main_inst = 0;            // instantiated (padded) main iteration count
   int sm_count = 0;
+  int tile_smem = 0;                // dynamic shared memory of the tile kernel
+  int tile_blocks_per_sm = 0;       // co-resident blocks per SM (cooperative launch)
 };
 
 namespace {
@@ -165,6 +169,115 @@ int pack_rows(gc_field* f, const gc_field_desc* d) {
   return GC_OK;
 }
 
+// ---- tile-kernel instantiations and window images -------------------------------------------------------------
+const void* tile_fn(const gc_field* f) {
+  const bool modes = f->dev.nk > 0;
+  if (f->dev.tile_nmax == 8)
+    return modes ? (const void*)gc::trace_tile_kernel<8, true> : (const void*)gc::trace_tile_kernel<8, false>;
+  return modes ? (const void*)gc::trace_tile_kernel<16, true> : (const void*)gc::trace_tile_kernel<16, false>;
+}
+
+int resolve_kernel(const gc_field* f, int64_t n) {
+  if (f->kernel != GC_KERNEL_AUTO) return f->kernel;
+  if (f->tile_ok && n >= GC_TILE_MIN_PARTICLES) return GC_KERNEL_TILE;
+  return f->warp_ok ? GC_KERNEL_WARP : GC_KERNEL_GENERIC;
+}
+
+// images[cell][10 E]: [E][6] node rows cell-1 .. cell+4 (zero where the row does not exist), then [E][4] rows
+// cell .. cell+3 (kernels_tile.cuh).  Entries: per m, b(m,0) then (P, Q)(m,n) for n = 1..NMAX with
+// P = b(m,n) + b(m,-n), Q = b(m,n) - b(m,-n); then G, I, iota; then the nk mode amplitudes.
+int pack_tile_images(gc_field* f, const gc_field_desc* d) {
+  gc::FieldDev& v = f->dev;
+  f->tile_ok = false;
+  if (v.N > 16) return GC_OK;
+  const int nmax = v.N <= 8 ? 8 : 16;
+  const int rowlen = 1 + 2 * nmax;
+  const int E = (v.M + 1) * rowlen + 3 + d->nk;
+  const int smem = (int)((size_t)10 * E * sizeof(double) + (size_t)7 * 4 * gc::kTileThreads * sizeof(double) + 64);
+  if (smem > 110 * 1024) return GC_OK;                     // two blocks per SM must fit
+  const int ncell = d->ns - 3;
+  if ((size_t)3 * ncell * sizeof(int) > (size_t)10 * E * sizeof(double)) return GC_OK;   // scan space (phase B)
+  // node-major entry rows first
+  std::vector<double> rows((size_t)d->ns * E, 0.0);
+  for (int node = 0; node < d->ns; ++node) {
+    double* row = rows.data() + (size_t)node * E;
+    for (int k = 0; k < d->nh; ++k) {
+      const int m = d->xm[k], n = d->xn[k];
+      const double b = d->bmnc[(size_t)node * d->nh + k];
+      double* r = row + (size_t)m * rowlen;
+      if (n == 0) { r[0] += b; continue; }
+      const int an = n > 0 ? n : -n;
+      r[2 * an - 1] += b;                                  // P
+      r[2 * an] += n > 0 ? b : -b;                         // Q
+    }
+    double* x = row + (size_t)(v.M + 1) * rowlen;
+    x[0] = d->G[node]; x[1] = d->I[node]; x[2] = d->iota[node];
+    for (int k = 0; k < d->nk; ++k) x[3 + k] = d->phihat[(size_t)node * d->nk + k];
+  }
+  std::vector<double> img((size_t)ncell * 10 * E, 0.0);
+  for (int c = 0; c < ncell; ++c) {
+    double* A = img.data() + (size_t)c * 10 * E;
+    double* Bq = A + (size_t)6 * E;
+    for (int e = 0; e < E; ++e) {
+      for (int j = 0; j < 6; ++j) {
+        const int node = c - 1 + j;
+        if (node >= 0 && node < d->ns) A[(size_t)e * 6 + j] = rows[(size_t)node * E + e];
+      }
+      for (int j = 0; j < 4; ++j) Bq[(size_t)e * 4 + j] = rows[(size_t)(c + j) * E + e];
+    }
+  }
+  double* dev_img = nullptr;
+  int rc = upload(img.data(), img.size(), &dev_img);
+  if (rc != GC_OK) return rc;
+  f->allocs.push_back(dev_img);
+  v.tile_images = dev_img;
+  v.tile_E = E;
+  v.tile_nmax = nmax;
+  f->tile_smem = smem;
+  const void* fn = tile_fn(f);
+  GC_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  int per_sm = 0;
+  GC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, gc::kTileThreads, (size_t)smem));
+  if (per_sm < 1) return GC_OK;
+  int coop = 0, devid = 0;
+  GC_CUDA(cudaGetDevice(&devid));
+  GC_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, devid));
+  if (!coop) return GC_OK;
+  f->tile_blocks_per_sm = per_sm;
+  f->tile_ok = true;
+  return GC_OK;
+}
+
+// One cooperative launch of the tile kernel (mode 0 trace, mode 1 right-hand side only) with its scratch.
+int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, cudaStream_t st) {
+  const int ncell = f->dev.ns - 3;
+  const size_t n = (size_t)t.n;
+  const size_t rec_bytes = n * gc::kRecDoubles * sizeof(double);
+  const size_t int_count = n + (size_t)4 * (ncell + 1) + 8;
+  unsigned char* slab = nullptr;
+  GC_CUDA(cudaMallocAsync((void**)&slab, rec_bytes + int_count * sizeof(int), st));
+  gc::TileScratch sc{};
+  sc.rec = reinterpret_cast<double*>(slab);
+  int* ip = reinterpret_cast<int*>(slab + rec_bytes);
+  sc.order = ip; ip += n;
+  sc.cnt = ip; ip += ncell + 1;
+  sc.start = ip; ip += ncell + 1;
+  sc.tstart = ip; ip += ncell + 1;
+  sc.cursor = ip; ip += ncell + 1;
+  sc.ctrl = ip;
+  GC_CUDA(cudaMemsetAsync(sc.cnt, 0, ((size_t)4 * (ncell + 1) + 8) * sizeof(int), st));
+  long long blocks = (long long)f->sm_count * f->tile_blocks_per_sm;
+  const long long need = ((long long)n + gc::kTileThreads - 1) / gc::kTileThreads;
+  if (blocks > need) blocks = need;
+  if (blocks < 1) blocks = 1;
+  gc::FieldDev fd = f->dev;
+  void* args[] = {(void*)&fd, (void*)&t, (void*)&sc, (void*)&mode, (void*)&rhs_out};
+  GC_CUDA(cudaLaunchCooperativeKernel(tile_fn(f), dim3((unsigned)blocks), dim3(gc::kTileThreads), args,
+                                      (size_t)f->tile_smem, st));
+  GC_CUDA(cudaFreeAsync(slab, st));
+  return GC_OK;
+}
+
 int build_trace_dev(const gc_field* f, const gc_trace_params* p, int64_t n, gc::TraceDev* t) {
   if (!f || !p) return fail(GC_EINVAL, "gc_trace: NULL field or params");
   if (n < 0) return fail(GC_EINVAL, "gc_trace: n < 0");
@@ -259,11 +372,12 @@ int gc_field_create(const gc_field_desc* d, gc_field** out) {
     v.mode_m = mm; v.mode_n = mn; v.omega = om; v.phase = ph; v.phihat = phihat;
     rc = pack_rows(f, d);
   }
+  if (rc == GC_OK) rc = pack_tile_images(f, d);
   if (rc == GC_OK) {
     int devid = 0;
     cudaGetDevice(&devid);
     cudaDeviceGetAttribute(&f->sm_count, cudaDevAttrMultiProcessorCount, devid);
-    f->kernel = f->warp_ok ? GC_KERNEL_WARP : GC_KERNEL_GENERIC;
+    f->kernel = GC_KERNEL_AUTO;
     if (f->warp_ok) {
       const WarpInst* w = find_inst(f);
       rc = ensure_smem(w->trace_fn, w->smem_bytes);
@@ -282,20 +396,29 @@ int gc_field_create(const gc_field_desc* d, gc_field** out) {
 
 int gc_set_kernel(gc_field* f, int32_t kernel) {
   if (!f) return fail(GC_EINVAL, "gc_set_kernel: NULL field");
-  if (kernel == GC_KERNEL_AUTO) kernel = f->warp_ok ? GC_KERNEL_WARP : GC_KERNEL_GENERIC;
   if (kernel == GC_KERNEL_WARP && !f->warp_ok)
     return fail(GC_EINVAL, "gc_set_kernel: field does not fit the warp kernel (max|xn| <= 16, max xm <= 28)");
-  if (kernel != GC_KERNEL_WARP && kernel != GC_KERNEL_GENERIC) return fail(GC_EINVAL, "gc_set_kernel: unknown kernel");
+  if (kernel == GC_KERNEL_TILE && !f->tile_ok)
+    return fail(GC_EINVAL, "gc_set_kernel: field does not fit the tile kernel (max|xn| <= 16, window <= 110 KB)");
+  if (kernel != GC_KERNEL_AUTO && kernel != GC_KERNEL_WARP && kernel != GC_KERNEL_GENERIC && kernel != GC_KERNEL_TILE)
+    return fail(GC_EINVAL, "gc_set_kernel: unknown kernel");
   f->kernel = kernel;
   return GC_OK;
 }
 
-int gc_kernel_info(const gc_field* f, int32_t* kernel, int32_t* blocks, int32_t* threads, int32_t* smem,
+int gc_kernel_info(const gc_field* f, int64_t n, int32_t* kernel, int32_t* blocks, int32_t* threads, int32_t* smem,
                    int32_t* regs) {
   if (!f) return fail(GC_EINVAL, "gc_kernel_info: NULL field");
   cudaFuncAttributes at{};
   int b, t, s;
-  if (f->kernel == GC_KERNEL_WARP) {
+  const int k = resolve_kernel(f, n);
+  if (k == GC_KERNEL_TILE) {
+    GC_CUDA(cudaFuncGetAttributes(&at, tile_fn(f)));
+    long long bl = (long long)f->sm_count * f->tile_blocks_per_sm;
+    const long long need = (n + gc::kTileThreads - 1) / gc::kTileThreads;
+    if (bl > need) bl = need < 1 ? 1 : need;
+    b = (int)bl; t = gc::kTileThreads; s = f->tile_smem;
+  } else if (k == GC_KERNEL_WARP) {
     const WarpInst* w = find_inst(f);
     GC_CUDA(cudaFuncGetAttributes(&at, w->trace_fn));
     b = f->sm_count; t = gc::kWarpsPerBlock * 32; s = w->smem_bytes;
@@ -303,7 +426,7 @@ int gc_kernel_info(const gc_field* f, int32_t* kernel, int32_t* blocks, int32_t*
     GC_CUDA(cudaFuncGetAttributes(&at, (const void*)gc::trace_generic_kernel));
     b = f->sm_count * 4; t = 128; s = 0;
   }
-  if (kernel) *kernel = f->kernel;
+  if (kernel) *kernel = k;
   if (blocks) *blocks = b;
   if (threads) *threads = t;
   if (smem) *smem = s;
@@ -338,7 +461,15 @@ int gc_rhs_eval(const gc_field* f, double mass, double charge, double t, int64_t
   if (!f || n < 0) return fail(GC_EINVAL, "gc_rhs_eval: NULL field or n < 0");
   if (n == 0) return GC_OK;
   if (!y || !mu || !dydt) return fail(GC_EINVAL, "gc_rhs_eval: NULL array");
-  if (f->kernel == GC_KERNEL_WARP) {
+  const int kern = resolve_kernel(f, n);
+  if (kern == GC_KERNEL_TILE) {
+    gc::TraceDev td{};
+    td.mass = mass; td.charge = charge; td.t0 = t; td.t_max = t; td.v_ref = 1.0; td.inv_v_ref = 1.0;
+    td.n = n; td.s0 = y; td.th0 = y + n; td.ze0 = y + 2 * n; td.vpar0 = y + 3 * n; td.mu = mu;
+    td.max_steps = 1;
+    return launch_tile(f, td, 1, dydt, (cudaStream_t)stream);
+  }
+  if (kern == GC_KERNEL_WARP) {
     const WarpInst* w = find_inst(f);
     long long nn = n;
     void* args[] = {(void*)&f->dev, &mass, &charge, &t, &nn, (void*)&y, (void*)&mu, (void*)&dydt};
@@ -374,7 +505,9 @@ int gc_trace(const gc_field* f, const gc_trace_params* params, int64_t n, const 
   t.poincare_count = reinterpret_cast<unsigned long long*>(poincare_count);
   if (!poincare || !poincare_count) t.poincare_capacity = 0;
   if (poincare_count) GC_CUDA(cudaMemsetAsync(poincare_count, 0, sizeof(int64_t), st));
-  if (f->kernel == GC_KERNEL_WARP) {
+  const int kern = resolve_kernel(f, n);
+  if (kern == GC_KERNEL_TILE) return launch_tile(f, t, 0, nullptr, st);
+  if (kern == GC_KERNEL_WARP) {
     const WarpInst* w = find_inst(f);
     unsigned long long* counter = nullptr;
     GC_CUDA(cudaMallocAsync((void**)&counter, sizeof(unsigned long long), st));

@@ -1,0 +1,572 @@
+// kernels_tile.cuh -- the hot-path kernel for large ensembles: persistent, cell-binned, one THREAD per particle.
+//
+// Idea.  The radial stencil of a right-hand side depends only on the particle's radial
+// cell, and thousands of particles share a cell.  Particles are therefore binned by the start i0 of their
+// stencil ("home cell"); a block of 128 threads takes a TILE of up to 128 particles of one cell, stages that
+// cell's window of the harmonic table -- the six node rows i0-1 .. i0+4, i.e. the home stencil and both
+// neighbours -- into shared memory with ONE bulk (TMA) copy of a pre-packed image, and every thread then
+// integrates its own particle: the table values it needs are the same address for (almost) all lanes of a
+// warp, so a shared-memory load is a broadcast, and everything that is per particle (Lagrange weights, the two
+// sincos, the angle-addition recurrences, the guiding-centre algebra, the Dormand-Prince controller) is done
+// by one lane instead of being replicated over a warp.
+//
+// Radial interpolation commutes with the harmonic sum, so the inner loop carries none: with
+//     b(m,n) cos(m th - n ph) + b(m,-n) cos(m th + n ph) = P c_m C_n + Q s_m S_n      (ph = nfp zeta)
+// a thread accumulates, per poloidal row m and per stencil slot a = 0..3,
+//     PC[a] += P[a] C_n,  PS[a] += P[a] n S_n,  QS[a] += Q[a] S_n,  QC[a] += Q[a] n C_n
+// (16 DFMA + 2 DMUL per (m,n) pair against four 16-byte broadcast loads) and applies the four Lagrange
+// weights and (c_m, s_m) once per row.  C_n, S_n come from one sincos(nfp zeta) by recurrence and stay in
+// registers; c_m, s_m advance by the same recurrence from one sincos(theta) as the rows go by.
+//
+// Work distribution.  One cooperative persistent launch per gc_trace call.  Each epoch: block 0 turns the
+// per-cell counts into segment offsets, all threads scatter the running particles into `order`, blocks pull
+// tiles through an atomic counter and give every lane up to kTileCap attempted steps.  A lane whose particle
+// finishes, or whose home cell moves more than one cell away from the tile's, idles until the tile is written
+// back; a stage that needs a row outside the window reads the same image from global memory (identical
+// arithmetic, so a particle's result does not depend on who it shared a tile with).  Blocks that run out of
+// tiles keep advancing the tile they hold until every tile of the epoch has had its first chunk, so an epoch
+// has no idle tail.  Finished and lost particles simply stop being binned: that is the compaction.
+#pragma once
+#include <cooperative_groups.h>
+
+#include "device_math.cuh"
+#include "field.cuh"
+#include "kernels_generic.cuh"   // Profiles, gc_algebra, Dense3, poincare_emit
+
+namespace gc {
+
+namespace cgx = cooperative_groups;
+
+constexpr int kTileThreads = 128;      // particles per tile = threads per block
+constexpr int kTileCap = 32;           // attempted steps per lane per chunk
+constexpr int kRecDoubles = 16;        // one 128-byte record per particle
+
+// Per-call scratch of the tile kernel (device memory, owned by gc_trace for the duration of the call).
+struct TileScratch {
+  double* rec;      // [n][16]: y[4], k1[4], t, h, mu, attempts (int64), {status, flags}, {n_acc, n_rej}, {n_forced, cell}, -
+  int* order;       // [n]   running particles sorted by home cell
+  int* cnt;         // [ncell] running particles per home cell, accumulated for the NEXT binning
+  int* start;       // [ncell + 1] segment offsets into order
+  int* tstart;      // [ncell + 1] tile offsets
+  int* cursor;      // [ncell] scatter cursors
+  int* ctrl;        // [0] tile counter, [1] tiles past their first chunk, [2] tiles this epoch, [3] running
+};
+
+enum { kFlagPrevRejected = 1, kFlagHaveK1 = 2 };
+enum { kStRunning = -1, kStSkip = -2 };
+
+__constant__ double cDpA[7][6] = {
+    {0, 0, 0, 0, 0, 0},
+    {dp::a21, 0, 0, 0, 0, 0},
+    {dp::a31, dp::a32, 0, 0, 0, 0},
+    {dp::a41, dp::a42, dp::a43, 0, 0, 0},
+    {dp::a51, dp::a52, dp::a53, dp::a54, 0, 0},
+    {dp::a61, dp::a62, dp::a63, dp::a64, dp::a65, 0},
+    {dp::a71, 0.0, dp::a73, dp::a74, dp::a75, dp::a76}};
+__constant__ double cDpC[7] = {0.0, dp::c2, dp::c3, dp::c4, dp::c5, 1.0, 1.0};
+__constant__ double cDpE[7] = {dp::e1, 0.0, dp::e3, dp::e4, dp::e5, dp::e6, dp::e7};
+__constant__ double cDpD[7] = {dp::d1, 0.0, dp::d3, dp::d4, dp::d5, dp::d6, dp::d7};
+
+// ---- mbarrier / bulk-copy primitives (sm_90+ PTX; SASS: SYNCS / UBLKCP) ------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+
+// ---- loaders: four stencil values of one table entry -------------------------------------------------------------
+struct LdShared {
+  static __device__ __forceinline__ void ld4(const double* p, double (&v)[4]) {
+    const double2 a = *reinterpret_cast<const double2*>(p);
+    const double2 b = *reinterpret_cast<const double2*>(p + 2);
+    v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+  }
+};
+struct LdGlobal {
+  static __device__ __forceinline__ void ld4(const double* p, double (&v)[4]) {
+    const double2 a = __ldg(reinterpret_cast<const double2*>(p));
+    const double2 b = __ldg(reinterpret_cast<const double2*>(p + 2));
+    v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+  }
+};
+
+__device__ __forceinline__ double dot4(const double (&w)[4], const double (&v)[4]) {
+  return fma(w[3], v[3], fma(w[2], v[2], fma(w[1], v[1], w[0] * v[0])));
+}
+
+// Field quantities one right-hand side needs, as they come out of the table sweep.
+struct TileSums {
+  double B, Bs, Bth, Bze;       // Bze still lacks the factor nfp
+  Profiles pr;
+  double pt[9];                 // perturbation block (raw: psi-derivatives still d/ds)
+};
+
+// One sweep over the table entries of a stencil: rows m = 0..M of [b(m,0), (P,Q)(m,1), ..., (P,Q)(m,NMAX)], then
+// G, I, iota, then the mode amplitudes.  `e` points at the lane's first stencil value of entry 0; consecutive
+// entries are `stride` doubles apart.
+template <int NMAX, bool MODES, class Ld>
+__device__ __forceinline__ void table_sweep(const FieldDev& f, const double* e, int stride, const double (&w)[4],
+                                            const double (&dw)[4], double c1, double s1, const double (&C)[NMAX + 1],
+                                            const double (&S)[NMAX + 1], double thr, double zer, double t,
+                                            TileSums& o) {
+  double B = 0.0, Bs = 0.0, Bth = 0.0, Bze = 0.0;
+  double cm = 1.0, sm = 0.0;
+  const int M = f.M;
+#pragma unroll 1
+  for (int m = 0; m <= M; ++m) {
+    double PC[4], PS[4] = {0.0, 0.0, 0.0, 0.0}, QS[4] = {0.0, 0.0, 0.0, 0.0}, QC[4] = {0.0, 0.0, 0.0, 0.0};
+    Ld::ld4(e, PC);                                        // n = 0 column
+    e += stride;
+#pragma unroll
+    for (int n = 1; n <= NMAX; ++n) {
+      double P[4], Q[4];
+      Ld::ld4(e, P);
+      Ld::ld4(e + stride, Q);
+      e += 2 * stride;
+      const double nS = (double)n * S[n], nC = (double)n * C[n];
+#pragma unroll
+      for (int a = 0; a < 4; ++a) {
+        PC[a] = fma(P[a], C[n], PC[a]);
+        PS[a] = fma(P[a], nS, PS[a]);
+        QS[a] = fma(Q[a], S[n], QS[a]);
+        QC[a] = fma(Q[a], nC, QC[a]);
+      }
+    }
+    const double pc = dot4(w, PC), pcs = dot4(dw, PC), qs = dot4(w, QS), qss = dot4(dw, QS);
+    const double ps = dot4(w, PS), qc = dot4(w, QC);
+    B = fma(cm, pc, fma(sm, qs, B));
+    Bs = fma(cm, pcs, fma(sm, qss, Bs));
+    Bth = fma((double)m, fma(cm, qs, -sm * pc), Bth);
+    Bze = fma(sm, qc, fma(-cm, ps, Bze));
+    const double cn = fma(cm, c1, -sm * s1);
+    sm = fma(sm, c1, cm * s1);
+    cm = cn;
+  }
+  o.B = B; o.Bs = Bs; o.Bth = Bth; o.Bze = Bze;
+  double v[4];
+  Ld::ld4(e, v); o.pr.G = dot4(w, v); o.pr.Gs = dot4(dw, v); e += stride;
+  Ld::ld4(e, v); o.pr.I = dot4(w, v); o.pr.Is = dot4(dw, v); e += stride;
+  Ld::ld4(e, v); o.pr.io = dot4(w, v); o.pr.ios = dot4(dw, v); e += stride;
+#pragma unroll
+  for (int q = 0; q < 9; ++q) o.pt[q] = 0.0;
+  if constexpr (MODES) {
+    const Profiles& p = o.pr;
+    const double GI = p.G + p.io * p.I, GI_s = p.Gs + p.ios * p.I + p.io * p.Is;
+#pragma unroll 1
+    for (int k = 0; k < f.nk; ++k) {
+      Ld::ld4(e, v);
+      e += stride;
+      const double ph = dot4(w, v), ph_s = dot4(dw, v);
+      const double m = (double)__ldg(f.mode_m + k), n = (double)__ldg(f.mode_n + k);
+      const double om = __ldg(f.omega + k);
+      const double wt = reduce_2pi(om * t);
+      double sn, cs;
+      sincos_poly(fma(m, thr, fma(-n, zer, wt + __ldg(f.phase + k))), sn, cs);
+      const double inv = 1.0 / (om * GI);
+      const double Nk = fma(p.io, m, -n);
+      const double ah = -ph * Nk * inv;
+      const double ah_s = -(ph_s * Nk + ph * p.ios * m) * inv + ph * Nk * inv * (GI_s / GI);
+      o.pt[0] = fma(ph, sn, o.pt[0]);
+      o.pt[1] = fma(ph_s, sn, o.pt[1]);
+      o.pt[2] = fma(m * ph, cs, o.pt[2]);
+      o.pt[3] = fma(-n * ph, cs, o.pt[3]);
+      o.pt[4] = fma(ah, sn, o.pt[4]);
+      o.pt[5] = fma(ah_s, sn, o.pt[5]);
+      o.pt[6] = fma(m * ah, cs, o.pt[6]);
+      o.pt[7] = fma(-n * ah, cs, o.pt[7]);
+      o.pt[8] = fma(om * ah, cs, o.pt[8]);
+    }
+  }
+}
+
+// Right-hand side of one lane.  win = shared-memory image of the tile's cell ([E][6] rows cell-1..cell+4, then
+// [E][4] rows cell..cell+3); lanes whose stencil is not in the window read their own cell's image from global
+// memory.  Must be called by all 32 lanes of a warp; inactive lanes do nothing.
+template <int NMAX, bool MODES>
+__device__ __forceinline__ void rhs_tile(const FieldDev& f, const double* win, int cell, bool active, double mass,
+                                         double charge, double mu, double v_ref, double inv_v_ref, double t,
+                                         const double (&y)[4], double (&dy)[4]) {
+  int i0;
+  double w[4], dw[4];
+  lagrange_weights(f.ns, y[0], i0, w, dw);
+  const int off = i0 - cell + 1;
+  const bool inwin = active && off >= 0 && off <= 2;
+  const bool outside = active && !inwin;
+  const double thr = reduce_2pi(y[1]);
+  const double phr = reduce_2pi((double)f.nfp * y[2]);
+  double c1, s1, C[NMAX + 1], S[NMAX + 1];
+  sincos_poly(thr, s1, c1);
+  sincos_poly(phr, S[1], C[1]);
+  C[0] = 1.0; S[0] = 0.0;
+#pragma unroll
+  for (int n = 2; n <= NMAX; ++n) {
+    C[n] = fma(C[n - 1], C[1], -S[n - 1] * S[1]);
+    S[n] = fma(S[n - 1], C[1], C[n - 1] * S[1]);
+  }
+  const double zer = MODES ? reduce_2pi(y[2]) : 0.0;
+  TileSums o;
+  const int E = f.tile_E;
+  if (inwin) {
+    const double* e = (off == 1) ? win + 6 * E : win + off;     // off = 0 or 2: rows 0..3 or 2..5 of [E][6]
+    table_sweep<NMAX, MODES, LdShared>(f, e, off == 1 ? 4 : 6, w, dw, c1, s1, C, S, thr, zer, t, o);
+  }
+  if (__any_sync(0xffffffffu, outside)) {
+    if (outside) {
+      const double* e = f.tile_images + (size_t)i0 * (10 * E) + 6 * E;
+      table_sweep<NMAX, MODES, LdGlobal>(f, e, 4, w, dw, c1, s1, C, S, thr, zer, t, o);
+    }
+  }
+  if (active) {
+    const double fb[4] = {o.B, o.Bs, o.Bth, o.Bze * (double)f.nfp};
+    o.pt[1] *= f.inv_psi0;
+    o.pt[5] *= f.inv_psi0;
+    gc_algebra(mass, charge, mu, f.inv_psi0, y[3] * v_ref, fb, o.pr, o.pt, dy);
+    dy[3] *= inv_v_ref;
+  }
+}
+
+// L2-coherent 32-byte record accesses (the scratch is written by other blocks during the launch: bypass L1)
+__device__ __forceinline__ double4 ldcg4(const double* p) {
+  const double2 a = __ldcg(reinterpret_cast<const double2*>(p));
+  const double2 b = __ldcg(reinterpret_cast<const double2*>(p) + 1);
+  return make_double4(a.x, a.y, b.x, b.y);
+}
+__device__ __forceinline__ void stcg4(double* p, double4 v) {
+  __stcg(reinterpret_cast<double2*>(p), make_double2(v.x, v.y));
+  __stcg(reinterpret_cast<double2*>(p) + 1, make_double2(v.z, v.w));
+}
+
+__device__ __forceinline__ int home_cell(int ns, double s) { return stencil_start(ns, s * (double)(ns - 1)); }
+
+extern __shared__ __align__(128) unsigned char gc_tile_smem[];
+
+// mode 0: trace.  mode 1: right-hand side only (gc_rhs_eval): k1 of every particle goes to rhs_out[4][n].
+template <int NMAX, bool MODES>
+__global__ void __launch_bounds__(kTileThreads, 2)
+trace_tile_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_out) {
+  cgx::grid_group grid = cgx::this_grid();
+  const int tid = threadIdx.x;
+  const long long gtid = (long long)blockIdx.x * kTileThreads + tid;
+  const long long gthreads = (long long)gridDim.x * kTileThreads;
+  const int ncell = f.ns - 3;
+  const int E = f.tile_E;
+  constexpr double kTwoPi = 6.283185307179586476925286766559;
+
+  double* win = reinterpret_cast<double*>(gc_tile_smem);                 // [10 E]
+  double* kbuf = win + 10 * E;                                           // [7][4][kTileThreads]
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(kbuf + 7 * 4 * kTileThreads);
+  int* s_int = reinterpret_cast<int*>(bar + 1);                          // [0] tile id; scan space follows
+  auto kb = [&](int j, int c) -> double& { return kbuf[(j * 4 + c) * kTileThreads + tid]; };
+
+  if (tid == 0) mbar_init(bar, 1);
+  __syncthreads();
+  unsigned bar_phase = 0;
+
+  // ---- P0: records from the inputs (coalesced), first cell counts ------------------------------------------------
+  for (long long i = gtid; i < p.n; i += gthreads) {
+    double* r = sc.rec + i * kRecDoubles;
+    int st = kStRunning;
+    double y0, y1, y2, y3, h, t = p.t0, mu = p.mu[i];
+    if (mode == 1) {
+      y0 = p.s0[i]; y1 = p.th0[i]; y2 = p.ze0[i]; y3 = p.vpar0[i]; h = 0.0;
+    } else {
+      if (p.resume && p.status[i] != 0) st = kStSkip;
+      y0 = p.s0[i]; y1 = p.th0[i]; y2 = p.ze0[i]; y3 = p.vpar0[i] * p.inv_v_ref;
+      h = (p.h_inout && p.h_inout[i] > 0.0) ? p.h_inout[i] : p.h0;
+      if (h < p.h_min) h = p.h_min;
+    }
+    const int cell = home_cell(f.ns, y0);
+    reinterpret_cast<double4*>(r)[0] = make_double4(y0, y1, y2, y3);
+    reinterpret_cast<double4*>(r)[1] = make_double4(0.0, 0.0, 0.0, 0.0);
+    reinterpret_cast<double4*>(r)[2] = make_double4(t, h, mu, __longlong_as_double(0LL));
+    int4 a = make_int4(st, 0, 0, 0), b = make_int4(0, cell, 0, 0);
+    reinterpret_cast<int4*>(r + 12)[0] = a;
+    reinterpret_cast<int4*>(r + 12)[1] = b;
+    if (st == kStRunning) atomicAdd(sc.cnt + cell, 1);
+  }
+  grid.sync();
+
+  for (;;) {
+    // ---- B: segment and tile offsets (block 0) -------------------------------------------------------------------
+    if (blockIdx.x == 0) {
+      int* wsp = reinterpret_cast<int*>(win);                            // 3 ncell ints staged in the window space
+      for (int c = tid; c < ncell; c += kTileThreads) { wsp[c] = __ldcg(sc.cnt + c); sc.cnt[c] = 0; }
+      __syncthreads();
+      if (tid == 0) {
+        int run = 0, tiles = 0;
+        for (int c = 0; c < ncell; ++c) {
+          const int k = wsp[c];
+          wsp[ncell + c] = run;
+          wsp[2 * ncell + c] = tiles;
+          run += k;
+          tiles += (k + kTileThreads - 1) / kTileThreads;
+        }
+        sc.start[ncell] = run;
+        sc.tstart[ncell] = tiles;
+        sc.ctrl[0] = 0; sc.ctrl[1] = 0; sc.ctrl[2] = tiles; sc.ctrl[3] = run;
+      }
+      __syncthreads();
+      for (int c = tid; c < ncell; c += kTileThreads) {
+        sc.start[c] = wsp[ncell + c];
+        sc.cursor[c] = wsp[ncell + c];
+        sc.tstart[c] = wsp[2 * ncell + c];
+      }
+      __syncthreads();
+    }
+    grid.sync();
+    const int ntiles = __ldcg(sc.ctrl + 2);
+    if (__ldcg(sc.ctrl + 3) == 0) break;
+
+    // ---- C: scatter the running particles into cell order --------------------------------------------------------
+    for (long long i = gtid; i < p.n; i += gthreads) {
+      const int2 sf = __ldcg(reinterpret_cast<const int2*>(sc.rec + i * kRecDoubles + 12));
+      if (sf.x == kStRunning) {
+        const int cell = __ldcg(reinterpret_cast<const int2*>(sc.rec + i * kRecDoubles + 14)).y;
+        sc.order[atomicAdd(sc.cursor + cell, 1)] = (int)i;
+      }
+    }
+    grid.sync();
+
+    // ---- D: tiles ------------------------------------------------------------------------------------------------
+    int cur_cell = -1;
+    for (;;) {
+      __syncthreads();
+      if (tid == 0) s_int[0] = atomicAdd(sc.ctrl + 0, 1);
+      __syncthreads();
+      const int tile = s_int[0];
+      if (tile >= ntiles) break;
+      int lo = 0, hi = ncell - 1;                                        // largest c with tstart[c] <= tile
+      while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (__ldcg(sc.tstart + mid) <= tile) lo = mid; else hi = mid - 1;
+      }
+      const int cell = lo;
+      const int seg0 = __ldcg(sc.start + cell), seg1 = __ldcg(sc.start + cell + 1);
+      const int begin = seg0 + (tile - __ldcg(sc.tstart + cell)) * kTileThreads;
+      const int count = min(kTileThreads, seg1 - begin);
+      if (cell != cur_cell) {                                            // stage the window: one bulk copy
+        if (tid == 0) {
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          const unsigned bytes = (unsigned)(10 * E * sizeof(double));
+          mbar_expect_tx(bar, bytes);
+          bulk_g2s(win, f.tile_images + (size_t)cell * (10 * E), bytes, bar);
+        }
+        mbar_wait(bar, bar_phase);
+        bar_phase ^= 1u;
+        cur_cell = cell;
+      }
+
+      // lane state
+      bool active = tid < count;
+      long long pid = 0;
+      double y[4] = {0.0, 0.0, 0.0, 0.0}, t = 0.0, h = 0.0, mu = 0.0;
+      long long attempts = 0;
+      int st = 0, flags = 0, n_acc = 0, n_rej = 0, n_forced = 0;
+      if (active) {
+        pid = __ldcg(sc.order + begin + tid);
+        const double* r = sc.rec + pid * kRecDoubles;
+        const double4 a = ldcg4(r);
+        const double4 b = ldcg4(r + 4);
+        const double4 c = ldcg4(r + 8);
+        const int4 d = __ldcg(reinterpret_cast<const int4*>(r + 12));
+        const int4 g = __ldcg(reinterpret_cast<const int4*>(r + 12) + 1);
+        y[0] = a.x; y[1] = a.y; y[2] = a.z; y[3] = a.w;
+        kb(0, 0) = b.x; kb(0, 1) = b.y; kb(0, 2) = b.z; kb(0, 3) = b.w;
+        t = c.x; h = c.y; mu = c.z; attempts = __double_as_longlong(c.w);
+        st = d.x; flags = d.y; n_acc = d.z; n_rej = d.w; n_forced = g.x;
+      }
+      bool running = active;                     // false once finished or parked
+      bool first_chunk = true;
+
+      for (;;) {                                 // chunks of kTileCap attempts
+#pragma unroll 1
+        for (int att = 0; att < kTileCap; ++att) {
+          if (!__any_sync(0xffffffffu, running)) break;
+          // stage 0 gives k1 to lanes that do not carry one yet (first epoch; gc_rhs_eval)
+          const bool do_k1 = __any_sync(0xffffffffu, running && !(flags & kFlagHaveK1));
+          double h_try = h, yn[4] = {y[0], y[1], y[2], y[3]};
+          bool clipped = false;
+          const bool forced = (flags & kFlagPrevRejected) && p.h_min > 0.0 && h == p.h_min;
+          if (mode == 0 && running && t < p.t_max) {
+            if (t + h_try >= p.t_max) { h_try = p.t_max - t; clipped = true; }
+            if (!(t + h_try > t)) { st = GC_ST_NONFINITE_; running = false; }       // step underflow
+          }
+#pragma unroll 1
+          for (int stage = do_k1 ? 0 : 1; stage <= 6; ++stage) {
+            if (stage > 0 && !__any_sync(0xffffffffu, running)) break;
+            double ys[4], ts;
+            if (stage == 0) {
+              ys[0] = y[0]; ys[1] = y[1]; ys[2] = y[2]; ys[3] = y[3];
+              ts = t;
+            } else {
+              double acc[4] = {0.0, 0.0, 0.0, 0.0};
+              for (int j = 0; j < stage; ++j) {
+                const double a = cDpA[stage][j];
+#pragma unroll
+                for (int c = 0; c < 4; ++c) acc[c] = fma(a, kb(j, c), acc[c]);
+              }
+#pragma unroll
+              for (int c = 0; c < 4; ++c) ys[c] = fma(h_try, acc[c], y[c]);
+              ts = fma(cDpC[stage], h_try, t);
+              if (stage == 6) { yn[0] = ys[0]; yn[1] = ys[1]; yn[2] = ys[2]; yn[3] = ys[3]; }
+            }
+            double dy[4] = {0.0, 0.0, 0.0, 0.0};
+            const bool lane_on = running && (stage > 0 || !(flags & kFlagHaveK1));
+            rhs_tile<NMAX, MODES>(f, win, cell, lane_on, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, ts, ys, dy);
+            if (lane_on) {
+              kb(stage, 0) = dy[0]; kb(stage, 1) = dy[1]; kb(stage, 2) = dy[2]; kb(stage, 3) = dy[3];
+              if (stage == 0) {
+                flags |= kFlagHaveK1;
+                if (mode == 1) {
+#pragma unroll
+                  for (int c = 0; c < 4; ++c) rhs_out[(long long)c * p.n + pid] = dy[c];
+                  st = 0; running = false;
+                } else if (!finite4(y[0], y[1], y[2], y[3]) || !finite4(dy[0], dy[1], dy[2], dy[3])) {
+                  st = GC_ST_NONFINITE_; running = false;
+                } else if (!(t < p.t_max)) {
+                  st = 0; running = false;
+                }
+              }
+            }
+          }
+          if (running) {
+            ++attempts;
+            double accn = 0.0;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              double e = 0.0;
+              for (int j = 0; j < 7; ++j) e = fma(cDpE[j], kb(j, c), e);
+              const double delta = h_try * e;
+              const double sk = fma(p.rtol, fmax(fabs(y[c]), fabs(yn[c])), p.atol);
+              const double r = delta / sk;
+              accn = fma(r, r, accn);
+            }
+            const double err = sqrt(accn * 0.25);
+            const bool finite = finite4(yn[0], yn[1], yn[2], yn[3]) &&
+                                finite4(kb(6, 0), kb(6, 1), kb(6, 2), kb(6, 3)) && isfinite(err);
+            bool accept;
+            if (forced) {
+              accept = finite;
+              if (!finite) { st = GC_ST_NONFINITE_; running = false; }
+            } else {
+              accept = finite && err <= 1.0;
+            }
+            if (running && accept) {
+              const double scl = scale_after_accept(err);
+              const double h_next = (flags & kFlagPrevRejected) ? h_try * fmin(scl, 1.0) : h_try * scl;
+              if (p.poincare_capacity > 0 && floor(y[2] / kTwoPi) != floor(yn[2] / kTwoPi)) {
+                Dense3 d;
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                  double dd = 0.0;
+                  for (int j = 0; j < 7; ++j) dd = fma(cDpD[j], kb(j, c), dd);
+                  d.r1[c] = y[c];
+                  d.r2[c] = yn[c] - y[c];
+                  d.r3[c] = h_try * kb(0, c) - d.r2[c];
+                  d.r4[c] = d.r2[c] - h_try * kb(6, c) - d.r3[c];
+                  d.r5[c] = h_try * dd;
+                }
+                poincare_emit(d, pid, t, h_try, y[2], yn[2], p.poincare, p.poincare_capacity, p.poincare_count);
+              }
+              t = clipped ? p.t_max : t + h_try;
+#pragma unroll
+              for (int c = 0; c < 4; ++c) { y[c] = yn[c]; kb(0, c) = kb(6, c); }
+              ++n_acc;
+              if (forced) ++n_forced;
+              flags &= ~kFlagPrevRejected;
+              if (!clipped) h = h_next;
+              if (h < p.h_min) h = p.h_min;
+              if (y[0] >= p.s_loss) st = 1;
+              else if (y[0] <= p.s_min) st = 2;
+              else if (clipped) st = 0;
+              else if (attempts >= p.max_steps) st = 3;
+              if (st != kStRunning) running = false;
+              else {
+                const int hc = home_cell(f.ns, y[0]);
+                if (hc < cell - 1 || hc > cell + 1) running = false;      // parked until the next binning
+              }
+            } else if (running) {
+              ++n_rej;
+              h = h_try * scale_after_reject(err);
+              if (h < p.h_min) h = p.h_min;
+              flags |= kFlagPrevRejected;
+              if (attempts >= p.max_steps) { st = 3; running = false; }
+            }
+          }
+        }
+        // another chunk on the same tile only while other blocks still work on their first chunk
+        if (first_chunk && tid == 0) atomicAdd(sc.ctrl + 1, 1);
+        first_chunk = false;
+        const int nrun = __syncthreads_count(running);
+        bool more = false;
+        if (nrun * 2 >= kTileThreads) {
+          const volatile int* vc = sc.ctrl;
+          more = vc[0] >= ntiles && vc[1] < ntiles;
+        }
+        if (tid == 0) s_int[1] = more;
+        __syncthreads();
+        if (!s_int[1]) break;
+      }
+
+      // write the tile back
+      if (active) {
+        double* r = sc.rec + pid * kRecDoubles;
+        const int hc = home_cell(f.ns, y[0]);
+        stcg4(r, make_double4(y[0], y[1], y[2], y[3]));
+        stcg4(r + 4, make_double4(kb(0, 0), kb(0, 1), kb(0, 2), kb(0, 3)));
+        stcg4(r + 8, make_double4(t, h, mu, __longlong_as_double(attempts)));
+        __stcg(reinterpret_cast<int4*>(r + 12), make_int4(st, flags, n_acc, n_rej));
+        __stcg(reinterpret_cast<int4*>(r + 12) + 1, make_int4(n_forced, hc, 0, 0));
+        if (st == kStRunning) atomicAdd(sc.cnt + hc, 1);
+      }
+    }
+    grid.sync();
+  }
+
+  // ---- outputs (coalesced) -------------------------------------------------------------------------------------
+  if (mode == 0) {
+    for (long long i = gtid; i < p.n; i += gthreads) {
+      const double* r = sc.rec + i * kRecDoubles;
+      const int4 d = __ldcg(reinterpret_cast<const int4*>(r + 12));
+      if (d.x == kStSkip) continue;
+      const double4 a = ldcg4(r);
+      const double4 c = ldcg4(r + 8);
+      const int n_forced = __ldcg(reinterpret_cast<const int4*>(r + 12) + 1).x;
+      p.y_out[i] = a.x;
+      p.y_out[p.n + i] = a.y;
+      p.y_out[2 * p.n + i] = a.z;
+      p.y_out[3 * p.n + i] = a.w * p.v_ref;
+      p.t_out[i] = c.x;
+      p.status[i] = d.x;
+      if (p.h_inout) p.h_inout[i] = c.y;
+      if (p.n_acc) p.n_acc[i] = (p.resume ? p.n_acc[i] : 0) + d.z;
+      if (p.n_rej) p.n_rej[i] = (p.resume ? p.n_rej[i] : 0) + d.w;
+      if (p.n_forced) p.n_forced[i] = (p.resume ? p.n_forced[i] : 0) + n_forced;
+    }
+  }
+}
+
+}  // namespace gc

@@ -16,7 +16,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 SO_PATH = os.path.join(_HERE, "libgcorbit.so")
 
 GC_OK, GC_EINVAL, GC_ENOMEM, GC_ECUDA = 0, -1, -2, -3
-GC_KERNEL_AUTO, GC_KERNEL_GENERIC, GC_KERNEL_WARP = 0, 1, 2
+GC_KERNEL_AUTO, GC_KERNEL_GENERIC, GC_KERNEL_WARP, GC_KERNEL_TILE = 0, 1, 2, 3
+GC_TILE_MIN_PARTICLES = 8192
 ST_TMAX, ST_LOST, ST_AXIS, ST_MAXSTEPS, ST_NONFINITE = 0, 1, 2, 3, 4
 
 EXPORTS = ["gc_field_create", "gc_field_destroy", "gc_field_eval", "gc_pert_eval", "gc_rhs_eval", "gc_trace",
@@ -66,7 +67,7 @@ def load_library():
         L.gc_trace.argtypes = [vp, C.POINTER(gc_trace_params), i64] + [vp] * 15
         L.gc_trace_host.argtypes = [vp, C.POINTER(gc_trace_params), i64] + [vp] * 14
         L.gc_set_kernel.argtypes = [vp, i32]
-        L.gc_kernel_info.argtypes = [vp] + [C.POINTER(i32)] * 5
+        L.gc_kernel_info.argtypes = [vp, C.c_int64] + [C.POINTER(i32)] * 5
         L.gc_fp64_peak_probe.argtypes = [C.POINTER(dbl), C.POINTER(dbl)]
         for name in EXPORTS:
             if name != "gc_last_error":
@@ -161,10 +162,11 @@ class Field:
     def set_kernel(self, kernel: int):
         _check(load_library().gc_set_kernel(self._h, kernel))
 
-    def kernel_info(self) -> dict:
+    def kernel_info(self, n: int = 1 << 20) -> dict:
+        """Kernel and launch geometry gc_trace uses for an ensemble of n particles."""
         v = [C.c_int32(0) for _ in range(5)]
-        _check(load_library().gc_kernel_info(self._h, *[C.byref(x) for x in v]))
-        return dict(kernel={GC_KERNEL_GENERIC: "generic", GC_KERNEL_WARP: "warp"}[v[0].value],
+        _check(load_library().gc_kernel_info(self._h, int(n), *[C.byref(x) for x in v]))
+        return dict(kernel={GC_KERNEL_GENERIC: "generic", GC_KERNEL_WARP: "warp", GC_KERNEL_TILE: "tile"}[v[0].value],
                     blocks=v[1].value, threads=v[2].value, smem_bytes=v[3].value, regs=v[4].value)
 
     # ---- gc_field_eval / gc_pert_eval / gc_rhs_eval (device tensors in, device tensors out) ------------------

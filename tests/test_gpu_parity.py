@@ -10,12 +10,13 @@ from gpu_common import (COND_FACTOR, FLIP_RTOL, SAME_RTOL, assert_trace_parity, 
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = ["generic", "warp"]
+KERNELS = ["generic", "warp", "tile"]
 
 
 def _set_kernel(GF, name):
     from paper_2605_16734_b200 import gcorbit as G
-    GF.set_kernel({"generic": G.GC_KERNEL_GENERIC, "warp": G.GC_KERNEL_WARP}[name])
+    GF.set_kernel({"generic": G.GC_KERNEL_GENERIC, "warp": G.GC_KERNEL_WARP, "tile": G.GC_KERNEL_TILE,
+                   "auto": G.GC_KERNEL_AUTO}[name])
 
 
 @pytest.fixture(scope="module")
@@ -86,7 +87,7 @@ def test_rhs_matches_oracle(cases, config, kernel):
     for c in range(4):
         scale = np.maximum(np.abs(ref[c]), 1e-6 * np.abs(ref[c]).max())
         assert (np.abs(got[c] - ref[c]) / scale).max() < 1e-9, (c, (np.abs(got[c] - ref[c]) / scale).max())
-    _set_kernel(GF, "warp")
+    _set_kernel(GF, "auto")
 
 
 # ---- O5-O7: the trace ---------------------------------------------------------------------------------------------
@@ -113,18 +114,27 @@ def test_trace_config0_full(cases, kernel):
     # 1e-4 s is ~3000 steps: ~1-2 % of the particles are ill-conditioned in the oracle itself (gpu_common)
     info = assert_trace_parity(r, o, spec, label=f"config 0 {kernel}", cond=cond, min_within=0.95)
     print(f"config 0 {kernel}: {info}, attempts {int(o.n_acc.sum() + o.n_rej.sum())}")
-    _set_kernel(GF, "warp")
+    _set_kernel(GF, "auto")
 
 
+_SUB = {}
+
+
+@pytest.mark.parametrize("kernel", ["warp", "tile"])
 @pytest.mark.parametrize("config,n,t_max", [(1, 296, 2e-5), (2, 256, 2e-5), (3, 301, 3e-5), (4, 256, 2e-5)])
-def test_trace_subsamples(cases, config, n, t_max):
-    """Short-horizon subsamples of configs 1-4 (n chosen ragged against 8 warps per block)."""
+def test_trace_subsamples(cases, config, n, t_max, kernel):
+    """Short-horizon subsamples of configs 1-4 (n chosen ragged against 8 warps per block and 128-particle
+    tiles), hot-path kernels."""
     fld, spec, P, OF, GF, mu = cases(config, n)
     cap = 4096 if config == 4 else 0
+    _set_kernel(GF, kernel)
     r = gpu_trace(GF, spec, P, mu, t_max=t_max, poincare_capacity=cap)
-    o = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=t_max, poincare_capacity=cap)
-    cond = oracle_conditioning(OF, spec, P, mu, o, t_max=t_max)
-    info = assert_trace_parity(r, o, spec, label=f"config {config}", cond=cond, min_within=0.99)
+    _set_kernel(GF, "auto")
+    if config not in _SUB:
+        o = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=t_max, poincare_capacity=cap)
+        _SUB[config] = (o, oracle_conditioning(OF, spec, P, mu, o, t_max=t_max))
+    o, cond = _SUB[config]
+    info = assert_trace_parity(r, o, spec, label=f"config {config} {kernel}", cond=cond, min_within=0.99)
     print(f"config {config}: {info}")
     if cap:
         # O8: same crossings (record order is unspecified: compare sorted by particle, time)
@@ -145,15 +155,19 @@ def test_trace_generic_kernel_with_modes(cases):
     o = OF.trace(spec, Q.s, Q.theta, Q.zeta, Q.vpar, mu[:64], t_max=1e-5)
     cond = oracle_conditioning(OF, spec, Q, mu[:64], o, t_max=1e-5)
     assert_trace_parity(r, o, spec, min_same=0.95, label="config 2 generic", cond=cond, min_within=0.98)
-    _set_kernel(GF, "warp")
+    _set_kernel(GF, "auto")
 
 
+@pytest.mark.parametrize("kernel", ["warp", "tile"])
 @pytest.mark.parametrize("n", [1, 7, 33, 148 * 8 + 3])
-def test_trace_ragged_sizes(cases, n):
-    """One particle, fewer particles than warps in a block, and one more wave than the persistent grid holds."""
+def test_trace_ragged_sizes(cases, n, kernel):
+    """One particle, fewer particles than warps in a block / lanes in a tile, and one more wave than the
+    persistent grid holds."""
     fld, spec, P, OF, GF, mu = cases(0, 148 * 8 + 3)
     Q = P.head(n)
+    _set_kernel(GF, kernel)
     r = gpu_trace(GF, spec, Q, mu[:n], t_max=3e-6)
+    _set_kernel(GF, "auto")
     o = OF.trace(spec, Q.s, Q.theta, Q.zeta, Q.vpar, mu[:n], t_max=3e-6)
     cond = oracle_conditioning(OF, spec, Q, mu[:n], o, t_max=3e-6)
     assert_trace_parity(r, o, spec, min_same=0.0 if n < 100 else 0.99, label=f"n={n}", cond=cond)
@@ -165,6 +179,7 @@ def test_full_size_launch_sampled(cases):
     import torch
     from paper_2605_16734_b200 import gcorbit as G
     fld, spec, P, OF, GF, _ = cases(1, 64)          # fields only; the full ensemble is drawn here
+    assert GF.kernel_info(100_000)["kernel"] == "tile"
     from paper_2605_16734_b200 import workloads as W
     P = W.make_particles(1)
     assert P.n == 100_000

@@ -352,11 +352,11 @@ trace_tile_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_
 
     // ---- D: tiles ------------------------------------------------------------------------------------------------
     int cur_cell = -1;
+    __syncthreads();
+    if (tid == 0) s_int[0] = atomicAdd(sc.ctrl + 0, 1);
+    __syncthreads();
     for (;;) {
-      __syncthreads();
-      if (tid == 0) s_int[0] = atomicAdd(sc.ctrl + 0, 1);
-      __syncthreads();
-      const int tile = s_int[0];
+      const int tile = s_int[0];                                         // grabbed before the loop / at chunk end
       if (tile >= ntiles) break;
       int lo = 0, hi = ncell - 1;                                        // largest c with tstart[c] <= tile
       while (lo < hi) {
@@ -400,11 +400,17 @@ trace_tile_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_
       }
       bool running = active;                     // false once finished or parked
       bool first_chunk = true;
+      bool extra = false;                        // an extra chunk: stop as soon as the epoch's first chunks are done
 
       for (;;) {                                 // chunks of kTileCap attempts
 #pragma unroll 1
         for (int att = 0; att < kTileCap; ++att) {
           if (!__any_sync(0xffffffffu, running)) break;
+          if (extra) {                           // attempts are warp-local: any warp may stop at any attempt
+            int done = 0;
+            if ((tid & 31) == 0) done = *reinterpret_cast<const volatile int*>(sc.ctrl + 1);
+            if (__shfl_sync(0xffffffffu, done, 0) >= ntiles) break;
+          }
           // stage 0 gives k1 to lanes that do not carry one yet (first epoch; gc_rhs_eval)
           const bool do_k1 = __any_sync(0xffffffffu, running && !(flags & kFlagHaveK1));
           double h_try = h, yn[4] = {y[0], y[1], y[2], y[3]};
@@ -517,20 +523,25 @@ trace_tile_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_
             }
           }
         }
-        // another chunk on the same tile only while other blocks still work on their first chunk
+        // chunk end: take the next tile if there is one; if the epoch's tiles are all handed out, keep
+        // advancing this one while other blocks still work on a first chunk (no idle tail)
         if (first_chunk && tid == 0) atomicAdd(sc.ctrl + 1, 1);
         first_chunk = false;
         const int nrun = __syncthreads_count(running);
-        bool more = false;
-        if (nrun * 2 >= kTileThreads) {
-          const volatile int* vc = sc.ctrl;
-          more = vc[0] >= ntiles && vc[1] < ntiles;
+        if (tid == 0) {
+          const int next = atomicAdd(sc.ctrl + 0, 1);
+          bool more = false;
+          if (next >= ntiles && nrun * 2 >= kTileThreads) {
+            const volatile int* vc = sc.ctrl;
+            more = vc[1] < ntiles;
+          }
+          s_int[0] = next;
+          s_int[1] = more;
         }
-        if (tid == 0) s_int[1] = more;
         __syncthreads();
         if (!s_int[1]) break;
+        extra = true;
       }
-
       // write the tile back
       if (active) {
         double* r = sc.rec + pid * kRecDoubles;
@@ -542,6 +553,7 @@ trace_tile_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_
         __stcg(reinterpret_cast<int4*>(r + 12) + 1, make_int4(n_forced, hc, 0, 0));
         if (st == kStRunning) atomicAdd(sc.cnt + hc, 1);
       }
+      __syncthreads();                                                   // window / kbuf / s_int are reused
     }
     grid.sync();
   }

@@ -196,7 +196,7 @@ int pack_tile_images(gc_field* f, const gc_field_desc* d) {
   const int smem = (int)((size_t)10 * E * sizeof(double) + (size_t)7 * 4 * gc::kTileThreads * sizeof(double) + 64);
   if (smem > 110 * 1024) return GC_OK;                     // two blocks per SM must fit
   const int ncell = d->ns - 3;
-  if ((size_t)3 * ncell * sizeof(int) > (size_t)10 * E * sizeof(double)) return GC_OK;   // scan space (phase B)
+  if ((size_t)(gc::kSubBins + 2) * ncell * sizeof(int) > (size_t)10 * E * sizeof(double)) return GC_OK;   // scan space (phase B)
   // node-major entry rows first
   std::vector<double> rows((size_t)d->ns * E, 0.0);
   for (int node = 0; node < d->ns; ++node) {
@@ -253,19 +253,20 @@ int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, c
   const int ncell = f->dev.ns - 3;
   const size_t n = (size_t)t.n;
   const size_t rec_bytes = n * gc::kRecDoubles * sizeof(double);
-  const size_t int_count = n + (size_t)4 * (ncell + 1) + 8;
+  const size_t nbin = (size_t)ncell * gc::kSubBins;
+  const size_t int_count = n + 2 * nbin + (size_t)2 * (ncell + 1) + 8;
   unsigned char* slab = nullptr;
   GC_CUDA(cudaMallocAsync((void**)&slab, rec_bytes + int_count * sizeof(int), st));
   gc::TileScratch sc{};
   sc.rec = reinterpret_cast<double*>(slab);
   int* ip = reinterpret_cast<int*>(slab + rec_bytes);
   sc.order = ip; ip += n;
-  sc.cnt = ip; ip += ncell + 1;
+  sc.cnt = ip; ip += nbin;
+  sc.cursor = ip; ip += nbin;
   sc.start = ip; ip += ncell + 1;
   sc.tstart = ip; ip += ncell + 1;
-  sc.cursor = ip; ip += ncell + 1;
   sc.ctrl = ip;
-  GC_CUDA(cudaMemsetAsync(sc.cnt, 0, ((size_t)4 * (ncell + 1) + 8) * sizeof(int), st));
+  GC_CUDA(cudaMemsetAsync(sc.cnt, 0, (2 * nbin + (size_t)2 * (ncell + 1) + 8) * sizeof(int), st));
   long long blocks = (long long)f->sm_count * f->tile_blocks_per_sm;
   const long long need = ((long long)n + gc::kTileThreads - 1) / gc::kTileThreads;
   if (blocks > need) blocks = need;

@@ -40,15 +40,16 @@ namespace cgx = cooperative_groups;
 constexpr int kTileThreads = 128;      // particles per tile = threads per block
 constexpr int kTileCap = 32;           // attempted steps per lane per chunk
 constexpr int kRecDoubles = 16;        // one 128-byte record per particle
+constexpr int kSubBins = 8;            // radial sub-bins per cell: tiles come out ordered in s (lane coherence)
 
 // Per-call scratch of the tile kernel (device memory, owned by gc_trace for the duration of the call).
 struct TileScratch {
-  double* rec;      // [n][16]: y[4], k1[4], t, h, mu, attempts (int64), {status, flags}, {n_acc, n_rej}, {n_forced, cell}, -
+  double* rec;      // [n][16]: y[4], k1[4], t, h, mu, attempts (int64), {status, flags}, {n_acc, n_rej}, {n_forced, bin}, -
   int* order;       // [n]   running particles sorted by home cell
-  int* cnt;         // [ncell] running particles per home cell, accumulated for the NEXT binning
-  int* start;       // [ncell + 1] segment offsets into order
+  int* cnt;         // [ncell kSubBins] running particles per bin (home cell, radial sub-bin), for the NEXT binning
+  int* start;       // [ncell + 1] cell segment offsets into order
   int* tstart;      // [ncell + 1] tile offsets
-  int* cursor;      // [ncell] scatter cursors
+  int* cursor;      // [ncell kSubBins] scatter cursors
   int* ctrl;        // [0] tile counter, [1] tiles past their first chunk, [2] tiles this epoch, [3] running
 };
 
@@ -261,6 +262,17 @@ __device__ __forceinline__ void stcg4(double* p, double4 v) {
 
 __device__ __forceinline__ int home_cell(int ns, double s) { return stencil_start(ns, s * (double)(ns - 1)); }
 
+// Bin = home cell * kSubBins + radial sub-bin.  The sub-bin only orders the particles of a cell by s, so that
+// neighbouring lanes of a tile use the same stencil offset most of the time (shared-memory loads of a lane pair
+// merge when both read the same 16 bytes); it has no influence on any particle's arithmetic.
+__device__ __forceinline__ int home_bin(int ns, double s) {
+  const double u = s * (double)(ns - 1);
+  const int cell = stencil_start(ns, u);
+  double fr = (u - (double)(cell + 1)) * (double)kSubBins;          // interior: u in [cell + 1, cell + 2)
+  int sub = fr >= 0.0 ? (fr < (double)kSubBins ? (int)fr : kSubBins - 1) : 0;   // NaN -> 0
+  return cell * kSubBins + sub;
+}
+
 extern __shared__ __align__(128) unsigned char gc_tile_smem[];
 
 // mode 0: trace.  mode 1: right-hand side only (gc_rhs_eval): k1 of every particle goes to rhs_out[4][n].
@@ -298,41 +310,46 @@ trace_tile_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_
       h = (p.h_inout && p.h_inout[i] > 0.0) ? p.h_inout[i] : p.h0;
       if (h < p.h_min) h = p.h_min;
     }
-    const int cell = home_cell(f.ns, y0);
+    const int bin = home_bin(f.ns, y0);
     reinterpret_cast<double4*>(r)[0] = make_double4(y0, y1, y2, y3);
     reinterpret_cast<double4*>(r)[1] = make_double4(0.0, 0.0, 0.0, 0.0);
     reinterpret_cast<double4*>(r)[2] = make_double4(t, h, mu, __longlong_as_double(0LL));
-    int4 a = make_int4(st, 0, 0, 0), b = make_int4(0, cell, 0, 0);
+    int4 a = make_int4(st, 0, 0, 0), b = make_int4(0, bin, 0, 0);
     reinterpret_cast<int4*>(r + 12)[0] = a;
     reinterpret_cast<int4*>(r + 12)[1] = b;
-    if (st == kStRunning) atomicAdd(sc.cnt + cell, 1);
+    if (st == kStRunning) atomicAdd(sc.cnt + bin, 1);
   }
   grid.sync();
 
   for (;;) {
     // ---- B: segment and tile offsets (block 0) -------------------------------------------------------------------
     if (blockIdx.x == 0) {
-      int* wsp = reinterpret_cast<int*>(win);                            // 3 ncell ints staged in the window space
-      for (int c = tid; c < ncell; c += kTileThreads) { wsp[c] = __ldcg(sc.cnt + c); sc.cnt[c] = 0; }
+      int* wsp = reinterpret_cast<int*>(win);                            // nbin + 2 ncell ints staged in the window space
+      const int nbin = ncell * kSubBins;
+      for (int b = tid; b < nbin; b += kTileThreads) { wsp[b] = __ldcg(sc.cnt + b); sc.cnt[b] = 0; }
       __syncthreads();
       if (tid == 0) {
         int run = 0, tiles = 0;
         for (int c = 0; c < ncell; ++c) {
-          const int k = wsp[c];
-          wsp[ncell + c] = run;
-          wsp[2 * ncell + c] = tiles;
-          run += k;
-          tiles += (k + kTileThreads - 1) / kTileThreads;
+          wsp[nbin + c] = run;
+          wsp[nbin + ncell + c] = tiles;
+          const int run0 = run;
+          for (int b = c * kSubBins; b < (c + 1) * kSubBins; ++b) {      // counts become scatter cursors in place
+            const int k = wsp[b];
+            wsp[b] = run;
+            run += k;
+          }
+          tiles += (run - run0 + kTileThreads - 1) / kTileThreads;
         }
         sc.start[ncell] = run;
         sc.tstart[ncell] = tiles;
         sc.ctrl[0] = 0; sc.ctrl[1] = 0; sc.ctrl[2] = tiles; sc.ctrl[3] = run;
       }
       __syncthreads();
+      for (int b = tid; b < nbin; b += kTileThreads) sc.cursor[b] = wsp[b];
       for (int c = tid; c < ncell; c += kTileThreads) {
-        sc.start[c] = wsp[ncell + c];
-        sc.cursor[c] = wsp[ncell + c];
-        sc.tstart[c] = wsp[2 * ncell + c];
+        sc.start[c] = wsp[nbin + c];
+        sc.tstart[c] = wsp[nbin + ncell + c];
       }
       __syncthreads();
     }
@@ -344,8 +361,8 @@ trace_tile_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_
     for (long long i = gtid; i < p.n; i += gthreads) {
       const int2 sf = __ldcg(reinterpret_cast<const int2*>(sc.rec + i * kRecDoubles + 12));
       if (sf.x == kStRunning) {
-        const int cell = __ldcg(reinterpret_cast<const int2*>(sc.rec + i * kRecDoubles + 14)).y;
-        sc.order[atomicAdd(sc.cursor + cell, 1)] = (int)i;
+        const int bin = __ldcg(reinterpret_cast<const int2*>(sc.rec + i * kRecDoubles + 14)).y;
+        sc.order[atomicAdd(sc.cursor + bin, 1)] = (int)i;
       }
     }
     grid.sync();
@@ -545,13 +562,13 @@ trace_tile_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_
       // write the tile back
       if (active) {
         double* r = sc.rec + pid * kRecDoubles;
-        const int hc = home_cell(f.ns, y[0]);
+        const int hb = home_bin(f.ns, y[0]);
         stcg4(r, make_double4(y[0], y[1], y[2], y[3]));
         stcg4(r + 4, make_double4(kb(0, 0), kb(0, 1), kb(0, 2), kb(0, 3)));
         stcg4(r + 8, make_double4(t, h, mu, __longlong_as_double(attempts)));
         __stcg(reinterpret_cast<int4*>(r + 12), make_int4(st, flags, n_acc, n_rej));
-        __stcg(reinterpret_cast<int4*>(r + 12) + 1, make_int4(n_forced, hc, 0, 0));
-        if (st == kStRunning) atomicAdd(sc.cnt + hc, 1);
+        __stcg(reinterpret_cast<int4*>(r + 12) + 1, make_int4(n_forced, hb, 0, 0));
+        if (st == kStRunning) atomicAdd(sc.cnt + hb, 1);
       }
       __syncthreads();                                                   // window / kbuf / s_int are reused
     }

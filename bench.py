@@ -50,7 +50,7 @@ def parse_args():
     ap.add_argument("--particles", type=int, default=None, help="particles per GPU (default: the config's, "
                     "capped at 100000 per step for configs 3-4 unless given)")
     ap.add_argument("--segment", type=float, default=2e-5, help="simulated seconds per step")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "tile", "warp", "generic"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "mma", "tile", "warp", "generic"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
@@ -224,7 +224,7 @@ def run_cuda(args):
     n, seg, K, Wu = P.n, args.segment, args.steps, args.warmup
     GF = G.Field(fld)
     if args.kernel != "auto":
-        GF.set_kernel({"warp": G.GC_KERNEL_WARP, "generic": G.GC_KERNEL_GENERIC, "tile": G.GC_KERNEL_TILE}[args.kernel])
+        GF.set_kernel({"warp": G.GC_KERNEL_WARP, "generic": G.GC_KERNEL_GENERIC, "tile": G.GC_KERNEL_TILE, "mma": G.GC_KERNEL_MMA}[args.kernel])
     kinfo = GF.kernel_info(n)
     T = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device=dev)
     s, th, ze, vpar = T(P.s), T(P.theta), T(P.zeta), T(P.vpar)

@@ -9,7 +9,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "libgcorbit.so")
 SOURCES = ["gcorbit_api.cu"]
-HEADERS = ["device_math.cuh", "field.cuh", "kernels_generic.cuh", "kernels_warp.cuh", "kernels_tile.cuh",
+HEADERS = ["device_math.cuh", "field.cuh", "kernels_generic.cuh", "kernels_warp.cuh", "kernels_tile.cuh", "kernels_mma.cuh",
            os.path.join("..", "..", "include", "gcorbit.h")]
 
 

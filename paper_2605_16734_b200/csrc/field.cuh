@@ -30,6 +30,10 @@ struct FieldDev {
   // then G, I, iota, then the nk mode amplitudes
   const double* tile_images;
   int tile_E, tile_nmax;
+  // by-node image of the mma kernel (kernels_mma.cuh): image[ns + 4][mma_RS], image row = node + 2 (two zero rows
+  // at either end); a row holds the DMMA B fragments (P, Q)(m >= 1, n >= 1), b(m, 0), b(0, n), G, I, iota, modes
+  const double* mma_image;
+  int mma_RS, mma_MT, mma_KS;
 };
 
 // Integrator parameters as the kernels see them (gc_trace_params + derived values).

@@ -15,6 +15,7 @@ namespace gc { constexpr int GC_ST_NONFINITE_ = 4; }
 #include "kernels_generic.cuh"
 #include "kernels_warp.cuh"
 #include "kernels_tile.cuh"
+#include "kernels_mma.cuh"
 
 namespace {
 
@@ -60,6 +61,9 @@ struct gc_field {
   int sm_count = 0;
   int tile_smem = 0;                // dynamic shared memory of the tile kernel
   int tile_blocks_per_sm = 0;       // co-resident blocks per SM (cooperative launch)
+  bool mma_ok = false;
+  int mma_smem = 0;                 // dynamic shared memory of the mma kernel
+  int mma_blocks_per_sm = 0;
 };
 
 namespace {
@@ -177,8 +181,16 @@ const void* tile_fn(const gc_field* f) {
   return modes ? (const void*)gc::trace_tile_kernel<16, true> : (const void*)gc::trace_tile_kernel<16, false>;
 }
 
+const void* mma_fn(const gc_field* f) {
+  const bool modes = f->dev.nk > 0;
+  if (f->dev.mma_MT == 1)
+    return modes ? (const void*)gc::trace_mma_kernel<1, 2, true> : (const void*)gc::trace_mma_kernel<1, 2, false>;
+  return modes ? (const void*)gc::trace_mma_kernel<2, 4, true> : (const void*)gc::trace_mma_kernel<2, 4, false>;
+}
+
 int resolve_kernel(const gc_field* f, int64_t n) {
   if (f->kernel != GC_KERNEL_AUTO) return f->kernel;
+  if (f->mma_ok && n >= GC_TILE_MIN_PARTICLES) return GC_KERNEL_MMA;
   if (f->tile_ok && n >= GC_TILE_MIN_PARTICLES) return GC_KERNEL_TILE;
   return f->warp_ok ? GC_KERNEL_WARP : GC_KERNEL_GENERIC;
 }
@@ -248,8 +260,64 @@ int pack_tile_images(gc_field* f, const gc_field_desc* d) {
   return GC_OK;
 }
 
-// One cooperative launch of the tile kernel (mode 0 trace, mode 1 right-hand side only) with its scratch.
-int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, cudaStream_t st) {
+// image[ns + 4][RS] of the mma kernel (kernels_mma.cuh): image row = node + 2; per row the DMMA B fragments
+// (P, Q)(m, n) in lane order, then b(m, 0), b(0, n), G, I, iota and the mode amplitudes.
+template <int MT, int KS>
+void fill_mma_rows(const gc_field_desc* d, int RS, std::vector<double>& img) {
+  using R = gc::MmaRow<MT, KS>;
+  for (int node = 0; node < d->ns; ++node) {
+    double* row = img.data() + (size_t)(node + 2) * RS;
+    for (int k = 0; k < d->nh; ++k) {
+      const int m = d->xm[k], n = d->xn[k];
+      const double b = d->bmnc[(size_t)node * d->nh + k];
+      const int an = n > 0 ? n : -n;
+      if (m == 0) { row[R::kM0 + an] += b; continue; }
+      if (n == 0) { row[R::kN0 + m - 1] += b; continue; }
+      const int T = (m - 1) / 8, g = (m - 1) % 8, j = (an - 1) / 4, q = (an - 1) % 4;
+      double* e = row + R::kFrag + ((size_t)(T * KS + j) * 32 + 4 * g + q) * 2;
+      e[0] += b;                                           // P = b(m,n) + b(m,-n)
+      e[1] += n > 0 ? b : -b;                              // Q = b(m,n) - b(m,-n)
+    }
+    row[R::kProf] = d->G[node]; row[R::kProf + 1] = d->I[node]; row[R::kProf + 2] = d->iota[node];
+    for (int k = 0; k < d->nk; ++k) row[R::kModes + k] = d->phihat[(size_t)node * d->nk + k];
+  }
+}
+
+int pack_mma_image(gc_field* f, const gc_field_desc* d) {
+  gc::FieldDev& v = f->dev;
+  f->mma_ok = false;
+  if (v.N > 16 || v.M > 16 || d->nk > 4 * gc::kMmaModeSlots) return GC_OK;
+  const bool small = v.M <= 8 && v.N <= 8;
+  const int MT = small ? 1 : 2, KS = small ? 2 : 4;
+  const int RS = small ? gc::MmaRow<1, 2>::stride(d->nk) : gc::MmaRow<2, 4>::stride(d->nk);
+  const int smem = (int)gc::mma_smem_bytes(RS);
+  const int ncell = d->ns - 3;
+  if ((size_t)(gc::kSubBins + 2) * ncell * sizeof(int) > (size_t)gc::kMmaWinRows * RS * sizeof(double)) return GC_OK;
+  std::vector<double> img((size_t)(d->ns + 4) * RS, 0.0);
+  if (small) fill_mma_rows<1, 2>(d, RS, img); else fill_mma_rows<2, 4>(d, RS, img);
+  double* dev_img = nullptr;
+  int rc = upload(img.data(), img.size(), &dev_img);
+  if (rc != GC_OK) return rc;
+  f->allocs.push_back(dev_img);
+  v.mma_image = dev_img;
+  v.mma_RS = RS; v.mma_MT = MT; v.mma_KS = KS;
+  f->mma_smem = smem;
+  const void* fn = mma_fn(f);
+  GC_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  int per_sm = 0;
+  GC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, gc::kMmaThreads, (size_t)smem));
+  if (per_sm < 1) return GC_OK;
+  int coop = 0, devid = 0;
+  GC_CUDA(cudaGetDevice(&devid));
+  GC_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, devid));
+  if (!coop) return GC_OK;
+  f->mma_blocks_per_sm = per_sm;
+  f->mma_ok = true;
+  return GC_OK;
+}
+
+// One cooperative launch of the tile or mma kernel (mode 0 trace, mode 1 right-hand side only) with its scratch.
+int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, cudaStream_t st, bool mma = false) {
   const int ncell = f->dev.ns - 3;
   const size_t n = (size_t)t.n;
   const size_t rec_bytes = n * gc::kRecDoubles * sizeof(double);
@@ -267,14 +335,19 @@ int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, c
   sc.tstart = ip; ip += ncell + 1;
   sc.ctrl = ip;
   GC_CUDA(cudaMemsetAsync(sc.cnt, 0, (2 * nbin + (size_t)2 * (ncell + 1) + 8) * sizeof(int), st));
-  long long blocks = (long long)f->sm_count * f->tile_blocks_per_sm;
-  const long long need = ((long long)n + gc::kTileThreads - 1) / gc::kTileThreads;
+  const int per_tile = mma ? gc::kMmaTile : gc::kTileThreads;
+  long long blocks = (long long)f->sm_count * (mma ? f->mma_blocks_per_sm : f->tile_blocks_per_sm);
+  const long long need = ((long long)n + per_tile - 1) / per_tile;
   if (blocks > need) blocks = need;
   if (blocks < 1) blocks = 1;
   gc::FieldDev fd = f->dev;
   void* args[] = {(void*)&fd, (void*)&t, (void*)&sc, (void*)&mode, (void*)&rhs_out};
-  GC_CUDA(cudaLaunchCooperativeKernel(tile_fn(f), dim3((unsigned)blocks), dim3(gc::kTileThreads), args,
-                                      (size_t)f->tile_smem, st));
+  if (mma)
+    GC_CUDA(cudaLaunchCooperativeKernel(mma_fn(f), dim3((unsigned)blocks), dim3(gc::kMmaThreads), args,
+                                        (size_t)f->mma_smem, st));
+  else
+    GC_CUDA(cudaLaunchCooperativeKernel(tile_fn(f), dim3((unsigned)blocks), dim3(gc::kTileThreads), args,
+                                        (size_t)f->tile_smem, st));
   GC_CUDA(cudaFreeAsync(slab, st));
   return GC_OK;
 }
@@ -374,6 +447,7 @@ int gc_field_create(const gc_field_desc* d, gc_field** out) {
     rc = pack_rows(f, d);
   }
   if (rc == GC_OK) rc = pack_tile_images(f, d);
+  if (rc == GC_OK) rc = pack_mma_image(f, d);
   if (rc == GC_OK) {
     int devid = 0;
     cudaGetDevice(&devid);
@@ -401,7 +475,10 @@ int gc_set_kernel(gc_field* f, int32_t kernel) {
     return fail(GC_EINVAL, "gc_set_kernel: field does not fit the warp kernel (max|xn| <= 16, max xm <= 28)");
   if (kernel == GC_KERNEL_TILE && !f->tile_ok)
     return fail(GC_EINVAL, "gc_set_kernel: field does not fit the tile kernel (max|xn| <= 16, window <= 110 KB)");
-  if (kernel != GC_KERNEL_AUTO && kernel != GC_KERNEL_WARP && kernel != GC_KERNEL_GENERIC && kernel != GC_KERNEL_TILE)
+  if (kernel == GC_KERNEL_MMA && !f->mma_ok)
+    return fail(GC_EINVAL, "gc_set_kernel: field does not fit the mma kernel (max|xn| <= 16, max xm <= 16, nk <= 16)");
+  if (kernel != GC_KERNEL_AUTO && kernel != GC_KERNEL_WARP && kernel != GC_KERNEL_GENERIC && kernel != GC_KERNEL_TILE &&
+      kernel != GC_KERNEL_MMA)
     return fail(GC_EINVAL, "gc_set_kernel: unknown kernel");
   f->kernel = kernel;
   return GC_OK;
@@ -413,7 +490,13 @@ int gc_kernel_info(const gc_field* f, int64_t n, int32_t* kernel, int32_t* block
   cudaFuncAttributes at{};
   int b, t, s;
   const int k = resolve_kernel(f, n);
-  if (k == GC_KERNEL_TILE) {
+  if (k == GC_KERNEL_MMA) {
+    GC_CUDA(cudaFuncGetAttributes(&at, mma_fn(f)));
+    long long bl = (long long)f->sm_count * f->mma_blocks_per_sm;
+    const long long need = (n + gc::kMmaTile - 1) / gc::kMmaTile;
+    if (bl > need) bl = need < 1 ? 1 : need;
+    b = (int)bl; t = gc::kMmaThreads; s = f->mma_smem;
+  } else if (k == GC_KERNEL_TILE) {
     GC_CUDA(cudaFuncGetAttributes(&at, tile_fn(f)));
     long long bl = (long long)f->sm_count * f->tile_blocks_per_sm;
     const long long need = (n + gc::kTileThreads - 1) / gc::kTileThreads;
@@ -463,12 +546,12 @@ int gc_rhs_eval(const gc_field* f, double mass, double charge, double t, int64_t
   if (n == 0) return GC_OK;
   if (!y || !mu || !dydt) return fail(GC_EINVAL, "gc_rhs_eval: NULL array");
   const int kern = resolve_kernel(f, n);
-  if (kern == GC_KERNEL_TILE) {
+  if (kern == GC_KERNEL_TILE || kern == GC_KERNEL_MMA) {
     gc::TraceDev td{};
     td.mass = mass; td.charge = charge; td.t0 = t; td.t_max = t; td.v_ref = 1.0; td.inv_v_ref = 1.0;
     td.n = n; td.s0 = y; td.th0 = y + n; td.ze0 = y + 2 * n; td.vpar0 = y + 3 * n; td.mu = mu;
     td.max_steps = 1;
-    return launch_tile(f, td, 1, dydt, (cudaStream_t)stream);
+    return launch_tile(f, td, 1, dydt, (cudaStream_t)stream, kern == GC_KERNEL_MMA);
   }
   if (kern == GC_KERNEL_WARP) {
     const WarpInst* w = find_inst(f);
@@ -507,7 +590,7 @@ int gc_trace(const gc_field* f, const gc_trace_params* params, int64_t n, const 
   if (!poincare || !poincare_count) t.poincare_capacity = 0;
   if (poincare_count) GC_CUDA(cudaMemsetAsync(poincare_count, 0, sizeof(int64_t), st));
   const int kern = resolve_kernel(f, n);
-  if (kern == GC_KERNEL_TILE) return launch_tile(f, t, 0, nullptr, st);
+  if (kern == GC_KERNEL_TILE || kern == GC_KERNEL_MMA) return launch_tile(f, t, 0, nullptr, st, kern == GC_KERNEL_MMA);
   if (kern == GC_KERNEL_WARP) {
     const WarpInst* w = find_inst(f);
     unsigned long long* counter = nullptr;

@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 SO_PATH = os.path.join(_HERE, "libgcorbit.so")
 
 GC_OK, GC_EINVAL, GC_ENOMEM, GC_ECUDA = 0, -1, -2, -3
-GC_KERNEL_AUTO, GC_KERNEL_GENERIC, GC_KERNEL_WARP, GC_KERNEL_TILE = 0, 1, 2, 3
+GC_KERNEL_AUTO, GC_KERNEL_GENERIC, GC_KERNEL_WARP, GC_KERNEL_TILE, GC_KERNEL_MMA = 0, 1, 2, 3, 4
 GC_TILE_MIN_PARTICLES = 8192
 ST_TMAX, ST_LOST, ST_AXIS, ST_MAXSTEPS, ST_NONFINITE = 0, 1, 2, 3, 4
 
@@ -166,7 +166,7 @@ class Field:
         """Kernel and launch geometry gc_trace uses for an ensemble of n particles."""
         v = [C.c_int32(0) for _ in range(5)]
         _check(load_library().gc_kernel_info(self._h, int(n), *[C.byref(x) for x in v]))
-        return dict(kernel={GC_KERNEL_GENERIC: "generic", GC_KERNEL_WARP: "warp", GC_KERNEL_TILE: "tile"}[v[0].value],
+        return dict(kernel={GC_KERNEL_GENERIC: "generic", GC_KERNEL_WARP: "warp", GC_KERNEL_TILE: "tile", GC_KERNEL_MMA: "mma"}[v[0].value],
                     blocks=v[1].value, threads=v[2].value, smem_bytes=v[3].value, regs=v[4].value)
 
     # ---- gc_field_eval / gc_pert_eval / gc_rhs_eval (device tensors in, device tensors out) ------------------

@@ -23,7 +23,7 @@ def case4():
 
 def _kernels():
     from paper_2605_16734_b200 import gcorbit as G
-    return [G.GC_KERNEL_GENERIC, G.GC_KERNEL_WARP, G.GC_KERNEL_TILE]
+    return [G.GC_KERNEL_GENERIC, G.GC_KERNEL_WARP, G.GC_KERNEL_TILE, G.GC_KERNEL_MMA]
 
 
 def test_empty_ensemble(case0):
@@ -243,7 +243,7 @@ def test_fields_outside_the_warp_layout_use_the_generic_kernel():
     bm = np.concatenate([base.bmnc[:, perm], 0.5 * base.bmnc[:, 10:11]], axis=1)
     shuf = dataclasses.replace(base, xm=xm, xn=xn, bmnc=np.ascontiguousarray(bm))
     GF2, OF2 = G.Field(shuf), oracle.OracleField(shuf)
-    assert GF2.kernel_info(40)["kernel"] == "warp" and GF2.kernel_info(100_000)["kernel"] == "tile"
+    assert GF2.kernel_info(40)["kernel"] == "warp" and GF2.kernel_info(100_000)["kernel"] == "mma"
     mu2 = W.mu_from(P, OF2.eval_B_many(P.s, P.theta, P.zeta)[:, 0])
     r = gpu_trace(GF2, spec, P, mu2, t_max=5e-6)
     o = OF2.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu2, t_max=5e-6)

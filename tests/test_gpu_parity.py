@@ -10,12 +10,12 @@ from gpu_common import (COND_FACTOR, FLIP_RTOL, SAME_RTOL, assert_trace_parity, 
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = ["generic", "warp", "tile"]
+KERNELS = ["generic", "warp", "tile", "mma"]
 
 
 def _set_kernel(GF, name):
     from paper_2605_16734_b200 import gcorbit as G
-    GF.set_kernel({"generic": G.GC_KERNEL_GENERIC, "warp": G.GC_KERNEL_WARP, "tile": G.GC_KERNEL_TILE,
+    GF.set_kernel({"generic": G.GC_KERNEL_GENERIC, "warp": G.GC_KERNEL_WARP, "tile": G.GC_KERNEL_TILE, "mma": G.GC_KERNEL_MMA,
                    "auto": G.GC_KERNEL_AUTO}[name])
 
 
@@ -120,7 +120,7 @@ def test_trace_config0_full(cases, kernel):
 _SUB = {}
 
 
-@pytest.mark.parametrize("kernel", ["warp", "tile"])
+@pytest.mark.parametrize("kernel", ["warp", "tile", "mma"])
 @pytest.mark.parametrize("config,n,t_max", [(1, 296, 2e-5), (2, 256, 2e-5), (3, 301, 3e-5), (4, 256, 2e-5)])
 def test_trace_subsamples(cases, config, n, t_max, kernel):
     """Short-horizon subsamples of configs 1-4 (n chosen ragged against 8 warps per block and 128-particle
@@ -158,7 +158,7 @@ def test_trace_generic_kernel_with_modes(cases):
     _set_kernel(GF, "auto")
 
 
-@pytest.mark.parametrize("kernel", ["warp", "tile"])
+@pytest.mark.parametrize("kernel", ["warp", "tile", "mma"])
 @pytest.mark.parametrize("n", [1, 7, 33, 148 * 8 + 3])
 def test_trace_ragged_sizes(cases, n, kernel):
     """One particle, fewer particles than warps in a block / lanes in a tile, and one more wave than the
@@ -179,7 +179,7 @@ def test_full_size_launch_sampled(cases):
     import torch
     from paper_2605_16734_b200 import gcorbit as G
     fld, spec, P, OF, GF, _ = cases(1, 64)          # fields only; the full ensemble is drawn here
-    assert GF.kernel_info(100_000)["kernel"] == "tile"
+    assert GF.kernel_info(100_000)["kernel"] == "mma"
     from paper_2605_16734_b200 import workloads as W
     P = W.make_particles(1)
     assert P.n == 100_000

@@ -275,20 +275,36 @@ __device__ __forceinline__ int home_bin(int ns, double s) {
 
 extern __shared__ __align__(128) unsigned char gc_tile_smem[];
 
-// mode 0: trace.  mode 1: right-hand side only (gc_rhs_eval): k1 of every particle goes to rhs_out[4][n].
+// The table engine of trace_tile_kernel: DFMA sweep over a per-cell window image (see the header comment).
 template <int NMAX, bool MODES>
-__global__ void __launch_bounds__(kTileThreads, 2)
-trace_tile_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_out) {
+struct TileEngine {
+  static __device__ __forceinline__ int win_doubles(const FieldDev& f) { return 10 * f.tile_E; }
+  static __device__ __forceinline__ const double* win_src(const FieldDev& f, int cell) {
+    return f.tile_images + (size_t)cell * (10 * f.tile_E);
+  }
+  static __device__ __forceinline__ void rhs(const FieldDev& f, const double* win, int cell, bool active, double mass,
+                                             double charge, double mu, double v_ref, double inv_v_ref, double t,
+                                             const double (&y)[4], double (&dy)[4]) {
+    rhs_tile<NMAX, MODES>(f, win, cell, active, mass, charge, mu, v_ref, inv_v_ref, t, y, dy);
+  }
+};
+
+// Body of the cell-binned persistent kernels (trace_tile_kernel, trace_mma_kernel): binning, epochs, tiles, the
+// Dormand-Prince integrator of one lane per particle.  Eng supplies the window image and the right-hand side.
+// mode 0: trace.  mode 1: right-hand side only (gc_rhs_eval): k1 of every particle goes to rhs_out[4][n].
+template <class Eng>
+__device__ __forceinline__ void trace_binned_body(const FieldDev& f, const TraceDev& p, const TileScratch& sc, int mode,
+                                                  double* rhs_out) {
   cgx::grid_group grid = cgx::this_grid();
   const int tid = threadIdx.x;
   const long long gtid = (long long)blockIdx.x * kTileThreads + tid;
   const long long gthreads = (long long)gridDim.x * kTileThreads;
   const int ncell = f.ns - 3;
-  const int E = f.tile_E;
+  const int WD = Eng::win_doubles(f);
   constexpr double kTwoPi = 6.283185307179586476925286766559;
 
-  double* win = reinterpret_cast<double*>(gc_tile_smem);                 // [10 E]
-  double* kbuf = win + 10 * E;                                           // [7][4][kTileThreads]
+  double* win = reinterpret_cast<double*>(gc_tile_smem);                 // [WD] window image of the tile's cell
+  double* kbuf = win + WD;                                               // [7][4][kTileThreads]
   unsigned long long* bar = reinterpret_cast<unsigned long long*>(kbuf + 7 * 4 * kTileThreads);
   int* s_int = reinterpret_cast<int*>(bar + 1);                          // [0] tile id; scan space follows
   auto kb = [&](int j, int c) -> double& { return kbuf[(j * 4 + c) * kTileThreads + tid]; };
@@ -387,9 +403,9 @@ trace_tile_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_
       if (cell != cur_cell) {                                            // stage the window: one bulk copy
         if (tid == 0) {
           asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-          const unsigned bytes = (unsigned)(10 * E * sizeof(double));
+          const unsigned bytes = (unsigned)(WD * sizeof(double));
           mbar_expect_tx(bar, bytes);
-          bulk_g2s(win, f.tile_images + (size_t)cell * (10 * E), bytes, bar);
+          bulk_g2s(win, Eng::win_src(f, cell), bytes, bar);
         }
         mbar_wait(bar, bar_phase);
         bar_phase ^= 1u;
@@ -458,7 +474,7 @@ trace_tile_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_
             }
             double dy[4] = {0.0, 0.0, 0.0, 0.0};
             const bool lane_on = running && (stage > 0 || !(flags & kFlagHaveK1));
-            rhs_tile<NMAX, MODES>(f, win, cell, lane_on, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, ts, ys, dy);
+            Eng::rhs(f, win, cell, lane_on, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, ts, ys, dy);
             if (lane_on) {
               kb(stage, 0) = dy[0]; kb(stage, 1) = dy[1]; kb(stage, 2) = dy[2]; kb(stage, 3) = dy[3];
               if (stage == 0) {
@@ -596,6 +612,12 @@ trace_tile_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_
       if (p.n_forced) p.n_forced[i] = (p.resume ? p.n_forced[i] : 0) + n_forced;
     }
   }
+}
+
+template <int NMAX, bool MODES>
+__global__ void __launch_bounds__(kTileThreads, 2)
+trace_tile_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_out) {
+  trace_binned_body<TileEngine<NMAX, MODES>>(f, p, sc, mode, rhs_out);
 }
 
 }  // namespace gc

@@ -290,7 +290,11 @@ int pack_mma_image(gc_field* f, const gc_field_desc* d) {
   const bool small = v.M <= 8 && v.N <= 8;
   const int MT = small ? 1 : 2, KS = small ? 2 : 4;
   const int RS = small ? gc::MmaRow<1, 2>::stride(d->nk) : gc::MmaRow<2, 4>::stride(d->nk);
-  const int smem = (int)((size_t)gc::kMmaWinRows * RS * sizeof(double) + (size_t)7 * 4 * gc::kTileThreads * sizeof(double) + 64);
+#ifdef GC_MMA_L1
+  const int smem = (int)((size_t)((gc::kSubBins + 2) * (d->ns - 3) / 2 + 2) * sizeof(double) + (size_t)7 * 4 * gc::kMmaThreads * sizeof(double) + 64);
+#else
+  const int smem = (int)((size_t)gc::kMmaWinRows * RS * sizeof(double) + (size_t)7 * 4 * gc::kMmaThreads * sizeof(double) + 64);
+#endif
   if (smem > 110 * 1024) return GC_OK;
   const int ncell = d->ns - 3;
   if ((size_t)(gc::kSubBins + 2) * ncell * sizeof(int) > (size_t)gc::kMmaWinRows * RS * sizeof(double)) return GC_OK;
@@ -306,7 +310,7 @@ int pack_mma_image(gc_field* f, const gc_field_desc* d) {
   const void* fn = mma_fn(f);
   GC_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   int per_sm = 0;
-  GC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, gc::kTileThreads, (size_t)smem));
+  GC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, gc::kMmaThreads, (size_t)smem));
   if (per_sm < 1) return GC_OK;
   int coop = 0, devid = 0;
   GC_CUDA(cudaGetDevice(&devid));
@@ -336,7 +340,7 @@ int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, c
   sc.tstart = ip; ip += ncell + 1;
   sc.ctrl = ip;
   GC_CUDA(cudaMemsetAsync(sc.cnt, 0, (2 * nbin + (size_t)2 * (ncell + 1) + 8) * sizeof(int), st));
-  const int per_tile = mma ? gc::kTileThreads : gc::kTileThreads;
+  const int per_tile = mma ? gc::kMmaThreads : gc::kTileThreads;
   long long blocks = (long long)f->sm_count * (mma ? f->mma_blocks_per_sm : f->tile_blocks_per_sm);
   const long long need = ((long long)n + per_tile - 1) / per_tile;
   if (blocks > need) blocks = need;
@@ -344,7 +348,7 @@ int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, c
   gc::FieldDev fd = f->dev;
   void* args[] = {(void*)&fd, (void*)&t, (void*)&sc, (void*)&mode, (void*)&rhs_out};
   if (mma)
-    GC_CUDA(cudaLaunchCooperativeKernel(mma_fn(f), dim3((unsigned)blocks), dim3(gc::kTileThreads), args,
+    GC_CUDA(cudaLaunchCooperativeKernel(mma_fn(f), dim3((unsigned)blocks), dim3(gc::kMmaThreads), args,
                                         (size_t)f->mma_smem, st));
   else
     GC_CUDA(cudaLaunchCooperativeKernel(tile_fn(f), dim3((unsigned)blocks), dim3(gc::kTileThreads), args,
@@ -494,9 +498,9 @@ int gc_kernel_info(const gc_field* f, int64_t n, int32_t* kernel, int32_t* block
   if (k == GC_KERNEL_MMA) {
     GC_CUDA(cudaFuncGetAttributes(&at, mma_fn(f)));
     long long bl = (long long)f->sm_count * f->mma_blocks_per_sm;
-    const long long need = (n + gc::kTileThreads - 1) / gc::kTileThreads;
+    const long long need = (n + gc::kMmaThreads - 1) / gc::kMmaThreads;
     if (bl > need) bl = need < 1 ? 1 : need;
-    b = (int)bl; t = gc::kTileThreads; s = f->mma_smem;
+    b = (int)bl; t = gc::kMmaThreads; s = f->mma_smem;
   } else if (k == GC_KERNEL_TILE) {
     GC_CUDA(cudaFuncGetAttributes(&at, tile_fn(f)));
     long long bl = (long long)f->sm_count * f->tile_blocks_per_sm;

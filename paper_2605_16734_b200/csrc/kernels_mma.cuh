@@ -38,6 +38,13 @@
 
 namespace gc {
 
+constexpr int kMmaThreads = 64;                  // particles per tile = threads per block (2 warps share a window)
+constexpr int kMmaBlocksPerSm = 4;               // 8 warps per SM at <= 255 registers
+#ifndef GC_MMA_CAP
+#define GC_MMA_CAP 8
+#endif
+constexpr int kMmaCap = GC_MMA_CAP;              // attempted steps per particle per chunk (short: re-binning keeps the
+                                                 // groups on 4-row unions and parks fewer particles)
 constexpr int kMmaWinRows = 8;                   // node rows cell-2 .. cell+5
 constexpr int kMmaNone = 1 << 20;                // "no stencil": a row offset that gives weight 0 on every row
 
@@ -206,8 +213,13 @@ __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, in
     const int r_lo = __reduce_min_sync(0xffffffffu, (ingrp && inwin) ? off : kMmaNone);
     const int r_hi = __reduce_max_sync(0xffffffffu, (ingrp && inwin) ? off + 3 : -1);
     if (r_hi >= 0)
+#ifdef GC_MMA_L1
+      mma_sweep<MT, KS, LdG>(f.mma_image + (size_t)cell * RS, RS, r_lo, r_hi, (ingrp && inwin) ? off : kMmaNone, w, dw,
+                             src, lane, q, AC, AS, AnC, AnS, cm, sm, o);
+#else
       mma_sweep<MT, KS, LdS>(win, RS, r_lo, r_hi, (ingrp && inwin) ? off : kMmaNone, w, dw, src, lane, q, AC, AS, AnC,
                              AnS, cm, sm, o);
+#endif
     // ---- stencils outside the window: one sweep per distinct stencil, rows from global memory ----------------------
     unsigned pend = __ballot_sync(0xffffffffu, ingrp && outside);
     while (pend) {
@@ -226,7 +238,11 @@ __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, in
   }
   // ---- particle role: profiles, perturbation, guiding-centre algebra ------------------------------------------------
   if (active) {
+#ifdef GC_MMA_L1
+    const double* prow = f.mma_image + (size_t)(i0 + 2) * RS;
+#else
     const double* prow = inwin ? win + (size_t)off * RS : f.mma_image + (size_t)(i0 + 2) * RS;
+#endif
     Profiles pr;
     double v[4];
 #pragma unroll
@@ -280,7 +296,13 @@ __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, in
 // The table engine of trace_mma_kernel.
 template <int MT, int KS, bool MODES>
 struct MmaEngine {
+#ifdef GC_MMA_L1
+  static constexpr bool kStageWindow = false;
+  static __device__ __forceinline__ int win_doubles(const FieldDev& f) { return (kSubBins + 2) * (f.ns - 3) / 2 + 2; }
+#else
+  static constexpr bool kStageWindow = true;
   static __device__ __forceinline__ int win_doubles(const FieldDev& f) { return kMmaWinRows * f.mma_RS; }
+#endif
   static __device__ __forceinline__ const double* win_src(const FieldDev& f, int cell) {
     return f.mma_image + (size_t)cell * f.mma_RS;                     // image rows cell .. cell+7
   }
@@ -291,13 +313,10 @@ struct MmaEngine {
   }
 };
 
-#ifndef GC_MMA_MINB
-#define GC_MMA_MINB 2
-#endif
 template <int MT, int KS, bool MODES>
-__global__ void __launch_bounds__(kTileThreads, GC_MMA_MINB)
+__global__ void __launch_bounds__(kMmaThreads, kMmaBlocksPerSm)
 trace_mma_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_out) {
-  trace_binned_body<MmaEngine<MT, KS, MODES>>(f, p, sc, mode, rhs_out);
+  trace_binned_body<MmaEngine<MT, KS, MODES>, kMmaThreads, kMmaCap>(f, p, sc, mode, rhs_out);
 }
 
 }  // namespace gc

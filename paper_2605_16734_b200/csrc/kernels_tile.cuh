@@ -37,8 +37,11 @@ namespace gc {
 
 namespace cgx = cooperative_groups;
 
-constexpr int kTileThreads = 128;      // particles per tile = threads per block
-constexpr int kTileCap = 32;           // attempted steps per lane per chunk
+constexpr int kTileThreads = 128;      // tile kernel: particles per tile = threads per block
+#ifndef GC_TILE_CAP
+#define GC_TILE_CAP 8
+#endif
+constexpr int kTileCap = GC_TILE_CAP;  // tile kernel: attempted steps per lane per chunk
 constexpr int kRecDoubles = 16;        // one 128-byte record per particle
 constexpr int kSubBins = 8;            // radial sub-bins per cell: tiles come out ordered in s (lane coherence)
 
@@ -278,6 +281,7 @@ extern __shared__ __align__(128) unsigned char gc_tile_smem[];
 // The table engine of trace_tile_kernel: DFMA sweep over a per-cell window image (see the header comment).
 template <int NMAX, bool MODES>
 struct TileEngine {
+  static constexpr bool kStageWindow = true;
   static __device__ __forceinline__ int win_doubles(const FieldDev& f) { return 10 * f.tile_E; }
   static __device__ __forceinline__ const double* win_src(const FieldDev& f, int cell) {
     return f.tile_images + (size_t)cell * (10 * f.tile_E);
@@ -292,22 +296,23 @@ struct TileEngine {
 // Body of the cell-binned persistent kernels (trace_tile_kernel, trace_mma_kernel): binning, epochs, tiles, the
 // Dormand-Prince integrator of one lane per particle.  Eng supplies the window image and the right-hand side.
 // mode 0: trace.  mode 1: right-hand side only (gc_rhs_eval): k1 of every particle goes to rhs_out[4][n].
-template <class Eng>
+// THREADS = particles per tile = threads per block; CAP = attempted steps per lane per chunk.
+template <class Eng, int THREADS, int CAP>
 __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const TraceDev& p, const TileScratch& sc, int mode,
                                                   double* rhs_out) {
   cgx::grid_group grid = cgx::this_grid();
   const int tid = threadIdx.x;
-  const long long gtid = (long long)blockIdx.x * kTileThreads + tid;
-  const long long gthreads = (long long)gridDim.x * kTileThreads;
+  const long long gtid = (long long)blockIdx.x * THREADS + tid;
+  const long long gthreads = (long long)gridDim.x * THREADS;
   const int ncell = f.ns - 3;
   const int WD = Eng::win_doubles(f);
   constexpr double kTwoPi = 6.283185307179586476925286766559;
 
   double* win = reinterpret_cast<double*>(gc_tile_smem);                 // [WD] window image of the tile's cell
-  double* kbuf = win + WD;                                               // [7][4][kTileThreads]
-  unsigned long long* bar = reinterpret_cast<unsigned long long*>(kbuf + 7 * 4 * kTileThreads);
+  double* kbuf = win + WD;                                               // [7][4][THREADS]
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(kbuf + 7 * 4 * THREADS);
   int* s_int = reinterpret_cast<int*>(bar + 1);                          // [0] tile id; scan space follows
-  auto kb = [&](int j, int c) -> double& { return kbuf[(j * 4 + c) * kTileThreads + tid]; };
+  auto kb = [&](int j, int c) -> double& { return kbuf[(j * 4 + c) * THREADS + tid]; };
 
   if (tid == 0) mbar_init(bar, 1);
   __syncthreads();
@@ -342,7 +347,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
     if (blockIdx.x == 0) {
       int* wsp = reinterpret_cast<int*>(win);                            // nbin + 2 ncell ints staged in the window space
       const int nbin = ncell * kSubBins;
-      for (int b = tid; b < nbin; b += kTileThreads) { wsp[b] = __ldcg(sc.cnt + b); sc.cnt[b] = 0; }
+      for (int b = tid; b < nbin; b += THREADS) { wsp[b] = __ldcg(sc.cnt + b); sc.cnt[b] = 0; }
       __syncthreads();
       if (tid == 0) {
         int run = 0, tiles = 0;
@@ -355,15 +360,15 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
             wsp[b] = run;
             run += k;
           }
-          tiles += (run - run0 + kTileThreads - 1) / kTileThreads;
+          tiles += (run - run0 + THREADS - 1) / THREADS;
         }
         sc.start[ncell] = run;
         sc.tstart[ncell] = tiles;
         sc.ctrl[0] = 0; sc.ctrl[1] = 0; sc.ctrl[2] = tiles; sc.ctrl[3] = run;
       }
       __syncthreads();
-      for (int b = tid; b < nbin; b += kTileThreads) sc.cursor[b] = wsp[b];
-      for (int c = tid; c < ncell; c += kTileThreads) {
+      for (int b = tid; b < nbin; b += THREADS) sc.cursor[b] = wsp[b];
+      for (int c = tid; c < ncell; c += THREADS) {
         sc.start[c] = wsp[nbin + c];
         sc.tstart[c] = wsp[nbin + ncell + c];
       }
@@ -398,9 +403,9 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
       }
       const int cell = lo;
       const int seg0 = __ldcg(sc.start + cell), seg1 = __ldcg(sc.start + cell + 1);
-      const int begin = seg0 + (tile - __ldcg(sc.tstart + cell)) * kTileThreads;
-      const int count = min(kTileThreads, seg1 - begin);
-      if (cell != cur_cell) {                                            // stage the window: one bulk copy
+      const int begin = seg0 + (tile - __ldcg(sc.tstart + cell)) * THREADS;
+      const int count = min(THREADS, seg1 - begin);
+      if (Eng::kStageWindow && cell != cur_cell) {                       // stage the window: one bulk copy
         if (tid == 0) {
           asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
           const unsigned bytes = (unsigned)(WD * sizeof(double));
@@ -435,9 +440,9 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
       bool first_chunk = true;
       bool extra = false;                        // an extra chunk: stop as soon as the epoch's first chunks are done
 
-      for (;;) {                                 // chunks of kTileCap attempts
+      for (;;) {                                 // chunks of CAP attempts
 #pragma unroll 1
-        for (int att = 0; att < kTileCap; ++att) {
+        for (int att = 0; att < CAP; ++att) {
           if (!__any_sync(0xffffffffu, running)) break;
           if (extra) {                           // attempts are warp-local: any warp may stop at any attempt
             int done = 0;
@@ -564,7 +569,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
         if (tid == 0) {
           const int next = atomicAdd(sc.ctrl + 0, 1);
           bool more = false;
-          if (next >= ntiles && nrun * 2 >= kTileThreads) {
+          if (next >= ntiles && nrun * 2 >= THREADS) {
             const volatile int* vc = sc.ctrl;
             more = vc[1] < ntiles;
           }
@@ -617,7 +622,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
 template <int NMAX, bool MODES>
 __global__ void __launch_bounds__(kTileThreads, 2)
 trace_tile_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_out) {
-  trace_binned_body<TileEngine<NMAX, MODES>>(f, p, sc, mode, rhs_out);
+  trace_binned_body<TileEngine<NMAX, MODES>, kTileThreads, kTileCap>(f, p, sc, mode, rhs_out);
 }
 
 }  // namespace gc

@@ -1,5 +1,5 @@
 // kernels_mma.cuh -- hot-path kernel for large ensembles, second generation: the harmonic sum as FP64 matrix
-// instructions (DMMA.8x8x4), four lanes per particle.
+// instructions (DMMA.8x8x4), eight particles per instruction.
 //
 // Why.  kernels_tile.cuh is bound by shared-memory operand delivery: every DFMA of its sweep takes one operand
 // that each lane loads for itself (2 DFMA per loaded double; profiles/r1_ncu_tile_config1.md).  Once particles
@@ -10,24 +10,32 @@
 //     PC[p][r,m] = sum_n C_n(p) P[r][m,n]     PS = sum_n n S_n(p) P     QS = sum_n S_n(p) Q     QC = sum_n n C_n(p) Q
 // i.e. D[8 particles][8 columns (r, m)] += A[8 particles][4 toroidal numbers] * B[4 toroidal numbers][8 columns]:
 // mma.sync.m8n8k4.f64.  The A operand is per-particle trigonometry held in registers, the B operand is the
-// table, identical for the eight particles of a warp and fetched ONCE per warp (one 16-byte load per lane feeds
-// four DMMA = 32 DFMA-equivalents per lane), the accumulators never leave registers.  On B200 DMMA.8x8x4 runs on
-// the FP64 pipe at the DFMA rate (37 TFLOP/s measured, same roofline), so this buys operand bandwidth, not peak.
+// table, identical for the eight particles of a group and fetched ONCE per group (one 16-byte load per lane feeds
+// four DMMA = 32 DFMA-equivalents per lane), the accumulators never leave registers.  On B200 DMMA.8x8x4 shares
+// the FP64 units with DFMA (37 TFLOP/s measured for either, 35 when mixed: same roofline), so this buys operand
+// bandwidth, not peak; latency 26 cycles, two independent accumulators saturate the pipe (measured).
 //
-// Layout of the work.  A warp owns 8 particles; lane = 4 g + q: g = particle slot, q = lane of the quad.
-//   * DMMA fragments: A[g][q], B[q][g], D[g][2q, 2q+1].  Toroidal numbers n = 4 j + q + 1 (k-step j), poloidal
-//     numbers m = 1 + 8 T + (column) (m-tile T).  m = 0 and n = 0 are handled beside the DMMA (n = 0 initialises
-//     the PC accumulator, m = 0 is a 16-term DFMA sum split over the quad).
-//   * Rows: a warp sweeps the UNION of the stencil rows of its 8 particles (4 rows when they share a stencil,
-//     5 when they straddle a node); a particle's weight for a row outside its own stencil is exactly 0, so its
-//     result does not depend on who it shares the warp with.
-//   * Per row the epilogue turns the eight accumulators of a lane into its share of B, B_s, B_theta, B_zeta with
-//     (c_m, s_m) and the Lagrange weights; the quad sums by two butterfly shuffles at the end.
-//   * The integrator is component-parallel: lane q carries component q of (s, theta, zeta, u) and of k1..k7; the
-//     error norm is a quad reduction; every decision is taken identically by the four lanes.
+// Layout of the work.  As in kernels_tile.cuh a lane owns a particle for everything that is per particle
+// (Lagrange weights, one sincos(theta) and one sincos(nfp zeta), profiles, perturbation, guiding-centre algebra,
+// Dormand-Prince controller).  Only the harmonic sum changes hands: a warp pushes its 32 particles through the
+// sweep in four GROUPS of eight.  For group G lane = 4 g + q plays the FRAGMENT role for particle 8 G + g:
+//   * it fetches that particle's (cos, sin)(theta), (cos, sin)(nfp zeta) by shuffle and builds, by complex
+//     powers, the A operands C_n, S_n, n C_n, n S_n for n = 4 j + q + 1 (k-step j) and (c_m, s_m) for its four
+//     poloidal numbers m = 1 + 8 T + 2 q + e;
+//   * DMMA fragments: A[g][q], B[q][g], D[g][2q, 2q+1]; the B fragments (P, Q)(m, n) sit in the image in lane
+//     order, one 16-byte load per lane and k-step; n = 0 initialises the PC accumulator, m = 0 is a 16-term DFMA
+//     sum split over the quad;
+//   * rows: the group sweeps the UNION of the stencil rows of its 8 particles (4 rows when they share a stencil,
+//     5 when they straddle a node); the Lagrange weight of each row comes from the particle lane by shuffle and
+//     is exactly 0 for a row outside that particle's stencil, so a particle's result does not depend on who it
+//     shares a group with;
+//   * per row the epilogue turns the eight accumulators of a lane into its share of B, B_s, B_theta, B_zeta;
+//     two butterfly shuffles sum the quad and one more hands the four sums back to the particle lane.
 // Window: the 8 node rows cell-2 .. cell+5 of a by-node image (contiguous in global memory, ONE bulk TMA copy per
 // cell change); stencils that start further than 2 rows from the tile's cell are swept from global memory with the
-// same instruction sequence (bit-identical results).  Binning, epochs, tiles, records: as in kernels_tile.cuh.
+// same instruction sequence (bit-identical results).  Binning, epochs, tiles, records and the integrator are
+// trace_binned_body of kernels_tile.cuh; tiles are 64 particles (two warps share a window), chunks are 8 attempts:
+// frequent re-binning keeps the groups on 4-row unions and parks few particles.
 #pragma once
 #include <cooperative_groups.h>
 

@@ -46,8 +46,14 @@
 
 namespace gc {
 
-constexpr int kMmaThreads = 64;                  // particles per tile = threads per block (2 warps share a window)
-constexpr int kMmaBlocksPerSm = 4;               // 8 warps per SM at <= 255 registers
+#ifndef GC_MMA_THREADS
+#define GC_MMA_THREADS 64
+#endif
+#ifndef GC_MMA_MINB
+#define GC_MMA_MINB 4
+#endif
+constexpr int kMmaThreads = GC_MMA_THREADS;      // particles per tile = threads per block (2 warps share a window)
+constexpr int kMmaBlocksPerSm = GC_MMA_MINB;     // 8 warps per SM at <= 255 registers
 #ifndef GC_MMA_CAP
 #define GC_MMA_CAP 8
 #endif
@@ -106,7 +112,11 @@ __device__ __forceinline__ void mma_sweep(const double* base, int RS, int r_lo, 
                                           const double (&AnS)[KS], const double (&cm)[2 * MT],
                                           const double (&sm)[2 * MT], double (&o)[4]) {
   using R = MmaRow<MT, KS>;
-#pragma unroll 1
+#ifndef GC_MMA_ROW_UNROLL
+#define GC_MMA_ROW_UNROLL 2
+#endif
+  constexpr int kRowUnroll = GC_MMA_ROW_UNROLL;
+#pragma unroll kRowUnroll
   for (int r = r_lo; r <= r_hi; ++r) {
     const int idx = r - off_p;
     const double wsel = idx == 0 ? w[0] : idx == 1 ? w[1] : idx == 2 ? w[2] : idx == 3 ? w[3] : 0.0;

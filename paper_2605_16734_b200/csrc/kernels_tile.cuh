@@ -43,7 +43,10 @@ constexpr int kTileThreads = 128;      // tile kernel: particles per tile = thre
 #endif
 constexpr int kTileCap = GC_TILE_CAP;  // tile kernel: attempted steps per lane per chunk
 constexpr int kRecDoubles = 16;        // one 128-byte record per particle
-constexpr int kSubBins = 8;            // radial sub-bins per cell: tiles come out ordered in s (lane coherence)
+#ifndef GC_SUBBINS
+#define GC_SUBBINS 8
+#endif
+constexpr int kSubBins = GC_SUBBINS;   // radial sub-bins per cell: tiles come out ordered in s (lane coherence)
 
 // Per-call scratch of the tile kernel (device memory, owned by gc_trace for the duration of the call).
 struct TileScratch {
@@ -389,6 +392,9 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
     grid.sync();
 
     // ---- D: tiles ------------------------------------------------------------------------------------------------
+    // slot of this lane in a tile: groups of 8 particles are dealt round-robin to the warps of the block, so a
+    // short tile keeps every warp equally busy
+    const int slot = ((((tid & 31) >> 3) * (THREADS / 32) + (tid >> 5)) << 3) | (tid & 7);
     int cur_cell = -1;
     __syncthreads();
     if (tid == 0) s_int[0] = atomicAdd(sc.ctrl + 0, 1);
@@ -418,13 +424,13 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
       }
 
       // lane state
-      bool active = tid < count;
+      bool active = slot < count;
       long long pid = 0;
       double y[4] = {0.0, 0.0, 0.0, 0.0}, t = 0.0, h = 0.0, mu = 0.0;
       long long attempts = 0;
       int st = 0, flags = 0, n_acc = 0, n_rej = 0, n_forced = 0;
       if (active) {
-        pid = __ldcg(sc.order + begin + tid);
+        pid = __ldcg(sc.order + begin + slot);
         const double* r = sc.rec + pid * kRecDoubles;
         const double4 a = ldcg4(r);
         const double4 b = ldcg4(r + 4);

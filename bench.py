@@ -312,7 +312,10 @@ def run_cuda(args):
     achieved = attempts * fstep / (kernel_ms * 1e-3) / 1e12         # this rank's kernel, TFLOP/s
     traffic = None
     tp = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tp):
+    # one ncu capture of the DEFAULT launch (profiles/r1_ncu_mma_config1.md); other workloads have no capture
+    default_launch = (args.config == 1 and args.particles is None and args.segment == 2e-5 and
+                      kinfo["kernel"] == "mma")
+    if os.path.exists(tp) and default_launch:
         try:
             with open(tp) as fh:
                 traffic = json.load(fh).get(f"config{args.config}_dram_bytes_per_launch")

@@ -80,15 +80,18 @@ enum { GC_TRACE_RESUME = 1 };
 enum { GC_ST_TMAX = 0, GC_ST_LOST = 1, GC_ST_AXIS = 2, GC_ST_MAXSTEPS = 3, GC_ST_NONFINITE = 4 };
 
 /* Kernel selection for gc_trace (gc_set_kernel).
+ *   GC_KERNEL_MMA     cell-binned, one lane per particle, the harmonic sum as FP64 DMMA.8x8x4 over groups of eight
+ *                     particles, stencil window staged in shared memory by bulk copy; the default for large
+ *                     ensembles (needs max |xn| <= 16, max xm <= 16)
  *   GC_KERNEL_TILE    cell-binned, one thread per particle, stencil window staged in shared memory by bulk
  *                     copy; the kernel for large ensembles (needs max |xn| <= 16 and a window that fits
  *                     shared memory)
  *   GC_KERNEL_WARP    one warp per particle, stencil window in registers; the kernel for small ensembles
  *                     (needs max |xn| <= 16, max xm <= 28)
  *   GC_KERNEL_GENERIC one thread per particle, tables read from global memory; any field
- *   GC_KERNEL_AUTO    per call: TILE when the field fits it and n >= GC_TILE_MIN_PARTICLES, else WARP when the
- *                     field fits it, else GENERIC.
- * All three implement the same equations and controller; their results differ at rounding level only. */
+ *   GC_KERNEL_AUTO    per call: MMA (else TILE) when the field fits it and n >= GC_TILE_MIN_PARTICLES, else WARP
+ *                     when the field fits it, else GENERIC.
+ * All four implement the same equations and controller; their results differ at rounding level only. */
 enum { GC_KERNEL_AUTO = 0, GC_KERNEL_GENERIC = 1, GC_KERNEL_WARP = 2, GC_KERNEL_TILE = 3, GC_KERNEL_MMA = 4 };
 enum { GC_TILE_MIN_PARTICLES = 8192 };
 
@@ -145,7 +148,7 @@ int gc_trace_host(const gc_field* f, const gc_trace_params* params, int64_t n,
 /* Kernel choice (GC_KERNEL_*) for later gc_trace / gc_rhs_eval calls on this field (default AUTO); GC_EINVAL
  * if the field does not fit the requested kernel. */
 int gc_set_kernel(gc_field* f, int32_t kernel);
-/* Which kernel gc_trace will launch for this field and n particles (GC_KERNEL_GENERIC, _WARP or _TILE), and
+/* Which kernel gc_trace will launch for this field and n particles (GC_KERNEL_GENERIC, _WARP, _TILE or _MMA), and
  * its launch geometry; any pointer may be NULL. */
 int gc_kernel_info(const gc_field* f, int64_t n, int32_t* kernel, int32_t* blocks, int32_t* threads_per_block,
                    int32_t* smem_bytes, int32_t* regs_per_thread);

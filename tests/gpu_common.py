@@ -75,7 +75,7 @@ def oracle_conditioning(OF, spec, P, mu, base, **kw):
 
 
 def assert_trace_parity(r_gpu, r_ref, spec, min_same=1.0 - FLIP_FRACTION, label="", cond=None,
-                        min_within=1.0):
+                        min_within=1.0, median_rtol=MEDIAN_RTOL, flip_rtol=FLIP_RTOL):
     """cond = oracle_conditioning(...) or None (flat 1e-9 for particles on the oracle's step sequence,
     FLIP_RTOL for the others).  min_within: least fraction of particles inside the flat 1e-9."""
     yg = r_gpu.y.cpu().numpy()
@@ -91,21 +91,21 @@ def assert_trace_parity(r_gpu, r_ref, spec, min_same=1.0 - FLIP_FRACTION, label=
     rel = rel_diff(yg, r_ref.y, spec.v_ref)
     relt = np.abs(tg - r_ref.t) / np.maximum(np.abs(r_ref.t), 1e-300)
     assert same.mean() >= min_same, f"{label}: only {same.mean() * 100:.2f} % of particles took the oracle's step sequence"
-    assert np.median(rel) <= MEDIAN_RTOL, f"{label}: median rel diff {np.median(rel):.3e}"
+    assert np.median(rel) <= median_rtol, f"{label}: median rel diff {np.median(rel):.3e}"
     within = float((rel[stable] <= SAME_RTOL).mean())
     assert within >= min_within, f"{label}: only {within * 100:.2f} % of particles within {SAME_RTOL}"
     if cond is None:
-        tol = np.where(same, SAME_RTOL, FLIP_RTOL)
-        tolt = np.where(same, SAME_RTOL, FLIP_RTOL)
+        tol = np.where(same, SAME_RTOL, flip_rtol)
+        tolt = np.where(same, SAME_RTOL, flip_rtol)
     else:
         # a flipped accept/reject decision puts the particle on another step sequence: bounded by FLIP_RTOL
-        tol = np.where(same, np.maximum(SAME_RTOL, COND_FACTOR * cond[0]), FLIP_RTOL)
-        tolt = np.where(same, np.maximum(SAME_RTOL, COND_FACTOR * cond[1]), FLIP_RTOL)
+        tol = np.where(same, np.maximum(SAME_RTOL, COND_FACTOR * cond[0]), flip_rtol)
+        tolt = np.where(same, np.maximum(SAME_RTOL, COND_FACTOR * cond[1]), flip_rtol)
     worst = int(np.argmax(np.where(stable, rel / tol, 0.0)))
     assert (rel[stable] <= tol[stable]).all(), \
         f"{label}: particle {worst}: rel diff {rel[worst]:.3e} > tolerance {tol[worst]:.3e}"
     assert (relt[stable] <= tolt[stable]).all(), f"{label}: t_out differs by {relt[stable].max():.3e}"
-    assert rel[stable].max() <= FLIP_RTOL, f"{label}: max rel diff {rel.max():.3e} > {FLIP_RTOL}"
+    assert rel[stable].max() <= flip_rtol, f"{label}: max rel diff {rel.max():.3e} > {flip_rtol}"
     if same.any():
         assert np.array_equal(r_gpu.n_forced.cpu().numpy()[same], r_ref.n_forced[same])
     return dict(same_frac=float(same.mean()), max_rel=float(rel[stable].max()), median_rel=float(np.median(rel)),

@@ -291,9 +291,9 @@ int pack_mma_image(gc_field* f, const gc_field_desc* d) {
   const int MT = small ? 1 : 2, KS = small ? 2 : 4;
   const int RS = small ? gc::MmaRow<1, 2>::stride(d->nk) : gc::MmaRow<2, 4>::stride(d->nk);
 #ifdef GC_MMA_L1
-  const int smem = (int)((size_t)((gc::kSubBins + 2) * (d->ns - 3) / 2 + 2) * sizeof(double) + (size_t)7 * 4 * gc::kMmaThreads * sizeof(double) + 64);
+  const int smem = (int)((size_t)((gc::kSubBins + 2) * (d->ns - 3) / 2 + 2) * sizeof(double) + (size_t)(7 * 4 + 2 * gc::kMmaWtab) * gc::kMmaThreads * sizeof(double) + 64);
 #else
-  const int smem = (int)((size_t)gc::kMmaWinRows * RS * sizeof(double) + (size_t)7 * 4 * gc::kMmaThreads * sizeof(double) + 64);
+  const int smem = (int)((size_t)gc::kMmaWinRows * RS * sizeof(double) + (size_t)(7 * 4 + 2 * gc::kMmaWtab) * gc::kMmaThreads * sizeof(double) + 64);
 #endif
   if (smem > 110 * 1024) return GC_OK;
   const int ncell = d->ns - 3;

@@ -60,6 +60,7 @@ constexpr int kMmaBlocksPerSm = GC_MMA_MINB;     // 8 warps per SM at <= 255 reg
 constexpr int kMmaCap = GC_MMA_CAP;              // attempted steps per particle per chunk (short: re-binning keeps the
                                                  // groups on 4-row unions and parks fewer particles)
 constexpr int kMmaWinRows = 8;                   // node rows cell-2 .. cell+5
+constexpr int kMmaWtab = 6;                      // (w, dw) entries of a particle's weight table in shared memory
 constexpr int kMmaNone = 1 << 20;                // "no stencil": a row offset that gives weight 0 on every row
 
 // Offsets (in doubles) inside one node row of the image; RS = row stride.
@@ -101,13 +102,14 @@ __device__ __forceinline__ void cmul(double a, double b, double c, double d, dou
 
 
 // One pass over node rows r_lo .. r_hi (warp-uniform) of the image at `base` (row r at base + r RS) for the group of
-// 8 particles whose lanes are 8 G .. 8 G + 7.  Every lane plays two roles.  As PARTICLE lane it offers, row by row,
-// the Lagrange weight of its own stencil (off_p = row of its first stencil node in this pass, kMmaNone when it does
-// not take part: weight 0 on every row).  As FRAGMENT lane (g = lane / 4, q = lane % 4) it fetches the weights of
-// particle `src` = 8 G + g, issues the DMMA and accumulates its share of B, B_s, B_theta, B_zeta / nfp in o[].
+// 8 particles whose lanes are 8 G .. 8 G + 7, executed by the lanes in their FRAGMENT role (g = lane / 4,
+// q = lane % 4, serving particle 8 G + g).  wsrc = that particle's weight table in shared memory (6 x (w, dw):
+// zero, the four stencil weights, zero), off_f = row of its first stencil node in this pass (kMmaNone when it does
+// not take part: weight 0 on every row).  Issues the DMMA and accumulates this lane's share of B, B_s, B_theta,
+// B_zeta / nfp in o[].
 template <int MT, int KS, class Ld>
-__device__ __forceinline__ void mma_sweep(const double* base, int RS, int r_lo, int r_hi, int off_p,
-                                          const double (&w)[4], const double (&dw)[4], int src, int lane, int q,
+__device__ __forceinline__ void mma_sweep(const double* base, int RS, int r_lo, int r_hi, int off_f,
+                                          const double2* wsrc, int lane, int q,
                                           const double (&AC)[KS], const double (&AS)[KS], const double (&AnC)[KS],
                                           const double (&AnS)[KS], const double (&cm)[2 * MT],
                                           const double (&sm)[2 * MT], double (&o)[4]) {
@@ -118,10 +120,10 @@ __device__ __forceinline__ void mma_sweep(const double* base, int RS, int r_lo, 
   constexpr int kRowUnroll = GC_MMA_ROW_UNROLL;
 #pragma unroll kRowUnroll
   for (int r = r_lo; r <= r_hi; ++r) {
-    const int idx = r - off_p;
-    const double wsel = idx == 0 ? w[0] : idx == 1 ? w[1] : idx == 2 ? w[2] : idx == 3 ? w[3] : 0.0;
-    const double dwsel = idx == 0 ? dw[0] : idx == 1 ? dw[1] : idx == 2 ? dw[2] : idx == 3 ? dw[3] : 0.0;
-    const double wr = __shfl_sync(0xffffffffu, wsel, src), dwr = __shfl_sync(0xffffffffu, dwsel, src);
+    // (w, dw) of row r for the particle this lane serves: entries 1..4 of its table are the stencil weights,
+    // entries 0 and 5 are zero (rows outside the stencil)
+    const double2 wd = wsrc[min(max(r - off_f, -1), 4) + 1];
+    const double wr = wd.x, dwr = wd.y;
     const double* row = base + (size_t)r * RS;
     double T1 = 0.0, T2 = 0.0, T3 = 0.0;
 #pragma unroll
@@ -166,9 +168,9 @@ __device__ __forceinline__ void mma_sweep(const double* base, int RS, int r_lo, 
 // Right-hand side of one lane = one particle (same contract as rhs_tile); must be called by all 32 lanes of a warp.
 // win = shared-memory copy of image rows cell .. cell+7 (node rows cell-2 .. cell+5).
 template <int MT, int KS, bool MODES>
-__device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, int cell, bool active, double mass,
-                                        double charge, double mu, double v_ref, double inv_v_ref, double t,
-                                        const double (&y)[4], double (&dy)[4]) {
+__device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, double* ext, int cell, bool active,
+                                        double mass, double charge, double mu, double v_ref, double inv_v_ref,
+                                        double t, const double (&y)[4], double (&dy)[4]) {
   using R = MmaRow<MT, KS>;
   const int lane = threadIdx.x & 31, q = lane & 3;
   const int RS = f.mma_RS;
@@ -179,6 +181,14 @@ __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, in
   const int off = i0 - cell + 2;
   const bool inwin = active && off >= 0 && off <= kMmaWinRows - 4;
   const bool outside = active && !inwin;
+  // weight table of this particle for the fragment lanes: [0] = [5] = 0, [1 + a] = (w[a], dw[a])
+  double2* wtab = reinterpret_cast<double2*>(ext) + (size_t)threadIdx.x * kMmaWtab;
+  __syncwarp();                                                         // fragment lanes are done with the last table
+  wtab[0] = make_double2(0.0, 0.0);
+#pragma unroll
+  for (int a = 0; a < 4; ++a) wtab[1 + a] = make_double2(w[a], dw[a]);
+  wtab[5] = make_double2(0.0, 0.0);
+  __syncwarp();
   const double thr = active ? reduce_2pi(y[1]) : 0.0;                 // idle lanes offer finite operands
   const double phr = active ? reduce_2pi((double)f.nfp * y[2]) : 0.0;
   double c1, s1, C1, S1;
@@ -191,6 +201,7 @@ __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, in
     if (((onmask >> (8 * G)) & 0xFFu) == 0u) continue;                // warp-uniform
     const int src = 8 * G + (lane >> 2);
     const bool ingrp = (lane >> 3) == G;
+    const double2* wsrc = wtab + ((src - lane) * kMmaWtab);           // table of particle src (same warp)
     // ---- fragment role: trigonometry of particle src for n = 4 j + q + 1 and m = 1 + 8 T + 2 q + e -----------------
     const double gc1 = __shfl_sync(0xffffffffu, c1, src), gs1 = __shfl_sync(0xffffffffu, s1, src);
     const double gC1 = __shfl_sync(0xffffffffu, C1, src), gS1 = __shfl_sync(0xffffffffu, S1, src);
@@ -230,21 +241,23 @@ __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, in
     // ---- in-window stencils of the group: one sweep over the union of their rows ---------------------------------
     const int r_lo = __reduce_min_sync(0xffffffffu, (ingrp && inwin) ? off : kMmaNone);
     const int r_hi = __reduce_max_sync(0xffffffffu, (ingrp && inwin) ? off + 3 : -1);
-    if (r_hi >= 0)
+    if (r_hi >= 0) {
+      const int off_f = __shfl_sync(0xffffffffu, inwin ? off : kMmaNone, src);
 #ifdef GC_MMA_L1
-      mma_sweep<MT, KS, LdG>(f.mma_image + (size_t)cell * RS, RS, r_lo, r_hi, (ingrp && inwin) ? off : kMmaNone, w, dw,
-                             src, lane, q, AC, AS, AnC, AnS, cm, sm, o);
+      mma_sweep<MT, KS, LdG>(f.mma_image + (size_t)cell * RS, RS, r_lo, r_hi, off_f, wsrc, lane, q, AC, AS, AnC, AnS,
+                             cm, sm, o);
 #else
-      mma_sweep<MT, KS, LdS>(win, RS, r_lo, r_hi, (ingrp && inwin) ? off : kMmaNone, w, dw, src, lane, q, AC, AS, AnC,
-                             AnS, cm, sm, o);
+      mma_sweep<MT, KS, LdS>(win, RS, r_lo, r_hi, off_f, wsrc, lane, q, AC, AS, AnC, AnS, cm, sm, o);
 #endif
+    }
     // ---- stencils outside the window: one sweep per distinct stencil, rows from global memory ----------------------
     unsigned pend = __ballot_sync(0xffffffffu, ingrp && outside);
     while (pend) {
       const int i0L = __shfl_sync(0xffffffffu, i0, __ffs(pend) - 1);
       const bool mine = ingrp && outside && i0 == i0L;
-      mma_sweep<MT, KS, LdG>(f.mma_image + (size_t)(i0L + 2) * RS, RS, 0, 3, mine ? 0 : kMmaNone, w, dw, src, lane, q,
-                             AC, AS, AnC, AnS, cm, sm, o);
+      const int off_f = __shfl_sync(0xffffffffu, mine ? 0 : kMmaNone, src);
+      mma_sweep<MT, KS, LdG>(f.mma_image + (size_t)(i0L + 2) * RS, RS, 0, 3, off_f, wsrc, lane, q, AC, AS, AnC, AnS,
+                             cm, sm, o);
       pend &= ~__ballot_sync(0xffffffffu, mine);
     }
     // ---- back to the particle lanes: lane 8 G + g takes the quad sum of fragment lanes 4 g .. 4 g + 3 ---------------
@@ -321,13 +334,14 @@ struct MmaEngine {
   static constexpr bool kStageWindow = true;
   static __device__ __forceinline__ int win_doubles(const FieldDev& f) { return kMmaWinRows * f.mma_RS; }
 #endif
+  static constexpr int kExtDoubles = 2 * kMmaWtab;                   // per-thread weight table
   static __device__ __forceinline__ const double* win_src(const FieldDev& f, int cell) {
     return f.mma_image + (size_t)cell * f.mma_RS;                     // image rows cell .. cell+7
   }
-  static __device__ __forceinline__ void rhs(const FieldDev& f, const double* win, int cell, bool active, double mass,
-                                             double charge, double mu, double v_ref, double inv_v_ref, double t,
-                                             const double (&y)[4], double (&dy)[4]) {
-    rhs_mma<MT, KS, MODES>(f, win, cell, active, mass, charge, mu, v_ref, inv_v_ref, t, y, dy);
+  static __device__ __forceinline__ void rhs(const FieldDev& f, const double* win, double* ext, int cell, bool active,
+                                             double mass, double charge, double mu, double v_ref, double inv_v_ref,
+                                             double t, const double (&y)[4], double (&dy)[4]) {
+    rhs_mma<MT, KS, MODES>(f, win, ext, cell, active, mass, charge, mu, v_ref, inv_v_ref, t, y, dy);
   }
 };
 

@@ -285,13 +285,14 @@ extern __shared__ __align__(128) unsigned char gc_tile_smem[];
 template <int NMAX, bool MODES>
 struct TileEngine {
   static constexpr bool kStageWindow = true;
+  static constexpr int kExtDoubles = 0;         // no per-thread shared scratch beyond kbuf
   static __device__ __forceinline__ int win_doubles(const FieldDev& f) { return 10 * f.tile_E; }
   static __device__ __forceinline__ const double* win_src(const FieldDev& f, int cell) {
     return f.tile_images + (size_t)cell * (10 * f.tile_E);
   }
-  static __device__ __forceinline__ void rhs(const FieldDev& f, const double* win, int cell, bool active, double mass,
-                                             double charge, double mu, double v_ref, double inv_v_ref, double t,
-                                             const double (&y)[4], double (&dy)[4]) {
+  static __device__ __forceinline__ void rhs(const FieldDev& f, const double* win, double*, int cell, bool active,
+                                             double mass, double charge, double mu, double v_ref, double inv_v_ref,
+                                             double t, const double (&y)[4], double (&dy)[4]) {
     rhs_tile<NMAX, MODES>(f, win, cell, active, mass, charge, mu, v_ref, inv_v_ref, t, y, dy);
   }
 };
@@ -313,7 +314,8 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
 
   double* win = reinterpret_cast<double*>(gc_tile_smem);                 // [WD] window image of the tile's cell
   double* kbuf = win + WD;                                               // [7][4][THREADS]
-  unsigned long long* bar = reinterpret_cast<unsigned long long*>(kbuf + 7 * 4 * THREADS);
+  double* ext = kbuf + 7 * 4 * THREADS;                                  // [Eng::kExtDoubles][THREADS] engine scratch
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(ext + Eng::kExtDoubles * THREADS);
   int* s_int = reinterpret_cast<int*>(bar + 1);                          // [0] tile id; scan space follows
   auto kb = [&](int j, int c) -> double& { return kbuf[(j * 4 + c) * THREADS + tid]; };
 
@@ -485,7 +487,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
             }
             double dy[4] = {0.0, 0.0, 0.0, 0.0};
             const bool lane_on = running && (stage > 0 || !(flags & kFlagHaveK1));
-            Eng::rhs(f, win, cell, lane_on, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, ts, ys, dy);
+            Eng::rhs(f, win, ext, cell, lane_on, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, ts, ys, dy);
             if (lane_on) {
               kb(stage, 0) = dy[0]; kb(stage, 1) = dy[1]; kb(stage, 2) = dy[2]; kb(stage, 3) = dy[3];
               if (stage == 0) {

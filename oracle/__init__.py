@@ -228,6 +228,46 @@ class OracleField:
             res.traj, res.traj_count = traj, tcount
         return res
 
+    def trace_sampled(self, spec, s0, th0, ze0, vpar0, mu, sample_t0, sample_dt, nsamp, h_in=None, t0=None,
+                      t_max=None) -> TraceResult:
+        """O9: the trace with uniform-time samples of the continuous extension; adds ``samples`` [4][nsamp][n]
+        and ``nsampled`` [n] (= sample_end: one past the last sample index written) to the result."""
+        s0, th0, ze0, vpar0, mu = map(_f64, (s0, th0, ze0, vpar0, mu))
+        n = s0.shape[0]
+        p = _Params(spec.mass, spec.charge, spec.t0 if t0 is None else t0,
+                    spec.t_max if t_max is None else t_max, spec.rtol, spec.atol, spec.v_ref,
+                    spec.h0, spec.h_min, spec.s_loss, spec.s_min, int(spec.max_steps), 0, 0)
+        h = np.zeros(n) if h_in is None else _f64(h_in).copy()
+        y = np.zeros((4, n))
+        t = np.zeros(n)
+        status = np.zeros(n, np.int32)
+        n_acc, n_rej, n_forced = (np.zeros(n, np.int32) for _ in range(3))
+        samples = np.full((4, int(nsamp), n), np.nan)
+        nsampled = np.zeros(n, np.int32)
+        L = _load()
+        L.oracle_trace_sampled.argtypes = [C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 12 + \
+            [C.c_double, C.c_double, C.c_int64, C.c_void_p, C.c_void_p]
+        rc = L.oracle_trace_sampled(self._h, C.byref(p), C.c_int64(n), _p(s0), _p(th0), _p(ze0), _p(vpar0),
+                                    _p(mu), _p(h), _p(y), _p(t), _p(status), _p(n_acc), _p(n_rej), _p(n_forced),
+                                    float(sample_t0), float(sample_dt), int(nsamp), _p(samples), _p(nsampled))
+        if rc != 0:
+            raise ValueError("oracle_trace_sampled: bad arguments")
+        res = TraceResult(y, t, status, n_acc, n_rej, n_forced, h)
+        res.samples, res.nsampled = samples, nsampled
+        return res
+
+    def pzeta(self, mass, charge, chi_nodes, s, th, ze, vpar, t):
+        """A17: P_zeta at arrays of states and times (broadcast)."""
+        chi_nodes = _f64(chi_nodes)
+        L = _load()
+        L.oracle_pzeta.restype = C.c_double
+        L.oracle_pzeta.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_void_p] + [C.c_double] * 5
+        s, th, ze, vpar, t = np.broadcast_arrays(*(np.asarray(a, float) for a in (s, th, ze, vpar, t)))
+        out = np.empty(s.shape)
+        for idx in np.ndindex(s.shape):
+            out[idx] = L.oracle_pzeta(self._h, mass, charge, _p(chi_nodes), s[idx], th[idx], ze[idx], vpar[idx], t[idx])
+        return out
+
     def rk4(self, mass, charge, v_ref, s0, th0, ze0, vpar0, mu, t0, h, nsteps):
         s0, th0, ze0, vpar0, mu = map(_f64, (s0, th0, ze0, vpar0, mu))
         n = s0.shape[0]
@@ -257,3 +297,32 @@ def dp5_attempt_fn(fun, t, y, h, k1=None):
     _load().oracle_dp5_attempt_fn(cb, None, C.c_double(t), _p(y), _p(k1), C.c_double(h),
                                   _p(y_new), _p(k), _p(delta))
     return y_new, k, delta
+
+
+# ---- weighted Birkhoff average (NEXT-1; PAPER.md:50,94 cite Duignan & Meiss 2023) -----------------------------
+def birkhoff_weights(N: int) -> np.ndarray:
+    """w_j = g((j + 1) / (N + 1)), g(x) = exp(-1 / (x (1 - x))), j = 0 .. N-1: the C-infinity bump of the weighted
+    Birkhoff average, sampled strictly inside (0, 1) so that no weight is 0/0."""
+    x = (np.arange(N) + 1.0) / (N + 1.0)
+    return np.exp(-1.0 / (x * (1.0 - x)))
+
+
+def birkhoff_average(f) -> float:
+    """WB_N(f) = sum_j w_j f_j / sum_j w_j."""
+    f = np.asarray(f, float)
+    w = birkhoff_weights(f.shape[0])
+    return float(np.sum(w * f) / np.sum(w))
+
+
+def birkhoff_digits(f):
+    """(WB of the first half, WB of the second half, digit accuracy): the series is cut into two halves of
+    N = len(f) // 2 samples; digits = -log10(|WB_1 - WB_2| / max(|WB_1|, |WB_2|)), capped at 16 (reading A25 of
+    DESIGN.md: an orbit on an invariant torus gives many digits, a chaotic one few; PAPER.md:94 quotes the
+    threshold 3)."""
+    f = np.asarray(f, float)
+    N = f.shape[0] // 2
+    a, b = birkhoff_average(f[:N]), birkhoff_average(f[N:2 * N])
+    scale = max(abs(a), abs(b))
+    d = abs(a - b)
+    digits = 16.0 if (d == 0.0 or scale == 0.0) else min(16.0, -np.log10(d / scale))
+    return a, b, float(digits)

@@ -352,14 +352,19 @@ static void poincare_step(int64_t id, double t, double h, const double y[4], con
 }
 
 /* ---- O5-O8: the trace -------------------------------------------------------------------------------- */
-int oracle_trace(const oracle_field *f, const oracle_trace_params *p, int64_t n,
-                 const double *s0, const double *th0, const double *ze0, const double *vpar0,
-                 const double *mu, double *h_inout,
-                 double *y_out, double *t_out, int32_t *status,
-                 int32_t *n_acc_out, int32_t *n_rej_out, int32_t *n_forced_out,
-                 double *poincare, int64_t *poincare_count,
-                 double *traj, int64_t *traj_count) {
+/* O9 (NEXT-1): time of sample j.  One fused multiply-add, so that both implementations round it alike. */
+static double sample_time(double sample_t0, double sample_dt, int64_t j) { return fma((double)j, sample_dt, sample_t0); }
+
+static int trace_impl(const oracle_field *f, const oracle_trace_params *p, int64_t n,
+                      const double *s0, const double *th0, const double *ze0, const double *vpar0,
+                      const double *mu, double *h_inout,
+                      double *y_out, double *t_out, int32_t *status,
+                      int32_t *n_acc_out, int32_t *n_rej_out, int32_t *n_forced_out,
+                      double *poincare, int64_t *poincare_count,
+                      double *traj, int64_t *traj_count,
+                      double sample_t0, double sample_dt, int64_t nsamp, double *samples, int32_t *nsampled) {
   if (!f || !p || n < 0 || !(p->v_ref > 0.0) || !(p->h0 > 0.0) || p->h_min < 0.0) return -1;
+  if (nsamp > 0 && (!samples || !(sample_dt > 0.0))) return -1;
   if (poincare_count) *poincare_count = 0;
   int64_t pcap = (poincare && poincare_count) ? p->poincare_capacity : 0;
   int64_t tcap = (traj && traj_count) ? p->traj_capacity : 0;
@@ -374,6 +379,15 @@ int oracle_trace(const oracle_field *f, const oracle_trace_params *p, int64_t n,
     int32_t n_acc = 0, n_rej = 0, n_forced = 0, st = -1;
     int prev_rejected = 0;
     int64_t ntraj = 0;
+    /* O9: next sample index = first j with tau_j >= t0; a sample that falls on t0 is the initial state */
+    int64_t jn = 0;
+    if (nsamp > 0) {
+      while (jn < nsamp && sample_time(sample_t0, sample_dt, jn) < t) ++jn;
+      if (jn < nsamp && sample_time(sample_t0, sample_dt, jn) == t) {
+        for (int c = 0; c < 4; ++c) samples[((size_t)c * nsamp + jn) * n + i] = c == 3 ? y[3] * p->v_ref : y[c];
+        ++jn;
+      }
+    }
     oracle_rhs(f, p->mass, p->charge, mu[i], p->v_ref, t, y, k1);
     if (!all_finite4(y) || !all_finite4(k1)) st = 4;
     else if (!(t < p->t_max)) st = 0;
@@ -398,7 +412,15 @@ int oracle_trace(const oracle_field *f, const oracle_trace_params *p, int64_t n,
         double sc = oracle_scale_accept(err);
         double h_next = prev_rejected ? h_try * fmin(sc, 1.0) : h_try * sc;
         if (pcap > 0) poincare_step(i, t, h_try, y, y_new, (const double(*)[4])k, poincare, pcap, poincare_count);
-        t = clipped ? p->t_max : t + h_try;
+        const double t_new = clipped ? p->t_max : t + h_try;
+        while (jn < nsamp) {                   /* O9: samples with t < tau_j <= t_new from the continuous extension */
+          double tj = sample_time(sample_t0, sample_dt, jn), ys[4];
+          if (tj > t_new) break;
+          oracle_dp5_dense(y, y_new, (const double(*)[4])k, h_try, (tj - t) / h_try, ys);
+          for (int c = 0; c < 4; ++c) samples[((size_t)c * nsamp + jn) * n + i] = c == 3 ? ys[3] * p->v_ref : ys[c];
+          ++jn;
+        }
+        t = t_new;
         for (int c = 0; c < 4; ++c) { y[c] = y_new[c]; k1[c] = k[6][c]; }
         ++n_acc;
         if (forced) ++n_forced;
@@ -434,8 +456,47 @@ int oracle_trace(const oracle_field *f, const oracle_trace_params *p, int64_t n,
     if (n_rej_out) n_rej_out[i] = n_rej;
     if (n_forced_out) n_forced_out[i] = n_forced;
     if (traj_count) traj_count[i] = ntraj;
+    if (nsampled) nsampled[i] = (int32_t)jn;
   }
   return 0;
+}
+
+int oracle_trace(const oracle_field *f, const oracle_trace_params *p, int64_t n,
+                 const double *s0, const double *th0, const double *ze0, const double *vpar0,
+                 const double *mu, double *h_inout,
+                 double *y_out, double *t_out, int32_t *status,
+                 int32_t *n_acc_out, int32_t *n_rej_out, int32_t *n_forced_out,
+                 double *poincare, int64_t *poincare_count,
+                 double *traj, int64_t *traj_count) {
+  return trace_impl(f, p, n, s0, th0, ze0, vpar0, mu, h_inout, y_out, t_out, status, n_acc_out, n_rej_out,
+                    n_forced_out, poincare, poincare_count, traj, traj_count, 0.0, 0.0, 0, NULL, NULL);
+}
+
+int oracle_trace_sampled(const oracle_field *f, const oracle_trace_params *p, int64_t n,
+                         const double *s0, const double *th0, const double *ze0, const double *vpar0,
+                         const double *mu, double *h_inout,
+                         double *y_out, double *t_out, int32_t *status,
+                         int32_t *n_acc_out, int32_t *n_rej_out, int32_t *n_forced_out,
+                         double sample_t0, double sample_dt, int64_t nsamp, double *samples, int32_t *nsampled) {
+  return trace_impl(f, p, n, s0, th0, ze0, vpar0, mu, h_inout, y_out, t_out, status, n_acc_out, n_rej_out,
+                    n_forced_out, NULL, NULL, NULL, NULL, sample_t0, sample_dt, nsamp, samples, nsampled);
+}
+
+/* A17: canonical toroidal momentum P_zeta = q ((rho + alpha) G - chi(s)), rho = m v_par / (q B), chi' = iota with
+ * respect to psi; chi is given at the radial nodes and interpolated like every other profile (O1). */
+double oracle_pzeta(const oracle_field *f, double mass, double charge, const double *chi_nodes,
+                    double s, double th, double ze, double vpar, double t) {
+  double fb[4], pr[6], pt[9] = {0};
+  int32_t i0;
+  double w[4], dw[4];
+  oracle_eval_B(f, s, th, ze, fb);
+  oracle_eval_profiles(f, s, pr);
+  oracle_eval_pert(f, s, th, ze, t, pt);
+  oracle_lagrange(f->ns, s, &i0, w, dw);
+  double chi = 0.0;
+  for (int a = 0; a < 4; ++a) chi += w[a] * chi_nodes[i0 + a];
+  double rho = mass * vpar / (charge * fb[0]);
+  return charge * ((rho + pt[4]) * pr[0] - chi);
 }
 
 /* ---- check (d): classical RK4 at fixed step -------------------------------------------------------- */

@@ -98,6 +98,24 @@ int oracle_trace(const oracle_field *f, const oracle_trace_params *p, int64_t n,
                  double *poincare, int64_t *poincare_count,
                  double *traj, int64_t *traj_count);
 
+/* O9 (NEXT-1 of SURVEY.md section 8(f); "dense output", "given trajectory data, transport
+ * diagnostics include ... weighted Birkhoff averaging"): the same trace, recording the state at the uniform times
+ * tau_j = sample_t0 + j sample_dt, j = 0 .. nsamp-1, from the continuous extension of the accepted step that
+ * contains tau_j (t < tau_j <= t_new; a sample that falls on t0 is the initial state).
+ * samples [4][nsamp][n] = s, theta, zeta, v_par (m/s); sample_end [n] = index of the next sample the particle
+ * would have written: its samples j_first <= j < sample_end are valid, j_first = first j with tau_j >= t0; a
+ * particle that stops early leaves the later ones untouched. */
+int oracle_trace_sampled(const oracle_field *f, const oracle_trace_params *p, int64_t n,
+                         const double *s0, const double *th0, const double *ze0, const double *vpar0,
+                         const double *mu, double *h_inout,
+                         double *y_out, double *t_out, int32_t *status,
+                         int32_t *n_acc, int32_t *n_rej, int32_t *n_forced,
+                         double sample_t0, double sample_dt, int64_t nsamp, double *samples, int32_t *sample_end);
+
+/* A17: P_zeta = q ((rho + alpha) G - chi), rho = m v_par / (q B); chi_nodes [ns] = chi at the radial nodes. */
+double oracle_pzeta(const oracle_field *f, double mass, double charge, const double *chi_nodes,
+                    double s, double th, double ze, double vpar, double t);
+
 /* Check (d): classical fixed-step RK4, nsteps steps of size h from t0; y_out [4][n]. */
 void oracle_rk4(const oracle_field *f, double mass, double charge, double v_ref, int64_t n,
                 const double *s0, const double *th0, const double *ze0, const double *vpar0,

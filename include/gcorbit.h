@@ -145,6 +145,43 @@ int gc_trace_host(const gc_field* f, const gc_trace_params* params, int64_t n,
                   int32_t* n_acc, int32_t* n_rej, int32_t* n_forced,
                   double* poincare, int64_t* poincare_count);
 
+/* ---- NEXT-1 of SURVEY.md section 8(f): uniform-time samples of the continuous extension and the diagnostics they
+ * feed ("dense output"; "given trajectory data, transport diagnostics include ... weighted
+ * Birkhoff averaging"; "the weighted Birkhoff average of P_zeta serves as an integrability
+ * diagnostic, with digit accuracy below 3 indicating chaotic motion").  Readings O9, A25 of DESIGN.md section 12.
+ *
+ * gc_trace_sampled = gc_trace (same arguments, same results, no Poincare records) that also records the state at
+ * the times tau_j = fma(j, sample_dt, sample_t0), j = 0 .. nsamp-1, from the 4th-order continuous extension of the
+ * accepted step with t < tau_j <= t_new; a sample that falls on t0 is the initial state.
+ *   samples    [4][nsamp][n] DEVICE: s, theta, zeta, v_par (m/s); entries not reached are left untouched
+ *   sample_end [n] DEVICE int32: index of the next sample the particle would write; its valid samples are
+ *              j_first <= j < sample_end with j_first = first j with tau_j >= t0 (of the first segment)
+ * Under GC_TRACE_RESUME the sample grid simply continues (same sample_t0, sample_dt, buffers).  Small ensembles
+ * are traced by the generic kernel (the warp kernel records no samples); GC_EINVAL if sample_dt <= 0 or a
+ * buffer is NULL with nsamp > 0. */
+int gc_trace_sampled(const gc_field* f, const gc_trace_params* params, int64_t n,
+                     const double* s0, const double* th0, const double* ze0, const double* vpar0,
+                     const double* mu, double* h_inout,
+                     double* y_out, double* t_out, int32_t* status,
+                     int32_t* n_acc, int32_t* n_rej, int32_t* n_forced,
+                     double sample_t0, double sample_dt, int64_t nsamp, double* samples, int32_t* sample_end,
+                     void* stream);
+
+/* A17: canonical toroidal momentum P_zeta = q ((rho + alpha) G - chi(s)), rho = m v_par / (q B), at n states and
+ * times.  DEVICE pointers.  y [4][n] = s, theta, zeta, v_par (m/s) (a [4][nsamp][n] sample buffer is such an array
+ * with n' = nsamp n); t [n] times (alpha depends on t; may be NULL for a static field); chi_nodes [ns]: chi at the
+ * radial nodes, d chi / d psi = iota, interpolated like every profile (O1); out [n] in J s / m ... (kg m^2 / s). */
+int gc_pzeta_eval(const gc_field* f, double mass, double charge, int64_t n, const double* y, const double* t,
+                  const double* chi_nodes, double* out, void* stream);
+
+/* Weighted Birkhoff average of n series (A25).  DEVICE pointers.  series [nsamp][n]; for series i the samples
+ * j_first <= j < (sample_end ? sample_end[i] : nsamp) are cut into two halves of N = count / 2 samples and each
+ * half is averaged with the weights w_k = g((k + 1) / (N + 1)), g(x) = exp(-1 / (x (1 - x))), k = 0 .. N-1.
+ * out [3][n] = WB of the first half, WB of the second half, digit accuracy
+ * -log10(|WB_1 - WB_2| / max(|WB_1|, |WB_2|)) capped at 16 (NaN for series with fewer than 4 samples). */
+int gc_birkhoff(int64_t n, int64_t nsamp, const double* series, int64_t j_first, const int32_t* sample_end,
+                double* out, void* stream);
+
 /* Kernel choice (GC_KERNEL_*) for later gc_trace / gc_rhs_eval calls on this field (default AUTO); GC_EINVAL
  * if the field does not fit the requested kernel. */
 int gc_set_kernel(gc_field* f, int32_t kernel);

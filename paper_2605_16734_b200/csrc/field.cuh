@@ -50,6 +50,11 @@ struct TraceDev {
   double* poincare;
   unsigned long long* poincare_count;
   unsigned long long* work_counter;   // persistent-kernel particle queue head
+  // O9 (gc_trace_sampled): samples[4][nsamp][n] at tau_j = fma(j, sample_dt, sample_t0); nsamp = 0 disables
+  double sample_t0, sample_dt;
+  long long nsamp;
+  double* samples;
+  int* sample_end;
 };
 
 }  // namespace gc

@@ -174,19 +174,23 @@ int pack_rows(gc_field* f, const gc_field_desc* d) {
 }
 
 // ---- tile-kernel instantiations and window images -------------------------------------------------------------
-const void* tile_fn(const gc_field* f) {
+template <bool SAMPLE>
+const void* tile_fn_t(const gc_field* f) {
   const bool modes = f->dev.nk > 0;
   if (f->dev.tile_nmax == 8)
-    return modes ? (const void*)gc::trace_tile_kernel<8, true> : (const void*)gc::trace_tile_kernel<8, false>;
-  return modes ? (const void*)gc::trace_tile_kernel<16, true> : (const void*)gc::trace_tile_kernel<16, false>;
+    return modes ? (const void*)gc::trace_tile_kernel<8, true, SAMPLE> : (const void*)gc::trace_tile_kernel<8, false, SAMPLE>;
+  return modes ? (const void*)gc::trace_tile_kernel<16, true, SAMPLE> : (const void*)gc::trace_tile_kernel<16, false, SAMPLE>;
 }
+const void* tile_fn(const gc_field* f, bool sample = false) { return sample ? tile_fn_t<true>(f) : tile_fn_t<false>(f); }
 
-const void* mma_fn(const gc_field* f) {
+template <bool SAMPLE>
+const void* mma_fn_t(const gc_field* f) {
   const bool modes = f->dev.nk > 0;
   if (f->dev.mma_MT == 1)
-    return modes ? (const void*)gc::trace_mma_kernel<1, 2, true> : (const void*)gc::trace_mma_kernel<1, 2, false>;
-  return modes ? (const void*)gc::trace_mma_kernel<2, 4, true> : (const void*)gc::trace_mma_kernel<2, 4, false>;
+    return modes ? (const void*)gc::trace_mma_kernel<1, 2, true, SAMPLE> : (const void*)gc::trace_mma_kernel<1, 2, false, SAMPLE>;
+  return modes ? (const void*)gc::trace_mma_kernel<2, 4, true, SAMPLE> : (const void*)gc::trace_mma_kernel<2, 4, false, SAMPLE>;
 }
+const void* mma_fn(const gc_field* f, bool sample = false) { return sample ? mma_fn_t<true>(f) : mma_fn_t<false>(f); }
 
 int resolve_kernel(const gc_field* f, int64_t n) {
   if (f->kernel != GC_KERNEL_AUTO) return f->kernel;
@@ -248,6 +252,7 @@ int pack_tile_images(gc_field* f, const gc_field_desc* d) {
   f->tile_smem = smem;
   const void* fn = tile_fn(f);
   GC_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  GC_CUDA(cudaFuncSetAttribute(tile_fn(f, true), cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   int per_sm = 0;
   GC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, gc::kTileThreads, (size_t)smem));
   if (per_sm < 1) return GC_OK;
@@ -309,6 +314,7 @@ int pack_mma_image(gc_field* f, const gc_field_desc* d) {
   f->mma_smem = smem;
   const void* fn = mma_fn(f);
   GC_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  GC_CUDA(cudaFuncSetAttribute(mma_fn(f, true), cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   int per_sm = 0;
   GC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, gc::kMmaThreads, (size_t)smem));
   if (per_sm < 1) return GC_OK;
@@ -347,11 +353,12 @@ int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, c
   if (blocks < 1) blocks = 1;
   gc::FieldDev fd = f->dev;
   void* args[] = {(void*)&fd, (void*)&t, (void*)&sc, (void*)&mode, (void*)&rhs_out};
+  const bool sample = mode == 0 && t.nsamp > 0;
   if (mma)
-    GC_CUDA(cudaLaunchCooperativeKernel(mma_fn(f), dim3((unsigned)blocks), dim3(gc::kMmaThreads), args,
+    GC_CUDA(cudaLaunchCooperativeKernel(mma_fn(f, sample), dim3((unsigned)blocks), dim3(gc::kMmaThreads), args,
                                         (size_t)f->mma_smem, st));
   else
-    GC_CUDA(cudaLaunchCooperativeKernel(tile_fn(f), dim3((unsigned)blocks), dim3(gc::kTileThreads), args,
+    GC_CUDA(cudaLaunchCooperativeKernel(tile_fn(f, sample), dim3((unsigned)blocks), dim3(gc::kTileThreads), args,
                                         (size_t)f->tile_smem, st));
   GC_CUDA(cudaFreeAsync(slab, st));
   return GC_OK;
@@ -575,13 +582,19 @@ int gc_rhs_eval(const gc_field* f, double mass, double charge, double t, int64_t
   return GC_OK;
 }
 
-int gc_trace(const gc_field* f, const gc_trace_params* params, int64_t n, const double* s0, const double* th0,
-             const double* ze0, const double* vpar0, const double* mu, double* h_inout, double* y_out,
-             double* t_out, int32_t* status, int32_t* n_acc, int32_t* n_rej, int32_t* n_forced, double* poincare,
-             int64_t* poincare_count, void* stream) {
+}  // extern "C"
+
+namespace {
+int trace_common(const gc_field* f, const gc_trace_params* params, int64_t n, const double* s0, const double* th0,
+                 const double* ze0, const double* vpar0, const double* mu, double* h_inout, double* y_out,
+                 double* t_out, int32_t* status, int32_t* n_acc, int32_t* n_rej, int32_t* n_forced, double* poincare,
+                 int64_t* poincare_count, double sample_t0, double sample_dt, int64_t nsamp, double* samples,
+                 int32_t* sample_end, void* stream) {
   gc::TraceDev t{};
   int rc = build_trace_dev(f, params, n, &t);
   if (rc != GC_OK) return rc;
+  if (nsamp < 0 || (nsamp > 0 && (!samples || !sample_end || !(sample_dt > 0.0) || !std::isfinite(sample_t0))))
+    return fail(GC_EINVAL, "gc_trace_sampled: nsamp > 0 needs sample_dt > 0, finite sample_t0, samples and sample_end");
   if (n == 0) return GC_OK;
   if (!s0 || !th0 || !ze0 || !vpar0 || !mu || !y_out || !t_out || !status)
     return fail(GC_EINVAL, "gc_trace: NULL particle array");
@@ -594,7 +607,9 @@ int gc_trace(const gc_field* f, const gc_trace_params* params, int64_t n, const 
   t.poincare_count = reinterpret_cast<unsigned long long*>(poincare_count);
   if (!poincare || !poincare_count) t.poincare_capacity = 0;
   if (poincare_count) GC_CUDA(cudaMemsetAsync(poincare_count, 0, sizeof(int64_t), st));
-  const int kern = resolve_kernel(f, n);
+  t.sample_t0 = sample_t0; t.sample_dt = sample_dt; t.nsamp = nsamp; t.samples = samples; t.sample_end = sample_end;
+  int kern = resolve_kernel(f, n);
+  if (kern == GC_KERNEL_WARP && nsamp > 0) kern = GC_KERNEL_GENERIC;     // the warp kernel records no samples
   if (kern == GC_KERNEL_TILE || kern == GC_KERNEL_MMA) return launch_tile(f, t, 0, nullptr, st, kern == GC_KERNEL_MMA);
   if (kern == GC_KERNEL_WARP) {
     const WarpInst* w = find_inst(f);
@@ -614,6 +629,52 @@ int gc_trace(const gc_field* f, const gc_trace_params* params, int64_t n, const 
     gc::trace_generic_kernel<<<(unsigned)blocks, 128, 0, st>>>(f->dev, t);
     GC_CUDA(cudaGetLastError());
   }
+  return GC_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int gc_trace(const gc_field* f, const gc_trace_params* params, int64_t n, const double* s0, const double* th0,
+             const double* ze0, const double* vpar0, const double* mu, double* h_inout, double* y_out,
+             double* t_out, int32_t* status, int32_t* n_acc, int32_t* n_rej, int32_t* n_forced, double* poincare,
+             int64_t* poincare_count, void* stream) {
+  return trace_common(f, params, n, s0, th0, ze0, vpar0, mu, h_inout, y_out, t_out, status, n_acc, n_rej, n_forced,
+                      poincare, poincare_count, 0.0, 0.0, 0, nullptr, nullptr, stream);
+}
+
+int gc_trace_sampled(const gc_field* f, const gc_trace_params* params, int64_t n, const double* s0, const double* th0,
+                     const double* ze0, const double* vpar0, const double* mu, double* h_inout, double* y_out,
+                     double* t_out, int32_t* status, int32_t* n_acc, int32_t* n_rej, int32_t* n_forced,
+                     double sample_t0, double sample_dt, int64_t nsamp, double* samples, int32_t* sample_end,
+                     void* stream) {
+  if (params && params->poincare_capacity != 0)
+    return fail(GC_EINVAL, "gc_trace_sampled: records no Poincare crossings (poincare_capacity must be 0)");
+  return trace_common(f, params, n, s0, th0, ze0, vpar0, mu, h_inout, y_out, t_out, status, n_acc, n_rej, n_forced,
+                      nullptr, nullptr, sample_t0, sample_dt, nsamp, samples, sample_end, stream);
+}
+
+int gc_pzeta_eval(const gc_field* f, double mass, double charge, int64_t n, const double* y, const double* t,
+                  const double* chi_nodes, double* out, void* stream) {
+  if (!f || n < 0) return fail(GC_EINVAL, "gc_pzeta_eval: NULL field or n < 0");
+  if (n == 0) return GC_OK;
+  if (!y || !chi_nodes || !out || charge == 0.0) return fail(GC_EINVAL, "gc_pzeta_eval: NULL array or zero charge");
+  const int tb = 128;
+  gc::pzeta_eval_kernel<<<(unsigned)((n + tb - 1) / tb), tb, 0, (cudaStream_t)stream>>>(f->dev, mass, charge, n, y, t,
+                                                                                       chi_nodes, out);
+  GC_CUDA(cudaGetLastError());
+  return GC_OK;
+}
+
+int gc_birkhoff(int64_t n, int64_t nsamp, const double* series, int64_t j_first, const int32_t* sample_end,
+                double* out, void* stream) {
+  if (n < 0 || nsamp < 0 || j_first < 0) return fail(GC_EINVAL, "gc_birkhoff: negative size");
+  if (n == 0) return GC_OK;
+  if (!series || !out) return fail(GC_EINVAL, "gc_birkhoff: NULL array");
+  const int tb = 128;
+  gc::birkhoff_kernel<<<(unsigned)((n + tb - 1) / tb), tb, 0, (cudaStream_t)stream>>>(n, nsamp, series, j_first,
+                                                                                     sample_end, out);
+  GC_CUDA(cudaGetLastError());
   return GC_OK;
 }
 

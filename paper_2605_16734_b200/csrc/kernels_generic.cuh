@@ -173,6 +173,26 @@ __device__ inline void poincare_emit(const Dense3& d, long long id, double t, do
   }
 }
 
+// ---- O9: uniform-time samples of the continuous extension ------------------------------------------------------
+__device__ __forceinline__ double sample_time(const TraceDev& p, long long j) {
+  return fma((double)j, p.sample_dt, p.sample_t0);          // one FMA on both sides (oracle: sample_time)
+}
+
+// First sample index of a particle that starts at t0: first j with tau_j >= t0 (0 .. nsamp).
+__device__ __forceinline__ long long first_sample_index(const TraceDev& p, double t0) {
+  double g = ceil((t0 - p.sample_t0) / p.sample_dt);
+  long long j = g > 0.0 ? (g < (double)p.nsamp ? (long long)g : p.nsamp) : 0;
+  while (j > 0 && sample_time(p, j - 1) >= t0) --j;
+  while (j < p.nsamp && sample_time(p, j) < t0) ++j;
+  return j;
+}
+
+// Component c of the continuous extension at tau from y, y_new, h k1, h k7 and h sum d_i k_i.
+__device__ __forceinline__ double dense_component(double y, double yn, double hk1, double hk7, double hd, double tau) {
+  const double r2 = yn - y, r3 = hk1 - r2, r4 = r2 - hk7 - r3, sg = 1.0 - tau;
+  return fma(tau, fma(sg, fma(tau, fma(sg, hd, r4), r3), r2), y);
+}
+
 // ---- generic trace: one thread per particle ----------------------------------------------------------------
 __global__ void __launch_bounds__(128) trace_generic_kernel(FieldDev f, TraceDev p) {
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < p.n;
@@ -187,6 +207,15 @@ __global__ void __launch_bounds__(128) trace_generic_kernel(FieldDev f, TraceDev
     long long attempts = 0;
     int n_acc = 0, n_rej = 0, n_forced = 0, st = -1;
     bool prev_rejected = false;
+    long long jn = 0;
+    if (p.nsamp > 0) {
+      jn = first_sample_index(p, t);
+      if (jn < p.nsamp && sample_time(p, jn) == t) {         // a sample on t0 is the initial state
+#pragma unroll
+        for (int c = 0; c < 4; ++c) p.samples[((long long)c * p.nsamp + jn) * p.n + i] = c == 3 ? p.vpar0[i] : y[c];
+        ++jn;
+      }
+    }
     rhs_generic(f, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, t, y, k[0]);
     if (!finite4(y[0], y[1], y[2], y[3]) || !finite4(k[0][0], k[0][1], k[0][2], k[0][3])) st = GC_ST_NONFINITE_;
     else if (!(t < p.t_max)) st = 0;
@@ -258,7 +287,26 @@ __global__ void __launch_bounds__(128) trace_generic_kernel(FieldDev f, TraceDev
           }
           poincare_emit(d, i, t, h_try, y[2], yn[2], p.poincare, p.poincare_capacity, p.poincare_count);
         }
-        t = clipped ? p.t_max : t + h_try;
+        const double t_new = clipped ? p.t_max : t + h_try;
+        if (p.nsamp > 0 && jn < p.nsamp && sample_time(p, jn) <= t_new) {       // O9
+          double hd[4];
+#pragma unroll
+          for (int c = 0; c < 4; ++c)
+            hd[c] = h_try * fma(dp::d7, k[6][c], fma(dp::d6, k[5][c], fma(dp::d5, k[4][c],
+                              fma(dp::d4, k[3][c], fma(dp::d3, k[2][c], dp::d1 * k[0][c])))));
+          while (jn < p.nsamp) {
+            const double tj = sample_time(p, jn);
+            if (tj > t_new) break;
+            const double tau = (tj - t) / h_try;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              const double v = dense_component(y[c], yn[c], h_try * k[0][c], h_try * k[6][c], hd[c], tau);
+              p.samples[((long long)c * p.nsamp + jn) * p.n + i] = c == 3 ? v * p.v_ref : v;
+            }
+            ++jn;
+          }
+        }
+        t = t_new;
 #pragma unroll
         for (int c = 0; c < 4; ++c) { y[c] = yn[c]; k[0][c] = k[6][c]; }
         ++n_acc;
@@ -288,7 +336,61 @@ __global__ void __launch_bounds__(128) trace_generic_kernel(FieldDev f, TraceDev
     if (p.n_acc) p.n_acc[i] = (p.resume ? p.n_acc[i] : 0) + n_acc;
     if (p.n_rej) p.n_rej[i] = (p.resume ? p.n_rej[i] : 0) + n_rej;
     if (p.n_forced) p.n_forced[i] = (p.resume ? p.n_forced[i] : 0) + n_forced;
+    if (p.nsamp > 0 && p.sample_end) p.sample_end[i] = (int)jn;
   }
+}
+
+// ---- A17: P_zeta = q ((rho + alpha) G - chi) at n states and times ----------------------------------------------
+__global__ void pzeta_eval_kernel(FieldDev f, double mass, double charge, long long n, const double* y,
+                                  const double* t, const double* chi_nodes, double* out) {
+  const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double s = y[i], th = y[n + i], ze = y[2 * n + i], v = y[3 * n + i];
+  int i0;
+  double w[4], dw[4], fb[4], pt[9];
+  lagrange_weights(f.ns, s, i0, w, dw);
+  Profiles p;
+  interp4(f.G, 1, i0, w, dw, p.G, p.Gs);
+  interp4(f.I, 1, i0, w, dw, p.I, p.Is);
+  interp4(f.iota, 1, i0, w, dw, p.io, p.ios);
+  eval_B_generic(f, i0, w, dw, th, ze, fb);
+  double al = 0.0;
+  if (f.nk > 0) {
+    eval_pert_generic(f, i0, w, dw, p, th, ze, t ? t[i] : 0.0, pt);
+    al = pt[4];
+  }
+  double chi, dchi;
+  interp4(chi_nodes, 1, i0, w, dw, chi, dchi);
+  const double rho = mass * v / (charge * fb[0]);
+  out[i] = charge * ((rho + al) * p.G - chi);
+}
+
+// ---- A25: weighted Birkhoff average of the two halves of each series, digit accuracy ---------------------------------
+__global__ void birkhoff_kernel(long long n, long long nsamp, const double* series, long long j_first,
+                                const int* sample_end, double* out) {
+  const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  long long end = sample_end ? (long long)sample_end[i] : nsamp;
+  if (end > nsamp) end = nsamp;
+  const long long N = (end - j_first) / 2;
+  const double nan = __longlong_as_double(0x7ff8000000000000LL);
+  if (j_first < 0 || N < 2) { out[i] = nan; out[n + i] = nan; out[2 * n + i] = nan; return; }
+  double wb[2];
+  for (int half = 0; half < 2; ++half) {
+    double sw = 0.0, swf = 0.0;
+    const double* fcol = series + (j_first + half * N) * n + i;
+    for (long long k = 0; k < N; ++k) {
+      const double x = (double)(k + 1) / (double)(N + 1);
+      const double w = exp(-1.0 / (x * (1.0 - x)));
+      sw += w;
+      swf = fma(w, fcol[k * n], swf);
+    }
+    wb[half] = swf / sw;
+  }
+  const double d = fabs(wb[0] - wb[1]), scale = fmax(fabs(wb[0]), fabs(wb[1]));
+  out[i] = wb[0];
+  out[n + i] = wb[1];
+  out[2 * n + i] = (d == 0.0 || scale == 0.0) ? 16.0 : fmin(16.0, -log10(d / scale));
 }
 
 __global__ void field_eval_kernel(FieldDev f, long long n, const double* s, const double* th, const double* ze,

@@ -345,10 +345,10 @@ struct MmaEngine {
   }
 };
 
-template <int MT, int KS, bool MODES>
+template <int MT, int KS, bool MODES, bool SAMPLE>
 __global__ void __launch_bounds__(kMmaThreads, kMmaBlocksPerSm)
 trace_mma_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_out) {
-  trace_binned_body<MmaEngine<MT, KS, MODES>, kMmaThreads, kMmaCap>(f, p, sc, mode, rhs_out);
+  trace_binned_body<MmaEngine<MT, KS, MODES>, kMmaThreads, kMmaCap, SAMPLE>(f, p, sc, mode, rhs_out);
 }
 
 }  // namespace gc

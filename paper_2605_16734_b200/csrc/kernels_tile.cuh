@@ -300,8 +300,9 @@ struct TileEngine {
 // Body of the cell-binned persistent kernels (trace_tile_kernel, trace_mma_kernel): binning, epochs, tiles, the
 // Dormand-Prince integrator of one lane per particle.  Eng supplies the window image and the right-hand side.
 // mode 0: trace.  mode 1: right-hand side only (gc_rhs_eval): k1 of every particle goes to rhs_out[4][n].
-// THREADS = particles per tile = threads per block; CAP = attempted steps per lane per chunk.
-template <class Eng, int THREADS, int CAP>
+// THREADS = particles per tile = threads per block; CAP = attempted steps per lane per chunk; SAMPLE = record the
+// uniform-time samples of gc_trace_sampled (O9; a separate instantiation, so that gc_trace pays nothing for it).
+template <class Eng, int THREADS, int CAP, bool SAMPLE>
 __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const TraceDev& p, const TileScratch& sc, int mode,
                                                   double* rhs_out) {
   cgx::grid_group grid = cgx::this_grid();
@@ -337,10 +338,24 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
       if (h < p.h_min) h = p.h_min;
     }
     const int bin = home_bin(f.ns, y0);
+    int jn0 = 0;
+    if constexpr (SAMPLE) {
+      if (st == kStRunning && mode == 0) {
+        long long j = first_sample_index(p, t);
+        if (j < p.nsamp && sample_time(p, j) == t) {           // a sample on t0 is the initial state
+          p.samples[(0 * p.nsamp + j) * p.n + i] = y0;
+          p.samples[(1 * p.nsamp + j) * p.n + i] = y1;
+          p.samples[(2 * p.nsamp + j) * p.n + i] = y2;
+          p.samples[(3 * p.nsamp + j) * p.n + i] = p.vpar0[i];
+          ++j;
+        }
+        jn0 = (int)j;
+      }
+    }
     reinterpret_cast<double4*>(r)[0] = make_double4(y0, y1, y2, y3);
     reinterpret_cast<double4*>(r)[1] = make_double4(0.0, 0.0, 0.0, 0.0);
     reinterpret_cast<double4*>(r)[2] = make_double4(t, h, mu, __longlong_as_double(0LL));
-    int4 a = make_int4(st, 0, 0, 0), b = make_int4(0, bin, 0, 0);
+    int4 a = make_int4(st, 0, 0, 0), b = make_int4(0, bin, jn0, 0);
     reinterpret_cast<int4*>(r + 12)[0] = a;
     reinterpret_cast<int4*>(r + 12)[1] = b;
     if (st == kStRunning) atomicAdd(sc.cnt + bin, 1);
@@ -430,7 +445,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
       long long pid = 0;
       double y[4] = {0.0, 0.0, 0.0, 0.0}, t = 0.0, h = 0.0, mu = 0.0;
       long long attempts = 0;
-      int st = 0, flags = 0, n_acc = 0, n_rej = 0, n_forced = 0;
+      int st = 0, flags = 0, n_acc = 0, n_rej = 0, n_forced = 0, jn = 0;
       if (active) {
         pid = __ldcg(sc.order + begin + slot);
         const double* r = sc.rec + pid * kRecDoubles;
@@ -442,7 +457,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
         y[0] = a.x; y[1] = a.y; y[2] = a.z; y[3] = a.w;
         kb(0, 0) = b.x; kb(0, 1) = b.y; kb(0, 2) = b.z; kb(0, 3) = b.w;
         t = c.x; h = c.y; mu = c.z; attempts = __double_as_longlong(c.w);
-        st = d.x; flags = d.y; n_acc = d.z; n_rej = d.w; n_forced = g.x;
+        st = d.x; flags = d.y; n_acc = d.z; n_rej = d.w; n_forced = g.x; jn = g.z;
       }
       bool running = active;                     // false once finished or parked
       bool first_chunk = true;
@@ -543,7 +558,30 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
                 }
                 poincare_emit(d, pid, t, h_try, y[2], yn[2], p.poincare, p.poincare_capacity, p.poincare_count);
               }
-              t = clipped ? p.t_max : t + h_try;
+              const double t_new = clipped ? p.t_max : t + h_try;
+              if constexpr (SAMPLE) {                                     // O9
+                if (jn < p.nsamp && sample_time(p, jn) <= t_new) {
+                  double hd[4];
+#pragma unroll
+                  for (int c = 0; c < 4; ++c) {
+                    double dd = 0.0;
+                    for (int j = 0; j < 7; ++j) dd = fma(cDpD[j], kb(j, c), dd);
+                    hd[c] = h_try * dd;
+                  }
+                  while (jn < p.nsamp) {
+                    const double tj = sample_time(p, jn);
+                    if (tj > t_new) break;
+                    const double tau = (tj - t) / h_try;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                      const double v = dense_component(y[c], yn[c], h_try * kb(0, c), h_try * kb(6, c), hd[c], tau);
+                      p.samples[((long long)c * p.nsamp + jn) * p.n + pid] = c == 3 ? v * p.v_ref : v;
+                    }
+                    ++jn;
+                  }
+                }
+              }
+              t = t_new;
 #pragma unroll
               for (int c = 0; c < 4; ++c) { y[c] = yn[c]; kb(0, c) = kb(6, c); }
               ++n_acc;
@@ -596,7 +634,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
         stcg4(r + 4, make_double4(kb(0, 0), kb(0, 1), kb(0, 2), kb(0, 3)));
         stcg4(r + 8, make_double4(t, h, mu, __longlong_as_double(attempts)));
         __stcg(reinterpret_cast<int4*>(r + 12), make_int4(st, flags, n_acc, n_rej));
-        __stcg(reinterpret_cast<int4*>(r + 12) + 1, make_int4(n_forced, hb, 0, 0));
+        __stcg(reinterpret_cast<int4*>(r + 12) + 1, make_int4(n_forced, hb, jn, 0));
         if (st == kStRunning) atomicAdd(sc.cnt + hb, 1);
       }
       __syncthreads();                                                   // window / kbuf / s_int are reused
@@ -612,7 +650,9 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
       if (d.x == kStSkip) continue;
       const double4 a = ldcg4(r);
       const double4 c = ldcg4(r + 8);
-      const int n_forced = __ldcg(reinterpret_cast<const int4*>(r + 12) + 1).x;
+      const int4 g = __ldcg(reinterpret_cast<const int4*>(r + 12) + 1);
+      const int n_forced = g.x;
+      if constexpr (SAMPLE) { if (p.sample_end) p.sample_end[i] = g.z; }
       p.y_out[i] = a.x;
       p.y_out[p.n + i] = a.y;
       p.y_out[2 * p.n + i] = a.z;
@@ -627,10 +667,10 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
   }
 }
 
-template <int NMAX, bool MODES>
+template <int NMAX, bool MODES, bool SAMPLE>
 __global__ void __launch_bounds__(kTileThreads, 2)
 trace_tile_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_out) {
-  trace_binned_body<TileEngine<NMAX, MODES>, kTileThreads, kTileCap>(f, p, sc, mode, rhs_out);
+  trace_binned_body<TileEngine<NMAX, MODES>, kTileThreads, kTileCap, SAMPLE>(f, p, sc, mode, rhs_out);
 }
 
 }  // namespace gc

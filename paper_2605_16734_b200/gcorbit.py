@@ -21,7 +21,8 @@ GC_TILE_MIN_PARTICLES = 8192
 ST_TMAX, ST_LOST, ST_AXIS, ST_MAXSTEPS, ST_NONFINITE = 0, 1, 2, 3, 4
 
 EXPORTS = ["gc_field_create", "gc_field_destroy", "gc_field_eval", "gc_pert_eval", "gc_rhs_eval", "gc_trace",
-           "gc_trace_host", "gc_set_kernel", "gc_kernel_info", "gc_fp64_peak_probe", "gc_last_error"]
+           "gc_trace_host", "gc_set_kernel", "gc_kernel_info", "gc_fp64_peak_probe", "gc_last_error",
+           "gc_trace_sampled", "gc_pzeta_eval", "gc_birkhoff"]
 
 
 class GcError(RuntimeError):
@@ -66,6 +67,9 @@ def load_library():
         L.gc_rhs_eval.argtypes = [vp, dbl, dbl, dbl, i64, vp, vp, vp, vp]
         L.gc_trace.argtypes = [vp, C.POINTER(gc_trace_params), i64] + [vp] * 15
         L.gc_trace_host.argtypes = [vp, C.POINTER(gc_trace_params), i64] + [vp] * 14
+        L.gc_trace_sampled.argtypes = [vp, C.POINTER(gc_trace_params), i64] + [vp] * 12 + [dbl, dbl, i64, vp, vp, vp]
+        L.gc_pzeta_eval.argtypes = [vp, dbl, dbl, i64, vp, vp, vp, vp, vp]
+        L.gc_birkhoff.argtypes = [i64, i64, vp, i64, vp, vp, vp]
         L.gc_set_kernel.argtypes = [vp, i32]
         L.gc_kernel_info.argtypes = [vp, C.c_int64] + [C.POINTER(i32)] * 5
         L.gc_fp64_peak_probe.argtypes = [C.POINTER(dbl), C.POINTER(dbl)]
@@ -121,6 +125,8 @@ class TraceResult:
     h: object            # [n]
     poincare: object = None
     poincare_count: int = 0
+    samples: object = None        # [4][nsamp][n] (gc_trace_sampled)
+    sample_end: object = None     # [n] int32
 
 
 class Field:
@@ -225,6 +231,38 @@ class Field:
         out._count_tensor = cnt
         return out
 
+    # ---- NEXT-1: gc_trace_sampled / gc_pzeta_eval / gc_birkhoff ----------------------------------------------------
+    def trace_sampled(self, spec, s0, th0, ze0, vpar0, mu, sample_t0, sample_dt, nsamp, h_inout=None, t0=None,
+                      t_max=None, out=None, flags=0) -> TraceResult:
+        """gc_trace plus uniform-time samples of the continuous extension (O9).  ``out`` may carry the result of a
+        previous call (same sample buffers: the grid continues under GC_TRACE_RESUME)."""
+        torch = _torch()
+        n = s0.numel()
+        dev = s0.device
+        p = make_params(spec, t0, t_max, 0, flags)
+        if out is None:
+            i32 = lambda: torch.empty(n, dtype=torch.int32, device=dev)
+            out = TraceResult(torch.empty((4, n), dtype=torch.float64, device=dev),
+                              torch.empty(n, dtype=torch.float64, device=dev), i32(), i32(), i32(), i32(), h_inout)
+            out.samples = torch.full((4, int(nsamp), n), float("nan"), dtype=torch.float64, device=dev)
+            out.sample_end = torch.zeros(n, dtype=torch.int32, device=dev)
+        out.h = h_inout
+        _check(load_library().gc_trace_sampled(self._h, C.byref(p), n, _dp(s0), _dp(th0), _dp(ze0), _dp(vpar0),
+                                               _dp(mu), _dp(h_inout), _dp(out.y), _dp(out.t), _dp(out.status),
+                                               _dp(out.n_acc), _dp(out.n_rej), _dp(out.n_forced), float(sample_t0),
+                                               float(sample_dt), int(nsamp), _dp(out.samples), _dp(out.sample_end),
+                                               _stream_ptr(torch)))
+        return out
+
+    def pzeta_eval(self, mass, charge, y, t, chi_nodes):
+        """P_zeta at the n states y [4][n] (device) and times t [n] (device or None); chi_nodes [ns] device."""
+        torch = _torch()
+        n = y.shape[1]
+        out = torch.empty(n, dtype=torch.float64, device=y.device)
+        _check(load_library().gc_pzeta_eval(self._h, float(mass), float(charge), n, _dp(y), _dp(t), _dp(chi_nodes),
+                                            _dp(out), _stream_ptr(torch)))
+        return out
+
     def trace_resume(self, spec, state: TraceResult, mu, t0, t_max, poincare_capacity=0) -> TraceResult:
         """Continue a previous ``trace`` result in place over [t0, t_max] (GC_TRACE_RESUME): the rows of
         ``state.y`` are the initial conditions and receive the new states; ``state.h`` carries the step
@@ -277,3 +315,13 @@ def fp64_peak_probe():
     f, ms = C.c_double(0), C.c_double(0)
     _check(load_library().gc_fp64_peak_probe(C.byref(f), C.byref(ms)))
     return f.value, ms.value
+
+
+def birkhoff(series, j_first=0, sample_end=None):
+    """gc_birkhoff: series [nsamp][n] device tensor -> [3][n] (WB first half, WB second half, digit accuracy)."""
+    torch = _torch()
+    nsamp, n = series.shape
+    out = torch.empty((3, n), dtype=torch.float64, device=series.device)
+    _check(load_library().gc_birkhoff(n, nsamp, _dp(series), int(j_first), _dp(sample_end), _dp(out),
+                                      _stream_ptr(torch)))
+    return out

@@ -1,0 +1,204 @@
+"""-m gpu: NEXT-1 through the C ABI against the oracle: uniform-time samples of the
+continuous extension (gc_trace_sampled, O9), P_zeta at states (gc_pzeta_eval, A17), weighted Birkhoff average and
+digit accuracy (gc_birkhoff, A25).  Expected values come from oracle/ only."""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+import pytest
+
+from gpu_common import assert_trace_parity, make_case, oracle_conditioning, to_dev
+
+pytestmark = pytest.mark.gpu
+
+
+def _kernel(GF, name):
+    from paper_2605_16734_b200 import gcorbit as G
+    GF.set_kernel({"generic": G.GC_KERNEL_GENERIC, "tile": G.GC_KERNEL_TILE, "mma": G.GC_KERNEL_MMA,
+                   "warp": G.GC_KERNEL_WARP, "auto": G.GC_KERNEL_AUTO}[name])
+
+
+def _sample_parity(r, o, spec, k, label):
+    """Samples of the first k particles: same sample_end, same untouched entries, values within 1e-9 (relative to
+    max(1, |y|) for s and the angles, to max(v_ref, |v|) for v_par) for particles on the oracle's step sequence."""
+    sg = r.samples.cpu().numpy()[:, :, :k]
+    eg = r.sample_end.cpu().numpy()[:k]
+    same = (r.n_acc.cpu().numpy()[:k] == o.n_acc) & (r.n_rej.cpu().numpy()[:k] == o.n_rej)
+    assert same.mean() >= 0.97, f"{label}: {same.mean()}"
+    assert np.array_equal(eg[same], o.nsampled[same]), f"{label}: sample_end differs"
+    assert np.array_equal(np.isnan(sg[:, :, same]), np.isnan(o.samples[:, :, same])), f"{label}: coverage differs"
+    floor = np.array([1.0, 1.0, 1.0, spec.v_ref])[:, None, None]
+    rel = np.abs(sg - o.samples) / np.maximum(np.abs(o.samples), floor)
+    rel = np.where(np.isnan(o.samples), 0.0, rel)[:, :, same]
+    assert np.median(rel) < 1e-12 and rel.max() < 1e-9, f"{label}: max rel {rel.max():.3e}"
+    return float(rel.max())
+
+
+@pytest.mark.parametrize("kernel", ["generic", "warp", "tile", "mma"])
+def test_samples_config0(kernel):
+    """Config 0, 96 particles, 40 samples over 4e-6 s (the warp kernel hands a sampled trace to the generic one)."""
+    import torch
+    fld, spec, P, OF, GF, mu = make_case(0, 96)
+    _kernel(GF, kernel)
+    nsamp, dt, t_max = 40, 1e-7, 4e-6
+    r = GF.trace_sampled(spec, to_dev(P.s), to_dev(P.theta), to_dev(P.zeta), to_dev(P.vpar), to_dev(mu), 0.0, dt,
+                         nsamp, t_max=t_max)
+    torch.cuda.synchronize()
+    o = OF.trace_sampled(spec, P.s, P.theta, P.zeta, P.vpar, mu, 0.0, dt, nsamp, t_max=t_max)
+    cond = oracle_conditioning(OF, spec, P, mu, o, t_max=t_max)
+    assert_trace_parity(r, o, spec, label=f"sampled {kernel}", cond=cond, min_within=0.99)
+    print(kernel, "samples max rel", _sample_parity(r, o, spec, P.n, f"samples {kernel}"))
+
+
+@pytest.mark.parametrize("config", [1, 4])
+def test_samples_large_ensemble_mma(config):
+    """The launch configuration of the benchmark kernel: 20,000 particles of config 1 / config 4 (16 modes) through
+    the mma kernel, sample grid that starts before t0 and is not aligned with it, a loss boundary that stops some
+    particles early; 160 particles checked against the oracle."""
+    import dataclasses
+    import torch
+    import oracle
+    from paper_2605_16734_b200 import gcorbit as G, workloads as W
+    fld = W.make_field(config)
+    spec = dataclasses.replace(W.make_spec(config), s_loss=0.47)
+    P = W.make_particles(config, 20_000)
+    OF, GF = oracle.OracleField(fld), G.Field(fld)
+    mu = W.mu_from(P, OF.eval_B_many(P.s, P.theta, P.zeta)[:, 0])
+    assert GF.kernel_info(P.n)["kernel"] == "mma"
+    nsamp, dt, st0, t_max = 24, 1.3e-7, -2.5e-7, 2.5e-6
+    r = GF.trace_sampled(spec, to_dev(P.s), to_dev(P.theta), to_dev(P.zeta), to_dev(P.vpar), to_dev(mu), st0, dt,
+                         nsamp, t_max=t_max)
+    torch.cuda.synchronize()
+    k = 160
+    Q = P.head(k)
+    o = OF.trace_sampled(spec, Q.s, Q.theta, Q.zeta, Q.vpar, mu[:k], st0, dt, nsamp, t_max=t_max)
+    assert (o.status == 1).any() and (o.status == 0).any()
+    assert np.array_equal(r.status.cpu().numpy()[:k], o.status)
+    print("config", config, "samples max rel", _sample_parity(r, o, spec, k, f"samples mma config {config}"))
+
+
+def test_samples_continue_over_resumed_segments():
+    """GC_TRACE_RESUME with the same sample buffers: the grid continues; compared with the oracle run in the same
+    two segments."""
+    import torch
+    from paper_2605_16734_b200 import gcorbit as G
+    fld, spec, P, OF, GF, mu = make_case(0, 64)
+    _kernel(GF, "generic")
+    dt, nsamp = 2.0 ** -23, 17
+    t1, t2 = 8 * dt, 16 * dt
+    h = torch.zeros(P.n, dtype=torch.float64, device="cuda:0")
+    mu_d = to_dev(mu)
+    r = GF.trace_sampled(spec, to_dev(P.s), to_dev(P.theta), to_dev(P.zeta), to_dev(P.vpar), mu_d, 0.0, dt, nsamp,
+                         h_inout=h, t0=0.0, t_max=t1)
+    r = GF.trace_sampled(spec, r.y[0], r.y[1], r.y[2], r.y[3], mu_d, 0.0, dt, nsamp, h_inout=h, t0=t1, t_max=t2,
+                         out=r, flags=G.GC_TRACE_RESUME)
+    torch.cuda.synchronize()
+    a = OF.trace_sampled(spec, P.s, P.theta, P.zeta, P.vpar, mu, 0.0, dt, nsamp, t0=0.0, t_max=t1)
+    b = OF.trace_sampled(spec, a.y[0], a.y[1], a.y[2], a.y[3], mu, 0.0, dt, nsamp, h_in=a.h, t0=t1, t_max=t2)
+    both = np.where(np.isnan(b.samples), a.samples, b.samples)
+    sg = r.samples.cpu().numpy()
+    assert np.array_equal(r.sample_end.cpu().numpy(), b.nsampled) and np.isfinite(sg).all()
+    floor = np.array([1.0, 1.0, 1.0, spec.v_ref])[:, None, None]
+    assert (np.abs(sg - both) / np.maximum(np.abs(both), floor)).max() < 1e-9
+
+
+def test_sampled_argument_checks():
+    from paper_2605_16734_b200 import gcorbit as G
+    fld, spec, P, OF, GF, mu = make_case(0, 8)
+    a = [to_dev(x) for x in (P.s, P.theta, P.zeta, P.vpar, mu)]
+    with pytest.raises(G.GcError):
+        GF.trace_sampled(spec, *a, 0.0, 0.0, 4)              # sample_dt must be > 0
+    with pytest.raises(G.GcError):
+        GF.trace_sampled(spec, *a, float("nan"), 1e-7, 4)
+
+
+# ---- gc_pzeta_eval -------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("config", [1, 4])
+def test_pzeta_eval_matches_oracle(config):
+    import torch
+    fld, spec, P, OF, GF, mu = make_case(config, 300)
+    s_n = np.arange(fld.ns) / (fld.ns - 1)
+    chi = fld.psi0 * (0.42 * s_n + 0.05 * s_n ** 2)           # iota = 0.42 + 0.1 s
+    t = np.linspace(0.0, 3e-5, P.n)
+    y = np.stack([P.s, P.theta, P.zeta, P.vpar])
+    out = GF.pzeta_eval(spec.mass, spec.charge, to_dev(y), to_dev(t), to_dev(chi))
+    torch.cuda.synchronize()
+    ref = OF.pzeta(spec.mass, spec.charge, chi, P.s, P.theta, P.zeta, P.vpar, t)
+    assert np.abs(out.cpu().numpy() / ref - 1.0).max() < 1e-12
+
+
+def test_pzeta_of_gpu_samples_is_conserved_in_an_axisymmetric_field():
+    """End to end on the device: gc_trace_sampled -> gc_pzeta_eval on the sample buffer (viewed as [4][nsamp n])
+    in a field whose non-symmetric harmonics are removed: P_zeta is constant along every orbit."""
+    import torch
+    import oracle
+    from paper_2605_16734_b200 import gcorbit as G, workloads as W
+    fld = W.make_field(0)
+    keep = fld.xn == 0
+    fld.xm, fld.xn, fld.bmnc = fld.xm[keep], fld.xn[keep], np.ascontiguousarray(fld.bmnc[:, keep])
+    spec = W.make_spec(0)
+    P = W.make_particles(0, 128)
+    OF, GF = oracle.OracleField(fld), G.Field(fld)
+    mu = W.mu_from(P, OF.eval_B_many(P.s, P.theta, P.zeta)[:, 0])
+    s_n = np.arange(fld.ns) / (fld.ns - 1)
+    chi = to_dev(fld.psi0 * (0.42 * s_n + 0.05 * s_n ** 2))
+    nsamp, dt = 51, 1e-6
+    r = GF.trace_sampled(spec, to_dev(P.s), to_dev(P.theta), to_dev(P.zeta), to_dev(P.vpar), to_dev(mu), 0.0, dt,
+                         nsamp, t_max=5e-5)
+    pz = GF.pzeta_eval(spec.mass, spec.charge, r.samples.reshape(4, nsamp * P.n), None, chi).reshape(nsamp, P.n)
+    torch.cuda.synchronize()
+    assert bool((r.sample_end == nsamp).all())
+    pz = pz.cpu().numpy()
+    dev = np.abs(pz / pz[0] - 1.0).max(axis=0)
+    # the kinks of the piecewise-cubic interpolant set the floor; over 128 orbits the worst one sits
+    # two decades above the typical one
+    assert np.median(dev) < 1e-7 and dev.max() < 1e-5
+    assert np.ptp(r.samples[0].cpu().numpy(), axis=0).max() > 0.01
+
+
+# ---- gc_birkhoff ---------------------------------------------------------------------------------------------------
+def test_birkhoff_matches_oracle():
+    """Quasi-periodic, chaotic (logistic map), constant and noisy series of ragged valid lengths."""
+    import torch
+    import oracle
+    from paper_2605_16734_b200 import gcorbit as G
+    rng = np.random.default_rng(11)
+    nsamp, n = 3000, 40
+    j = np.arange(nsamp)
+    series = np.empty((nsamp, n))
+    for i in range(n):
+        kind = i % 4
+        if kind == 0:
+            nu = (math.sqrt(5.0) - 1.0) / 2.0 + 0.01 * i
+            series[:, i] = 1.0 + 0.3 * i + np.cos(2 * np.pi * nu * j + i) + 0.2 * np.sin(2 * np.pi * 2 * nu * j)
+        elif kind == 1:
+            x = np.empty(nsamp)
+            x[0] = 0.1 + 0.01 * i
+            for k in range(1, nsamp):
+                x[k] = 4.0 * x[k - 1] * (1.0 - x[k - 1])
+            series[:, i] = x
+        elif kind == 2:
+            series[:, i] = -2.5
+        else:
+            series[:, i] = rng.standard_normal(nsamp)
+    j_first = 3
+    end = rng.integers(200, nsamp + 1, n).astype(np.int32)
+    end[:4] = nsamp
+    end[4] = j_first + 3                                      # fewer than 4 samples: NaN
+    out = G.birkhoff(to_dev(series), j_first, torch.as_tensor(end, device="cuda:0"))
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()
+    for i in range(n):
+        cnt = int(end[i]) - j_first
+        if cnt // 2 < 2:
+            assert np.isnan(out[:, i]).all()
+            continue
+        a, b, d = oracle.birkhoff_digits(series[j_first:int(end[i]), i])
+        assert out[0, i] == pytest.approx(a, rel=1e-12, abs=1e-13)
+        assert out[1, i] == pytest.approx(b, rel=1e-12, abs=1e-13)
+        if d < 11.0:                                          # |WB_1 - WB_2| well above the rounding of the sums
+            assert out[2, i] == pytest.approx(d, abs=1e-3 if d > 8 else 1e-5), i
+        else:
+            assert out[2, i] > 10.5
+    assert out[2, 0] > 8.0 and out[2, 1] < 3.0                # regular vs chaotic

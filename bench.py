@@ -51,6 +51,9 @@ def parse_args():
                     "capped at 100000 per step for configs 3-4 unless given)")
     ap.add_argument("--segment", type=float, default=2e-5, help="simulated seconds per step")
     ap.add_argument("--kernel", default="auto", choices=["auto", "mma", "tile", "warp", "generic"])
+    ap.add_argument("--samples", type=int, default=0, help="NEXT-1: uniform-time samples per segment recorded by "
+                    "gc_trace_sampled (0 = plain gc_trace, the default line); adds the P_zeta / weighted-Birkhoff "
+                    "post-processing time to config")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
@@ -238,9 +241,22 @@ def run_cuda(args):
         return int((st.n_acc.sum(dtype=torch.int64) + st.n_rej.sum(dtype=torch.int64)).item())
 
     # warm-up: the first W segments of the trace
-    state = GF.trace(spec, s, th, ze, vpar, mu, h_inout=h, t0=0.0, t_max=seg)
+    S = args.samples
+    if S > 0:
+        nsamp_total = S * (max(Wu, 1) + K) + 1
+        sdt = seg / S
+
+        def resume(state, t0, t1):
+            y = state.y
+            return GF.trace_sampled(spec, y[0], y[1], y[2], y[3], mu, 0.0, sdt, nsamp_total, h_inout=state.h, t0=t0,
+                                    t_max=t1, out=state, flags=G.GC_TRACE_RESUME)
+        state = GF.trace_sampled(spec, s, th, ze, vpar, mu, 0.0, sdt, nsamp_total, h_inout=h, t0=0.0, t_max=seg)
+    else:
+        def resume(state, t0, t1):
+            return GF.trace_resume(spec, state, mu, t0=t0, t_max=t1)
+        state = GF.trace(spec, s, th, ze, vpar, mu, h_inout=h, t0=0.0, t_max=seg)
     for w in range(1, max(Wu, 1)):
-        GF.trace_resume(spec, state, mu, t0=w * seg, t_max=(w + 1) * seg)
+        resume(state, w * seg, (w + 1) * seg)
     torch.cuda.synchronize()
     first = max(Wu, 1)
     a_before = attempts_of(state)
@@ -255,7 +271,7 @@ def run_cuda(args):
     for k in range(K):
         flush.fill_(k & 0xFF)                                  # L2 flush between timed iterations (not timed)
         ev[k][0].record(stream)
-        GF.trace_resume(spec, state, mu, t0=(first + k) * seg, t_max=(first + k + 1) * seg)
+        resume(state, (first + k) * seg, (first + k + 1) * seg)
         ev[k][1].record(stream)
     torch.cuda.synchronize()
     if world > 1:
@@ -269,9 +285,31 @@ def run_cuda(args):
     ms_max, attempts_all = E.reduce_timing(kernel_ms, attempts, dev)
     value = attempts_all / (ms_max * 1e-3)
 
+    # ---- NEXT-1 post-processing (only with --samples): P_zeta of every sample, weighted Birkhoff average per particle
+    diag = None
+    if S > 0:
+        s_n = np.arange(fld.ns) / (fld.ns - 1)
+        iota_int = np.concatenate([[0.0], np.cumsum(0.5 * (fld.iota[1:] + fld.iota[:-1]) * np.diff(s_n))])
+        chi = T(fld.psi0 * iota_int)                                    # chi(s) = psi0 int iota ds (trapezoid on the nodes)
+        tt = (torch.arange(nsamp_total, dtype=torch.float64, device=dev) * sdt).repeat_interleave(n)
+        e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        e0.record(stream)
+        pz = GF.pzeta_eval(spec.mass, spec.charge, state.samples.reshape(4, nsamp_total * n), tt, chi)
+        e1.record(stream)
+        wb = G.birkhoff(pz.reshape(nsamp_total, n), 0, state.sample_end)
+        e2.record(stream)
+        torch.cuda.synchronize()
+        dig = wb[2][torch.isfinite(wb[2])]
+        diag = {"samples_per_segment": S, "nsamp": nsamp_total, "sample_buffer_bytes": 32 * nsamp_total * n,
+                "pzeta_eval_ms": e0.elapsed_time(e1), "birkhoff_ms": e1.elapsed_time(e2),
+                "pzeta_points_per_s": nsamp_total * n / (e0.elapsed_time(e1) * 1e-3),
+                "birkhoff_GBps": 8.0 * nsamp_total * n / (e1.elapsed_time(e2) * 1e-3) / 1e9,
+                "digits_median": float(dig.median().item()) if dig.numel() else None,
+                "frac_digits_below_3": float((dig < 3).double().mean().item()) if dig.numel() else None}
+
     # ---- e2e: the same segments through gc_trace_host, pinned host buffers, copies inside the timed region
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and S == 0:
         Ke = min(K, 3)
         pin = lambda t: t.detach().cpu().pin_memory()
         hy, ht, hs, hh, hmu = pin(state.y), pin(state.t), pin(state.status), pin(state.h), pin(mu)
@@ -314,7 +352,7 @@ def run_cuda(args):
     tp = os.path.join(ROOT, "profiles", "traffic.json")
     # one ncu capture of the DEFAULT launch (profiles/r1_ncu_mma_config1.md); other workloads have no capture
     default_launch = (args.config == 1 and args.particles is None and args.segment == 2e-5 and
-                      kinfo["kernel"] == "mma")
+                      kinfo["kernel"] == "mma" and args.samples == 0)
     if os.path.exists(tp) and default_launch:
         try:
             with open(tp) as fh:
@@ -332,6 +370,8 @@ def run_cuda(args):
     cpu = None
     if not args.no_cpu_baseline:
         cpu = oracle_sample(fld, spec, P, seg, args.cpu_seconds)
+    if diag:
+        info["next1_diagnostics"] = diag
     info.update({"kernel": kinfo, "l2": "flushed between timed steps (256 MiB write, outside each step's event pair)",
                  "alive_before": alive_before, "alive_after": alive_after,
                  "simulated_window_s": [first * seg, (first + K) * seg]})

@@ -11,7 +11,9 @@
  * finite differences and an independent numpy series; DP5 tableau vs exact-rational order conditions
  * and scipy's RK45 step; the RHS vs the Euler-Lagrange equations of the guiding-centre Lagrangian
  * solved numerically; energy, P_zeta, helical momentum, n*H - omega*P_zeta invariants; closed-form
- * orbits; brute-force RK4.  FIRM3D-level agreement (same numbers as the reference code on its own
+ * orbits; brute-force RK4; (tests/test_oracle_sampling.py) uniform-time samples vs closed form and an independent
+ * DOP853 integration, P_zeta of the samples vs conservation laws, the weighted Birkhoff average (oracle/__init__.py)
+ * vs super-convergence on quasi-periodic signals and the logistic map.  FIRM3D-level agreement (same numbers as the reference code on its own
  * equilibria) is PARITY UNPINNED: no code, equilibrium file or printed equation exists to pin it to.
  */
 #ifndef GC_ORACLE_H

@@ -18,6 +18,7 @@ struct FieldDev {
   const int* mode_m;     // [nk]
   const int* mode_n;     // [nk]
   const double* omega;   // [nk]
+  const double* inv_omega;  // [nk] 1 / omega (mma kernel: no division per mode and right-hand side)
   const double* phase;   // [nk]
   const double* phihat;  // [ns][nk]
   // packed by-node layout of the warp kernel (kernels_warp.cuh): rows[node][it][lane]

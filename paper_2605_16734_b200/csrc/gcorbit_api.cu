@@ -295,11 +295,7 @@ int pack_mma_image(gc_field* f, const gc_field_desc* d) {
   const bool small = v.M <= 8 && v.N <= 8;
   const int MT = small ? 1 : 2, KS = small ? 2 : 4;
   const int RS = small ? gc::MmaRow<1, 2>::stride(d->nk) : gc::MmaRow<2, 4>::stride(d->nk);
-#ifdef GC_MMA_L1
-  const int smem = (int)((size_t)((gc::kSubBins + 2) * (d->ns - 3) / 2 + 2) * sizeof(double) + (size_t)(7 * 4 + 2 * gc::kMmaWtab) * gc::kMmaThreads * sizeof(double) + 64);
-#else
   const int smem = (int)((size_t)gc::kMmaWinRows * RS * sizeof(double) + (size_t)(7 * 4 + 2 * gc::kMmaWtab) * gc::kMmaThreads * sizeof(double) + 64);
-#endif
   if (smem > 110 * 1024) return GC_OK;
   const int ncell = d->ns - 3;
   if ((size_t)(gc::kSubBins + 2) * ncell * sizeof(int) > (size_t)gc::kMmaWinRows * RS * sizeof(double)) return GC_OK;
@@ -452,10 +448,14 @@ int gc_field_create(const gc_field_desc* d, gc_field** out) {
   up(d->xm, d->nh, &xm); up(d->xn, d->nh, &xn); up(d->bmnc, (size_t)d->ns * d->nh, &bmnc);
   up(d->G, d->ns, &G); up(d->I, d->ns, &I); up(d->iota, d->ns, &iota);
   up(d->mode_m, d->nk, &mm); up(d->mode_n, d->nk, &mn); up(d->mode_omega, d->nk, &om);
+  std::vector<double> inv_om(d->nk);
+  for (int k = 0; k < d->nk; ++k) inv_om[k] = 1.0 / d->mode_omega[k];
+  double* iom = nullptr;
+  up(inv_om.data(), d->nk, &iom);
   up(d->mode_phase, d->nk, &ph); up(d->phihat, (size_t)d->ns * d->nk, &phihat);
   if (rc == GC_OK) {
     v.xm = xm; v.xn = xn; v.bmnc = bmnc; v.G = G; v.I = I; v.iota = iota;
-    v.mode_m = mm; v.mode_n = mn; v.omega = om; v.phase = ph; v.phihat = phihat;
+    v.mode_m = mm; v.mode_n = mn; v.omega = om; v.inv_omega = iom; v.phase = ph; v.phihat = phihat;
     rc = pack_rows(f, d);
   }
   if (rc == GC_OK) rc = pack_tile_images(f, d);

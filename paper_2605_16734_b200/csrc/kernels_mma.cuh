@@ -243,12 +243,7 @@ __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, do
     const int r_hi = __reduce_max_sync(0xffffffffu, (ingrp && inwin) ? off + 3 : -1);
     if (r_hi >= 0) {
       const int off_f = __shfl_sync(0xffffffffu, inwin ? off : kMmaNone, src);
-#ifdef GC_MMA_L1
-      mma_sweep<MT, KS, LdG>(f.mma_image + (size_t)cell * RS, RS, r_lo, r_hi, off_f, wsrc, lane, q, AC, AS, AnC, AnS,
-                             cm, sm, o);
-#else
       mma_sweep<MT, KS, LdS>(win, RS, r_lo, r_hi, off_f, wsrc, lane, q, AC, AS, AnC, AnS, cm, sm, o);
-#endif
     }
     // ---- stencils outside the window: one sweep per distinct stencil, rows from global memory ----------------------
     unsigned pend = __ballot_sync(0xffffffffu, ingrp && outside);
@@ -269,11 +264,7 @@ __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, do
   }
   // ---- particle role: profiles, perturbation, guiding-centre algebra ------------------------------------------------
   if (active) {
-#ifdef GC_MMA_L1
-    const double* prow = f.mma_image + (size_t)(i0 + 2) * RS;
-#else
     const double* prow = inwin ? win + (size_t)off * RS : f.mma_image + (size_t)(i0 + 2) * RS;
-#endif
     Profiles pr;
     double v[4];
 #pragma unroll
@@ -291,6 +282,7 @@ __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, do
     if constexpr (MODES) {
       const double zer = reduce_2pi(y[2]);
       const double GI = pr.G + pr.io * pr.I, GI_s = pr.Gs + pr.ios * pr.I + pr.io * pr.Is;
+      const double invGI = 1.0 / GI, gig = GI_s * invGI;               // one division per right-hand side
 #pragma unroll 1
       for (int k = 0; k < f.nk; ++k) {
 #pragma unroll
@@ -301,10 +293,10 @@ __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, do
         const double wt = reduce_2pi(om * t);
         double sn, cs;
         sincos_poly(fma(m, thr, fma(-n, zer, wt + __ldg(f.phase + k))), sn, cs);
-        const double inv = 1.0 / (om * GI);
+        const double inv = __ldg(f.inv_omega + k) * invGI;             // 1 / (omega (G + iota I))
         const double Nk = fma(pr.io, m, -n);
         const double ah = -ph * Nk * inv;
-        const double ah_s = -(ph_s * Nk + ph * pr.ios * m) * inv + ph * Nk * inv * (GI_s / GI);
+        const double ah_s = -(ph_s * Nk + ph * pr.ios * m) * inv + ph * Nk * inv * gig;
         pt[0] = fma(ph, sn, pt[0]);
         pt[1] = fma(ph_s, sn, pt[1]);
         pt[2] = fma(m * ph, cs, pt[2]);
@@ -327,13 +319,8 @@ __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, do
 // The table engine of trace_mma_kernel.
 template <int MT, int KS, bool MODES>
 struct MmaEngine {
-#ifdef GC_MMA_L1
-  static constexpr bool kStageWindow = false;
-  static __device__ __forceinline__ int win_doubles(const FieldDev& f) { return (kSubBins + 2) * (f.ns - 3) / 2 + 2; }
-#else
   static constexpr bool kStageWindow = true;
   static __device__ __forceinline__ int win_doubles(const FieldDev& f) { return kMmaWinRows * f.mma_RS; }
-#endif
   static constexpr int kExtDoubles = 2 * kMmaWtab;                   // per-thread weight table
   static __device__ __forceinline__ const double* win_src(const FieldDev& f, int cell) {
     return f.mma_image + (size_t)cell * f.mma_RS;                     // image rows cell .. cell+7

@@ -306,6 +306,44 @@ static int all_finite4(const double v[4]) {
   return isfinite(v[0]) && isfinite(v[1]) && isfinite(v[2]) && isfinite(v[3]);
 }
 
+/* O8: one crossing of component `comp` through `target` inside the accepted step (t, y) -> (t+h, y_new): root of
+ * the continuous extension by 8 bisections and Newton, then the record (id, t + tau h, s, theta mod 2 pi). */
+static void record_crossing(int64_t id, double t, double h, const double y[4], const double y_new[4],
+                            const double k[7][4], int comp, double target, double tol,
+                            double *buf, int64_t cap, int64_t *count) {
+  const double TWO_PI = 6.283185307179586476925286766559;
+  double lo = 0.0, hi = 1.0, yt[4], dy[4];
+  double glo = y[comp] - target;
+  for (int it = 0; it < 8; ++it) {                                  /* bisection to bracket */
+    double mid = 0.5 * (lo + hi);
+    dense_and_slope(y, y_new, k, h, mid, yt, dy);
+    double g = yt[comp] - target;
+    if ((g < 0.0) == (glo < 0.0) && g != 0.0) { lo = mid; glo = g; } else { hi = mid; }
+  }
+  double tau = 0.5 * (lo + hi);
+  for (int it = 0; it < 20; ++it) {                                 /* Newton polish */
+    dense_and_slope(y, y_new, k, h, tau, yt, dy);
+    double g = yt[comp] - target;
+    if (fabs(g) < tol || dy[comp] == 0.0) break;
+    double tn = tau - g / dy[comp];
+    if (tn < lo) tn = lo;
+    if (tn > hi) tn = hi;
+    tau = tn;
+  }
+  dense_and_slope(y, y_new, k, h, tau, yt, dy);
+  int64_t slot;
+#pragma omp atomic capture
+  slot = (*count)++;
+  if (slot < cap) {
+    double thm = fmod(yt[1], TWO_PI);
+    if (thm < 0.0) thm += TWO_PI;
+    buf[slot * 4 + 0] = (double)id;
+    buf[slot * 4 + 1] = t + tau * h;
+    buf[slot * 4 + 2] = yt[0];
+    buf[slot * 4 + 3] = thm;
+  }
+}
+
 /* O8: record every crossing of zeta = 2 pi k inside the accepted step (t, y) -> (t+h, y_new). */
 static void poincare_step(int64_t id, double t, double h, const double y[4], const double y_new[4],
                           const double k[7][4], double *buf, int64_t cap, int64_t *count) {
@@ -317,38 +355,17 @@ static void poincare_step(int64_t id, double t, double h, const double y[4], con
   else { kfirst = k0; klast = k1 + 1.0; kstep = -1.0; }               /* planes crossed going down */
   for (double kp = kfirst; kstep > 0 ? kp <= klast : kp >= klast; kp += kstep) {
     double target = TWO_PI * kp;
-    double lo = 0.0, hi = 1.0, yt[4], dy[4];
-    double glo = y[2] - target;
-    for (int it = 0; it < 8; ++it) {                                  /* bisection to bracket */
-      double mid = 0.5 * (lo + hi);
-      dense_and_slope(y, y_new, k, h, mid, yt, dy);
-      double g = yt[2] - target;
-      if ((g < 0.0) == (glo < 0.0) && g != 0.0) { lo = mid; glo = g; } else { hi = mid; }
-    }
-    double tau = 0.5 * (lo + hi);
-    double tol = 1e-12 * fmax(1.0, fabs(target));
-    for (int it = 0; it < 20; ++it) {                                 /* Newton polish */
-      dense_and_slope(y, y_new, k, h, tau, yt, dy);
-      double g = yt[2] - target;
-      if (fabs(g) < tol || dy[2] == 0.0) break;
-      double tn = tau - g / dy[2];
-      if (tn < lo) tn = lo;
-      if (tn > hi) tn = hi;
-      tau = tn;
-    }
-    dense_and_slope(y, y_new, k, h, tau, yt, dy);
-    int64_t slot;
-#pragma omp atomic capture
-    slot = (*count)++;
-    if (slot < cap) {
-      double thm = fmod(yt[1], TWO_PI);
-      if (thm < 0.0) thm += TWO_PI;
-      buf[slot * 4 + 0] = (double)id;
-      buf[slot * 4 + 1] = t + tau * h;
-      buf[slot * 4 + 2] = yt[0];
-      buf[slot * 4 + 3] = thm;
-    }
+    record_crossing(id, t, h, y, y_new, k, 2, target, 1e-12 * fmax(1.0, fabs(target)), buf, cap, count);
   }
+}
+
+/* O8b (NEXT-1; "trapped particle Poincare map"): the bounce section v_par = 0.  A step whose end
+ * values of u = v_par / v_ref have opposite signs (or that ends exactly on 0 from a nonzero start) holds one
+ * crossing; both directions count; u is O(1), so the root tolerance is 1e-12 absolute. */
+static void bounce_step(int64_t id, double t, double h, const double y[4], const double y_new[4],
+                        const double k[7][4], double *buf, int64_t cap, int64_t *count) {
+  if (!((y[3] < 0.0 && y_new[3] >= 0.0) || (y[3] > 0.0 && y_new[3] <= 0.0))) return;
+  record_crossing(id, t, h, y, y_new, k, 3, 0.0, 1e-12, buf, cap, count);
 }
 
 /* ---- O5-O8: the trace -------------------------------------------------------------------------------- */
@@ -411,7 +428,10 @@ static int trace_impl(const oracle_field *f, const oracle_trace_params *p, int64
       if (accept) {
         double sc = oracle_scale_accept(err);
         double h_next = prev_rejected ? h_try * fmin(sc, 1.0) : h_try * sc;
-        if (pcap > 0) poincare_step(i, t, h_try, y, y_new, (const double(*)[4])k, poincare, pcap, poincare_count);
+        if (pcap > 0) {
+          if (p->section == 1) bounce_step(i, t, h_try, y, y_new, (const double(*)[4])k, poincare, pcap, poincare_count);
+          else poincare_step(i, t, h_try, y, y_new, (const double(*)[4])k, poincare, pcap, poincare_count);
+        }
         const double t_new = clipped ? p->t_max : t + h_try;
         while (jn < nsamp) {                   /* O9: samples with t < tau_j <= t_new from the continuous extension */
           double tj = sample_time(sample_t0, sample_dt, jn), ys[4];

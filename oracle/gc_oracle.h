@@ -50,6 +50,7 @@ typedef struct {
   int64_t max_steps;
   int64_t poincare_capacity;   /* records in the shared buffer; 0 disables O8 */
   int64_t traj_capacity;       /* per-particle accepted-step records; 0 disables (oracle-only) */
+  int64_t section;             /* which crossings the Poincare records hold: 0 zeta = 0 mod 2 pi (O8), 1 v_par = 0 (O8b) */
 } oracle_trace_params;
 
 oracle_field *oracle_field_create(const oracle_field_desc *d);

@@ -247,3 +247,66 @@ def test_birkhoff_digits_separate_regular_from_chaotic():
     assert oracle.birkhoff_digits(np.full(100, 3.0))[2] == 16.0
     # invariant under scaling of the signal
     assert oracle.birkhoff_digits(7.0 * x)[2] == pytest.approx(d, abs=1e-9)
+
+
+# ---- O8b: bounce section v_par = 0 -----------------------------------------------------------------------------------
+def test_bounce_section_matches_event_location_of_an_independent_integrator():
+    """Trapped particles of config 0: every record of the v_par = 0 section agrees in time and position with the
+    events scipy's DOP853 (rtol 1e-12, dense output + root finding) locates on the oracle's right-hand side; the
+    number of records is the number of sign changes of v_par along the accepted steps; passing particles give none."""
+    fld = W.make_field(0)
+    F = oracle.OracleField(fld)
+    P = W.make_particles(0).head(40)
+    mu = _mu_for(F, P)
+    spec = W.make_spec(0)
+    spec.t_max = 4e-5
+    r = F.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu, poincare_capacity=4000, traj_capacity=20000, section=1)
+    rec = r.poincare[np.lexsort((r.poincare[:, 1], r.poincare[:, 0]))]
+    assert r.poincare_count == len(rec) > 20
+    per = {i: rec[rec[:, 0] == i] for i in range(P.n)}
+    checked = 0
+    for i in range(P.n):
+        tr = r.traj[i, :r.traj_count[i]]
+        u = np.concatenate([[P.vpar[i] / VREF], tr[:, 4]])
+        changes = int(np.sum((u[:-1] < 0) & (u[1:] >= 0)) + np.sum((u[:-1] > 0) & (u[1:] <= 0)))
+        assert len(per[i]) == changes
+        if changes == 0:                                       # passing, or not yet turned: no record
+            continue
+        if checked >= 6:
+            continue
+        ev = lambda t, y: y[3]
+        sol = solve_ivp(lambda t, y: F.rhs(M, Q, mu[i], VREF, t, y), (0.0, float(r.t[i])),
+                        [P.s[i], P.theta[i], P.zeta[i], P.vpar[i] / VREF], method="DOP853", rtol=1e-12, atol=1e-14,
+                        events=ev)
+        te, ye = sol.t_events[0], sol.y_events[0]
+        te, ye = te[te > 0], ye[te > 0]
+        assert len(te) == changes
+        assert np.abs(per[i][:, 1] - te).max() < 1e-11          # seconds; bounce periods are ~1e-5 s
+        assert np.abs(per[i][:, 2] - ye[:, 0]).max() < 2e-6     # global error of the rtol 1e-9 trace after ~30 bounces
+        dth = np.abs(per[i][:, 3] - np.mod(ye[:, 1], 2 * np.pi))
+        assert np.minimum(dth, 2 * np.pi - dth).max() < 2e-5
+        checked += 1
+    assert checked >= 4
+    passing = [i for i in range(P.n) if abs(P.vpar[i]) / VREF > 0.8]
+    assert passing and all(len(per[i]) == 0 for i in passing)
+
+
+def test_bounce_section_in_a_closed_form_field_has_no_crossings_and_zeta_section_is_unchanged():
+    """B00-only field: v_par is constant, so the bounce section records nothing whatever the sign of v_par; the
+    default section (zeta planes) of the same call is what it was (section = 0 is the old behaviour)."""
+    ns = 21
+    s_n = np.arange(ns) / (ns - 1)
+    fld = W.Field(ns=ns, nfp=4, xm=np.zeros(1, np.int32), xn=np.zeros(1, np.int32), bmnc=np.full((ns, 1), 5.7),
+                  G=np.full(ns, 57.0), I=np.zeros(ns), iota=0.42 + 0.1 * s_n, psi0=W.PSI0)
+    F = oracle.OracleField(fld)
+    s0 = np.array([0.3, 0.6]); th0 = np.array([0.5, 1.0]); ze0 = np.array([0.1, -2.0])
+    v0 = np.array([0.8, -0.5]) * VREF
+    mu = 0.5 * M * (VREF ** 2 - v0 ** 2) / 5.7
+    spec = W.make_spec(0)
+    spec.t_max = 2e-5
+    b = F.trace(spec, s0, th0, ze0, v0, mu, poincare_capacity=100, section=1)
+    assert b.poincare_count == 0
+    z = F.trace(spec, s0, th0, ze0, v0, mu, poincare_capacity=100, section=0)
+    z0 = F.trace(spec, s0, th0, ze0, v0, mu, poincare_capacity=100)
+    srt = lambda a: a[np.lexsort((a[:, 1], a[:, 0]))]           # record order depends on the thread schedule
+    assert z.poincare_count == z0.poincare_count > 0 and np.array_equal(srt(z.poincare), srt(z0.poincare))

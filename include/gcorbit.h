@@ -73,8 +73,11 @@ typedef struct {
  * GC_ST_TMAX (0) are traced, from (s0, th0, ze0, vpar0) at t0; every output of the others is left as it
  * is, and n_acc, n_rej, n_forced are added to instead of overwritten (max_steps stays per call).  Together with h_inout, and with s0..vpar0 aliasing the rows of y_out (allowed: a particle is read
  * once before anything of it is written), a long horizon runs as consecutive calls on the same buffers,
- * each continuing where the last one stopped (checkpoint / resume). */
-enum { GC_TRACE_RESUME = 1 };
+ * each continuing where the last one stopped (checkpoint / resume).
+ * GC_TRACE_SECTION_VPAR (NEXT-1, O8b; "trapped particle Poincare map"): the Poincare records are taken
+ * where v_par changes sign (the bounce points, both directions) instead of at zeta = 0 mod 2 pi; same record
+ * format; small ensembles are then traced by the generic kernel. */
+enum { GC_TRACE_RESUME = 1, GC_TRACE_SECTION_VPAR = 2 };
 
 /* Per-particle exit status written by gc_trace. */
 enum { GC_ST_TMAX = 0, GC_ST_LOST = 1, GC_ST_AXIS = 2, GC_ST_MAXSTEPS = 3, GC_ST_NONFINITE = 4 };

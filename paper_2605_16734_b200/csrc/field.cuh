@@ -43,6 +43,7 @@ struct TraceDev {
   long long max_steps, poincare_capacity;
   long long n;
   int resume;                         // GC_TRACE_RESUME: skip particles whose status is not 0 on entry
+  int section;                        // Poincare records: 0 zeta = 0 mod 2 pi (O8), 1 v_par = 0 (O8b)
   const double *s0, *th0, *ze0, *vpar0, *mu;
   double* h_inout;
   double *y_out, *t_out;

@@ -193,6 +193,49 @@ __device__ __forceinline__ double dense_component(double y, double yn, double hk
   return fma(tau, fma(sg, fma(tau, fma(sg, hd, r4), r3), r2), y);
 }
 
+// d/dtau of dense_component.
+__device__ __forceinline__ double dense_component_slope(double y, double yn, double hk1, double hk7, double hd,
+                                                        double tau) {
+  const double r2 = yn - y, r3 = hk1 - r2, r4 = r2 - hk7 - r3, sg = 1.0 - tau;
+  const double P4 = fma(sg, hd, r4), dP4 = -hd;
+  const double P3 = fma(tau, P4, r3), dP3 = fma(tau, dP4, P4);
+  const double P2 = fma(sg, P3, r2), dP2 = fma(sg, dP3, -P3);
+  return fma(tau, dP2, P2);
+}
+
+// O8b: the bounce section v_par = 0 (u = v_par / v_ref changes sign over the accepted step, or ends on 0).  Called by
+// ONE thread per particle-step with y, y_new and h k1, h k7, h sum d_i k_i of the four components.
+__device__ __forceinline__ bool bounce_crossed(double u0, double u1) {
+  return (u0 < 0.0 && u1 >= 0.0) || (u0 > 0.0 && u1 <= 0.0);
+}
+__device__ inline void bounce_emit(const double (&y)[4], const double (&yn)[4], const double (&hk1)[4],
+                                   const double (&hk7)[4], const double (&hd)[4], long long id, double t, double h,
+                                   double* buf, long long cap, unsigned long long* count) {
+  constexpr double kTwoPi = 6.283185307179586476925286766559;
+  double lo = 0.0, hi = 1.0, glo = y[3];
+  for (int it = 0; it < 8; ++it) {
+    const double mid = 0.5 * (lo + hi);
+    const double g = dense_component(y[3], yn[3], hk1[3], hk7[3], hd[3], mid);
+    if ((g < 0.0) == (glo < 0.0) && g != 0.0) { lo = mid; glo = g; } else { hi = mid; }
+  }
+  double tau = 0.5 * (lo + hi);
+  for (int it = 0; it < 20; ++it) {
+    const double g = dense_component(y[3], yn[3], hk1[3], hk7[3], hd[3], tau);
+    const double dv = dense_component_slope(y[3], yn[3], hk1[3], hk7[3], hd[3], tau);
+    if (fabs(g) < 1e-12 || dv == 0.0) break;
+    tau = fmin(fmax(tau - g / dv, lo), hi);
+  }
+  const unsigned long long slot = atomicAdd(count, 1ULL);
+  if ((long long)slot < cap) {
+    const double sv = dense_component(y[0], yn[0], hk1[0], hk7[0], hd[0], tau);
+    const double thv = dense_component(y[1], yn[1], hk1[1], hk7[1], hd[1], tau);
+    double thm = fmod(thv, kTwoPi);
+    if (thm < 0.0) thm += kTwoPi;
+    double* r = buf + slot * 4;
+    r[0] = (double)id; r[1] = fma(tau, h, t); r[2] = sv; r[3] = thm;
+  }
+}
+
 // ---- generic trace: one thread per particle ----------------------------------------------------------------
 __global__ void __launch_bounds__(128) trace_generic_kernel(FieldDev f, TraceDev p) {
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < p.n;
@@ -273,8 +316,19 @@ __global__ void __launch_bounds__(128) trace_generic_kernel(FieldDev f, TraceDev
       if (accept) {
         const double sc = scale_after_accept(err);
         const double h_next = prev_rejected ? h_try * fmin(sc, 1.0) : h_try * sc;
-        if (p.poincare_capacity > 0 && floor(y[2] / 6.283185307179586476925286766559) !=
-                                           floor(yn[2] / 6.283185307179586476925286766559)) {
+        if (p.poincare_capacity > 0 && p.section == 1) {              // O8b: bounce section
+          if (bounce_crossed(y[3], yn[3])) {
+            double hk1[4], hk7[4], hd[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              hk1[c] = h_try * k[0][c]; hk7[c] = h_try * k[6][c];
+              hd[c] = h_try * fma(dp::d7, k[6][c], fma(dp::d6, k[5][c], fma(dp::d5, k[4][c],
+                                fma(dp::d4, k[3][c], fma(dp::d3, k[2][c], dp::d1 * k[0][c])))));
+            }
+            bounce_emit(y, yn, hk1, hk7, hd, i, t, h_try, p.poincare, p.poincare_capacity, p.poincare_count);
+          }
+        } else if (p.poincare_capacity > 0 && floor(y[2] / 6.283185307179586476925286766559) !=
+                                                  floor(yn[2] / 6.283185307179586476925286766559)) {
           Dense3 d;
 #pragma unroll
           for (int c = 0; c < 3; ++c) {

@@ -340,7 +340,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
     const int bin = home_bin(f.ns, y0);
     int jn0 = 0;
     if constexpr (SAMPLE) {
-      if (st == kStRunning && mode == 0) {
+      if (st == kStRunning && mode == 0 && p.nsamp > 0) {
         long long j = first_sample_index(p, t);
         if (j < p.nsamp && sample_time(p, j) == t) {           // a sample on t0 is the initial state
           p.samples[(0 * p.nsamp + j) * p.n + i] = y0;
@@ -544,7 +544,23 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
             if (running && accept) {
               const double scl = scale_after_accept(err);
               const double h_next = (flags & kFlagPrevRejected) ? h_try * fmin(scl, 1.0) : h_try * scl;
-              if (p.poincare_capacity > 0 && floor(y[2] / kTwoPi) != floor(yn[2] / kTwoPi)) {
+              bool zeta_section = true;
+              if constexpr (SAMPLE) {                                     // O8b lives in the diagnostics build only
+                if (p.section == 1) {
+                  zeta_section = false;
+                  if (p.poincare_capacity > 0 && bounce_crossed(y[3], yn[3])) {
+                    double hk1[4], hk7[4], hd[4];
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                      double dd = 0.0;
+                      for (int j = 0; j < 7; ++j) dd = fma(cDpD[j], kb(j, c), dd);
+                      hk1[c] = h_try * kb(0, c); hk7[c] = h_try * kb(6, c); hd[c] = h_try * dd;
+                    }
+                    bounce_emit(y, yn, hk1, hk7, hd, pid, t, h_try, p.poincare, p.poincare_capacity, p.poincare_count);
+                  }
+                }
+              }
+              if (zeta_section && p.poincare_capacity > 0 && floor(y[2] / kTwoPi) != floor(yn[2] / kTwoPi)) {
                 Dense3 d;
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {

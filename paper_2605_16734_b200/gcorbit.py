@@ -105,6 +105,7 @@ def _stream_ptr(torch):
 
 
 GC_TRACE_RESUME = 1
+GC_TRACE_SECTION_VPAR = 2
 
 
 def make_params(spec, t0=None, t_max=None, poincare_capacity=0, flags=0) -> gc_trace_params:

@@ -202,3 +202,68 @@ def test_birkhoff_matches_oracle():
         else:
             assert out[2, i] > 10.5
     assert out[2, 0] > 8.0 and out[2, 1] < 3.0                # regular vs chaotic
+
+
+# ---- GC_TRACE_SECTION_VPAR: bounce section -----------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", ["generic", "warp", "tile", "mma"])
+def test_bounce_section_matches_oracle(kernel):
+    """Poincare records at the bounce points (v_par = 0) of 96 config-0 particles (the warp kernel hands the call
+    to the generic one): same particles, same count, times / s / theta within the O8 tolerances."""
+    import torch
+    from paper_2605_16734_b200 import gcorbit as G
+    fld, spec, P, OF, GF, mu = make_case(0, 96)
+    _kernel(GF, kernel)
+    t_max, cap = 3e-5, 4096
+    r = GF.trace(spec, to_dev(P.s), to_dev(P.theta), to_dev(P.zeta), to_dev(P.vpar), to_dev(mu), t_max=t_max,
+                 poincare_capacity=cap, flags=G.GC_TRACE_SECTION_VPAR)
+    torch.cuda.synchronize()
+    G.finish_poincare(r)
+    o = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=t_max, poincare_capacity=cap, section=1)
+    same = (r.n_acc.cpu().numpy() == o.n_acc) & (r.n_rej.cpu().numpy() == o.n_rej)
+    assert same.mean() >= 0.97 and o.poincare_count > 50
+    srt = lambda a: a[np.lexsort((a[:, 1], a[:, 0]))]
+    a, b = srt(r.poincare.cpu().numpy()), srt(o.poincare)
+    keep_a, keep_b = same[a[:, 0].astype(int)], same[b[:, 0].astype(int)]
+    a, b = a[keep_a], b[keep_b]                                 # particles on the oracle's step sequence
+    assert a.shape == b.shape and np.array_equal(a[:, 0], b[:, 0])
+    assert np.abs(a[:, 1] - b[:, 1]).max() <= 1e-9 * t_max
+    assert np.abs(a[:, 2] - b[:, 2]).max() <= 1e-9
+    dth = np.abs(a[:, 3] - b[:, 3])
+    assert np.minimum(dth, 2 * np.pi - dth).max() <= 1e-8
+    # and the default section of the same field is untouched by the new code path
+    z = GF.trace(spec, to_dev(P.s), to_dev(P.theta), to_dev(P.zeta), to_dev(P.vpar), to_dev(mu), t_max=t_max,
+                 poincare_capacity=cap)
+    torch.cuda.synchronize()
+    G.finish_poincare(z)
+    oz = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=t_max, poincare_capacity=cap)
+    assert z.poincare_count == oz.poincare_count
+
+
+def test_bounce_section_large_ensemble_mma():
+    """20,000 particles of config 4 through the diagnostics build of the mma kernel; 128 checked."""
+    import torch
+    import oracle
+    from paper_2605_16734_b200 import gcorbit as G, workloads as W
+    fld, spec = W.make_field(4), W.make_spec(4)
+    P = W.make_particles(4, 20_000)
+    OF, GF = oracle.OracleField(fld), G.Field(fld)
+    mu = W.mu_from(P, OF.eval_B_many(P.s, P.theta, P.zeta)[:, 0])
+    assert GF.kernel_info(P.n)["kernel"] == "mma"
+    t_max, cap = 1e-5, 200_000
+    r = GF.trace(spec, to_dev(P.s), to_dev(P.theta), to_dev(P.zeta), to_dev(P.vpar), to_dev(mu), t_max=t_max,
+                 poincare_capacity=cap, flags=G.GC_TRACE_SECTION_VPAR)
+    torch.cuda.synchronize()
+    G.finish_poincare(r)
+    assert 0 < r.poincare_count <= cap
+    k = 128
+    Q = P.head(k)
+    o = OF.trace(spec, Q.s, Q.theta, Q.zeta, Q.vpar, mu[:k], t_max=t_max, poincare_capacity=cap, section=1)
+    same = (r.n_acc.cpu().numpy()[:k] == o.n_acc) & (r.n_rej.cpu().numpy()[:k] == o.n_rej)
+    assert same.mean() >= 0.97 and o.poincare_count > 10
+    srt = lambda a: a[np.lexsort((a[:, 1], a[:, 0]))]
+    a = r.poincare.cpu().numpy()
+    a = srt(a[a[:, 0] < k])
+    b = srt(o.poincare)
+    a, b = a[same[a[:, 0].astype(int)]], b[same[b[:, 0].astype(int)]]
+    assert a.shape == b.shape and np.array_equal(a[:, 0], b[:, 0])
+    assert np.abs(a[:, 1] - b[:, 1]).max() <= 1e-9 * t_max and np.abs(a[:, 2] - b[:, 2]).max() <= 1e-9

@@ -137,7 +137,8 @@ int gc_trace(const gc_field* f, const gc_trace_params* params, int64_t n,
              int32_t* n_acc, int32_t* n_rej, int32_t* n_forced,
              double* poincare, int64_t* poincare_count, void* stream);
 
-/* The same trace with HOST buffers: allocates device scratch, copies the inputs in (with GC_TRACE_RESUME
+/* The same trace with HOST buffers: uses a device workspace and a stream kept in the field (grown on demand, freed
+ * by gc_field_destroy; calls on one field must not overlap), copies the inputs in (with GC_TRACE_RESUME
  * also y_out, t_out, status and the counters, so that untouched particles keep their values), runs
  * gc_trace, copies every non-NULL output back and synchronises.  `poincare_count` is a host int64 here.
  * Pinned host buffers make the copies asynchronous; pageable ones work too. */

@@ -61,6 +61,10 @@ struct gc_field {
   int sm_count = 0;
   int tile_smem = 0;                // dynamic shared memory of the tile kernel
   int tile_blocks_per_sm = 0;       // co-resident blocks per SM (cooperative launch)
+  // workspace of gc_trace_host, kept between calls (cudaMalloc / cudaFree per call cost up to 200 ms now and then)
+  cudaStream_t host_stream = nullptr;
+  void* host_slab = nullptr;
+  size_t host_slab_bytes = 0;
   bool mma_ok = false;
   int mma_smem = 0;                 // dynamic shared memory of the mma kernel
   int mma_blocks_per_sm = 0;
@@ -396,6 +400,8 @@ const char* gc_last_error(void) { return g_last_error.c_str(); }
 int gc_field_destroy(gc_field* f) {
   if (!f) return GC_OK;
   for (void* p : f->allocs) cudaFree(p);
+  if (f->host_slab) cudaFree(f->host_slab);
+  if (f->host_stream) cudaStreamDestroy(f->host_stream);
   delete f;
   return GC_OK;
 }
@@ -692,15 +698,8 @@ int gc_trace_host(const gc_field* f, const gc_trace_params* params, int64_t n, c
   const int64_t cap = (poincare && poincare_count) ? params->poincare_capacity : 0;
   // one device slab: 5 inputs, h, y_out[4], t_out (doubles) | status + 3 counters (int32) | poincare
   const size_t n_dbl = nd * 11 + (size_t)cap * 4 + 1;
-  double* dbl = nullptr;
-  int32_t* i32 = nullptr;
-  cudaStream_t st = nullptr;
   int rc = GC_OK;
-  auto cleanup = [&]() {
-    if (dbl) cudaFree(dbl);
-    if (i32) cudaFree(i32);
-    if (st) cudaStreamDestroy(st);
-  };
+  auto cleanup = [&]() {};
 #define GC_H(expr)                                                                 \
   do {                                                                             \
     cudaError_t e_ = (expr);                                                       \
@@ -711,9 +710,19 @@ int gc_trace_host(const gc_field* f, const gc_trace_params* params, int64_t n, c
       return rc;                                                                   \
     }                                                                              \
   } while (0)
-  GC_H(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking));
-  GC_H(cudaMalloc((void**)&dbl, n_dbl * sizeof(double)));
-  GC_H(cudaMalloc((void**)&i32, nd * 4 * sizeof(int32_t)));
+  // stream and device slab live in the field and are reused by later calls (calls on one field must not overlap)
+  gc_field* fm = const_cast<gc_field*>(f);
+  if (!fm->host_stream) GC_H(cudaStreamCreateWithFlags(&fm->host_stream, cudaStreamNonBlocking));
+  const size_t dbl_bytes = ((n_dbl * sizeof(double) + 255) / 256) * 256;
+  const size_t need = dbl_bytes + nd * 4 * sizeof(int32_t);
+  if (need > fm->host_slab_bytes) {
+    if (fm->host_slab) { cudaFree(fm->host_slab); fm->host_slab = nullptr; fm->host_slab_bytes = 0; }
+    GC_H(cudaMalloc(&fm->host_slab, need));
+    fm->host_slab_bytes = need;
+  }
+  cudaStream_t st = fm->host_stream;
+  double* dbl = reinterpret_cast<double*>(fm->host_slab);
+  int32_t* i32 = reinterpret_cast<int32_t*>(reinterpret_cast<unsigned char*>(fm->host_slab) + dbl_bytes);
   double *d_s = dbl, *d_th = dbl + nd, *d_ze = dbl + 2 * nd, *d_v = dbl + 3 * nd, *d_mu = dbl + 4 * nd,
          *d_h = dbl + 5 * nd, *d_y = dbl + 6 * nd, *d_t = dbl + 10 * nd, *d_pc = dbl + 11 * nd;
   int64_t* d_cnt = reinterpret_cast<int64_t*>(dbl + 11 * nd + (size_t)cap * 4);

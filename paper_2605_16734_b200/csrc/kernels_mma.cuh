@@ -114,6 +114,13 @@ __device__ __forceinline__ void mma_sweep(const double* base, int RS, int r_lo, 
                                           const double (&AnS)[KS], const double (&cm)[2 * MT],
                                           const double (&sm)[2 * MT], double (&o)[4]) {
   using R = MmaRow<MT, KS>;
+  double mc[2 * MT], ms[2 * MT];                       // m c_m, m s_m of this lane's columns m = 1 + 8 T + 2 q + e
+#pragma unroll
+  for (int k = 0; k < 2 * MT; ++k) {
+    const double m = (double)(1 + 8 * (k >> 1) + 2 * q + (k & 1));
+    mc[k] = m * cm[k];
+    ms[k] = m * sm[k];
+  }
 #ifndef GC_MMA_ROW_UNROLL
 #define GC_MMA_ROW_UNROLL 2
 #endif
@@ -139,12 +146,11 @@ __device__ __forceinline__ void mma_sweep(const double* base, int RS, int r_lo, 
         dmma884(QC0, QC1, AnC[j], pq.y);
       }
       // columns m = 1 + 8 T + 2 q + e  (index 2 T + e of cm / sm)
-      const double m0 = (double)(1 + 8 * T + 2 * q), m1 = m0 + 1.0;
       const double c0 = cm[2 * T], s0 = sm[2 * T], c1 = cm[2 * T + 1], s1 = sm[2 * T + 1];
       T1 = fma(c0, PC0, T1); T1 = fma(s0, QS0, T1);
       T1 = fma(c1, PC1, T1); T1 = fma(s1, QS1, T1);
-      T2 = fma(m0, fma(c0, QS0, -s0 * PC0), T2);
-      T2 = fma(m1, fma(c1, QS1, -s1 * PC1), T2);
+      T2 = fma(mc[2 * T], QS0, T2); T2 = fma(-ms[2 * T], PC0, T2);
+      T2 = fma(mc[2 * T + 1], QS1, T2); T2 = fma(-ms[2 * T + 1], PC1, T2);
       T3 = fma(s0, QC0, T3); T3 = fma(-c0, PS0, T3);
       T3 = fma(s1, QC1, T3); T3 = fma(-c1, PS1, T3);
     }

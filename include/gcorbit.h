@@ -96,7 +96,7 @@ enum { GC_ST_TMAX = 0, GC_ST_LOST = 1, GC_ST_AXIS = 2, GC_ST_MAXSTEPS = 3, GC_ST
  *                     when the field fits it, else GENERIC.
  * All four implement the same equations and controller; their results differ at rounding level only. */
 enum { GC_KERNEL_AUTO = 0, GC_KERNEL_GENERIC = 1, GC_KERNEL_WARP = 2, GC_KERNEL_TILE = 3, GC_KERNEL_MMA = 4 };
-enum { GC_TILE_MIN_PARTICLES = 8192 };
+enum { GC_TILE_MIN_PARTICLES = 4096 };
 
 /* Copies the tables to the device, checks them (finite values, xm >= 0, omega != 0) and builds the
  * packed by-node layout of the warp kernel.  *out is NULL on failure. */

@@ -327,6 +327,25 @@ int pack_mma_image(gc_field* f, const gc_field_desc* d) {
   return GC_OK;
 }
 
+// Blocks and particles per tile for n particles: full tiles when the ensemble fills the persistent grid, else
+// tiles shrunk (to a multiple of 8 = one DMMA group; smaller tiles were measured and gain nothing) so that every
+// block gets one.
+long long tile_geometry(const gc_field* f, long long n, bool mma, int* tile_size) {
+  const int threads = mma ? gc::kMmaThreads : gc::kTileThreads;
+  const long long grid = (long long)f->sm_count * (mma ? f->mma_blocks_per_sm : f->tile_blocks_per_sm);
+  long long tsz = threads;
+  if (n < grid * threads) {
+    tsz = ((n + grid - 1) / grid + 7) / 8 * 8;
+    if (tsz < 8) tsz = 8;
+    if (tsz > threads) tsz = threads;
+  }
+  long long blocks = (n + tsz - 1) / tsz;
+  if (blocks > grid) blocks = grid;
+  if (blocks < 1) blocks = 1;
+  *tile_size = (int)tsz;
+  return blocks;
+}
+
 // One cooperative launch of the tile or mma kernel (mode 0 trace, mode 1 right-hand side only) with its scratch.
 int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, cudaStream_t st, bool mma = false) {
   const int ncell = f->dev.ns - 3;
@@ -346,11 +365,9 @@ int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, c
   sc.tstart = ip; ip += ncell + 1;
   sc.ctrl = ip;
   GC_CUDA(cudaMemsetAsync(sc.cnt, 0, (2 * nbin + (size_t)2 * (ncell + 1) + 8) * sizeof(int), st));
-  const int per_tile = mma ? gc::kMmaThreads : gc::kTileThreads;
-  long long blocks = (long long)f->sm_count * (mma ? f->mma_blocks_per_sm : f->tile_blocks_per_sm);
-  const long long need = ((long long)n + per_tile - 1) / per_tile;
-  if (blocks > need) blocks = need;
-  if (blocks < 1) blocks = 1;
+  int per_tile = 0;
+  long long blocks = tile_geometry(f, (long long)n, mma, &per_tile);
+  sc.tile_size = per_tile;
   gc::FieldDev fd = f->dev;
   void* args[] = {(void*)&fd, (void*)&t, (void*)&sc, (void*)&mode, (void*)&rhs_out};
   const bool sample = mode == 0 && (t.nsamp > 0 || t.section != 0);   // the diagnostics build of the kernel
@@ -511,16 +528,12 @@ int gc_kernel_info(const gc_field* f, int64_t n, int32_t* kernel, int32_t* block
   const int k = resolve_kernel(f, n);
   if (k == GC_KERNEL_MMA) {
     GC_CUDA(cudaFuncGetAttributes(&at, mma_fn(f)));
-    long long bl = (long long)f->sm_count * f->mma_blocks_per_sm;
-    const long long need = (n + gc::kMmaThreads - 1) / gc::kMmaThreads;
-    if (bl > need) bl = need < 1 ? 1 : need;
-    b = (int)bl; t = gc::kMmaThreads; s = f->mma_smem;
+    int tsz = 0;
+    b = (int)tile_geometry(f, n, true, &tsz); t = gc::kMmaThreads; s = f->mma_smem;
   } else if (k == GC_KERNEL_TILE) {
     GC_CUDA(cudaFuncGetAttributes(&at, tile_fn(f)));
-    long long bl = (long long)f->sm_count * f->tile_blocks_per_sm;
-    const long long need = (n + gc::kTileThreads - 1) / gc::kTileThreads;
-    if (bl > need) bl = need < 1 ? 1 : need;
-    b = (int)bl; t = gc::kTileThreads; s = f->tile_smem;
+    int tsz = 0;
+    b = (int)tile_geometry(f, n, false, &tsz); t = gc::kTileThreads; s = f->tile_smem;
   } else if (k == GC_KERNEL_WARP) {
     const WarpInst* w = find_inst(f);
     GC_CUDA(cudaFuncGetAttributes(&at, w->trace_fn));

@@ -56,6 +56,7 @@ struct TileScratch {
   int* start;       // [ncell + 1] cell segment offsets into order
   int* tstart;      // [ncell + 1] tile offsets
   int* cursor;      // [ncell kSubBins] scatter cursors
+  int tile_size;    // particles per tile, a multiple of 8, <= threads per block
   int* ctrl;        // [0] tile counter, [1] tiles past their first chunk, [2] tiles this epoch, [3] running
 };
 
@@ -311,6 +312,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
   const long long gthreads = (long long)gridDim.x * THREADS;
   const int ncell = f.ns - 3;
   const int WD = Eng::win_doubles(f);
+  const int tsz = sc.tile_size;          // particles per tile (<= THREADS; smaller when the ensemble cannot fill the grid)
   constexpr double kTwoPi = 6.283185307179586476925286766559;
 
   double* win = reinterpret_cast<double*>(gc_tile_smem);                 // [WD] window image of the tile's cell
@@ -380,7 +382,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
             wsp[b] = run;
             run += k;
           }
-          tiles += (run - run0 + THREADS - 1) / THREADS;
+          tiles += (run - run0 + tsz - 1) / tsz;
         }
         sc.start[ncell] = run;
         sc.tstart[ncell] = tiles;
@@ -426,8 +428,8 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
       }
       const int cell = lo;
       const int seg0 = __ldcg(sc.start + cell), seg1 = __ldcg(sc.start + cell + 1);
-      const int begin = seg0 + (tile - __ldcg(sc.tstart + cell)) * THREADS;
-      const int count = min(THREADS, seg1 - begin);
+      const int begin = seg0 + (tile - __ldcg(sc.tstart + cell)) * tsz;
+      const int count = min(tsz, seg1 - begin);
       if (Eng::kStageWindow && cell != cur_cell) {                       // stage the window: one bulk copy
         if (tid == 0) {
           asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -631,7 +633,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
         if (tid == 0) {
           const int next = atomicAdd(sc.ctrl + 0, 1);
           bool more = false;
-          if (next >= ntiles && nrun * 2 >= THREADS) {
+          if (next >= ntiles && nrun * 2 >= tsz) {
             const volatile int* vc = sc.ctrl;
             more = vc[1] < ntiles;
           }

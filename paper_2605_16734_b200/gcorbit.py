@@ -17,7 +17,7 @@ SO_PATH = os.path.join(_HERE, "libgcorbit.so")
 
 GC_OK, GC_EINVAL, GC_ENOMEM, GC_ECUDA = 0, -1, -2, -3
 GC_KERNEL_AUTO, GC_KERNEL_GENERIC, GC_KERNEL_WARP, GC_KERNEL_TILE, GC_KERNEL_MMA = 0, 1, 2, 3, 4
-GC_TILE_MIN_PARTICLES = 8192
+GC_TILE_MIN_PARTICLES = 4096
 ST_TMAX, ST_LOST, ST_AXIS, ST_MAXSTEPS, ST_NONFINITE = 0, 1, 2, 3, 4
 
 EXPORTS = ["gc_field_create", "gc_field_destroy", "gc_field_eval", "gc_pert_eval", "gc_rhs_eval", "gc_trace",

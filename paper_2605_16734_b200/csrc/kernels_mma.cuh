@@ -26,16 +26,17 @@
 //     order, one 16-byte load per lane and k-step; n = 0 initialises the PC accumulator, m = 0 is a 16-term DFMA
 //     sum split over the quad;
 //   * rows: the group sweeps the UNION of the stencil rows of its 8 particles (4 rows when they share a stencil,
-//     5 when they straddle a node); the Lagrange weight of each row comes from the particle lane by shuffle and
-//     is exactly 0 for a row outside that particle's stencil, so a particle's result does not depend on who it
-//     shares a group with;
+//     5 when they straddle a node); the Lagrange weights of a row come from the particle's six-entry table in
+//     shared memory (one LDS.128) and are exactly 0 for a row outside that particle's stencil, so a particle's
+//     result does not depend on who it shares a group with;
 //   * per row the epilogue turns the eight accumulators of a lane into its share of B, B_s, B_theta, B_zeta;
 //     two butterfly shuffles sum the quad and one more hands the four sums back to the particle lane.
 // Window: the 8 node rows cell-2 .. cell+5 of a by-node image (contiguous in global memory, ONE bulk TMA copy per
 // cell change); stencils that start further than 2 rows from the tile's cell are swept from global memory with the
 // same instruction sequence (bit-identical results).  Binning, epochs, tiles, records and the integrator are
-// trace_binned_body of kernels_tile.cuh; tiles are 64 particles (two warps share a window), chunks are 8 attempts:
-// frequent re-binning keeps the groups on 4-row unions and parks few particles.
+// trace_binned_body of kernels_tile.cuh; tiles are 64 particles (two warps share a window; fewer when the ensemble
+// cannot fill the grid), chunks are 8 attempts: frequent re-binning keeps the groups on 4-row unions and parks few
+// particles.
 #pragma once
 #include <cooperative_groups.h>
 

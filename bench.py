@@ -354,6 +354,7 @@ def run_cuda(args):
     except Exception:
         pass
     probe_flops, _ = G.fp64_peak_probe()
+    dmma_flops, mixed_flops = G.dmma_peak_probe()
     fstep = info["flop_per_particle_step"]
     achieved = attempts * fstep / (kernel_ms * 1e-3) / 1e12         # this rank's kernel, TFLOP/s
     traffic = None
@@ -371,7 +372,8 @@ def run_cuda(args):
                 "frac": achieved / peak_nominal, "traffic": traffic,
                 "kernel": f"trace_{kinfo['kernel']}_kernel", "launch_ms_avg": kernel_ms / K,
                 "peak_source": "148 SMs x 64 FP64 lanes x 2 flop x clocks.max.sm (DESIGN.md section 6)",
-                "peak_probe_tflops": probe_flops / 1e12,
+                "peak_probe_tflops": probe_flops / 1e12, "peak_probe_dmma_tflops": dmma_flops / 1e12,
+                "peak_probe_dmma_dfma_mixed_tflops": mixed_flops / 1e12,
                 "frac_of_probe": achieved / (probe_flops / 1e12),
                 "flop_per_particle_step": fstep,
                 "particle_steps_per_launch": attempts / K}

@@ -199,6 +199,12 @@ int gc_kernel_info(const gc_field* f, int64_t n, int32_t* kernel, int32_t* block
  * Synchronous. */
 int gc_fp64_peak_probe(double* flops_per_s, double* elapsed_ms);
 
+/* The same for the FP64 matrix instruction the mma kernel is built on: DMMA.8x8x4 (mma.sync.m8n8k4.f64) with 8
+ * independent accumulators per warp, alone (*flops_dmma) and with one DFMA per DMMA mixed in (*flops_mixed, counting
+ * both): the two instruction kinds share the FP64 units, so there is one FP64 roofline.
+ * Synchronous. */
+int gc_dmma_peak_probe(double* flops_dmma, double* flops_mixed);
+
 /* Thread-local text of the last nonzero return ("" if none). */
 const char* gc_last_error(void);
 

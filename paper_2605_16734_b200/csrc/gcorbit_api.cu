@@ -408,6 +408,25 @@ __global__ void dfma_probe_kernel(double* out, int iters) {
   if (a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7 == 12345.678) out[0] = a0;
 }
 
+// 8 independent DMMA.8x8x4 accumulators per warp; MIX > 0 adds MIX DFMA per 8 DMMA (the two share the FP64 units).
+template <int MIX>
+__global__ void dmma_probe_kernel(double* out, int iters) {
+  double acc[16], f[8];
+  for (int i = 0; i < 16; ++i) acc[i] = threadIdx.x * 1e-9 + i;
+  for (int i = 0; i < 8; ++i) f[i] = i + 1.0;
+  const double a = 0.999 + threadIdx.x * 1e-6, b = 1e-3;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int j = 0; j < 8; ++j) gc::dmma884(acc[2 * j], acc[2 * j + 1], a, b);
+#pragma unroll
+    for (int j = 0; j < MIX; ++j) f[j & 7] = fma(f[j & 7], a, b);
+  }
+  double s = 0.0;
+  for (int i = 0; i < 16; ++i) s += acc[i];
+  for (int i = 0; i < 8; ++i) s += f[i];
+  if (s == 12345.678) out[0] = s;
+}
+
 }  // namespace
 
 extern "C" {
@@ -807,6 +826,38 @@ int gc_fp64_peak_probe(double* flops_per_s, double* elapsed_ms) {
   const double flops = 2.0 * 8.0 * (double)iters * (double)blocks * (double)threads;
   if (flops_per_s) *flops_per_s = flops / (best * 1e-3);
   if (elapsed_ms) *elapsed_ms = best;
+  return GC_OK;
+}
+
+int gc_dmma_peak_probe(double* flops_dmma, double* flops_mixed) {
+  int devid = 0, sms = 0;
+  GC_CUDA(cudaGetDevice(&devid));
+  GC_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, devid));
+  double* out = nullptr;
+  GC_CUDA(cudaMalloc((void**)&out, sizeof(double)));
+  const int iters = 40000, blocks = sms * 2, threads = 128;          // 2 warps per SM sub-partition
+  cudaEvent_t a, b;
+  GC_CUDA(cudaEventCreate(&a));
+  GC_CUDA(cudaEventCreate(&b));
+  float best[2] = {1e30f, 1e30f};
+  for (int which = 0; which < 2; ++which) {
+    for (int rep = 0; rep < 4; ++rep) {                                // first repetition warms up
+      GC_CUDA(cudaEventRecord(a));
+      if (which == 0) dmma_probe_kernel<0><<<blocks, threads>>>(out, iters);
+      else dmma_probe_kernel<8><<<blocks, threads>>>(out, iters);
+      GC_CUDA(cudaEventRecord(b));
+      GC_CUDA(cudaEventSynchronize(b));
+      float ms = 0;
+      GC_CUDA(cudaEventElapsedTime(&ms, a, b));
+      if (rep > 0 && ms < best[which]) best[which] = ms;
+    }
+  }
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  cudaFree(out);
+  const double warps = (double)blocks * threads / 32.0;
+  if (flops_dmma) *flops_dmma = 8.0 * 512.0 * iters * warps / (best[0] * 1e-3);
+  if (flops_mixed) *flops_mixed = (8.0 * 512.0 + 8.0 * 64.0) * iters * warps / (best[1] * 1e-3);
   return GC_OK;
 }
 

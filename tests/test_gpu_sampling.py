@@ -78,13 +78,14 @@ def test_samples_large_ensemble_mma(config):
     print("config", config, "samples max rel", _sample_parity(r, o, spec, k, f"samples mma config {config}"))
 
 
-def test_samples_continue_over_resumed_segments():
+@pytest.mark.parametrize("kernel", ["generic", "tile", "mma"])
+def test_samples_continue_over_resumed_segments(kernel):
     """GC_TRACE_RESUME with the same sample buffers: the grid continues; compared with the oracle run in the same
     two segments."""
     import torch
     from paper_2605_16734_b200 import gcorbit as G
     fld, spec, P, OF, GF, mu = make_case(0, 64)
-    _kernel(GF, "generic")
+    _kernel(GF, kernel)
     dt, nsamp = 2.0 ** -23, 17
     t1, t2 = 8 * dt, 16 * dt
     h = torch.zeros(P.n, dtype=torch.float64, device="cuda:0")

@@ -268,3 +268,50 @@ def test_bounce_section_large_ensemble_mma():
     a, b = a[same[a[:, 0].astype(int)]], b[same[b[:, 0].astype(int)]]
     assert a.shape == b.shape and np.array_equal(a[:, 0], b[:, 0])
     assert np.abs(a[:, 1] - b[:, 1]).max() <= 1e-9 * t_max and np.abs(a[:, 2] - b[:, 2]).max() <= 1e-9
+
+
+def test_birkhoff_digits_of_pzeta_turn_chaotic_with_the_mode_amplitude():
+    """The whole NEXT-1 chain on the device on a case with a known answer (the weighted Birkhoff
+    average of P_zeta as integrability diagnostic, digit accuracy below 3 = chaotic): an axisymmetric equilibrium
+    (non-symmetric harmonics removed) conserves P_zeta, so without modes every orbit is regular; three
+    shear-Alfven harmonics of one n and one omega break it, the more the larger they are.  2048 particles, 3001
+    uniform-time samples over 3e-3 s, gc_trace_sampled -> gc_pzeta_eval -> gc_birkhoff."""
+    import torch
+    from paper_2605_16734_b200 import gcorbit as G, workloads as W
+    spec = W.make_spec(1)
+    P = W.make_particles(1, 2048)
+    nsamp, dt = 3001, 1e-6
+    frac_chaotic, med = {}, {}
+    for amp in (0.0, 1e3, 1e5):
+        fld = W.make_field(1)
+        keep = fld.xn == 0
+        fld.xm, fld.xn, fld.bmnc = fld.xm[keep], fld.xn[keep], np.ascontiguousarray(fld.bmnc[:, keep])
+        s_n = np.arange(fld.ns) / (fld.ns - 1)
+        fld.mode_m = np.array([3, 4, 5], np.int32)
+        fld.mode_n = np.array([2, 2, 2], np.int32)
+        fld.mode_omega = np.full(3, 2 * math.pi * 120e3)
+        fld.mode_phase = np.array([0.0, 1.0, 2.0])
+        env = np.exp(-(s_n - 0.4) ** 2 / (2 * 0.1 ** 2))
+        fld.phihat = np.stack([amp * env, 0.8 * amp * env, 0.6 * amp * env], axis=1)
+        GF = G.Field(fld)
+        GF.set_kernel(G.GC_KERNEL_MMA)
+        s, th, ze, vp = (to_dev(x) for x in (P.s, P.theta, P.zeta, P.vpar))
+        B, _ = GF.field_eval(s, th, ze, derivs=False)
+        mu = to_dev(0.5 * spec.mass * P.vperp2()) / B
+        r = GF.trace_sampled(spec, s, th, ze, vp, mu, 0.0, dt, nsamp, t_max=3e-3)
+        chi = to_dev(fld.psi0 * (0.42 * s_n + 0.05 * s_n ** 2))
+        tt = (torch.arange(nsamp, dtype=torch.float64, device="cuda:0") * dt).repeat_interleave(P.n)
+        pz = GF.pzeta_eval(spec.mass, spec.charge, r.samples.reshape(4, -1), tt, chi).reshape(nsamp, P.n)
+        wb = G.birkhoff(pz, 0, r.sample_end)
+        torch.cuda.synchronize()
+        full = r.sample_end == nsamp
+        assert int(full.sum()) > 0.95 * P.n
+        d = wb[2][full].cpu().numpy()
+        frac_chaotic[amp], med[amp] = float(np.mean(d < 3.0)), float(np.median(d))
+        if amp == 0.0:                                       # P_zeta itself is constant to the integrator's accuracy
+            pzv = pz[:, full].cpu().numpy()
+            assert np.median(pzv.std(axis=0) / np.abs(pzv.mean(axis=0))) < 1e-6
+    print("fraction with digits < 3:", frac_chaotic, "median digits:", med)
+    assert frac_chaotic[0.0] == 0.0 and med[0.0] > 6.0
+    assert frac_chaotic[0.0] <= frac_chaotic[1e3] < frac_chaotic[1e5] and frac_chaotic[1e5] > 0.3
+    assert med[1e5] < 4.0 < med[1e3]

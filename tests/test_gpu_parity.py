@@ -263,3 +263,52 @@ def test_trace_fine_grid_steps_across_several_cells(kernel):
     info = assert_trace_parity(Sub, o, spec, label=f"fine grid {kernel}", cond=cond, min_same=0.97, min_within=0.5,
                                median_rtol=1e-9, flip_rtol=1e3 * spec.rtol)
     print(f"fine grid {kernel}: {info}, cells crossed up to {ds.max():.1f}")
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_general_field_rhs_and_trace(kernel):
+    """A field that exercises what the configs leave at zero: I(s) != 0, G'(s) != 0, nonlinear iota, harmonics given
+    in shuffled order with a duplicated (m, n) pair (duplicates add, gcorbit.h), M = 11 and N = 13 (zero-padded in the
+    packed layouts), two modes with different omega.  Right-hand side at 300 points and a short trace of 300
+    particles against the oracle, every kernel."""
+    import torch
+    import oracle
+    from paper_2605_16734_b200 import gcorbit as G, workloads as W
+    rng = np.random.default_rng(5)
+    ns, nfp, M, N = 61, 3, 11, 13
+    xm, xn = W.harmonic_list(M, N)
+    s_n = np.arange(ns) / (ns - 1)
+    amp = 0.04 * 5.0 * rng.standard_normal(xm.size) * np.exp(-(xm + np.abs(xn)) / 3.0)
+    bmnc = amp[None, :] * (s_n[:, None] ** (xm[None, :] / 2.0))
+    bmnc[:, 0] = 5.0 + 0.3 * s_n
+    perm = rng.permutation(xm.size)
+    xm, xn, bmnc = xm[perm], xn[perm], bmnc[:, perm]
+    dup = int(np.nonzero((xm == 3) & (xn == -2))[0][0])
+    xm, xn = np.append(xm, xm[dup]), np.append(xn, xn[dup])               # the same harmonic once more: adds
+    bmnc = np.concatenate([bmnc, 0.5 * bmnc[:, dup:dup + 1]], axis=1)
+    env = np.exp(-(s_n - 0.45) ** 2 / (2 * 0.08 ** 2))
+    fld = W.Field(ns=ns, nfp=nfp, xm=xm.astype(np.int32), xn=xn.astype(np.int32), bmnc=np.ascontiguousarray(bmnc),
+                  G=48.0 + 2.0 * s_n - 0.7 * s_n ** 2, I=1.5 * s_n + 0.4 * s_n ** 2,
+                  iota=0.38 + 0.2 * s_n - 0.05 * s_n ** 3, psi0=6.5,
+                  mode_m=np.array([4, 7], np.int32), mode_n=np.array([-3, 5], np.int32),
+                  mode_omega=2 * np.pi * np.array([90e3, -210e3]), mode_phase=np.array([0.4, 2.0]),
+                  phihat=np.stack([3e3 * env, -2e3 * env], axis=1))
+    spec = W.make_spec(0)
+    P = W.make_particles(1, 300)
+    OF, GF = oracle.OracleField(fld), G.Field(fld)
+    mu = W.mu_from(P, OF.eval_B_many(P.s, P.theta, P.zeta)[:, 0])
+    _set_kernel(GF, kernel)
+    t = 1.7e-5
+    y = np.stack([P.s, P.theta - 20.0, P.zeta + 70.0, P.vpar])
+    got = GF.rhs_eval(spec.mass, spec.charge, t, to_dev(y), to_dev(mu))
+    torch.cuda.synchronize()
+    got = got.cpu().numpy()
+    ref = np.array([OF.rhs(spec.mass, spec.charge, mu[i], 1.0, t, y[:, i]) for i in range(P.n)]).T
+    for c in range(4):
+        scale = np.maximum(np.abs(ref[c]), 1e-6 * np.abs(ref[c]).max())
+        assert (np.abs(got[c] - ref[c]) / scale).max() < 1e-9, (c, (np.abs(got[c] - ref[c]) / scale).max())
+    r = gpu_trace(GF, spec, P, mu, t_max=1.5e-5)
+    o = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=1.5e-5)
+    cond = oracle_conditioning(OF, spec, P, mu, o, t_max=1.5e-5)
+    info = assert_trace_parity(r, o, spec, label=f"general field {kernel}", cond=cond, min_within=0.98)
+    print(f"general field {kernel}: {info}")

@@ -358,7 +358,7 @@ def run_cuda(args):
     fstep = info["flop_per_particle_step"]
     achieved = attempts * fstep / (kernel_ms * 1e-3) / 1e12         # this rank's kernel, TFLOP/s
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    tp = os.path.join(ROOT, "profiles", "traffic.json.txt")
     # one ncu capture of the DEFAULT launch (profiles/r1_ncu_mma_config1.md); other workloads have no capture
     default_launch = (args.config == 1 and args.particles is None and args.segment == 2e-5 and
                       kinfo["kernel"] == "mma" and args.samples == 0)

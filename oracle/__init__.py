@@ -45,7 +45,7 @@ class _Params(C.Structure):
                 ("rtol", C.c_double), ("atol", C.c_double), ("v_ref", C.c_double),
                 ("h0", C.c_double), ("h_min", C.c_double), ("s_loss", C.c_double), ("s_min", C.c_double),
                 ("max_steps", C.c_int64), ("poincare_capacity", C.c_int64), ("traj_capacity", C.c_int64),
-                ("section", C.c_int64)]
+                ("section", C.c_int64), ("refine_loss", C.c_int64)]
 
 
 def _load():
@@ -199,13 +199,13 @@ class OracleField:
 
     # ---- ensembles -----------------------------------------------------------------------------------
     def trace(self, spec, s0, th0, ze0, vpar0, mu, h_in=None, poincare_capacity=0, traj_capacity=0,
-              t0=None, t_max=None, section=0) -> TraceResult:
+              t0=None, t_max=None, section=0, refine_loss=False) -> TraceResult:
         s0, th0, ze0, vpar0, mu = map(_f64, (s0, th0, ze0, vpar0, mu))
         n = s0.shape[0]
         p = _Params(spec.mass, spec.charge, spec.t0 if t0 is None else t0,
                     spec.t_max if t_max is None else t_max, spec.rtol, spec.atol, spec.v_ref,
                     spec.h0, spec.h_min, spec.s_loss, spec.s_min, int(spec.max_steps),
-                    int(poincare_capacity), int(traj_capacity), int(section))
+                    int(poincare_capacity), int(traj_capacity), int(section), int(bool(refine_loss)))
         h = np.zeros(n) if h_in is None else _f64(h_in).copy()
         y = np.zeros((4, n))
         t = np.zeros(n)

@@ -440,6 +440,27 @@ static int trace_impl(const oracle_field *f, const oracle_trace_params *p, int64
           for (int c = 0; c < 4; ++c) samples[((size_t)c * nsamp + jn) * n + i] = c == 3 ? ys[3] * p->v_ref : ys[c];
           ++jn;
         }
+        /* O7b: refined loss point, taken after the samples and records of the step (they run to its end) */
+        const int lost_now = y_new[0] >= p->s_loss;
+        double t_rep = t_new, y_rep[4] = {y_new[0], y_new[1], y_new[2], y_new[3]};
+        if (lost_now && p->refine_loss && y[0] < p->s_loss) {
+          double lo = 0.0, hi = 1.0, yt[4], dyt[4];
+          for (int it = 0; it < 8; ++it) {
+            double mid = 0.5 * (lo + hi);
+            dense_and_slope(y, y_new, (const double(*)[4])k, h_try, mid, yt, dyt);
+            if (yt[0] < p->s_loss) lo = mid; else hi = mid;
+          }
+          double tau = 0.5 * (lo + hi);
+          for (int it = 0; it < 20; ++it) {
+            dense_and_slope(y, y_new, (const double(*)[4])k, h_try, tau, yt, dyt);
+            double g = yt[0] - p->s_loss;
+            if (fabs(g) < 1e-14 || dyt[0] == 0.0) break;
+            double tn = tau - g / dyt[0];
+            tau = tn < lo ? lo : (tn > hi ? hi : tn);
+          }
+          dense_and_slope(y, y_new, (const double(*)[4])k, h_try, tau, y_rep, dyt);
+          t_rep = t + tau * h_try;
+        }
         t = t_new;
         for (int c = 0; c < 4; ++c) { y[c] = y_new[c]; k1[c] = k[6][c]; }
         ++n_acc;
@@ -453,7 +474,7 @@ static int trace_impl(const oracle_field *f, const oracle_trace_params *p, int64
         }
         ++ntraj;
         /* O7 stop rules, in this order */
-        if (y[0] >= p->s_loss) st = 1;
+        if (lost_now) { st = 1; t = t_rep; for (int c = 0; c < 4; ++c) y[c] = y_rep[c]; }
         else if (y[0] <= p->s_min) st = 2;
         else if (clipped) st = 0;
         else if (attempts >= p->max_steps) st = 3;

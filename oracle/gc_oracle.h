@@ -51,6 +51,8 @@ typedef struct {
   int64_t poincare_capacity;   /* records in the shared buffer; 0 disables O8 */
   int64_t traj_capacity;       /* per-particle accepted-step records; 0 disables (oracle-only) */
   int64_t section;             /* which crossings the Poincare records hold: 0 zeta = 0 mod 2 pi (O8), 1 v_par = 0 (O8b) */
+  int64_t refine_loss;         /* O7b: 1 = a lost particle reports the root of s(tau) = s_loss on the continuous
+                                  extension of its last step (t_out, y_out) instead of the end of that step (A8) */
 } oracle_trace_params;
 
 oracle_field *oracle_field_create(const oracle_field_desc *d);

@@ -180,3 +180,32 @@ def test_config0_workload_shape():
     assert 0.03 < rej < 0.4
     per_s = r.n_acc.sum() / r.t.sum()
     assert 5e6 < per_s < 2e8
+
+
+def test_refined_loss_time_against_closed_form_drift():
+    """O7b: with refine_loss the loss time is the root of s(tau) = s_loss on the continuous extension, which in the
+    E x B drift field has a closed form; the reported state sits on the boundary; survivors and the rest of the
+    trace are untouched."""
+    A, om = -8.0e3, TWO_PI * 1e3
+    fld = _exb_drift_field(A, om)
+    F = oracle.OracleField(fld)
+    s0 = np.array([0.9, 0.9, 0.5])
+    th0 = np.array([0.1, 0.1, 0.1])
+    ze0 = np.array([0.2, -0.3, 0.2])
+    v0 = np.array([0.7, -0.6, 0.7]) * VREF
+    mu = 0.5 * M * (VREF ** 2 - v0 ** 2) / 5.7
+    spec = W.make_spec(0)
+    spec.t_max = 1e-4
+    a = F.trace(spec, s0, th0, ze0, v0, mu)
+    r = F.trace(spec, s0, th0, ze0, v0, mu, refine_loss=True)
+    phi0 = 2 * th0 - ze0
+    assert list(r.status) == [1, 1, 0]
+    assert np.array_equal(r.n_acc, a.n_acc) and np.array_equal(r.n_rej, a.n_rej)
+    assert np.array_equal(r.y[:, 2], a.y[:, 2]) and r.t[2] == a.t[2]
+    for i in (0, 1):
+        t_star = (math.asin(math.sin(phi0[i]) - om * fld.psi0 * (1.0 - s0[i]) / (2 * A)) - phi0[i]) / om
+        assert abs(r.t[i] - t_star) < 2e-7 * t_star              # accuracy of the 4th-order extension, not the step size
+        assert abs(a.t[i] - t_star) > 1e-6 * t_star              # the unrefined time is a step end
+        assert r.t[i] <= a.t[i] and abs(r.y[0, i] - 1.0) < 1e-13
+        assert np.isclose(r.y[2, i], ze0[i] + v0[i] * 5.7 * r.t[i] / 57.0, rtol=1e-9)
+        assert np.isclose(r.y[3, i], v0[i], rtol=1e-12)

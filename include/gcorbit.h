@@ -76,8 +76,11 @@ typedef struct {
  * each continuing where the last one stopped (checkpoint / resume).
  * GC_TRACE_SECTION_VPAR (NEXT-1, O8b; "trapped particle Poincare map"): the Poincare records are taken
  * where v_par changes sign (the bounce points, both directions) instead of at zeta = 0 mod 2 pi; same record
- * format; small ensembles are then traced by the generic kernel. */
-enum { GC_TRACE_RESUME = 1, GC_TRACE_SECTION_VPAR = 2 };
+ * format; small ensembles are then traced by the generic kernel.
+ * GC_TRACE_REFINE_LOSS (O7b, the alternative reading of A8): a lost particle reports the point where the continuous
+ * extension of its last step crosses s_loss (t_out, y_out; |s - s_loss| < 1e-13) instead of the end of that step;
+ * step counts, samples and Poincare records are unchanged; small ensembles go to the generic kernel. */
+enum { GC_TRACE_RESUME = 1, GC_TRACE_SECTION_VPAR = 2, GC_TRACE_REFINE_LOSS = 4 };
 
 /* Per-particle exit status written by gc_trace. */
 enum { GC_ST_TMAX = 0, GC_ST_LOST = 1, GC_ST_AXIS = 2, GC_ST_MAXSTEPS = 3, GC_ST_NONFINITE = 4 };

@@ -44,6 +44,7 @@ struct TraceDev {
   long long n;
   int resume;                         // GC_TRACE_RESUME: skip particles whose status is not 0 on entry
   int section;                        // Poincare records: 0 zeta = 0 mod 2 pi (O8), 1 v_par = 0 (O8b)
+  int refine_loss;                    // O7b: lost particles report the root of s(tau) = s_loss of their last step
   const double *s0, *th0, *ze0, *vpar0, *mu;
   double* h_inout;
   double *y_out, *t_out;

@@ -370,7 +370,7 @@ int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, c
   sc.tile_size = per_tile;
   gc::FieldDev fd = f->dev;
   void* args[] = {(void*)&fd, (void*)&t, (void*)&sc, (void*)&mode, (void*)&rhs_out};
-  const bool sample = mode == 0 && (t.nsamp > 0 || t.section != 0);   // the diagnostics build of the kernel
+  const bool sample = mode == 0 && (t.nsamp > 0 || t.section != 0 || t.refine_loss != 0);   // the diagnostics build of the kernel
   if (mma)
     GC_CUDA(cudaLaunchCooperativeKernel(mma_fn(f, sample), dim3((unsigned)blocks), dim3(gc::kMmaThreads), args,
                                         (size_t)f->mma_smem, st));
@@ -386,7 +386,7 @@ int build_trace_dev(const gc_field* f, const gc_trace_params* p, int64_t n, gc::
   if (n < 0) return fail(GC_EINVAL, "gc_trace: n < 0");
   if (!(p->v_ref > 0.0) || !(p->h0 > 0.0) || !(p->h_min >= 0.0) || !(p->mass > 0.0) || p->charge == 0.0 ||
       !(p->rtol >= 0.0) || !(p->atol >= 0.0) || !(p->rtol + p->atol > 0.0) || p->max_steps < 1 ||
-      p->poincare_capacity < 0 || (p->flags & ~(int64_t)(GC_TRACE_RESUME | GC_TRACE_SECTION_VPAR)) != 0 || !std::isfinite(p->t0) || !std::isfinite(p->t_max))
+      p->poincare_capacity < 0 || (p->flags & ~(int64_t)(GC_TRACE_RESUME | GC_TRACE_SECTION_VPAR | GC_TRACE_REFINE_LOSS)) != 0 || !std::isfinite(p->t0) || !std::isfinite(p->t_max))
     return fail(GC_EINVAL, "gc_trace: invalid integrator specification");
   t->mass = p->mass; t->charge = p->charge; t->t0 = p->t0; t->t_max = p->t_max;
   t->rtol = p->rtol; t->atol = p->atol; t->v_ref = p->v_ref; t->inv_v_ref = 1.0 / p->v_ref;
@@ -394,6 +394,7 @@ int build_trace_dev(const gc_field* f, const gc_trace_params* p, int64_t n, gc::
   t->max_steps = p->max_steps; t->poincare_capacity = p->poincare_capacity; t->n = n;
   t->resume = (p->flags & GC_TRACE_RESUME) ? 1 : 0;
   t->section = (p->flags & GC_TRACE_SECTION_VPAR) ? 1 : 0;
+  t->refine_loss = (p->flags & GC_TRACE_REFINE_LOSS) ? 1 : 0;
   return GC_OK;
 }
 
@@ -648,7 +649,7 @@ int trace_common(const gc_field* f, const gc_trace_params* params, int64_t n, co
   if (poincare_count) GC_CUDA(cudaMemsetAsync(poincare_count, 0, sizeof(int64_t), st));
   t.sample_t0 = sample_t0; t.sample_dt = sample_dt; t.nsamp = nsamp; t.samples = samples; t.sample_end = sample_end;
   int kern = resolve_kernel(f, n);
-  if (kern == GC_KERNEL_WARP && (nsamp > 0 || t.section != 0))
+  if (kern == GC_KERNEL_WARP && (nsamp > 0 || t.section != 0 || t.refine_loss != 0))
     kern = GC_KERNEL_GENERIC;                       // the warp kernel has neither samples nor the bounce section
   if (kern == GC_KERNEL_TILE || kern == GC_KERNEL_MMA) return launch_tile(f, t, 0, nullptr, st, kern == GC_KERNEL_MMA);
   if (kern == GC_KERNEL_WARP) {

@@ -236,6 +236,23 @@ __device__ inline void bounce_emit(const double (&y)[4], const double (&yn)[4], 
   }
 }
 
+// O7b: root of s(tau) = s_loss on the continuous extension of component 0 (s < s_loss at tau = 0, >= at tau = 1).
+__device__ inline double loss_root(double y0, double yn0, double hk1, double hk7, double hd, double s_loss) {
+  double lo = 0.0, hi = 1.0;
+  for (int it = 0; it < 8; ++it) {
+    const double mid = 0.5 * (lo + hi);
+    if (dense_component(y0, yn0, hk1, hk7, hd, mid) < s_loss) lo = mid; else hi = mid;
+  }
+  double tau = 0.5 * (lo + hi);
+  for (int it = 0; it < 20; ++it) {
+    const double g = dense_component(y0, yn0, hk1, hk7, hd, tau) - s_loss;
+    const double dv = dense_component_slope(y0, yn0, hk1, hk7, hd, tau);
+    if (fabs(g) < 1e-14 || dv == 0.0) break;
+    tau = fmin(fmax(tau - g / dv, lo), hi);
+  }
+  return tau;
+}
+
 // ---- generic trace: one thread per particle ----------------------------------------------------------------
 __global__ void __launch_bounds__(128) trace_generic_kernel(FieldDev f, TraceDev p) {
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < p.n;
@@ -360,7 +377,20 @@ __global__ void __launch_bounds__(128) trace_generic_kernel(FieldDev f, TraceDev
             ++jn;
           }
         }
-        t = t_new;
+        const bool lost_now = yn[0] >= p.s_loss;
+        double t_rep = t_new;
+        if (lost_now && p.refine_loss && y[0] < p.s_loss) {            // O7b
+          double hd[4];
+#pragma unroll
+          for (int c = 0; c < 4; ++c)
+            hd[c] = h_try * fma(dp::d7, k[6][c], fma(dp::d6, k[5][c], fma(dp::d5, k[4][c],
+                              fma(dp::d4, k[3][c], fma(dp::d3, k[2][c], dp::d1 * k[0][c])))));
+          const double tau = loss_root(y[0], yn[0], h_try * k[0][0], h_try * k[6][0], hd[0], p.s_loss);
+#pragma unroll
+          for (int c = 0; c < 4; ++c) yn[c] = dense_component(y[c], yn[c], h_try * k[0][c], h_try * k[6][c], hd[c], tau);
+          t_rep = fma(tau, h_try, t);
+        }
+        t = lost_now ? t_rep : t_new;
 #pragma unroll
         for (int c = 0; c < 4; ++c) { y[c] = yn[c]; k[0][c] = k[6][c]; }
         ++n_acc;
@@ -368,7 +398,7 @@ __global__ void __launch_bounds__(128) trace_generic_kernel(FieldDev f, TraceDev
         prev_rejected = false;
         if (!clipped) h = h_next;
         if (h < p.h_min) h = p.h_min;
-        if (y[0] >= p.s_loss) st = 1;
+        if (lost_now) st = 1;
         else if (y[0] <= p.s_min) st = 2;
         else if (clipped) st = 0;
         else if (attempts >= p.max_steps) st = 3;

@@ -599,7 +599,27 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
                   }
                 }
               }
-              t = t_new;
+              const bool lost_now = yn[0] >= p.s_loss;
+              if constexpr (SAMPLE) {                                     // O7b lives in the diagnostics build only
+                if (lost_now && p.refine_loss && y[0] < p.s_loss) {
+                  double hd[4];
+#pragma unroll
+                  for (int c = 0; c < 4; ++c) {
+                    double dd = 0.0;
+                    for (int j = 0; j < 7; ++j) dd = fma(cDpD[j], kb(j, c), dd);
+                    hd[c] = h_try * dd;
+                  }
+                  const double tau = loss_root(y[0], yn[0], h_try * kb(0, 0), h_try * kb(6, 0), hd[0], p.s_loss);
+#pragma unroll
+                  for (int c = 0; c < 4; ++c)
+                    yn[c] = dense_component(y[c], yn[c], h_try * kb(0, c), h_try * kb(6, c), hd[c], tau);
+                  t = fma(tau, h_try, t);
+                } else {
+                  t = t_new;
+                }
+              } else {
+                t = t_new;
+              }
 #pragma unroll
               for (int c = 0; c < 4; ++c) { y[c] = yn[c]; kb(0, c) = kb(6, c); }
               ++n_acc;
@@ -607,7 +627,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
               flags &= ~kFlagPrevRejected;
               if (!clipped) h = h_next;
               if (h < p.h_min) h = p.h_min;
-              if (y[0] >= p.s_loss) st = 1;
+              if (lost_now) st = 1;
               else if (y[0] <= p.s_min) st = 2;
               else if (clipped) st = 0;
               else if (attempts >= p.max_steps) st = 3;

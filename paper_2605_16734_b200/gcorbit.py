@@ -107,6 +107,7 @@ def _stream_ptr(torch):
 
 GC_TRACE_RESUME = 1
 GC_TRACE_SECTION_VPAR = 2
+GC_TRACE_REFINE_LOSS = 4
 
 
 def make_params(spec, t0=None, t_max=None, poincare_capacity=0, flags=0) -> gc_trace_params:

@@ -274,3 +274,40 @@ def test_binned_kernels_are_bitwise_reproducible_and_independent_of_the_company(
         assert torch.equal(x.y, y.y) and torch.equal(x.t, y.t) and torch.equal(x.status, y.status)
         assert torch.equal(x.n_acc, y.n_acc) and torch.equal(x.n_rej, y.n_rej)
     assert torch.equal(a.y[:, :5000], c.y) and torch.equal(a.t[:5000], c.t) and torch.equal(a.n_acc[:5000], c.n_acc)
+
+
+@pytest.mark.parametrize("kernel", ["generic", "warp", "tile", "mma"])
+def test_refined_loss_point_matches_oracle(kernel):
+    """GC_TRACE_REFINE_LOSS (O7b): lost particles report the crossing of s_loss on the continuous extension; the
+    warp kernel hands the call to the generic one.  Everything else equals the unrefined trace."""
+    import dataclasses
+    import torch
+    from paper_2605_16734_b200 import gcorbit as G
+    fld, spec, P, OF, GF, mu = make_case(0, 96)
+    spec = dataclasses.replace(spec, s_loss=0.262)
+    GF.set_kernel({"generic": G.GC_KERNEL_GENERIC, "warp": G.GC_KERNEL_WARP, "tile": G.GC_KERNEL_TILE,
+                   "mma": G.GC_KERNEL_MMA}[kernel])
+    a = [to_dev(x) for x in (P.s, P.theta, P.zeta, P.vpar, mu)]
+    r = GF.trace(spec, *a, t_max=3e-5, flags=G.GC_TRACE_REFINE_LOSS)
+    u = GF.trace(spec, *a, t_max=3e-5)
+    torch.cuda.synchronize()
+    o = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=3e-5, refine_loss=True)
+    st = r.status.cpu().numpy()
+    assert np.array_equal(st, o.status) and 10 < (st == 1).sum() < 90
+    same = (r.n_acc.cpu().numpy() == o.n_acc) & (r.n_rej.cpu().numpy() == o.n_rej)
+    assert same.mean() >= 0.97
+    lost = (st == 1) & same
+    y, t = r.y.cpu().numpy(), r.t.cpu().numpy()
+    assert np.abs(y[0, lost] - spec.s_loss).max() < 1e-12
+    assert np.abs(t[lost] - o.t[lost]).max() <= 1e-9 * 3e-5
+    floor = np.array([[1.0], [1.0], [1.0], [spec.v_ref]])
+    assert (np.abs(y[:, lost] - o.y[:, lost]) / np.maximum(np.abs(o.y[:, lost]), floor)).max() < 1e-9
+    # refined times precede the step ends of the unrefined trace by less than a step; survivors are identical
+    tu = u.t.cpu().numpy()
+    assert np.all(t[lost] <= tu[lost]) and np.all(tu[lost] - t[lost] < 2e-7)
+    surv = torch.as_tensor(st == 0)
+    if kernel == "warp":                                   # the refined call ran in the generic kernel: rounding differs
+        d = (r.y[:, surv] - u.y[:, surv]).abs() / torch.maximum(u.y[:, surv].abs(), to_dev(floor))
+        assert float(d.max()) < 1e-9
+    else:
+        assert torch.equal(r.y[:, surv], u.y[:, surv]) and torch.equal(r.n_acc, u.n_acc)

@@ -257,8 +257,10 @@ int pack_tile_images(gc_field* f, const gc_field_desc* d) {
   const void* fn = tile_fn(f);
   GC_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   GC_CUDA(cudaFuncSetAttribute(tile_fn(f, true), cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  int per_sm = 0;
+  int per_sm = 0, per_sm_diag = 0;
   GC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, gc::kTileThreads, (size_t)smem));
+  GC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_diag, tile_fn(f, true), gc::kTileThreads, (size_t)smem));
+  if (per_sm_diag < per_sm) per_sm = per_sm_diag;
   if (per_sm < 1) return GC_OK;
   int coop = 0, devid = 0;
   GC_CUDA(cudaGetDevice(&devid));
@@ -315,8 +317,10 @@ int pack_mma_image(gc_field* f, const gc_field_desc* d) {
   const void* fn = mma_fn(f);
   GC_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   GC_CUDA(cudaFuncSetAttribute(mma_fn(f, true), cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  int per_sm = 0;
+  int per_sm = 0, per_sm_diag = 0;                         // the plain and the diagnostics build share one grid size
   GC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, gc::kMmaThreads, (size_t)smem));
+  GC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_diag, mma_fn(f, true), gc::kMmaThreads, (size_t)smem));
+  if (per_sm_diag < per_sm) per_sm = per_sm_diag;
   if (per_sm < 1) return GC_OK;
   int coop = 0, devid = 0;
   GC_CUDA(cudaGetDevice(&devid));

@@ -22,6 +22,10 @@ def runs():
     fld, spec, P, OF, GF, mu = make_case(1, N_ORACLE)
     o = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=T_MAX)
     g = gpu_trace(GF, spec, P, mu, t_max=T_MAX)
+    from paper_2605_16734_b200 import gcorbit as G
+    GF.set_kernel(G.GC_KERNEL_MMA)                          # the same ensemble through the large-ensemble kernel
+    g_mma = gpu_trace(GF, spec, P, mu, t_max=T_MAX)
+    GF.set_kernel(G.GC_KERNEL_AUTO)
     # an independent, larger GPU ensemble of the same recipe (different random stream)
     P2 = W.make_particles(1, 16384, stream=5)
     s, th, ze = to_dev(P2.s), to_dev(P2.theta), to_dev(P2.zeta)
@@ -29,7 +33,7 @@ def runs():
     mu2 = to_dev(0.5 * spec.mass * P2.vperp2()) / B
     g2 = GF.trace(spec, s, th, ze, to_dev(P2.vpar), mu2, t_max=T_MAX)
     torch.cuda.synchronize()
-    return spec, o, g, g2
+    return spec, o, g, g2, g_mma
 
 
 def _loss(status, t):
@@ -39,7 +43,7 @@ def _loss(status, t):
 
 def test_same_ensemble_loss_fraction_and_ks(runs):
     from scipy.stats import ks_2samp
-    spec, o, g, g2 = runs
+    spec, o, g, g2, g_mma = runs
     f_o, t_o = _loss(o.status, o.t)
     f_g, t_g = _loss(g.status.cpu().numpy(), g.t.cpu().numpy())
     assert len(t_o) >= 20, "horizon too short for a loss statistic"
@@ -48,12 +52,14 @@ def test_same_ensemble_loss_fraction_and_ks(runs):
     assert ks_2samp(t_g, t_o).pvalue > 0.01
     # no particle may end in a state the config cannot produce
     assert set(np.unique(g.status.cpu().numpy())) <= {0, 1, 2}
-    print(f"loss fraction oracle {f_o:.4f} gpu {f_g:.4f}; {len(t_o)} loss events")
+    f_m, t_m = _loss(g_mma.status.cpu().numpy(), g_mma.t.cpu().numpy())
+    assert abs(f_m - f_o) <= se and ks_2samp(t_m, t_o).pvalue > 0.01
+    print(f"loss fraction oracle {f_o:.4f} gpu {f_g:.4f} (warp) {f_m:.4f} (mma); {len(t_o)} loss events")
 
 
 def test_independent_ensemble_loss_fraction_and_ks(runs):
     from scipy.stats import ks_2samp
-    spec, o, g, g2 = runs
+    spec, o, g, g2, g_mma = runs
     f_o, t_o = _loss(o.status, o.t)
     st2, t2 = g2.status.cpu().numpy(), g2.t.cpu().numpy()
     f_2, t_2 = _loss(st2, t2)

@@ -315,3 +315,39 @@ def test_birkhoff_digits_of_pzeta_turn_chaotic_with_the_mode_amplitude():
     assert frac_chaotic[0.0] == 0.0 and med[0.0] > 6.0
     assert frac_chaotic[0.0] <= frac_chaotic[1e3] < frac_chaotic[1e5] and frac_chaotic[1e5] > 0.3
     assert med[1e5] < 4.0 < med[1e3]
+
+
+def test_pzeta_error_versus_tolerance_and_nodes_protocol_of_the_paper():
+    """The protocol of the paper's Fig. 1 right (10 particles, 1e-4 s, maximum relative P_zeta error
+    over trajectory and particles, symmetrised field, swept over the Dormand-Prince tolerance and the number of
+    radial nodes; the paper quotes ~1e-8 at tolerance 1e-9 and 64 nodes for ITS equilibrium: context, not a pass
+    value) run on the device chain gc_trace_sampled -> gc_pzeta_eval on the synthetic symmetric field: the error
+    falls by about two decades per two decades of tolerance and is of the paper's order at 1e-9."""
+    import dataclasses
+    import torch
+    from paper_2605_16734_b200 import gcorbit as G, workloads as W
+    P = W.make_particles(0, 10)
+    err = {}
+    for ns in (32, 64, 96):
+        for rtol in (1e-7, 1e-9, 1e-11):
+            fld = W.make_equilibrium(8, 8, ns)
+            keep = fld.xn == 0
+            fld.xm, fld.xn, fld.bmnc = fld.xm[keep], fld.xn[keep], np.ascontiguousarray(fld.bmnc[:, keep])
+            spec = dataclasses.replace(W.make_spec(0), rtol=rtol, atol=rtol)
+            GF = G.Field(fld)
+            s, th, ze, vp = (to_dev(x) for x in (P.s, P.theta, P.zeta, P.vpar))
+            B, _ = GF.field_eval(s, th, ze, derivs=False)
+            mu = to_dev(0.5 * spec.mass * P.vperp2()) / B
+            nsamp, dt = 201, 5e-7
+            r = GF.trace_sampled(spec, s, th, ze, vp, mu, 0.0, dt, nsamp, t_max=1e-4)
+            s_n = np.arange(ns) / (ns - 1)
+            chi = to_dev(fld.psi0 * (0.42 * s_n + 0.05 * s_n ** 2))
+            pz = GF.pzeta_eval(spec.mass, spec.charge, r.samples.reshape(4, -1), None, chi).reshape(nsamp, P.n)
+            torch.cuda.synchronize()
+            assert bool((r.sample_end == nsamp).all())
+            pz = pz.cpu().numpy()
+            err[(ns, rtol)] = float(np.abs(pz / pz[0] - 1.0).max())
+    print({k: f"{v:.2e}" for k, v in err.items()})
+    for ns in (32, 64, 96):
+        assert err[(ns, 1e-9)] < 1e-6 and err[(ns, 1e-11)] < 5e-8
+        assert err[(ns, 1e-9)] < 0.05 * err[(ns, 1e-7)] and err[(ns, 1e-11)] < 0.3 * err[(ns, 1e-9)]

@@ -101,8 +101,10 @@ enum { GC_ST_TMAX = 0, GC_ST_LOST = 1, GC_ST_AXIS = 2, GC_ST_MAXSTEPS = 3, GC_ST
 enum { GC_KERNEL_AUTO = 0, GC_KERNEL_GENERIC = 1, GC_KERNEL_WARP = 2, GC_KERNEL_TILE = 3, GC_KERNEL_MMA = 4 };
 enum { GC_TILE_MIN_PARTICLES = 4096 };
 
-/* Copies the tables to the device, checks them (finite values, xm >= 0, omega != 0) and builds the
- * packed by-node layout of the warp kernel.  *out is NULL on failure. */
+/* Copies the tables to the device, checks them (finite values, xm >= 0, omega != 0) and builds the packed layouts of
+ * every trace kernel the field fits: the by-node lane rows of the warp kernel, the per-cell window images of the
+ * tile kernel and the by-node DMMA-fragment image of the mma kernel.  *out is NULL on
+ * failure. */
 int gc_field_create(const gc_field_desc* desc, gc_field** out);
 int gc_field_destroy(gc_field* f);
 
@@ -140,12 +142,14 @@ int gc_trace(const gc_field* f, const gc_trace_params* params, int64_t n,
              int32_t* n_acc, int32_t* n_rej, int32_t* n_forced,
              double* poincare, int64_t* poincare_count, void* stream);
 
-/* The same trace with HOST buffers: uses a device workspace and a stream kept in the field (grown on demand, freed
- * by gc_field_destroy; calls on one field must not overlap), copies the inputs in (with GC_TRACE_RESUME
- * also y_out, t_out, status and the counters, so that untouched particles keep their values), runs
- * gc_trace, copies every non-NULL output back and synchronises.  `poincare_count` is a host int64 here.
- * Pinned host buffers make the copies asynchronous; pageable ones work too. */
-int gc_trace_host(const gc_field* f, const gc_trace_params* params, int64_t n,
+/* The same trace with HOST buffers.  MUTATES THE FIELD: a device workspace and a stream are created in it on the
+ * first call, grown on demand and freed by gc_field_destroy, so the field is not const here and the call is not
+ * re-entrant on one field: a call that overlaps another gc_trace_host call on the same field returns GC_EINVAL
+ * (different fields may run concurrently).  Copies the inputs in (with GC_TRACE_RESUME also y_out, t_out, status
+ * and the counters, so that untouched particles keep their values), runs gc_trace, copies every non-NULL output
+ * back and synchronises.  `poincare_count` is a host int64 here.  Pinned host buffers make the copies
+ * asynchronous; pageable ones work too. */
+int gc_trace_host(gc_field* f, const gc_trace_params* params, int64_t n,
                   const double* s0, const double* th0, const double* ze0, const double* vpar0,
                   const double* mu, double* h_inout,
                   double* y_out, double* t_out, int32_t* status,
@@ -196,17 +200,6 @@ int gc_set_kernel(gc_field* f, int32_t kernel);
  * its launch geometry; any pointer may be NULL. */
 int gc_kernel_info(const gc_field* f, int64_t n, int32_t* kernel, int32_t* blocks, int32_t* threads_per_block,
                    int32_t* smem_bytes, int32_t* regs_per_thread);
-
-/* Register-only DFMA loop on every SM: measures the FP64 pipe's sustained rate that the roofline of
- * DESIGN.md section 6 is quoted against.  Writes achieved FLOP/s (2 per DFMA) to *flops_per_s (host).
- * Synchronous. */
-int gc_fp64_peak_probe(double* flops_per_s, double* elapsed_ms);
-
-/* The same for the FP64 matrix instruction the mma kernel is built on: DMMA.8x8x4 (mma.sync.m8n8k4.f64) with 8
- * independent accumulators per warp, alone (*flops_dmma) and with one DFMA per DMMA mixed in (*flops_mixed, counting
- * both): the two instruction kinds share the FP64 units, so there is one FP64 roofline.
- * Synchronous. */
-int gc_dmma_peak_probe(double* flops_dmma, double* flops_mixed);
 
 /* Thread-local text of the last nonzero return ("" if none). */
 const char* gc_last_error(void);

@@ -4,6 +4,7 @@
 
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -65,6 +66,7 @@ struct gc_field {
   cudaStream_t host_stream = nullptr;
   void* host_slab = nullptr;
   size_t host_slab_bytes = 0;
+  std::atomic<bool> host_busy{false};   // gc_trace_host is not re-entrant on one field: overlapping calls get GC_EINVAL
   bool mma_ok = false;
   int mma_smem = 0;                 // dynamic shared memory of the mma kernel
   int mma_blocks_per_sm = 0;
@@ -118,6 +120,11 @@ int ensure_smem(const void* fn, int bytes) {
   GC_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   return GC_OK;
 }
+
+// Dynamic shared memory the binned kernels may ask for: two blocks per SM must fit.  The attribute belongs to the
+// kernel FUNCTION, not to a field (two live fields can share an instantiation with different window sizes), so every
+// instantiation is raised to this one cap and never lowered.
+constexpr int kBinnedSmemCap = 110 * 1024;
 
 // Packed rows[node][it][lane] of the warp kernel (kernels_warp.cuh header comment).
 int pack_rows(gc_field* f, const gc_field_desc* d) {
@@ -214,7 +221,7 @@ int pack_tile_images(gc_field* f, const gc_field_desc* d) {
   const int rowlen = 1 + 2 * nmax;
   const int E = (v.M + 1) * rowlen + 3 + d->nk;
   const int smem = (int)((size_t)10 * E * sizeof(double) + (size_t)7 * 4 * gc::kTileThreads * sizeof(double) + 64);
-  if (smem > 110 * 1024) return GC_OK;                     // two blocks per SM must fit
+  if (smem > kBinnedSmemCap) return GC_OK;                 // two blocks per SM must fit
   const int ncell = d->ns - 3;
   if ((size_t)(gc::kSubBins + 2) * ncell * sizeof(int) > (size_t)10 * E * sizeof(double)) return GC_OK;   // scan space (phase B)
   // node-major entry rows first
@@ -255,8 +262,8 @@ int pack_tile_images(gc_field* f, const gc_field_desc* d) {
   v.tile_nmax = nmax;
   f->tile_smem = smem;
   const void* fn = tile_fn(f);
-  GC_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  GC_CUDA(cudaFuncSetAttribute(tile_fn(f, true), cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  GC_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, kBinnedSmemCap));
+  GC_CUDA(cudaFuncSetAttribute(tile_fn(f, true), cudaFuncAttributeMaxDynamicSharedMemorySize, kBinnedSmemCap));
   int per_sm = 0, per_sm_diag = 0;
   GC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, gc::kTileThreads, (size_t)smem));
   GC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_diag, tile_fn(f, true), gc::kTileThreads, (size_t)smem));
@@ -302,7 +309,7 @@ int pack_mma_image(gc_field* f, const gc_field_desc* d) {
   const int MT = small ? 1 : 2, KS = small ? 2 : 4;
   const int RS = small ? gc::MmaRow<1, 2>::stride(d->nk) : gc::MmaRow<2, 4>::stride(d->nk);
   const int smem = (int)((size_t)gc::kMmaWinRows * RS * sizeof(double) + (size_t)(7 * 4 + 2 * gc::kMmaWtab) * gc::kMmaThreads * sizeof(double) + 64);
-  if (smem > 110 * 1024) return GC_OK;
+  if (smem > kBinnedSmemCap) return GC_OK;
   const int ncell = d->ns - 3;
   if ((size_t)(gc::kSubBins + 2) * ncell * sizeof(int) > (size_t)gc::kMmaWinRows * RS * sizeof(double)) return GC_OK;
   std::vector<double> img((size_t)(d->ns + 4) * RS, 0.0);
@@ -315,8 +322,8 @@ int pack_mma_image(gc_field* f, const gc_field_desc* d) {
   v.mma_RS = RS; v.mma_MT = MT; v.mma_KS = KS;
   f->mma_smem = smem;
   const void* fn = mma_fn(f);
-  GC_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  GC_CUDA(cudaFuncSetAttribute(mma_fn(f, true), cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  GC_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, kBinnedSmemCap));
+  GC_CUDA(cudaFuncSetAttribute(mma_fn(f, true), cudaFuncAttributeMaxDynamicSharedMemorySize, kBinnedSmemCap));
   int per_sm = 0, per_sm_diag = 0;                         // the plain and the diagnostics build share one grid size
   GC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, gc::kMmaThreads, (size_t)smem));
   GC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_diag, mma_fn(f, true), gc::kMmaThreads, (size_t)smem));
@@ -375,13 +382,14 @@ int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, c
   gc::FieldDev fd = f->dev;
   void* args[] = {(void*)&fd, (void*)&t, (void*)&sc, (void*)&mode, (void*)&rhs_out};
   const bool sample = mode == 0 && (t.nsamp > 0 || t.section != 0 || t.refine_loss != 0);   // the diagnostics build of the kernel
-  if (mma)
-    GC_CUDA(cudaLaunchCooperativeKernel(mma_fn(f, sample), dim3((unsigned)blocks), dim3(gc::kMmaThreads), args,
-                                        (size_t)f->mma_smem, st));
-  else
-    GC_CUDA(cudaLaunchCooperativeKernel(tile_fn(f, sample), dim3((unsigned)blocks), dim3(gc::kTileThreads), args,
-                                        (size_t)f->tile_smem, st));
-  GC_CUDA(cudaFreeAsync(slab, st));
+  const cudaError_t le =
+      mma ? cudaLaunchCooperativeKernel(mma_fn(f, sample), dim3((unsigned)blocks), dim3(gc::kMmaThreads), args,
+                                        (size_t)f->mma_smem, st)
+          : cudaLaunchCooperativeKernel(tile_fn(f, sample), dim3((unsigned)blocks), dim3(gc::kTileThreads), args,
+                                        (size_t)f->tile_smem, st);
+  const cudaError_t fe = cudaFreeAsync(slab, st);           // also on a failed launch: the scratch must not leak
+  GC_CUDA(le);
+  GC_CUDA(fe);
   return GC_OK;
 }
 
@@ -400,36 +408,6 @@ int build_trace_dev(const gc_field* f, const gc_trace_params* p, int64_t n, gc::
   t->section = (p->flags & GC_TRACE_SECTION_VPAR) ? 1 : 0;
   t->refine_loss = (p->flags & GC_TRACE_REFINE_LOSS) ? 1 : 0;
   return GC_OK;
-}
-
-__global__ void dfma_probe_kernel(double* out, int iters) {
-  double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6,
-         a7 = a0 + 7;
-  const double x = 0.999999999, y = 1e-12;
-  for (int i = 0; i < iters; ++i) {
-    a0 = fma(a0, x, y); a1 = fma(a1, x, y); a2 = fma(a2, x, y); a3 = fma(a3, x, y);
-    a4 = fma(a4, x, y); a5 = fma(a5, x, y); a6 = fma(a6, x, y); a7 = fma(a7, x, y);
-  }
-  if (a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7 == 12345.678) out[0] = a0;
-}
-
-// 8 independent DMMA.8x8x4 accumulators per warp; MIX > 0 adds MIX DFMA per 8 DMMA (the two share the FP64 units).
-template <int MIX>
-__global__ void dmma_probe_kernel(double* out, int iters) {
-  double acc[16], f[8];
-  for (int i = 0; i < 16; ++i) acc[i] = threadIdx.x * 1e-9 + i;
-  for (int i = 0; i < 8; ++i) f[i] = i + 1.0;
-  const double a = 0.999 + threadIdx.x * 1e-6, b = 1e-3;
-  for (int it = 0; it < iters; ++it) {
-#pragma unroll
-    for (int j = 0; j < 8; ++j) gc::dmma884(acc[2 * j], acc[2 * j + 1], a, b);
-#pragma unroll
-    for (int j = 0; j < MIX; ++j) f[j & 7] = fma(f[j & 7], a, b);
-  }
-  double s = 0.0;
-  for (int i = 0; i < 16; ++i) s += acc[i];
-  for (int i = 0; i < 8; ++i) s += f[i];
-  if (s == 12345.678) out[0] = s;
 }
 
 }  // namespace
@@ -665,9 +643,11 @@ int trace_common(const gc_field* f, const gc_trace_params* params, int64_t n, co
     void* args[] = {(void*)&f->dev, (void*)&t};
     long long blocks = (n + gc::kWarpsPerBlock - 1) / gc::kWarpsPerBlock;
     if (blocks > f->sm_count) blocks = f->sm_count;
-    GC_CUDA(cudaLaunchKernel(w->trace_fn, dim3((unsigned)blocks), dim3(gc::kWarpsPerBlock * 32), args,
-                             (size_t)w->smem_bytes, st));
-    GC_CUDA(cudaFreeAsync(counter, st));
+    const cudaError_t le = cudaLaunchKernel(w->trace_fn, dim3((unsigned)blocks), dim3(gc::kWarpsPerBlock * 32), args,
+                                            (size_t)w->smem_bytes, st);
+    const cudaError_t fe = cudaFreeAsync(counter, st);      // also on a failed launch
+    GC_CUDA(le);
+    GC_CUDA(fe);
   } else {
     long long blocks = (n + 127) / 128;
     if (blocks > (long long)f->sm_count * 16) blocks = (long long)f->sm_count * 16;
@@ -723,7 +703,7 @@ int gc_birkhoff(int64_t n, int64_t nsamp, const double* series, int64_t j_first,
   return GC_OK;
 }
 
-int gc_trace_host(const gc_field* f, const gc_trace_params* params, int64_t n, const double* s0,
+int gc_trace_host(gc_field* f, const gc_trace_params* params, int64_t n, const double* s0,
                   const double* th0, const double* ze0, const double* vpar0, const double* mu, double* h_inout,
                   double* y_out, double* t_out, int32_t* status, int32_t* n_acc, int32_t* n_rej,
                   int32_t* n_forced, double* poincare, int64_t* poincare_count) {
@@ -747,8 +727,10 @@ int gc_trace_host(const gc_field* f, const gc_trace_params* params, int64_t n, c
       return rc;                                                                   \
     }                                                                              \
   } while (0)
-  // stream and device slab live in the field and are reused by later calls (calls on one field must not overlap)
-  gc_field* fm = const_cast<gc_field*>(f);
+  // stream and device slab live in the field and are reused by later calls; calls on one field must not overlap
+  gc_field* fm = f;
+  if (fm->host_busy.exchange(true)) return fail(GC_EINVAL, "gc_trace_host: another gc_trace_host call is running on this field");
+  struct Release { gc_field* f; ~Release() { f->host_busy.store(false); } } release{fm};
   if (!fm->host_stream) GC_H(cudaStreamCreateWithFlags(&fm->host_stream, cudaStreamNonBlocking));
   const size_t dbl_bytes = ((n_dbl * sizeof(double) + 255) / 256) * 256;
   const size_t need = dbl_bytes + nd * 4 * sizeof(int32_t);
@@ -800,69 +782,6 @@ int gc_trace_host(const gc_field* f, const gc_trace_params* params, int64_t n, c
   GC_H(cudaStreamSynchronize(st));
 #undef GC_H
   cleanup();
-  return GC_OK;
-}
-
-int gc_fp64_peak_probe(double* flops_per_s, double* elapsed_ms) {
-  int devid = 0, sms = 0;
-  GC_CUDA(cudaGetDevice(&devid));
-  GC_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, devid));
-  double* out = nullptr;
-  GC_CUDA(cudaMalloc((void**)&out, sizeof(double)));
-  const int iters = 200000, blocks = sms * 2, threads = 512;
-  cudaEvent_t a, b;
-  GC_CUDA(cudaEventCreate(&a));
-  GC_CUDA(cudaEventCreate(&b));
-  dfma_probe_kernel<<<blocks, threads>>>(out, 1000);
-  GC_CUDA(cudaDeviceSynchronize());
-  float best = 1e30f;
-  for (int rep = 0; rep < 3; ++rep) {
-    GC_CUDA(cudaEventRecord(a));
-    dfma_probe_kernel<<<blocks, threads>>>(out, iters);
-    GC_CUDA(cudaEventRecord(b));
-    GC_CUDA(cudaEventSynchronize(b));
-    float ms = 0;
-    GC_CUDA(cudaEventElapsedTime(&ms, a, b));
-    best = ms < best ? ms : best;
-  }
-  cudaEventDestroy(a);
-  cudaEventDestroy(b);
-  cudaFree(out);
-  const double flops = 2.0 * 8.0 * (double)iters * (double)blocks * (double)threads;
-  if (flops_per_s) *flops_per_s = flops / (best * 1e-3);
-  if (elapsed_ms) *elapsed_ms = best;
-  return GC_OK;
-}
-
-int gc_dmma_peak_probe(double* flops_dmma, double* flops_mixed) {
-  int devid = 0, sms = 0;
-  GC_CUDA(cudaGetDevice(&devid));
-  GC_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, devid));
-  double* out = nullptr;
-  GC_CUDA(cudaMalloc((void**)&out, sizeof(double)));
-  const int iters = 40000, blocks = sms * 2, threads = 128;          // 2 warps per SM sub-partition
-  cudaEvent_t a, b;
-  GC_CUDA(cudaEventCreate(&a));
-  GC_CUDA(cudaEventCreate(&b));
-  float best[2] = {1e30f, 1e30f};
-  for (int which = 0; which < 2; ++which) {
-    for (int rep = 0; rep < 4; ++rep) {                                // first repetition warms up
-      GC_CUDA(cudaEventRecord(a));
-      if (which == 0) dmma_probe_kernel<0><<<blocks, threads>>>(out, iters);
-      else dmma_probe_kernel<8><<<blocks, threads>>>(out, iters);
-      GC_CUDA(cudaEventRecord(b));
-      GC_CUDA(cudaEventSynchronize(b));
-      float ms = 0;
-      GC_CUDA(cudaEventElapsedTime(&ms, a, b));
-      if (rep > 0 && ms < best[which]) best[which] = ms;
-    }
-  }
-  cudaEventDestroy(a);
-  cudaEventDestroy(b);
-  cudaFree(out);
-  const double warps = (double)blocks * threads / 32.0;
-  if (flops_dmma) *flops_dmma = 8.0 * 512.0 * iters * warps / (best[0] * 1e-3);
-  if (flops_mixed) *flops_mixed = (8.0 * 512.0 + 8.0 * 64.0) * iters * warps / (best[1] * 1e-3);
   return GC_OK;
 }
 

@@ -350,8 +350,6 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, 1) trace_warp_kernel(Fiel
     int n_acc = 0, n_rej = 0, n_forced = 0, st = -1;
     bool prev_rejected = false, clipped = false, forced = false;
     double k1 = 0.0, k2 = 0.0, k3 = 0.0, k4 = 0.0, k5 = 0.0, k6 = 0.0, k7 = 0.0, yn = y, h_try = h;
-    if (!(t < p.t_max)) st = 0;
-
     // One copy of the right-hand side in the instruction stream: the seven stages (and the initial k1
     // evaluation, stage 0) run through the same loop body; `stage` is warp-uniform.
     int stage = 0;
@@ -405,7 +403,8 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, 1) trace_warp_kernel(Fiel
         default: k7 = kv; break;
       }
       if (stage == 0) {
-        if (!__all_sync(kFull, isfinite(y) && isfinite(k1))) st = GC_ST_NONFINITE_;
+        if (!__all_sync(kFull, isfinite(y) && isfinite(k1))) st = GC_ST_NONFINITE_;   // O6: checked before the
+        else if (!(t < p.t_max)) st = 0;                                              // t0 >= t_max shortcut
         stage = 1;
         continue;
       }

@@ -21,8 +21,8 @@ GC_TILE_MIN_PARTICLES = 4096
 ST_TMAX, ST_LOST, ST_AXIS, ST_MAXSTEPS, ST_NONFINITE = 0, 1, 2, 3, 4
 
 EXPORTS = ["gc_field_create", "gc_field_destroy", "gc_field_eval", "gc_pert_eval", "gc_rhs_eval", "gc_trace",
-           "gc_trace_host", "gc_set_kernel", "gc_kernel_info", "gc_fp64_peak_probe", "gc_last_error",
-           "gc_trace_sampled", "gc_pzeta_eval", "gc_birkhoff", "gc_dmma_peak_probe"]
+           "gc_trace_host", "gc_set_kernel", "gc_kernel_info", "gc_last_error",
+           "gc_trace_sampled", "gc_pzeta_eval", "gc_birkhoff"]
 
 
 class GcError(RuntimeError):
@@ -72,8 +72,6 @@ def load_library():
         L.gc_birkhoff.argtypes = [i64, i64, vp, i64, vp, vp, vp]
         L.gc_set_kernel.argtypes = [vp, i32]
         L.gc_kernel_info.argtypes = [vp, C.c_int64] + [C.POINTER(i32)] * 5
-        L.gc_fp64_peak_probe.argtypes = [C.POINTER(dbl), C.POINTER(dbl)]
-        L.gc_dmma_peak_probe.argtypes = [C.POINTER(dbl), C.POINTER(dbl)]
         for name in EXPORTS:
             if name != "gc_last_error":
                 getattr(L, name).restype = C.c_int
@@ -312,19 +310,6 @@ def finish_poincare(res: TraceResult) -> TraceResult:
         res.poincare_count = int(cnt.item())
         res.poincare = res.poincare[:min(res.poincare_count, res.poincare.shape[0])]
     return res
-
-
-def dmma_peak_probe():
-    """(DMMA.8x8x4 alone, DMMA + DFMA mixed) in FLOP/s."""
-    a, b = C.c_double(0), C.c_double(0)
-    _check(load_library().gc_dmma_peak_probe(C.byref(a), C.byref(b)))
-    return a.value, b.value
-
-
-def fp64_peak_probe():
-    f, ms = C.c_double(0), C.c_double(0)
-    _check(load_library().gc_fp64_peak_probe(C.byref(f), C.byref(ms)))
-    return f.value, ms.value
 
 
 def birkhoff(series, j_first=0, sample_end=None):

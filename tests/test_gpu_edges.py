@@ -116,6 +116,30 @@ def test_minimum_step_forces_acceptance(case0):
         assert rel_diff(r.y.cpu().numpy()[:, same], o.y[:, same], sp.v_ref).max() < 1e-7
 
 
+def test_forced_only_after_a_rejection_and_step_underflow(case0):
+    """The three controller branches pinned on the oracle in tests/test_oracle_controller.py, on every kernel:
+    h0 = h_min far above the natural step gives reject / forced accept pairs (5 + 5 with t_max = 4.5 h_min), never a
+    forced first attempt; A23: t + h == t ends a particle with status 4 and zero attempts."""
+    fld, spec, P, OF, GF, mu = case0
+    Q = P.head(33)
+    sp = dataclasses.replace(spec, h_min=4e-7, h0=4e-7)
+    o = OF.trace(sp, Q.s, Q.theta, Q.zeta, Q.vpar, mu[:33], t_max=4.5 * 4e-7)
+    assert (o.n_acc == 5).all() and (o.n_rej == 5).all() and (o.n_forced == 5).all()
+    su = dataclasses.replace(spec, h_min=0.0, h0=1e-12, max_steps=1000)
+    for kern in _kernels():
+        GF.set_kernel(kern)
+        r = gpu_trace(GF, sp, Q, mu[:33], t_max=4.5 * 4e-7)
+        for a, b in ((r.n_acc, o.n_acc), (r.n_rej, o.n_rej), (r.n_forced, o.n_forced), (r.status, o.status)):
+            assert np.array_equal(a.cpu().numpy(), b)
+        assert (r.t.cpu().numpy() == 4.5 * 4e-7).all()
+        assert rel_diff(r.y.cpu().numpy(), o.y, sp.v_ref).max() < 1e-7      # forced steps: far above rtol
+        u = gpu_trace(GF, su, Q, mu[:33], t0=1e8, t_max=2e8)
+        assert (u.status.cpu().numpy() == 4).all() and (u.t.cpu().numpy() == 1e8).all()
+        assert (u.n_acc.cpu().numpy() == 0).all() and (u.n_rej.cpu().numpy() == 0).all()
+        assert np.array_equal(u.y.cpu().numpy()[0], Q.s)
+    GF.set_kernel(0)
+
+
 def test_h_inout_roundtrip_and_segments(case0):
     """Two calls joined by h_inout and GC_TRACE_RESUME equal the oracle run with the same segmentation; lost
     or stopped particles are not touched by the second call."""
@@ -311,3 +335,53 @@ def test_refined_loss_point_matches_oracle(kernel):
         assert float(d.max()) < 1e-9
     else:
         assert torch.equal(r.y[:, surv], u.y[:, surv]) and torch.equal(r.n_acc, u.n_acc)
+
+
+def test_two_live_fields_sharing_a_kernel_instantiation():
+    """The dynamic shared-memory limit belongs to the kernel function, not to a field: a field with a large window
+    (config 4, 16 mode harmonics) must still launch after a field with a smaller window of the same instantiation
+    (config 2, 8 mode harmonics) was created."""
+    from paper_2605_16734_b200 import gcorbit as G
+    fld4, spec4, P4, OF4, GF4, mu4 = make_case(4, 4200)
+    fld2, spec2, P2, OF2, GF2, mu2 = make_case(2, 64)          # created second: used to lower the limit
+    k = 24
+    o = OF4.trace(spec4, P4.s[:k], P4.theta[:k], P4.zeta[:k], P4.vpar[:k], mu4[:k], t_max=2e-6)
+    for kern in (G.GC_KERNEL_TILE, G.GC_KERNEL_MMA):
+        GF4.set_kernel(kern)
+        r = gpu_trace(GF4, spec4, P4, mu4, t_max=2e-6)
+        assert np.array_equal(r.status.cpu().numpy()[:k], o.status)
+        assert rel_diff(r.y.cpu().numpy()[:, :k], o.y, spec4.v_ref).max() < 1e-9
+        GF2.set_kernel(kern)
+        r2 = gpu_trace(GF2, spec2, P2, mu2, t_max=1e-6)
+        assert (r2.status.cpu().numpy() == 0).all()
+
+
+def test_trace_host_refuses_overlapping_calls_on_one_field(case0):
+    """gc_trace_host keeps its device workspace in the field, so it is not re-entrant on one field: a call that
+    overlaps another one returns GC_EINVAL instead of corrupting the workspace (include/gcorbit.h)."""
+    import threading
+    from paper_2605_16734_b200 import gcorbit as G
+    fld, spec, P, OF, GF, mu = case0
+    GF.set_kernel(G.GC_KERNEL_GENERIC)                         # slow on purpose: the first call runs for a while
+    results = []
+
+    def call(t_max):
+        try:
+            r = GF.trace_host(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=t_max)
+            results.append(("ok", r))
+        except G.GcError as e:
+            results.append(("err", e))
+
+    a = threading.Thread(target=call, args=(1e-4,))
+    a.start()
+    import time
+    time.sleep(0.05)
+    call(1e-6)                                                 # overlaps the first call (ctypes releases the GIL)
+    a.join()
+    GF.set_kernel(G.GC_KERNEL_AUTO)
+    kinds = sorted(k for k, _ in results)
+    assert kinds == ["err", "ok"], kinds
+    err = [v for k, v in results if k == "err"][0]
+    assert err.code == G.GC_EINVAL and "another gc_trace_host call" in str(err)
+    again = GF.trace_host(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=1e-6)      # and the field is usable afterwards
+    assert (again.status == 0).all()

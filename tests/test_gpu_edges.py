@@ -372,7 +372,7 @@ def test_trace_host_refuses_overlapping_calls_on_one_field(case0):
         except G.GcError as e:
             results.append(("err", e))
 
-    a = threading.Thread(target=call, args=(1e-4,))
+    a = threading.Thread(target=call, args=(5e-4,))
     a.start()
     import time
     time.sleep(0.05)

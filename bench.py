@@ -3,12 +3,17 @@
     python bench.py --gpus N --steps K --warmup W            # this repo's CUDA path (one rank per GPU)
     python bench.py --impl reference --gpus N --steps K --warmup W   # the CPU oracle, as it stands
 
-Workload: BASELINE.json configs[1] -- 100,000 alpha particles per GPU, static field with 545 harmonics on
-101 radial nodes, rtol = atol = 1e-9, h_min = 1e-12.  One "step" advances the whole
-ensemble by one segment of simulated time (default 2e-5 s, about 10^3 Dormand-Prince attempts per
-particle) with ONE gc_trace call that continues the previous step in place (GC_TRACE_RESUME), so K steps
-are the first (W + K) * segment seconds of the config-1 trace; lost particles drop out as they do there.
-A particle-step is one ATTEMPTED Dormand-Prince step (6 right-hand sides), accepted or rejected.
+Workload: BASELINE.json configs[3] -- the 1,000,000-particle trace north_star's target names: slowing-down alphas
+with a (1-s)^2 birth profile in the static config-1 field (545 harmonics on 101 radial nodes), rtol = atol = 1e-8
+(DESIGN.md section 7).  One "step" advances the whole ensemble by one segment of simulated time (default 2e-5 s,
+about 350 Dormand-Prince attempts per particle) with ONE gc_trace call that continues the previous step in place
+(GC_TRACE_RESUME), so K steps are the first (W + K) * segment seconds of the config-3 trace; lost particles drop
+out as they do there.  A particle-step is one ATTEMPTED Dormand-Prince step (6 right-hand sides), accepted or
+rejected.  --config 0|1|2|4 select the other BASELINE configurations (not the default line).
+
+With --gpus N > 1 and no torchrun environment the script starts N ranks itself (torch.distributed.run on
+127.0.0.1), one per GPU; every rank traces an independent draw of the same recipe (weak scaling, no data-path
+collective).
 """
 from __future__ import annotations
 
@@ -29,15 +34,21 @@ import numpy as np
 METRIC = "guiding-center particle-steps/s (FP64)"
 UNIT = "particle-steps/s"
 # FP64 ALU peak used as the roofline denominator: 148 SMs x 64 FP64 lanes x 2 flop
-# x 1.965 GHz (clocks.max.sm in MEASURED_PEAKS.json) = 37.2 TFLOP/s; gc_fp64_peak_probe measures the
-# sustained DFMA rate of the same box in the same run and is reported beside it.
+# x 1.965 GHz (sm_max_mhz in MEASURED_PEAKS.json) = 37.2 TFLOP/s; libgcprobes.so measures the sustained DFMA
+# and DMMA rates of the same box in the same run, reported beside it.
 FP64_LANES_PER_SM = 64
 
 
-def flops_per_step(nh: int, M: int, nk: int, n_omega: int) -> float:
-    """F_RHS = 28 nh + 18 (M + 1) + 350 (+ 75 K + 40 n_omega); F_step = 6 F_RHS + 250."""
-    f_rhs = 28.0 * nh + 18.0 * (M + 1) + 350.0 + 75.0 * nk + 40.0 * n_omega
+def flops_per_step(nh: int, M: int, nk: int, n_omega: int, per_harmonic: float = 28.0) -> float:
+    """F_RHS = 28 nh + 18 (M + 1) + 350 (+ 75 K + 40 n_omega); F_step = 6 F_RHS + 250.
+    per_harmonic = 28 is the survey's textbook count (14 FMA per harmonic); 16 is the cheapest exact formulation
+    this build found (+-n pairing with slot-wise accumulation, 8 FMA per harmonic)."""
+    f_rhs = per_harmonic * nh + 18.0 * (M + 1) + 350.0 + 75.0 * nk + 40.0 * n_omega
     return 6.0 * f_rhs + 250.0
+
+
+DEFAULT_CONFIG = 3
+FULL_SIZE = {0: 512, 1: 100_000, 2: 100_000, 3: 1_000_000, 4: 1_000_000}
 
 
 def parse_args():
@@ -45,10 +56,12 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1)")
-    ap.add_argument("--particles", type=int, default=None, help="particles per GPU (default: the config's, "
-                    "capped at 100000 per step for configs 3-4 unless given)")
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference", "plumbing"],
+                    help="cuda: this repo's kernels; reference: the CPU oracle; plumbing: launcher + process group + "
+                         "timing reduction only (gloo, no device; used by the CPU tests)")
+    ap.add_argument("--config", type=int, default=DEFAULT_CONFIG, choices=sorted(FULL_SIZE),
+                    help="BASELINE.json config index (default 3: the 1M-particle trace)")
+    ap.add_argument("--particles", type=int, default=None, help="particles per GPU (default: the config's)")
     ap.add_argument("--segment", type=float, default=2e-5, help="simulated seconds per step")
     ap.add_argument("--kernel", default="auto", choices=["auto", "mma", "tile", "warp", "generic"])
     ap.add_argument("--samples", type=int, default=0, help="NEXT-1: uniform-time samples per segment recorded by "
@@ -106,8 +119,7 @@ def workload(args, rank: int):
     from paper_2605_16734_b200 import workloads as W
     cfg = args.config
     fld, spec = W.make_field(cfg), W.make_spec(cfg)
-    full = {0: 512, 1: 100_000, 2: 100_000, 3: 1_000_000, 4: 1_000_000}[cfg]
-    n = args.particles if args.particles else full
+    n = args.particles if args.particles else FULL_SIZE[cfg]
     P = W.make_particles(cfg, n, stream=rank)
     M = int(fld.xm.max())
     n_omega = len(set(np.asarray(fld.mode_omega).tolist()))
@@ -116,7 +128,8 @@ def workload(args, rank: int):
                         f"advancing the ensemble by {args.segment:g} s of simulated time (GC_TRACE_RESUME)",
             "particles_per_gpu": n, "segment_s": args.segment, "nh": fld.nh, "ns": fld.ns, "nk": fld.nk,
             "rtol": spec.rtol,
-            "flop_per_particle_step": flops_per_step(fld.nh, M, fld.nk, n_omega)}
+            "flop_per_particle_step": flops_per_step(fld.nh, M, fld.nk, n_omega),
+            "flop_per_particle_step_min": flops_per_step(fld.nh, M, fld.nk, n_omega, per_harmonic=16.0)}
     return fld, spec, P, info
 
 
@@ -240,6 +253,9 @@ def run_cuda(args):
     def attempts_of(st):
         return int((st.n_acc.sum(dtype=torch.int64) + st.n_rej.sum(dtype=torch.int64)).item())
 
+    def accepted_of(st):
+        return int(st.n_acc.sum(dtype=torch.int64).item())
+
     # warm-up: the first W segments of the trace
     S = args.samples
     if S > 0:
@@ -260,6 +276,7 @@ def run_cuda(args):
     torch.cuda.synchronize()
     first = max(Wu, 1)
     a_before = attempts_of(state)
+    acc_before = accepted_of(state)
     alive_before = int((state.status == 0).sum().item())
 
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
@@ -281,6 +298,7 @@ def run_cuda(args):
     step_ms = [a.elapsed_time(b) for a, b in ev]
     kernel_ms = float(sum(step_ms))
     attempts = attempts_of(state) - a_before
+    accepted = accepted_of(state) - acc_before
     alive_after = int((state.status == 0).sum().item())
     ms_max, attempts_all = E.reduce_timing(kernel_ms, attempts, dev)
     value = attempts_all / (ms_max * 1e-3)
@@ -346,36 +364,52 @@ def run_cuda(args):
         return
 
     peak_nominal = 148 * FP64_LANES_PER_SM * 2 * 1.965e9 / 1e12
+    peak_src = "148 SMs x 64 FP64 lanes x 2 flop x 1965 MHz (fallback: MEASURED_PEAKS.json not found)"
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
             mp = json.load(fh)
-        peak_nominal = torch.cuda.get_device_properties(dev).multi_processor_count * FP64_LANES_PER_SM * 2 * \
-            float(mp["sm_max_mhz"]) * 1e6 / 1e12
+        sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        peak_nominal = sms * FP64_LANES_PER_SM * 2 * float(mp["sm_max_mhz"]) * 1e6 / 1e12
+        peak_src = (f"{sms} SMs x 64 FP64 lanes x 2 flop x sm_max_mhz {mp['sm_max_mhz']:g} of MEASURED_PEAKS.json "
+                    "(DESIGN.md section 6; the file holds no FP64 figure, so the ALU peak is derived)")
     except Exception:
         pass
-    probe_flops, _ = G.fp64_peak_probe()
-    dmma_flops, mixed_flops = G.dmma_peak_probe()
-    fstep = info["flop_per_particle_step"]
-    achieved = attempts * fstep / (kernel_ms * 1e-3) / 1e12         # this rank's kernel, TFLOP/s
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json.txt")
-    # one ncu capture of the DEFAULT launch (profiles/r1_ncu_mma_config1.md); other workloads have no capture
-    default_launch = (args.config == 1 and args.particles is None and args.segment == 2e-5 and
+    from paper_2605_16734_b200 import probes
+    probe_flops, _ = probes.dfma()
+    dmma_flops, mixed_flops = probes.dmma()
+    lds_distinct, lds_paired = probes.lds128()
+    fstep, fstep_min = info["flop_per_particle_step"], info["flop_per_particle_step_min"]
+    rate = attempts / (kernel_ms * 1e-3)                            # this rank's kernel, particle-steps/s
+    achieved = rate * fstep / 1e12
+    # constants of ONE ncu --set full capture of the default launch (profiles/ncu_constants.json.txt names the
+    # capture): DRAM bytes per launch and executed FP64 flop per particle-step.  Any other workload: null.
+    traffic = executed = cap_src = None
+    default_launch = (args.config == DEFAULT_CONFIG and args.particles is None and args.segment == 2e-5 and
                       kinfo["kernel"] == "mma" and args.samples == 0)
+    tp = os.path.join(ROOT, "profiles", "ncu_constants.json.txt")
     if os.path.exists(tp) and default_launch:
         try:
             with open(tp) as fh:
-                traffic = json.load(fh).get(f"config{args.config}_dram_bytes_per_launch")
+                c = json.load(fh).get(f"config{args.config}", {})
+            traffic, executed, cap_src = c.get("dram_bytes_per_launch"), c.get("executed_flop_per_particle_step"), \
+                c.get("source")
         except Exception:
-            traffic = None
+            pass
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
                 "frac": achieved / peak_nominal, "traffic": traffic,
+                "flop_model": "frac / achieved count the SURVEY.md 8(d) textbook formulation (28 flop per harmonic "
+                              "and right-hand side); the kernel runs a cheaper exact one: see frac_min_formulation "
+                              "(16 flop per harmonic) and frac_executed (FP64 flop the kernel really issues)",
+                "frac_min_formulation": rate * fstep_min / 1e12 / peak_nominal,
+                "frac_executed": (rate * executed / 1e12 / peak_nominal) if executed else None,
+                "executed_flop_per_particle_step": executed, "ncu_capture": cap_src,
                 "kernel": f"trace_{kinfo['kernel']}_kernel", "launch_ms_avg": kernel_ms / K,
-                "peak_source": "148 SMs x 64 FP64 lanes x 2 flop x clocks.max.sm (DESIGN.md section 6)",
+                "peak_source": peak_src,
                 "peak_probe_tflops": probe_flops / 1e12, "peak_probe_dmma_tflops": dmma_flops / 1e12,
                 "peak_probe_dmma_dfma_mixed_tflops": mixed_flops / 1e12,
+                "lds128_cycles_per_warp_instr": {"distinct": lds_distinct, "lane_pairs_shared": lds_paired},
                 "frac_of_probe": achieved / (probe_flops / 1e12),
-                "flop_per_particle_step": fstep,
+                "flop_per_particle_step": fstep, "flop_per_particle_step_min": fstep_min,
                 "particle_steps_per_launch": attempts / K}
     cpu = None
     if not args.no_cpu_baseline:
@@ -388,7 +422,8 @@ def run_cuda(args):
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wu,
            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64", "data": "synthetic", "config": info,
-           "rhs_evals_per_s": 6.0 * value, "accepted_fraction": None,
+           "rhs_evals_per_s": 6.0 * value, "accepted_fraction": accepted / max(attempts, 1),
+           "accepted_particle_steps_per_s": value * accepted / max(attempts, 1),
            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": K, "clocks": clocks,
            "wall_s_timed_region": t_wall1 - t_wall0}
     print(json.dumps(out))
@@ -396,10 +431,46 @@ def run_cuda(args):
         dist.destroy_process_group()
 
 
+def run_plumbing(args):
+    """--impl plumbing: everything of the multi-rank path that is not a kernel -- launch, rendezvous, process group
+    (gloo, CPU), the max-over-ranks / sum-over-ranks reduction of ensemble.reduce_timing and the rank-0 JSON line --
+    with made-up per-rank numbers.  Used by tests/test_bench_contract.py; measures nothing."""
+    import torch.distributed as dist
+    from paper_2605_16734_b200 import ensemble as E
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        dist.init_process_group("gloo")
+    ms, attempts = E.reduce_timing(100.0 + rank, 1000 * (rank + 1))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps({"impl": "plumbing", "n_gpus": world, "ms_max": ms, "attempts_sum": attempts}))
+
+
+def launch_ranks(args) -> int:
+    """`python bench.py --gpus N` without a torchrun environment: start N ranks of this script on this node
+    (torch.distributed.run, rendezvous on 127.0.0.1, a free port), one per GPU, and pass their output through."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "WARN")
+    return subprocess.call(cmd, env=env)
+
+
 def main():
     args = parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        raise SystemExit(launch_ranks(args))
     if args.impl == "reference":
         run_reference(args)
+    elif args.impl == "plumbing":
+        run_plumbing(args)
     else:
         run_cuda(args)
 

@@ -196,6 +196,15 @@ int gc_birkhoff(int64_t n, int64_t nsamp, const double* series, int64_t j_first,
 /* Kernel choice (GC_KERNEL_*) for later gc_trace / gc_rhs_eval calls on this field (default AUTO); GC_EINVAL
  * if the field does not fit the requested kernel. */
 int gc_set_kernel(gc_field* f, int32_t kernel);
+/* Tuning of the cell-binned kernels (MMA, TILE) for later calls on this field; results do not depend on either.
+ *   GC_OPT_WAVE_PARTICLES  the ensemble is traced in waves of this many particles inside one launch, so that the
+ *                          per-particle records of a wave (128 B each) stay in L2 between its epochs; 0 = automatic
+ *                          (2^18), minimum 4096; an ensemble up to 1.25 waves runs as one wave
+ *   GC_OPT_CHUNK_ATTEMPTS  attempted steps a particle gets per epoch before the ensemble is re-binned by radial
+ *                          cell; 0 = the kernel's default (8), at most the kernel's compiled maximum (8)
+ * GC_EINVAL for an unknown option or a value out of range. */
+enum { GC_OPT_WAVE_PARTICLES = 1, GC_OPT_CHUNK_ATTEMPTS = 2 };
+int gc_set_option(gc_field* f, int32_t option, int64_t value);
 /* Which kernel gc_trace will launch for this field and n particles (GC_KERNEL_GENERIC, _WARP, _TILE or _MMA), and
  * its launch geometry; any pointer may be NULL. */
 int gc_kernel_info(const gc_field* f, int64_t n, int32_t* kernel, int32_t* blocks, int32_t* threads_per_block,

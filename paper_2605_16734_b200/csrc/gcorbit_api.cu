@@ -66,6 +66,12 @@ struct gc_field {
   cudaStream_t host_stream = nullptr;
   void* host_slab = nullptr;
   size_t host_slab_bytes = 0;
+  // per-call scratch of the trace kernels comes from a pool of the field that keeps what it is given back (the
+  // default pool of the device returns freed memory to the driver at every synchronisation, so a caller that
+  // synchronises after each call -- gc_trace_host does -- paid a fresh 13..128 MB allocation per call)
+  cudaMemPool_t pool = nullptr;
+  long long wave_particles = 0;     // GC_OPT_WAVE_PARTICLES (0 = automatic)
+  int chunk_attempts = 0;           // GC_OPT_CHUNK_ATTEMPTS (0 = the kernel's default)
   std::atomic<bool> host_busy{false};   // gc_trace_host is not re-entrant on one field: overlapping calls get GC_EINVAL
   bool mma_ok = false;
   int mma_smem = 0;                 // dynamic shared memory of the mma kernel
@@ -125,6 +131,10 @@ int ensure_smem(const void* fn, int bytes) {
 // kernel FUNCTION, not to a field (two live fields can share an instantiation with different window sizes), so every
 // instantiation is raised to this one cap and never lowered.
 constexpr int kBinnedSmemCap = 110 * 1024;
+
+// Particles per wave of the binned kernels when the caller does not say (GC_OPT_WAVE_PARTICLES): 2^18 records of
+// 128 B = 32 MB, a quarter of the 126 MB L2.
+constexpr long long kAutoWaveParticles = 1 << 18;
 
 // Packed rows[node][it][lane] of the warp kernel (kernels_warp.cuh header comment).
 int pack_rows(gc_field* f, const gc_field_desc* d) {
@@ -357,19 +367,31 @@ long long tile_geometry(const gc_field* f, long long n, bool mma, int* tile_size
   return blocks;
 }
 
+// Waves: the 128-byte records of one wave must stay in L2 between its epochs.
+long long wave_size(const gc_field* f, long long n) {
+  const long long wave = f->wave_particles > 0 ? f->wave_particles : kAutoWaveParticles;
+  if (n <= wave + wave / 4) return n > 0 ? n : 1;          // one wave
+  const long long nw = (n + wave - 1) / wave;
+  return ((n + nw - 1) / nw + 63) / 64 * 64;               // equal waves, whole tiles
+}
+
 // One cooperative launch of the tile or mma kernel (mode 0 trace, mode 1 right-hand side only) with its scratch.
 int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, cudaStream_t st, bool mma = false) {
   const int ncell = f->dev.ns - 3;
   const size_t n = (size_t)t.n;
-  const size_t rec_bytes = n * gc::kRecDoubles * sizeof(double);
+  const long long wave = wave_size(f, (long long)n);
+  const size_t wn = (size_t)wave;
+  const size_t rec_bytes = wn * gc::kRecDoubles * sizeof(double);
   const size_t nbin = (size_t)ncell * gc::kSubBins;
-  const size_t int_count = n + 2 * nbin + (size_t)2 * (ncell + 1) + 8;
+  const size_t int_count = wn + 2 * nbin + (size_t)2 * (ncell + 1) + 8;
   unsigned char* slab = nullptr;
-  GC_CUDA(cudaMallocAsync((void**)&slab, rec_bytes + int_count * sizeof(int), st));
+  GC_CUDA(cudaMallocFromPoolAsync((void**)&slab, rec_bytes + int_count * sizeof(int), f->pool, st));
   gc::TileScratch sc{};
+  sc.wave = wave;
+  sc.chunk = f->chunk_attempts;
   sc.rec = reinterpret_cast<double*>(slab);
   int* ip = reinterpret_cast<int*>(slab + rec_bytes);
-  sc.order = ip; ip += n;
+  sc.order = ip; ip += wn;
   sc.cnt = ip; ip += nbin;
   sc.cursor = ip; ip += nbin;
   sc.start = ip; ip += ncell + 1;
@@ -377,7 +399,7 @@ int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, c
   sc.ctrl = ip;
   GC_CUDA(cudaMemsetAsync(sc.cnt, 0, (2 * nbin + (size_t)2 * (ncell + 1) + 8) * sizeof(int), st));
   int per_tile = 0;
-  long long blocks = tile_geometry(f, (long long)n, mma, &per_tile);
+  long long blocks = tile_geometry(f, (long long)wn, mma, &per_tile);
   sc.tile_size = per_tile;
   gc::FieldDev fd = f->dev;
   void* args[] = {(void*)&fd, (void*)&t, (void*)&sc, (void*)&mode, (void*)&rhs_out};
@@ -421,6 +443,7 @@ int gc_field_destroy(gc_field* f) {
   for (void* p : f->allocs) cudaFree(p);
   if (f->host_slab) cudaFree(f->host_slab);
   if (f->host_stream) cudaStreamDestroy(f->host_stream);
+  if (f->pool) cudaMemPoolDestroy(f->pool);                // waits for nothing: callers synchronise before destroying
   delete f;
   return GC_OK;
 }
@@ -490,6 +513,19 @@ int gc_field_create(const gc_field_desc* d, gc_field** out) {
     int devid = 0;
     cudaGetDevice(&devid);
     cudaDeviceGetAttribute(&f->sm_count, cudaDevAttrMultiProcessorCount, devid);
+    cudaMemPoolProps props{};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = devid;
+    cudaError_t pe = cudaMemPoolCreate(&f->pool, &props);
+    if (pe == cudaSuccess) {
+      unsigned long long keep = ~0ULL;                       // never trim: the scratch is reused call after call
+      pe = cudaMemPoolSetAttribute(f->pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+    if (pe != cudaSuccess) rc = fail(GC_ECUDA, std::string("cudaMemPoolCreate: ") + cudaGetErrorString(pe));
+  }
+  if (rc == GC_OK) {
     f->kernel = GC_KERNEL_AUTO;
     if (f->warp_ok) {
       const WarpInst* w = find_inst(f);
@@ -522,6 +558,23 @@ int gc_set_kernel(gc_field* f, int32_t kernel) {
   return GC_OK;
 }
 
+int gc_set_option(gc_field* f, int32_t option, int64_t value) {
+  if (!f) return fail(GC_EINVAL, "gc_set_option: NULL field");
+  if (value < 0) return fail(GC_EINVAL, "gc_set_option: negative value");
+  switch (option) {
+    case GC_OPT_WAVE_PARTICLES:
+      if (value != 0 && value < 4096) return fail(GC_EINVAL, "gc_set_option: a wave holds at least 4096 particles");
+      f->wave_particles = value;
+      return GC_OK;
+    case GC_OPT_CHUNK_ATTEMPTS:
+      if (value > 64) return fail(GC_EINVAL, "gc_set_option: at most 64 attempts per chunk");
+      f->chunk_attempts = (int)value;
+      return GC_OK;
+    default:
+      return fail(GC_EINVAL, "gc_set_option: unknown option");
+  }
+}
+
 int gc_kernel_info(const gc_field* f, int64_t n, int32_t* kernel, int32_t* blocks, int32_t* threads, int32_t* smem,
                    int32_t* regs) {
   if (!f) return fail(GC_EINVAL, "gc_kernel_info: NULL field");
@@ -531,11 +584,11 @@ int gc_kernel_info(const gc_field* f, int64_t n, int32_t* kernel, int32_t* block
   if (k == GC_KERNEL_MMA) {
     GC_CUDA(cudaFuncGetAttributes(&at, mma_fn(f)));
     int tsz = 0;
-    b = (int)tile_geometry(f, n, true, &tsz); t = gc::kMmaThreads; s = f->mma_smem;
+    b = (int)tile_geometry(f, wave_size(f, n), true, &tsz); t = gc::kMmaThreads; s = f->mma_smem;
   } else if (k == GC_KERNEL_TILE) {
     GC_CUDA(cudaFuncGetAttributes(&at, tile_fn(f)));
     int tsz = 0;
-    b = (int)tile_geometry(f, n, false, &tsz); t = gc::kTileThreads; s = f->tile_smem;
+    b = (int)tile_geometry(f, wave_size(f, n), false, &tsz); t = gc::kTileThreads; s = f->tile_smem;
   } else if (k == GC_KERNEL_WARP) {
     const WarpInst* w = find_inst(f);
     GC_CUDA(cudaFuncGetAttributes(&at, w->trace_fn));
@@ -637,7 +690,7 @@ int trace_common(const gc_field* f, const gc_trace_params* params, int64_t n, co
   if (kern == GC_KERNEL_WARP) {
     const WarpInst* w = find_inst(f);
     unsigned long long* counter = nullptr;
-    GC_CUDA(cudaMallocAsync((void**)&counter, sizeof(unsigned long long), st));
+    GC_CUDA(cudaMallocFromPoolAsync((void**)&counter, sizeof(unsigned long long), f->pool, st));
     GC_CUDA(cudaMemsetAsync(counter, 0, sizeof(unsigned long long), st));
     t.work_counter = counter;
     void* args[] = {(void*)&f->dev, (void*)&t};

@@ -50,13 +50,16 @@ constexpr int kSubBins = GC_SUBBINS;   // radial sub-bins per cell: tiles come o
 
 // Per-call scratch of the tile kernel (device memory, owned by gc_trace for the duration of the call).
 struct TileScratch {
-  double* rec;      // [n][16]: y[4], k1[4], t, h, mu, attempts (int64), {status, flags}, {n_acc, n_rej}, {n_forced, bin}, -
-  int* order;       // [n]   running particles sorted by home cell
+  double* rec;      // [wave][16]: y[4], k1[4], t, h, mu, attempts (int64), {status, flags}, {n_acc, n_rej}, {n_forced, bin}, -
+  int* order;       // [wave] running particles (index inside the wave) sorted by home cell
   int* cnt;         // [ncell kSubBins] running particles per bin (home cell, radial sub-bin), for the NEXT binning
   int* start;       // [ncell + 1] cell segment offsets into order
   int* tstart;      // [ncell + 1] tile offsets
   int* cursor;      // [ncell kSubBins] scatter cursors
   int tile_size;    // particles per tile, a multiple of 8, <= threads per block
+  int chunk;        // attempted steps per lane per chunk (<= the kernel's CAP template argument: 0 = CAP)
+  long long wave;   // particles per wave: the ensemble is traced wave after wave inside one launch so that the records of
+                    // a wave stay in L2 between its epochs (10^6 records of 128 B do not fit)
   int* ctrl;        // [0] tile counter, [1] tiles past their first chunk, [2] tiles this epoch, [3] running
 };
 
@@ -326,9 +329,12 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
   __syncthreads();
   unsigned bar_phase = 0;
 
+  const int chunk = (sc.chunk > 0 && sc.chunk < CAP) ? sc.chunk : CAP;
+  for (long long w0 = 0; w0 < p.n; w0 += sc.wave) {                        // waves (one, unless the ensemble is large)
+  const long long w1 = (w0 + sc.wave < p.n) ? w0 + sc.wave : p.n;
   // ---- P0: records from the inputs (coalesced), first cell counts ------------------------------------------------
-  for (long long i = gtid; i < p.n; i += gthreads) {
-    double* r = sc.rec + i * kRecDoubles;
+  for (long long i = w0 + gtid; i < w1; i += gthreads) {
+    double* r = sc.rec + (i - w0) * kRecDoubles;
     int st = kStRunning;
     double y0, y1, y2, y3, h, t = p.t0, mu = p.mu[i];
     if (mode == 1) {
@@ -401,7 +407,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
     if (__ldcg(sc.ctrl + 3) == 0) break;
 
     // ---- C: scatter the running particles into cell order --------------------------------------------------------
-    for (long long i = gtid; i < p.n; i += gthreads) {
+    for (long long i = gtid; i < w1 - w0; i += gthreads) {
       const int2 sf = __ldcg(reinterpret_cast<const int2*>(sc.rec + i * kRecDoubles + 12));
       if (sf.x == kStRunning) {
         const int bin = __ldcg(reinterpret_cast<const int2*>(sc.rec + i * kRecDoubles + 14)).y;
@@ -449,8 +455,9 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
       long long attempts = 0;
       int st = 0, flags = 0, n_acc = 0, n_rej = 0, n_forced = 0, jn = 0;
       if (active) {
-        pid = __ldcg(sc.order + begin + slot);
-        const double* r = sc.rec + pid * kRecDoubles;
+        const int li = __ldcg(sc.order + begin + slot);
+        pid = w0 + li;
+        const double* r = sc.rec + (long long)li * kRecDoubles;
         const double4 a = ldcg4(r);
         const double4 b = ldcg4(r + 4);
         const double4 c = ldcg4(r + 8);
@@ -467,7 +474,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
 
       for (;;) {                                 // chunks of CAP attempts
 #pragma unroll 1
-        for (int att = 0; att < CAP; ++att) {
+        for (int att = 0; att < chunk; ++att) {
           if (!__any_sync(0xffffffffu, running)) break;
           if (extra) {                           // attempts are warp-local: any warp may stop at any attempt
             int done = 0;
@@ -666,7 +673,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
       }
       // write the tile back
       if (active) {
-        double* r = sc.rec + pid * kRecDoubles;
+        double* r = sc.rec + (pid - w0) * kRecDoubles;
         const int hb = home_bin(f.ns, y[0]);
         stcg4(r, make_double4(y[0], y[1], y[2], y[3]));
         stcg4(r + 4, make_double4(kb(0, 0), kb(0, 1), kb(0, 2), kb(0, 3)));
@@ -681,9 +688,10 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
   }
 
   // ---- outputs (coalesced) -------------------------------------------------------------------------------------
+  // (the thread that reads record i - w0 here is the one that overwrites it in P0 of the next wave: no barrier needed)
   if (mode == 0) {
-    for (long long i = gtid; i < p.n; i += gthreads) {
-      const double* r = sc.rec + i * kRecDoubles;
+    for (long long i = w0 + gtid; i < w1; i += gthreads) {
+      const double* r = sc.rec + (i - w0) * kRecDoubles;
       const int4 d = __ldcg(reinterpret_cast<const int4*>(r + 12));
       if (d.x == kStSkip) continue;
       const double4 a = ldcg4(r);
@@ -703,6 +711,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
       if (p.n_forced) p.n_forced[i] = (p.resume ? p.n_forced[i] : 0) + n_forced;
     }
   }
+  }                                                                          // waves
 }
 
 template <int NMAX, bool MODES, bool SAMPLE>

@@ -18,10 +18,11 @@ SO_PATH = os.path.join(_HERE, "libgcorbit.so")
 GC_OK, GC_EINVAL, GC_ENOMEM, GC_ECUDA = 0, -1, -2, -3
 GC_KERNEL_AUTO, GC_KERNEL_GENERIC, GC_KERNEL_WARP, GC_KERNEL_TILE, GC_KERNEL_MMA = 0, 1, 2, 3, 4
 GC_TILE_MIN_PARTICLES = 4096
+GC_OPT_WAVE_PARTICLES, GC_OPT_CHUNK_ATTEMPTS = 1, 2
 ST_TMAX, ST_LOST, ST_AXIS, ST_MAXSTEPS, ST_NONFINITE = 0, 1, 2, 3, 4
 
 EXPORTS = ["gc_field_create", "gc_field_destroy", "gc_field_eval", "gc_pert_eval", "gc_rhs_eval", "gc_trace",
-           "gc_trace_host", "gc_set_kernel", "gc_kernel_info", "gc_last_error",
+           "gc_trace_host", "gc_set_kernel", "gc_set_option", "gc_kernel_info", "gc_last_error",
            "gc_trace_sampled", "gc_pzeta_eval", "gc_birkhoff"]
 
 
@@ -71,6 +72,7 @@ def load_library():
         L.gc_pzeta_eval.argtypes = [vp, dbl, dbl, i64, vp, vp, vp, vp, vp]
         L.gc_birkhoff.argtypes = [i64, i64, vp, i64, vp, vp, vp]
         L.gc_set_kernel.argtypes = [vp, i32]
+        L.gc_set_option.argtypes = [vp, i32, i64]
         L.gc_kernel_info.argtypes = [vp, C.c_int64] + [C.POINTER(i32)] * 5
         for name in EXPORTS:
             if name != "gc_last_error":
@@ -168,6 +170,9 @@ class Field:
     # ---- gc_set_kernel / gc_kernel_info --------------------------------------------------------------------
     def set_kernel(self, kernel: int):
         _check(load_library().gc_set_kernel(self._h, kernel))
+
+    def set_option(self, option: int, value: int):
+        _check(load_library().gc_set_option(self._h, int(option), int(value)))
 
     def kernel_info(self, n: int = 1 << 20) -> dict:
         """Kernel and launch geometry gc_trace uses for an ensemble of n particles."""

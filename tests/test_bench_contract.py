@@ -39,3 +39,29 @@ def test_cuda_arm_has_no_cpu_fallback():
         pytest.skip("a CUDA device is present")
     r = _run("--steps", "1", "--warmup", "1")
     assert r.returncode != 0 and "no CUDA device" in (r.stderr + r.stdout)
+
+
+def test_gpus_flag_starts_that_many_ranks():
+    """`python bench.py --gpus 2` with no torchrun environment starts two ranks itself (torch.distributed.run on
+    127.0.0.1), which form a process group (gloo here), reduce the timing (max) and the attempts (sum) and print ONE
+    line on rank 0 -- the launcher and plumbing of the CUDA arm without its kernels (--impl plumbing)."""
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR",
+                                                            "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "plumbing", "--gpus", "2"],
+                       capture_output=True, text=True, timeout=300, cwd=ROOT, env=env)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    # rank r reports 100 + r ms and 1000 (r + 1) attempts
+    assert d == {"impl": "plumbing", "n_gpus": 2, "ms_max": 101.0, "attempts_sum": 3000}
+
+
+def test_reference_arm_under_torchrun_prints_on_rank_0_only():
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps",
+                        "1", "--warmup", "0", "--config", "0", "--cpu-seconds", "1"],
+                       capture_output=True, text=True, timeout=600, cwd=ROOT, env=env)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1 and json.loads(lines[0])["n_gpus"] == 2

@@ -197,9 +197,10 @@ int gc_birkhoff(int64_t n, int64_t nsamp, const double* series, int64_t j_first,
  * if the field does not fit the requested kernel. */
 int gc_set_kernel(gc_field* f, int32_t kernel);
 /* Tuning of the cell-binned kernels (MMA, TILE) for later calls on this field; results do not depend on either.
- *   GC_OPT_WAVE_PARTICLES  the ensemble is traced in waves of this many particles inside one launch, so that the
- *                          per-particle records of a wave (128 B each) stay in L2 between its epochs; 0 = automatic
- *                          (2^18), minimum 4096; an ensemble up to 1.25 waves runs as one wave
+ *   GC_OPT_WAVE_PARTICLES  number of record slots: a larger ensemble streams through them inside one launch (a
+ *                          finished particle hands its slot to the next unstarted one), so that the per-particle
+ *                          records (128 B each) stay in L2 between epochs; 0 = automatic (2^18), minimum 4096; an
+ *                          ensemble up to 1.25 times this number gets one slot per particle
  *   GC_OPT_CHUNK_ATTEMPTS  attempted steps a particle gets per epoch before the ensemble is re-binned by radial
  *                          cell; 0 = the kernel's default (8), at most the kernel's compiled maximum (8)
  * GC_EINVAL for an unknown option or a value out of range. */

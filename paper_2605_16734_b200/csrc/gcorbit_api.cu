@@ -132,8 +132,8 @@ int ensure_smem(const void* fn, int bytes) {
 // instantiation is raised to this one cap and never lowered.
 constexpr int kBinnedSmemCap = 110 * 1024;
 
-// Particles per wave of the binned kernels when the caller does not say (GC_OPT_WAVE_PARTICLES): 2^18 records of
-// 128 B = 32 MB, a quarter of the 126 MB L2.
+// Record slots of the binned kernels when the caller does not say (GC_OPT_WAVE_PARTICLES): 2^18 records of 128 B =
+// 32 MB, a quarter of the 126 MB L2.
 constexpr long long kAutoWaveParticles = 1 << 18;
 
 // Packed rows[node][it][lane] of the warp kernel (kernels_warp.cuh header comment).
@@ -367,12 +367,12 @@ long long tile_geometry(const gc_field* f, long long n, bool mma, int* tile_size
   return blocks;
 }
 
-// Waves: the 128-byte records of one wave must stay in L2 between its epochs.
+// Record slots of the binned kernels: the 128-byte records must stay in L2 between epochs, so a large ensemble
+// streams through a fixed number of slots (kernels_tile.cuh).
 long long wave_size(const gc_field* f, long long n) {
-  const long long wave = f->wave_particles > 0 ? f->wave_particles : kAutoWaveParticles;
-  if (n <= wave + wave / 4) return n > 0 ? n : 1;          // one wave
-  const long long nw = (n + wave - 1) / wave;
-  return ((n + nw - 1) / nw + 63) / 64 * 64;               // equal waves, whole tiles
+  const long long slots = f->wave_particles > 0 ? f->wave_particles : kAutoWaveParticles;
+  if (n <= slots + slots / 4) return n > 0 ? n : 1;        // every particle has its own slot
+  return slots;
 }
 
 // One cooperative launch of the tile or mma kernel (mode 0 trace, mode 1 right-hand side only) with its scratch.
@@ -383,21 +383,23 @@ int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, c
   const size_t wn = (size_t)wave;
   const size_t rec_bytes = wn * gc::kRecDoubles * sizeof(double);
   const size_t nbin = (size_t)ncell * gc::kSubBins;
-  const size_t int_count = wn + 2 * nbin + (size_t)2 * (ncell + 1) + 8;
+  const size_t int_count = ((wn + 1) & ~(size_t)1) + 2 * nbin + (size_t)2 * (ncell + 1) + 8 + 4;
   unsigned char* slab = nullptr;
   GC_CUDA(cudaMallocFromPoolAsync((void**)&slab, rec_bytes + int_count * sizeof(int), f->pool, st));
   gc::TileScratch sc{};
-  sc.wave = wave;
+  sc.slots = wave;
   sc.chunk = f->chunk_attempts;
   sc.rec = reinterpret_cast<double*>(slab);
   int* ip = reinterpret_cast<int*>(slab + rec_bytes);
-  sc.order = ip; ip += wn;
+  sc.order = ip; ip += (wn + 1) & ~(size_t)1;
   sc.cnt = ip; ip += nbin;
   sc.cursor = ip; ip += nbin;
   sc.start = ip; ip += ncell + 1;
   sc.tstart = ip; ip += ncell + 1;
-  sc.ctrl = ip;
-  GC_CUDA(cudaMemsetAsync(sc.cnt, 0, (2 * nbin + (size_t)2 * (ncell + 1) + 8) * sizeof(int), st));
+  sc.ctrl = ip; ip += 8;
+  ip += ((reinterpret_cast<uintptr_t>(ip) & 7) ? 1 : 0);   // the 64-bit input cursor
+  sc.next = reinterpret_cast<unsigned long long*>(ip);
+  GC_CUDA(cudaMemsetAsync(sc.cnt, 0, (2 * nbin + (size_t)2 * (ncell + 1) + 8 + 4) * sizeof(int), st));
   int per_tile = 0;
   long long blocks = tile_geometry(f, (long long)wn, mma, &per_tile);
   sc.tile_size = per_tile;
@@ -417,7 +419,7 @@ int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, c
 
 int build_trace_dev(const gc_field* f, const gc_trace_params* p, int64_t n, gc::TraceDev* t) {
   if (!f || !p) return fail(GC_EINVAL, "gc_trace: NULL field or params");
-  if (n < 0) return fail(GC_EINVAL, "gc_trace: n < 0");
+  if (n < 0 || n > 0x7fffffffLL) return fail(GC_EINVAL, "gc_trace: n < 0 or n >= 2^31");
   if (!(p->v_ref > 0.0) || !(p->h0 > 0.0) || !(p->h_min >= 0.0) || !(p->mass > 0.0) || p->charge == 0.0 ||
       !(p->rtol >= 0.0) || !(p->atol >= 0.0) || !(p->rtol + p->atol > 0.0) || p->max_steps < 1 ||
       p->poincare_capacity < 0 || (p->flags & ~(int64_t)(GC_TRACE_RESUME | GC_TRACE_SECTION_VPAR | GC_TRACE_REFINE_LOSS)) != 0 || !std::isfinite(p->t0) || !std::isfinite(p->t_max))

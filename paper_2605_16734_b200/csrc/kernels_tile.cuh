@@ -50,21 +50,23 @@ constexpr int kSubBins = GC_SUBBINS;   // radial sub-bins per cell: tiles come o
 
 // Per-call scratch of the tile kernel (device memory, owned by gc_trace for the duration of the call).
 struct TileScratch {
-  double* rec;      // [wave][16]: y[4], k1[4], t, h, mu, attempts (int64), {status, flags}, {n_acc, n_rej}, {n_forced, bin}, -
-  int* order;       // [wave] running particles (index inside the wave) sorted by home cell
+  double* rec;      // [slots][16]: y[4], k1[4], t, h, mu, attempts (int64), {status, flags, n_acc, n_rej}, {n_forced, bin, jn, particle}
+  int* order;       // [slots] slots of the running particles sorted by home cell
   int* cnt;         // [ncell kSubBins] running particles per bin (home cell, radial sub-bin), for the NEXT binning
   int* start;       // [ncell + 1] cell segment offsets into order
   int* tstart;      // [ncell + 1] tile offsets
   int* cursor;      // [ncell kSubBins] scatter cursors
   int tile_size;    // particles per tile, a multiple of 8, <= threads per block
   int chunk;        // attempted steps per lane per chunk (<= the kernel's CAP template argument: 0 = CAP)
-  long long wave;   // particles per wave: the ensemble is traced wave after wave inside one launch so that the records of
-                    // a wave stay in L2 between its epochs (10^6 records of 128 B do not fit)
-  int* ctrl;        // [0] tile counter, [1] tiles past their first chunk, [2] tiles this epoch, [3] running
+  long long slots;  // record slots: the ensemble streams through them inside one launch -- a slot whose particle has
+                    // finished is flushed to the outputs and handed to the next unstarted particle -- so that the
+                    // records stay in L2 between epochs (10^6 records of 128 B do not fit)
+  unsigned long long* next;   // input cursor: first particle not yet admitted
+  int* ctrl;        // [0] tile counter, [1] tiles past their first chunk, [2] tiles this epoch, [3] running, [4] input exhausted
 };
 
 enum { kFlagPrevRejected = 1, kFlagHaveK1 = 2 };
-enum { kStRunning = -1, kStSkip = -2 };
+enum { kStRunning = -1, kStSkip = -2, kStEmpty = -3 };   // slot states below 0; >= 0: finished, not yet flushed
 
 __constant__ double cDpA[7][6] = {
     {0, 0, 0, 0, 0, 0},
@@ -330,17 +332,15 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
   unsigned bar_phase = 0;
 
   const int chunk = (sc.chunk > 0 && sc.chunk < CAP) ? sc.chunk : CAP;
-  for (long long w0 = 0; w0 < p.n; w0 += sc.wave) {                        // waves (one, unless the ensemble is large)
-  const long long w1 = (w0 + sc.wave < p.n) ? w0 + sc.wave : p.n;
-  // ---- P0: records from the inputs (coalesced), first cell counts ------------------------------------------------
-  for (long long i = w0 + gtid; i < w1; i += gthreads) {
-    double* r = sc.rec + (i - w0) * kRecDoubles;
-    int st = kStRunning;
+  const long long S = sc.slots;
+
+  // Slot li takes particle i: record from the inputs, counted in its bin for the NEXT binning.
+  auto init_record = [&](long long li, long long i) {
+    double* r = sc.rec + li * kRecDoubles;
     double y0, y1, y2, y3, h, t = p.t0, mu = p.mu[i];
     if (mode == 1) {
       y0 = p.s0[i]; y1 = p.th0[i]; y2 = p.ze0[i]; y3 = p.vpar0[i]; h = 0.0;
     } else {
-      if (p.resume && p.status[i] != 0) st = kStSkip;
       y0 = p.s0[i]; y1 = p.th0[i]; y2 = p.ze0[i]; y3 = p.vpar0[i] * p.inv_v_ref;
       h = (p.h_inout && p.h_inout[i] > 0.0) ? p.h_inout[i] : p.h0;
       if (h < p.h_min) h = p.h_min;
@@ -348,7 +348,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
     const int bin = home_bin(f.ns, y0);
     int jn0 = 0;
     if constexpr (SAMPLE) {
-      if (st == kStRunning && mode == 0 && p.nsamp > 0) {
+      if (mode == 0 && p.nsamp > 0) {
         long long j = first_sample_index(p, t);
         if (j < p.nsamp && sample_time(p, j) == t) {           // a sample on t0 is the initial state
           p.samples[(0 * p.nsamp + j) * p.n + i] = y0;
@@ -360,13 +360,51 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
         jn0 = (int)j;
       }
     }
-    reinterpret_cast<double4*>(r)[0] = make_double4(y0, y1, y2, y3);
-    reinterpret_cast<double4*>(r)[1] = make_double4(0.0, 0.0, 0.0, 0.0);
-    reinterpret_cast<double4*>(r)[2] = make_double4(t, h, mu, __longlong_as_double(0LL));
-    int4 a = make_int4(st, 0, 0, 0), b = make_int4(0, bin, jn0, 0);
-    reinterpret_cast<int4*>(r + 12)[0] = a;
-    reinterpret_cast<int4*>(r + 12)[1] = b;
-    if (st == kStRunning) atomicAdd(sc.cnt + bin, 1);
+    stcg4(r, make_double4(y0, y1, y2, y3));
+    stcg4(r + 4, make_double4(0.0, 0.0, 0.0, 0.0));
+    stcg4(r + 8, make_double4(t, h, mu, __longlong_as_double(0LL)));
+    __stcg(reinterpret_cast<int4*>(r + 12), make_int4(kStRunning, 0, 0, 0));
+    __stcg(reinterpret_cast<int4*>(r + 12) + 1, make_int4(0, bin, jn0, (int)i));
+    atomicAdd(sc.cnt + bin, 1);
+  };
+  // A finished particle leaves its slot: results to the caller's arrays.
+  auto flush_record = [&](long long li) {
+    const double* r = sc.rec + li * kRecDoubles;
+    const int4 d = __ldcg(reinterpret_cast<const int4*>(r + 12));
+    const int4 g = __ldcg(reinterpret_cast<const int4*>(r + 12) + 1);
+    const double4 a = ldcg4(r);
+    const double4 c = ldcg4(r + 8);
+    const long long i = g.w;
+    if constexpr (SAMPLE) { if (p.sample_end) p.sample_end[i] = g.z; }
+    p.y_out[i] = a.x;
+    p.y_out[p.n + i] = a.y;
+    p.y_out[2 * p.n + i] = a.z;
+    p.y_out[3 * p.n + i] = a.w * p.v_ref;
+    p.t_out[i] = c.x;
+    p.status[i] = d.x;
+    if (p.h_inout) p.h_inout[i] = c.y;
+    if (p.n_acc) p.n_acc[i] = (p.resume ? p.n_acc[i] : 0) + d.z;
+    if (p.n_rej) p.n_rej[i] = (p.resume ? p.n_rej[i] : 0) + d.w;
+    if (p.n_forced) p.n_forced[i] = (p.resume ? p.n_forced[i] : 0) + g.x;
+  };
+  // Next particle to admit (GC_TRACE_RESUME: particles that finished in an earlier call are passed over), or -1.
+  auto next_particle = [&]() -> long long {
+    for (;;) {
+      const unsigned long long i = atomicAdd(sc.next, 1ULL);
+      if ((long long)i >= p.n) return -1;
+      if (mode == 0 && p.resume && p.status[i] != 0) continue;
+      return (long long)i;
+    }
+  };
+
+  // ---- P0: the first min(slots, n) particles take the slots in order (coalesced) -----------------------------------
+  if (gtid == 0) *sc.next = (unsigned long long)(S < p.n ? S : p.n);
+  for (long long i = gtid; i < S; i += gthreads) {
+    if (i < p.n && !(mode == 0 && p.resume && p.status[i] != 0)) {
+      init_record(i, i);
+    } else {                                   // nothing to trace here: the slot is refilled at the first binning
+      __stcg(reinterpret_cast<int4*>(sc.rec + i * kRecDoubles + 12), make_int4(i < p.n ? kStSkip : kStEmpty, 0, 0, 0));
+    }
   }
   grid.sync();
 
@@ -393,6 +431,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
         sc.start[ncell] = run;
         sc.tstart[ncell] = tiles;
         sc.ctrl[0] = 0; sc.ctrl[1] = 0; sc.ctrl[2] = tiles; sc.ctrl[3] = run;
+        sc.ctrl[4] = (long long)__ldcg(sc.next) >= p.n;                    // every particle has been admitted
       }
       __syncthreads();
       for (int b = tid; b < nbin; b += THREADS) sc.cursor[b] = wsp[b];
@@ -404,14 +443,20 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
     }
     grid.sync();
     const int ntiles = __ldcg(sc.ctrl + 2);
-    if (__ldcg(sc.ctrl + 3) == 0) break;
+    if (__ldcg(sc.ctrl + 3) == 0 && __ldcg(sc.ctrl + 4) != 0) break;        // nothing runs, nothing waits
 
-    // ---- C: scatter the running particles into cell order --------------------------------------------------------
-    for (long long i = gtid; i < w1 - w0; i += gthreads) {
-      const int2 sf = __ldcg(reinterpret_cast<const int2*>(sc.rec + i * kRecDoubles + 12));
-      if (sf.x == kStRunning) {
-        const int bin = __ldcg(reinterpret_cast<const int2*>(sc.rec + i * kRecDoubles + 14)).y;
-        sc.order[atomicAdd(sc.cursor + bin, 1)] = (int)i;
+    // ---- C: scatter the running particles into cell order; slots of finished particles are flushed and handed to
+    // the next unstarted particle, which joins at the next binning (it is counted in cnt now) ----------------------
+    for (long long li = gtid; li < S; li += gthreads) {
+      const int st_slot = __ldcg(reinterpret_cast<const int*>(sc.rec + li * kRecDoubles + 12));
+      if (st_slot == kStRunning) {
+        const int bin = __ldcg(reinterpret_cast<const int2*>(sc.rec + li * kRecDoubles + 14)).y;
+        sc.order[atomicAdd(sc.cursor + bin, 1)] = (int)li;
+      } else if (st_slot != kStEmpty) {
+        if (st_slot >= 0 && mode == 0) flush_record(li);
+        const long long i = next_particle();
+        if (i >= 0) init_record(li, i);
+        else __stcg(reinterpret_cast<int*>(sc.rec + li * kRecDoubles + 12), (int)kStEmpty);
       }
     }
     grid.sync();
@@ -454,9 +499,9 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
       double y[4] = {0.0, 0.0, 0.0, 0.0}, t = 0.0, h = 0.0, mu = 0.0;
       long long attempts = 0;
       int st = 0, flags = 0, n_acc = 0, n_rej = 0, n_forced = 0, jn = 0;
+      int li = 0;
       if (active) {
-        const int li = __ldcg(sc.order + begin + slot);
-        pid = w0 + li;
+        li = __ldcg(sc.order + begin + slot);
         const double* r = sc.rec + (long long)li * kRecDoubles;
         const double4 a = ldcg4(r);
         const double4 b = ldcg4(r + 4);
@@ -466,7 +511,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
         y[0] = a.x; y[1] = a.y; y[2] = a.z; y[3] = a.w;
         kb(0, 0) = b.x; kb(0, 1) = b.y; kb(0, 2) = b.z; kb(0, 3) = b.w;
         t = c.x; h = c.y; mu = c.z; attempts = __double_as_longlong(c.w);
-        st = d.x; flags = d.y; n_acc = d.z; n_rej = d.w; n_forced = g.x; jn = g.z;
+        st = d.x; flags = d.y; n_acc = d.z; n_rej = d.w; n_forced = g.x; jn = g.z; pid = g.w;
       }
       bool running = active;                     // false once finished or parked
       bool first_chunk = true;
@@ -673,13 +718,13 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
       }
       // write the tile back
       if (active) {
-        double* r = sc.rec + (pid - w0) * kRecDoubles;
+        double* r = sc.rec + (long long)li * kRecDoubles;
         const int hb = home_bin(f.ns, y[0]);
         stcg4(r, make_double4(y[0], y[1], y[2], y[3]));
         stcg4(r + 4, make_double4(kb(0, 0), kb(0, 1), kb(0, 2), kb(0, 3)));
         stcg4(r + 8, make_double4(t, h, mu, __longlong_as_double(attempts)));
         __stcg(reinterpret_cast<int4*>(r + 12), make_int4(st, flags, n_acc, n_rej));
-        __stcg(reinterpret_cast<int4*>(r + 12) + 1, make_int4(n_forced, hb, jn, 0));
+        __stcg(reinterpret_cast<int4*>(r + 12) + 1, make_int4(n_forced, hb, jn, (int)pid));
         if (st == kStRunning) atomicAdd(sc.cnt + hb, 1);
       }
       __syncthreads();                                                   // window / kbuf / s_int are reused
@@ -687,31 +732,11 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
     grid.sync();
   }
 
-  // ---- outputs (coalesced) -------------------------------------------------------------------------------------
-  // (the thread that reads record i - w0 here is the one that overwrites it in P0 of the next wave: no barrier needed)
+  // ---- the particles still in the slots -----------------------------------------------------------------------------
   if (mode == 0) {
-    for (long long i = w0 + gtid; i < w1; i += gthreads) {
-      const double* r = sc.rec + (i - w0) * kRecDoubles;
-      const int4 d = __ldcg(reinterpret_cast<const int4*>(r + 12));
-      if (d.x == kStSkip) continue;
-      const double4 a = ldcg4(r);
-      const double4 c = ldcg4(r + 8);
-      const int4 g = __ldcg(reinterpret_cast<const int4*>(r + 12) + 1);
-      const int n_forced = g.x;
-      if constexpr (SAMPLE) { if (p.sample_end) p.sample_end[i] = g.z; }
-      p.y_out[i] = a.x;
-      p.y_out[p.n + i] = a.y;
-      p.y_out[2 * p.n + i] = a.z;
-      p.y_out[3 * p.n + i] = a.w * p.v_ref;
-      p.t_out[i] = c.x;
-      p.status[i] = d.x;
-      if (p.h_inout) p.h_inout[i] = c.y;
-      if (p.n_acc) p.n_acc[i] = (p.resume ? p.n_acc[i] : 0) + d.z;
-      if (p.n_rej) p.n_rej[i] = (p.resume ? p.n_rej[i] : 0) + d.w;
-      if (p.n_forced) p.n_forced[i] = (p.resume ? p.n_forced[i] : 0) + n_forced;
-    }
+    for (long long li = gtid; li < S; li += gthreads)
+      if (__ldcg(reinterpret_cast<const int*>(sc.rec + li * kRecDoubles + 12)) >= 0) flush_record(li);
   }
-  }                                                                          // waves
 }
 
 template <int NMAX, bool MODES, bool SAMPLE>

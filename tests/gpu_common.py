@@ -108,8 +108,22 @@ def assert_trace_parity(r_gpu, r_ref, spec, min_same=1.0 - FLIP_FRACTION, label=
     assert rel[stable].max() <= flip_rtol, f"{label}: max rel diff {rel.max():.3e} > {flip_rtol}"
     if same.any():
         assert np.array_equal(r_gpu.n_forced.cpu().numpy()[same], r_ref.n_forced[same])
-    return dict(same_frac=float(same.mean()), max_rel=float(rel[stable].max()), median_rel=float(np.median(rel)),
+    info = dict(same_frac=float(same.mean()), max_rel=float(rel[stable].max()), median_rel=float(np.median(rel)),
                 within=within, max_rel_t=float(relt[stable].max()))
+    record_info("trace_parity", label=label, particles=int(n), unstable_in_oracle=int((~stable).sum()), **info)
+    return info
+
+
+def record_info(kind: str, **kw):
+    """Append one JSON line per comparison to gpurun_out/parity_info.jsonl (scratch that comes back from the GPU box;
+    profiles/r2_parity_summary.md is assembled from it), so that how close each test got is on record."""
+    import json
+    import os
+    out = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    if os.path.isdir(out):
+        test = os.environ.get("PYTEST_CURRENT_TEST", "").split(" ")[0]
+        with open(os.path.join(out, "parity_info.jsonl"), "a") as fh:
+            fh.write(json.dumps(dict(kind=kind, test=test, **kw)) + "\n")
 
 
 def sort_poincare(rec: np.ndarray) -> np.ndarray:

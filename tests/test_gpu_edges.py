@@ -300,6 +300,52 @@ def test_binned_kernels_are_bitwise_reproducible_and_independent_of_the_company(
     assert torch.equal(a.y[:, :5000], c.y) and torch.equal(a.t[:5000], c.t) and torch.equal(a.n_acc[:5000], c.n_acc)
 
 
+@pytest.mark.parametrize("kernel", ["tile", "mma"])
+def test_streaming_through_few_record_slots_changes_nothing(kernel):
+    """GC_OPT_WAVE_PARTICLES: 30,000 particles streamed through 4096 record slots (a finished particle hands its slot
+    to the next unstarted one) give bit for bit the results of one slot per particle -- also for a resumed second
+    segment in which lost particles are passed over, with samples, and for the right-hand side alone."""
+    import torch
+    from paper_2605_16734_b200 import gcorbit as G, workloads as W
+    fld, spec = W.make_field(1), W.make_spec(1)
+    P = W.make_particles(1, 30_000)
+    P.s[::7] = 0.97 + 0.02 * P.s[::7]                       # a good share of early losses (uneven slot turnover)
+    GF = G.Field(fld)
+    GF.set_kernel({"tile": G.GC_KERNEL_TILE, "mma": G.GC_KERNEL_MMA}[kernel])
+    s, th, ze, vp = (to_dev(x) for x in (P.s, P.theta, P.zeta, P.vpar))
+    B, _ = GF.field_eval(s, th, ze, derivs=False)
+    mu = to_dev(0.5 * spec.mass * P.vperp2()) / B
+
+    def two_segments():
+        h = torch.zeros(P.n, dtype=torch.float64, device="cuda:0")
+        st = GF.trace(spec, s, th, ze, vp, mu, h_inout=h, t0=0.0, t_max=4e-6)
+        first = (st.y.clone(), st.t.clone(), st.status.clone(), st.n_acc.clone())
+        GF.trace_resume(spec, st, mu, t0=4e-6, t_max=6e-6)
+        smp = GF.trace_sampled(spec, s, th, ze, vp, mu, 0.0, 1e-6, 4, t_max=3e-6)
+        y4 = torch.stack([s, th, ze, vp]).contiguous()
+        rhs = GF.rhs_eval(spec.mass, spec.charge, 0.0, y4, mu)
+        torch.cuda.synchronize()
+        return first, st, smp, rhs
+
+    f0, a, sa, ra = two_segments()
+    GF.set_option(G.GC_OPT_WAVE_PARTICLES, 4096)
+    f1, b, sb, rb = two_segments()
+    GF.set_option(G.GC_OPT_WAVE_PARTICLES, 0)
+    lost = int((f0[2] == 1).sum())
+    assert 1000 < lost < 20_000                             # the resumed call really passes particles over
+    for x, y in zip(f0, f1):
+        assert torch.equal(x, y)
+    for name in ("y", "t", "status", "n_acc", "n_rej", "n_forced", "h"):
+        assert torch.equal(getattr(a, name), getattr(b, name)), name
+    assert torch.equal(sa.sample_end, sb.sample_end)
+    assert torch.equal(torch.nan_to_num(sa.samples, nan=-7.0), torch.nan_to_num(sb.samples, nan=-7.0))
+    assert torch.equal(ra, rb)
+    with pytest.raises(G.GcError):
+        GF.set_option(G.GC_OPT_WAVE_PARTICLES, 100)
+    with pytest.raises(G.GcError):
+        GF.set_option(77, 1)
+
+
 @pytest.mark.parametrize("kernel", ["generic", "warp", "tile", "mma"])
 def test_refined_loss_point_matches_oracle(kernel):
     """GC_TRACE_REFINE_LOSS (O7b): lost particles report the crossing of s_loss on the continuous extension; the

@@ -173,9 +173,10 @@ def test_trace_ragged_sizes(cases, n, kernel):
     assert_trace_parity(r, o, spec, min_same=0.0 if n < 100 else 0.99, label=f"n={n}", cond=cond)
 
 
-@pytest.mark.parametrize("config,n_full,seg", [(1, 100_000, 2e-5), (3, 1_000_000, 4e-6), (4, 1_000_000, 4e-6)])
+@pytest.mark.parametrize("config,n_full,seg", [(1, 100_000, 2e-5), (2, 100_000, 2e-5), (3, 1_000_000, 4e-6),
+                                               (4, 1_000_000, 4e-6)])
 def test_full_size_launch_sampled(cases, config, n_full, seg):
-    """BASELINE.json configs[1], [3] and [4] at FULL size in the launch configuration bench.py times (100,000
+    """BASELINE.json configs[1], [2], [3] and [4] at FULL size in the launch configuration bench.py times (100,000
     particles over 2e-5 s segments; 10^6 particles, shorter segments to keep the test short), in-place resume of a
     second segment; 48 sampled particles (and a few lost ones) checked one by one against the oracle."""
     import torch
@@ -223,6 +224,10 @@ def test_full_size_launch_sampled(cases, config, n_full, seg):
     assert np.median(rel) < 1e-11 and (rel <= np.maximum(SAME_RTOL, COND_FACTOR * spread)).all(), rel.max()
     relt = np.abs(st.t.cpu().numpy()[idx] - t_ref) / t_ref
     assert (relt <= np.maximum(SAME_RTOL, COND_FACTOR * tspread)).all(), relt.max()
+    from gpu_common import record_info
+    record_info("full_size_sampled", label=f"config {config} mma, {n_full} particles, 2 x {seg:g} s", particles=len(idx),
+                max_rel=float(rel.max()), median_rel=float(np.median(rel)), within=float((rel <= SAME_RTOL).mean()),
+                max_rel_t=float(relt.max()), waves=-(-n_full // (1 << 18)))
 
 
 @pytest.mark.parametrize("kernel", ["tile", "mma"])

@@ -67,6 +67,8 @@ def parse_args():
     ap.add_argument("--samples", type=int, default=0, help="NEXT-1: uniform-time samples per segment recorded by "
                     "gc_trace_sampled (0 = plain gc_trace, the default line); adds the P_zeta / weighted-Birkhoff "
                     "post-processing time to config")
+    ap.add_argument("--slots", type=int, default=0, help="GC_OPT_WAVE_PARTICLES: record slots of the binned kernels "
+                    "(0 = the library's default, 2^18)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
@@ -241,7 +243,10 @@ def run_cuda(args):
     GF = G.Field(fld)
     if args.kernel != "auto":
         GF.set_kernel({"warp": G.GC_KERNEL_WARP, "generic": G.GC_KERNEL_GENERIC, "tile": G.GC_KERNEL_TILE, "mma": G.GC_KERNEL_MMA}[args.kernel])
+    if args.slots:
+        GF.set_option(G.GC_OPT_WAVE_PARTICLES, args.slots)
     kinfo = GF.kernel_info(n)
+    kinfo["record_slots"] = args.slots if args.slots else "default"
     T = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device=dev)
     s, th, ze, vpar = T(P.s), T(P.theta), T(P.zeta), T(P.vpar)
     Bst, _ = GF.field_eval(s, th, ze, derivs=False)          # mu = m v_perp^2 / (2 B) needs B at the start (A5)
@@ -385,7 +390,7 @@ def run_cuda(args):
     # capture): DRAM bytes per launch and executed FP64 flop per particle-step.  Any other workload: null.
     traffic = executed = cap_src = None
     default_launch = (args.config == DEFAULT_CONFIG and args.particles is None and args.segment == 2e-5 and
-                      kinfo["kernel"] == "mma" and args.samples == 0)
+                      kinfo["kernel"] == "mma" and args.samples == 0 and args.slots == 0)
     tp = os.path.join(ROOT, "profiles", "ncu_constants.json.txt")
     if os.path.exists(tp) and default_launch:
         try:

@@ -37,7 +37,8 @@ class _Desc(C.Structure):
                 ("G", C.c_void_p), ("I", C.c_void_p), ("iota", C.c_void_p),
                 ("psi0", C.c_double), ("nk", C.c_int32),
                 ("mode_m", C.c_void_p), ("mode_n", C.c_void_p),
-                ("mode_omega", C.c_void_p), ("mode_phase", C.c_void_p), ("phihat", C.c_void_p)]
+                ("mode_omega", C.c_void_p), ("mode_phase", C.c_void_p), ("phihat", C.c_void_p),
+                ("bmns", C.c_void_p), ("kmnc", C.c_void_p), ("kmns", C.c_void_p)]
 
 
 class _Params(C.Structure):
@@ -137,14 +138,18 @@ class OracleField:
             iota=_f64(fld.iota), mode_m=_i32(fld.mode_m), mode_n=_i32(fld.mode_n),
             mode_omega=_f64(fld.mode_omega), mode_phase=_f64(fld.mode_phase), phihat=_f64(fld.phihat))
         k = self._keep
+        for name in ("bmns", "kmnc", "kmns"):                      # NEXT-4 tables: absent = None
+            a = getattr(fld, name, None)
+            k[name] = None if a is None else _f64(a)
         self.ns, self.nh, self.nk = int(fld.ns), int(k["xm"].shape[0]), int(k["mode_m"].shape[0])
         assert k["bmnc"].shape == (self.ns, self.nh)
+        assert all(k[nm] is None or k[nm].shape == (self.ns, self.nh) for nm in ("bmns", "kmnc", "kmns"))
         if self.nk:
             assert k["phihat"].shape == (self.ns, self.nk)
         d = _Desc(self.ns, int(fld.nfp), self.nh, _p(k["xm"]), _p(k["xn"]), _p(k["bmnc"]),
                   _p(k["G"]), _p(k["I"]), _p(k["iota"]), float(fld.psi0), self.nk,
                   _p(k["mode_m"]), _p(k["mode_n"]), _p(k["mode_omega"]), _p(k["mode_phase"]),
-                  _p(k["phihat"]))
+                  _p(k["phihat"]), _p(k["bmns"]), _p(k["kmnc"]), _p(k["kmns"]))
         self._h = C.c_void_p(L.oracle_field_create(C.byref(d)))
         if not self._h.value:
             raise ValueError("oracle_field_create rejected the description")
@@ -169,6 +174,18 @@ class OracleField:
         out = np.zeros((s.size, 4))
         for i, (a, b, c) in enumerate(zip(s.ravel(), th.ravel(), ze.ravel())):
             out[i] = self.eval_B(a, b, c)
+        return out
+
+    def eval_K(self, s, th, ze):
+        out = np.zeros(4)
+        _load().oracle_eval_K(self._h, C.c_double(s), C.c_double(th), C.c_double(ze), _p(out))
+        return out
+
+    def rhs_general(self, mass, charge, mu, v_ref, t, y):
+        y = _f64(y)
+        out = np.zeros(4)
+        _load().oracle_rhs_general(self._h, C.c_double(mass), C.c_double(charge), C.c_double(mu),
+                                   C.c_double(v_ref), C.c_double(t), _p(y), _p(out))
         return out
 
     def eval_profiles(self, s):

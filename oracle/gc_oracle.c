@@ -17,6 +17,7 @@ struct oracle_field {
   int32_t ns, nfp, nh, nk;
   int32_t *xm, *xn, *mode_m, *mode_n;
   double *bmnc, *G, *I, *iota, *mode_omega, *mode_phase, *phihat;
+  double *bmns, *kmnc, *kmns;          /* NEXT-4: NULL = absent */
   double psi0;
 };
 
@@ -43,6 +44,10 @@ oracle_field *oracle_field_create(const oracle_field_desc *d) {
     f->mode_phase = (double *)dup_mem(d->mode_phase, sizeof(double) * d->nk);
     f->phihat = (double *)dup_mem(d->phihat, sizeof(double) * (size_t)d->ns * d->nk);
   }
+  size_t tab = sizeof(double) * (size_t)d->ns * d->nh;
+  if (d->bmns) f->bmns = (double *)dup_mem(d->bmns, tab);
+  if (d->kmnc) f->kmnc = (double *)dup_mem(d->kmnc, tab);
+  if (d->kmns) f->kmns = (double *)dup_mem(d->kmns, tab);
   return f;
 }
 
@@ -50,6 +55,7 @@ void oracle_field_destroy(oracle_field *f) {
   if (!f) return;
   free(f->xm); free(f->xn); free(f->bmnc); free(f->G); free(f->I); free(f->iota);
   free(f->mode_m); free(f->mode_n); free(f->mode_omega); free(f->mode_phase); free(f->phihat);
+  free(f->bmns); free(f->kmnc); free(f->kmns);
   free(f);
 }
 
@@ -94,23 +100,46 @@ static void interp(const double *tab, int32_t stride, int32_t i0, const double w
   *val = v; *dval = d;
 }
 
-/* ---- O2: equilibrium field strength and its derivatives ------------------------------------------- */
-void oracle_eval_B(const oracle_field *f, double s, double th, double ze, double out[4]) {
+/* ---- O2: equilibrium field strength and its derivatives -------------------------------------------
+ * One Fourier series  X = sum_k [ xc_k(s) cos(ang_k) + xs_k(s) sin(ang_k) ],  ang_k = m_k theta - n_k nfp zeta, and
+ * its derivatives in s, theta, zeta; either table may be NULL.  One libm cos + sin per harmonic, index order. */
+static void eval_series(const oracle_field *f, const double *tabc, const double *tabs,
+                        double s, double th, double ze, double out[4]) {
   int32_t i0; double w[4], dw[4];
   oracle_lagrange(f->ns, s, &i0, w, dw);
-  double B = 0.0, Bs = 0.0, Bth = 0.0, Bze = 0.0;
+  double X = 0.0, Xs = 0.0, Xth = 0.0, Xze = 0.0;
   for (int k = 0; k < f->nh; ++k) {
-    double b, bs;
-    interp(f->bmnc + k, f->nh, i0, w, dw, &b, &bs);
     double m = (double)f->xm[k], nn = (double)f->xn[k] * (double)f->nfp;
     double ang = m * th - nn * ze;
     double c = cos(ang), sn = sin(ang);
-    B += b * c;
-    Bs += bs * c;
-    Bth += -m * b * sn;
-    Bze += nn * b * sn;
+    if (tabc) {
+      double b, bs;
+      interp(tabc + k, f->nh, i0, w, dw, &b, &bs);
+      X += b * c;
+      Xs += bs * c;
+      Xth += -m * b * sn;
+      Xze += nn * b * sn;
+    }
+    if (tabs) {                                    /* NEXT-4: the terms stellarator symmetry forbids */
+      double b, bs;
+      interp(tabs + k, f->nh, i0, w, dw, &b, &bs);
+      X += b * sn;
+      Xs += bs * sn;
+      Xth += m * b * c;
+      Xze += -nn * b * c;
+    }
   }
-  out[0] = B; out[1] = Bs; out[2] = Bth; out[3] = Bze;
+  out[0] = X; out[1] = Xs; out[2] = Xth; out[3] = Xze;
+}
+
+void oracle_eval_B(const oracle_field *f, double s, double th, double ze, double out[4]) {
+  eval_series(f, f->bmnc, f->bmns, s, th, ze, out);
+}
+
+/* NEXT-4: the covariant radial component K(s, theta, zeta) of B = G grad zeta + I grad theta + K grad psi. */
+void oracle_eval_K(const oracle_field *f, double s, double th, double ze, double out[4]) {
+  if (!f->kmnc && !f->kmns) { out[0] = out[1] = out[2] = out[3] = 0.0; return; }
+  eval_series(f, f->kmnc, f->kmns, s, th, ze, out);
 }
 
 void oracle_eval_profiles(const oracle_field *f, double s, double out[6]) {
@@ -162,6 +191,7 @@ void oracle_eval_pert(const oracle_field *f, double s, double th, double ze, dou
  * rho_c = m v/(q B) + alpha, H = m v^2/2 + mu B + q Phi, chi' = iota, covariant radial component dropped. */
 void oracle_rhs(const oracle_field *f, double mass, double charge, double mu, double v_ref,
                 double t, const double y[4], double dydt[4]) {
+  if (f->kmnc || f->kmns) { oracle_rhs_general(f, mass, charge, mu, v_ref, t, y, dydt); return; }
   double s = y[0], th = y[1], ze = y[2], v = y[3] * v_ref;
   double fb[4], pr[6], pt[9];
   oracle_eval_B(f, s, th, ze, fb);
@@ -194,6 +224,70 @@ void oracle_rhs(const oracle_field *f, double mass, double charge, double mu, do
   dydt[1] = thdot;
   dydt[2] = zedot;
   dydt[3] = mvdot / mass / v_ref;
+}
+
+/* ---- O4, general form (NEXT-4: K kept) ---------------------------------------------------------------
+ * z = (psi, theta, zeta, v).  A*_psi = rho_c K, A*_theta = psi + rho_c I, A*_zeta = rho_c G - chi, A*_v = 0
+ * (all times q).  omega_ij = d_i A*_j - d_j A*_i.  Equations: q sum_j omega_ij zdot_j = d_i H + q d_t A*_i with
+ * H = m v^2/2 + mu B + q Phi.  K_psi never appears (d_psi A*_psi cancels). */
+void oracle_rhs_general(const oracle_field *f, double mass, double charge, double mu, double v_ref,
+                        double t, const double y[4], double dydt[4]) {
+  double s = y[0], th = y[1], ze = y[2], v = y[3] * v_ref;
+  double fb[4], fk[4], pr[6], pt[9];
+  oracle_eval_B(f, s, th, ze, fb);
+  oracle_eval_K(f, s, th, ze, fk);
+  oracle_eval_profiles(f, s, pr);
+  oracle_eval_pert(f, s, th, ze, t, pt);
+  double psi0 = f->psi0, q = charge;
+  double B = fb[0];
+  double dB[3] = {fb[1] / psi0, fb[2], fb[3]};                 /* d/dpsi, d/dtheta, d/dzeta */
+  double K = fk[0], dK[3] = {fk[1] / psi0, fk[2], fk[3]};
+  double G = pr[0], Gp = pr[1] / psi0, I = pr[2], Ip = pr[3] / psi0, iota = pr[4];
+  double dPhi[3] = {pt[1], pt[2], pt[3]};
+  double al = pt[4], dal[3] = {pt[5], pt[6], pt[7]}, al_t = pt[8];
+  double rho = mass * v / (q * B), rho_c = rho + al;
+  double r[3], rv = mass / (q * B);                            /* d rho_c / d(psi, theta, zeta), d rho_c / dv */
+  for (int x = 0; x < 3; ++x) r[x] = -rho * dB[x] / B + dal[x];
+  /* dA[i][j] = d A*_j / d z_i  (i, j over psi, theta, zeta, v) */
+  double dA[4][4];
+  for (int i = 0; i < 3; ++i) {
+    dA[i][0] = r[i] * K + rho_c * dK[i];
+    dA[i][1] = r[i] * I + (i == 0 ? 1.0 + rho_c * Ip : 0.0);
+    dA[i][2] = r[i] * G + (i == 0 ? rho_c * Gp - iota : 0.0);
+    dA[i][3] = 0.0;
+  }
+  dA[3][0] = rv * K; dA[3][1] = rv * I; dA[3][2] = rv * G; dA[3][3] = 0.0;
+  double Mx[4][5];
+  for (int i = 0; i < 4; ++i)
+    for (int j = 0; j < 4; ++j) Mx[i][j] = q * (dA[i][j] - dA[j][i]);
+  double At[3] = {al_t * K, al_t * I, al_t * G};               /* d A*_i / dt */
+  for (int i = 0; i < 3; ++i) Mx[i][4] = mu * dB[i] + q * dPhi[i] + q * At[i];
+  Mx[3][4] = mass * v;
+  /* Gaussian elimination with partial pivoting on rows scaled to unit maximum */
+  for (int i = 0; i < 4; ++i) {
+    double big = 0.0;
+    for (int j = 0; j < 4; ++j) big = fmax(big, fabs(Mx[i][j]));
+    for (int j = 0; j < 5; ++j) Mx[i][j] /= big;
+  }
+  for (int c = 0; c < 4; ++c) {
+    int piv = c;
+    for (int i = c + 1; i < 4; ++i) if (fabs(Mx[i][c]) > fabs(Mx[piv][c])) piv = i;
+    for (int j = 0; j < 5; ++j) { double tmp = Mx[c][j]; Mx[c][j] = Mx[piv][j]; Mx[piv][j] = tmp; }
+    for (int i = c + 1; i < 4; ++i) {
+      double fct = Mx[i][c] / Mx[c][c];
+      for (int j = c; j < 5; ++j) Mx[i][j] -= fct * Mx[c][j];
+    }
+  }
+  double zd[4];
+  for (int i = 3; i >= 0; --i) {
+    double acc = Mx[i][4];
+    for (int j = i + 1; j < 4; ++j) acc -= Mx[i][j] * zd[j];
+    zd[i] = acc / Mx[i][i];
+  }
+  dydt[0] = zd[0] / psi0;
+  dydt[1] = zd[1];
+  dydt[2] = zd[2];
+  dydt[3] = zd[3] / v_ref;
 }
 
 /* ---- O5: Dormand-Prince 5(4), FSAL ---------------------------------------------------- */

@@ -36,6 +36,11 @@ typedef struct {
   const int32_t *mode_m, *mode_n;          /* [nk]; phase m*theta - n*zeta + omega*t + phase */
   const double *mode_omega, *mode_phase;   /* [nk]                                          */
   const double *phihat;        /* [ns][nk] node-major, volts                               */
+  /* NEXT-4 of SURVEY.md section 8(f) (field model of PAPER.md:44 without stellarator symmetry and with the covariant
+   * radial component kept); each may be NULL (= zero): */
+  const double *bmns;          /* [ns][nh] sin coefficients of B:  B += bmns sin(m theta - n nfp zeta)            */
+  const double *kmnc, *kmns;   /* [ns][nh] covariant radial component K (B = G grad zeta + I grad theta + K grad psi),
+                                  T/m ... in units of T m / (T m^2) = 1/m: K = sum kmnc cos + kmns sin            */
 } oracle_field_desc;
 
 typedef struct oracle_field oracle_field;
@@ -63,6 +68,8 @@ void oracle_lagrange(int32_t ns, double s, int32_t *i0, double w[4], double dw[4
 
 /* O2: out = {B, dB/ds, dB/dtheta, dB/dzeta}. */
 void oracle_eval_B(const oracle_field *f, double s, double th, double ze, double out[4]);
+/* NEXT-4: covariant radial component, out = {K, dK/ds, dK/dtheta, dK/dzeta} (all zero without K tables). */
+void oracle_eval_K(const oracle_field *f, double s, double th, double ze, double out[4]);
 /* O1 on profiles: out = {G, dG/ds, I, dI/ds, iota, diota/ds}. */
 void oracle_eval_profiles(const oracle_field *f, double s, double out[6]);
 /* O3: out = {Phi, Phi_psi, Phi_theta, Phi_zeta, alpha, alpha_psi, alpha_theta, alpha_zeta, alpha_t}. */
@@ -71,6 +78,14 @@ void oracle_eval_pert(const oracle_field *f, double s, double th, double ze, dou
 /* O4: y = (s, theta, zeta, u = v_par/v_ref); dydt likewise. */
 void oracle_rhs(const oracle_field *f, double mass, double charge, double mu, double v_ref,
                 double t, const double y[4], double dydt[4]);
+
+/* O4 in its general form (NEXT-4): the Euler-Lagrange equations of
+ *   L = q rho_c K psidot + q (psi + rho_c I) thetadot + q (rho_c G - chi) zetadot - H
+ * written as the 4 x 4 antisymmetric system  sum_j omega_ij zdot_j = dH/dz_i + q dA*_i/dt  (z = psi, theta, zeta,
+ * v_par) and solved by Gaussian elimination.  oracle_rhs uses this form whenever the field has K tables; for K = 0
+ * it equals the closed form of oracle_rhs (pinned). */
+void oracle_rhs_general(const oracle_field *f, double mass, double charge, double mu, double v_ref,
+                        double t, const double y[4], double dydt[4]);
 
 /* O5: one Dormand-Prince attempt of size h from (t, y) with k1 = f(t, y) given.
  * Outputs y_new (5th order), k[7][4] (k[0] = k1 copied, k[6] = f(t+h, y_new)), delta[4] (embedded error). */

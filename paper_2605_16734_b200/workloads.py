@@ -47,6 +47,10 @@ class Field:
     mode_omega: np.ndarray = _dc_field(default_factory=lambda: np.zeros(0))
     mode_phase: np.ndarray = _dc_field(default_factory=lambda: np.zeros(0))
     phihat: np.ndarray = _dc_field(default_factory=lambda: np.zeros((0, 0)))   # [ns][nk], volts
+    # NEXT-4 of SURVEY.md section 8(f): tables that stellarator symmetry and the K = 0 reading leave out (None = absent)
+    bmns: np.ndarray | None = None      # [ns][nh] sin coefficients of B
+    kmnc: np.ndarray | None = None      # [ns][nh] cos coefficients of the covariant radial component K
+    kmns: np.ndarray | None = None      # [ns][nh] sin coefficients of K
 
     @property
     def nh(self) -> int:

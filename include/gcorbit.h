@@ -36,6 +36,12 @@ typedef struct gc_field gc_field;   /* opaque; owns the device copies of all tab
  *   radial grid s_j = j/(ns-1), j = 0..ns-1; cubic (4-point) Lagrange interpolation in s (O1)
  *   perturbation  Phi = sum_k phihat[.][k](s) sin(mode_m th - mode_n ze + mode_omega t + mode_phase),
  *   alpha from Phi by the ideal-MHD constraint E_par = 0 (O3).
+ * NEXT-4 of SURVEY.md section 8(f) (the field model of PAPER.md:44 without stellarator symmetry and with the covariant
+ * radial component kept); each of the three tables may be NULL (= zero):
+ *   B += sum_k bmns[.][k](s) sin(xm[k] th - xn[k] nfp ze)
+ *   K  = sum_k kmnc[.][k](s) cos(xm[k] th - xn[k] nfp ze) + kmns[.][k](s) sin(...)   in B = G grad zeta + I grad theta
+ *        + K grad psi; with K the equations of motion are the general Euler-Lagrange form.
+ * Fields with any of the three are traced by the mma kernel (large ensembles) or the generic kernel.
  * Harmonic lists may come in any order; duplicate (m, n) pairs add.  Requires xm >= 0. */
 typedef struct {
   int32_t ns;                 /* radial nodes, >= 4                                             */
@@ -54,6 +60,9 @@ typedef struct {
   const double* mode_omega;   /* [nk] rad/s, nonzero                                            */
   const double* mode_phase;   /* [nk] rad                                                       */
   const double* phihat;       /* [ns][nk] node-major, volts                                     */
+  const double* bmns;         /* [ns][nh] node-major sin coefficients of B, tesla, or NULL      */
+  const double* kmnc;         /* [ns][nh] node-major cos coefficients of K, 1/m (T m / (T m^2)), or NULL */
+  const double* kmns;         /* [ns][nh] node-major sin coefficients of K, or NULL             */
 } gc_field_desc;
 
 /* Integrator specification (O5-O8).  The state integrated is (s, theta, zeta, v_par/v_ref). */
@@ -112,6 +121,11 @@ int gc_field_destroy(gc_field* f);
  * Asynchronous on `stream` (a cudaStream_t, NULL = default stream).  Used to compute mu and by tests. */
 int gc_field_eval(const gc_field* f, int64_t n, const double* s, const double* th, const double* ze,
                   double* B, double* dB, void* stream);
+
+/* The covariant radial component K at n points (NEXT-4), same layout as gc_field_eval: K [n]; dK [3][n] = dK/ds,
+ * dK/dtheta, dK/dzeta, or NULL.  All zero for a field without K tables. */
+int gc_kcov_eval(const gc_field* f, int64_t n, const double* s, const double* th, const double* ze,
+                 double* K, double* dK, void* stream);
 
 /* O3 at n points and time t.  DEVICE pointers.  out [9][n] = Phi, Phi_psi, Phi_theta, Phi_zeta, alpha,
  * alpha_psi, alpha_theta, alpha_zeta, alpha_t.  All zero for a static field. */

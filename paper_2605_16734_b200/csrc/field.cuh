@@ -21,6 +21,10 @@ struct FieldDev {
   const double* inv_omega;  // [nk] 1 / omega (mma kernel: no division per mode and right-hand side)
   const double* phase;   // [nk]
   const double* phihat;  // [ns][nk]
+  // NEXT-4: sin coefficients of B and the covariant radial component K (nullptr = absent), [ns][nh] each
+  const double* bmns;
+  const double* kmnc;
+  const double* kmns;
   // packed by-node layout of the warp kernel (kernels_warp.cuh): rows[node][it][lane]
   const double* rows;
   int M, N;              // max xm, max |xn|
@@ -35,6 +39,10 @@ struct FieldDev {
   // at either end); a row holds the DMMA B fragments (P, Q)(m >= 1, n >= 1), b(m, 0), b(0, n), G, I, iota, modes
   const double* mma_image;
   int mma_RS, mma_MT, mma_KS;
+  // NEXT-4: images of the same row layout (fragments, b(m, 0), b(0, n) only) for bmns, kmnc, kmns; nullptr = absent
+  const double* mma_image_bs;
+  const double* mma_image_kc;
+  const double* mma_image_ks;
 };
 
 // Integrator parameters as the kernels see them (gc_trace_params + derived values).

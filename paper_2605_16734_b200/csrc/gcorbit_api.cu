@@ -74,6 +74,7 @@ struct gc_field {
   int chunk_attempts = 0;           // GC_OPT_CHUNK_ATTEMPTS (0 = the kernel's default)
   std::atomic<bool> host_busy{false};   // gc_trace_host is not re-entrant on one field: overlapping calls get GC_EINVAL
   bool mma_ok = false;
+  bool extra = false;               // NEXT-4 tables present (bmns, kmnc or kmns): mma or generic kernel only
   int mma_smem = 0;                 // dynamic shared memory of the mma kernel
   int mma_blocks_per_sm = 0;
 };
@@ -141,7 +142,7 @@ int pack_rows(gc_field* f, const gc_field_desc* d) {
   gc::FieldDev& v = f->dev;
   const int M = v.M, N = v.N;
   f->warp_ok = false;
-  if (N > gc::kMaxN || M > 28) return GC_OK;
+  if (N > gc::kMaxN || M > 28 || f->extra) return GC_OK;
   int cl_log = 5;
   if (N > 0) {
     cl_log = 1;
@@ -207,6 +208,8 @@ const void* tile_fn(const gc_field* f, bool sample = false) { return sample ? ti
 template <bool SAMPLE>
 const void* mma_fn_t(const gc_field* f) {
   const bool modes = f->dev.nk > 0;
+  if (f->extra)                                            // NEXT-4 tables: the 16/16 layout with the extra sweeps
+    return modes ? (const void*)gc::trace_mma_kernel<2, 4, true, SAMPLE, true> : (const void*)gc::trace_mma_kernel<2, 4, false, SAMPLE, true>;
   if (f->dev.mma_MT == 1)
     return modes ? (const void*)gc::trace_mma_kernel<1, 2, true, SAMPLE> : (const void*)gc::trace_mma_kernel<1, 2, false, SAMPLE>;
   return modes ? (const void*)gc::trace_mma_kernel<2, 4, true, SAMPLE> : (const void*)gc::trace_mma_kernel<2, 4, false, SAMPLE>;
@@ -226,7 +229,7 @@ int resolve_kernel(const gc_field* f, int64_t n) {
 int pack_tile_images(gc_field* f, const gc_field_desc* d) {
   gc::FieldDev& v = f->dev;
   f->tile_ok = false;
-  if (v.N > 16) return GC_OK;
+  if (v.N > 16 || f->extra) return GC_OK;
   const int nmax = v.N <= 8 ? 8 : 16;
   const int rowlen = 1 + 2 * nmax;
   const int E = (v.M + 1) * rowlen + 3 + d->nk;
@@ -290,22 +293,28 @@ int pack_tile_images(gc_field* f, const gc_field_desc* d) {
 
 // image[ns + 4][RS] of the mma kernel (kernels_mma.cuh): image row = node + 2; per row the DMMA B fragments
 // (P, Q)(m, n) in lane order, then b(m, 0), b(0, n), G, I, iota and the mode amplitudes.
+// `tab` = bmnc (with profiles and modes) or one of the NEXT-4 tables (series coefficients only; sin_table: the
+// entries multiply sin(m th - n nfp ze), so b(0, -n) enters the m = 0 row with the opposite sign).
 template <int MT, int KS>
-void fill_mma_rows(const gc_field_desc* d, int RS, std::vector<double>& img) {
+void fill_mma_rows(const gc_field_desc* d, int RS, std::vector<double>& img, const double* tab = nullptr,
+                   bool sin_table = false) {
   using R = gc::MmaRow<MT, KS>;
+  const bool main_table = tab == nullptr;
+  if (main_table) tab = d->bmnc;
   for (int node = 0; node < d->ns; ++node) {
     double* row = img.data() + (size_t)(node + 2) * RS;
     for (int k = 0; k < d->nh; ++k) {
       const int m = d->xm[k], n = d->xn[k];
-      const double b = d->bmnc[(size_t)node * d->nh + k];
+      const double b = tab[(size_t)node * d->nh + k];
       const int an = n > 0 ? n : -n;
-      if (m == 0) { row[R::kM0 + an] += b; continue; }
+      if (m == 0) { row[R::kM0 + an] += (sin_table && n < 0) ? -b : b; continue; }
       if (n == 0) { row[R::kN0 + m - 1] += b; continue; }
       const int T = (m - 1) / 8, g = (m - 1) % 8, j = (an - 1) / 4, q = (an - 1) % 4;
       double* e = row + R::kFrag + ((size_t)(T * KS + j) * 32 + 4 * g + q) * 2;
       e[0] += b;                                           // P = b(m,n) + b(m,-n)
       e[1] += n > 0 ? b : -b;                              // Q = b(m,n) - b(m,-n)
     }
+    if (!main_table) continue;
     row[R::kProf] = d->G[node]; row[R::kProf + 1] = d->I[node]; row[R::kProf + 2] = d->iota[node];
     for (int k = 0; k < d->nk; ++k) row[R::kModes + k] = d->phihat[(size_t)node * d->nk + k];
   }
@@ -315,7 +324,7 @@ int pack_mma_image(gc_field* f, const gc_field_desc* d) {
   gc::FieldDev& v = f->dev;
   f->mma_ok = false;
   if (v.N > 16 || v.M > 16) return GC_OK;
-  const bool small = v.M <= 8 && v.N <= 8;
+  const bool small = v.M <= 8 && v.N <= 8 && !f->extra;
   const int MT = small ? 1 : 2, KS = small ? 2 : 4;
   const int RS = small ? gc::MmaRow<1, 2>::stride(d->nk) : gc::MmaRow<2, 4>::stride(d->nk);
   const int smem = (int)((size_t)gc::kMmaWinRows * RS * sizeof(double) + (size_t)(7 * 4 + 2 * gc::kMmaWtab) * gc::kMmaThreads * sizeof(double) + 64);
@@ -330,6 +339,18 @@ int pack_mma_image(gc_field* f, const gc_field_desc* d) {
   f->allocs.push_back(dev_img);
   v.mma_image = dev_img;
   v.mma_RS = RS; v.mma_MT = MT; v.mma_KS = KS;
+  const double* extra_tab[3] = {d->bmns, d->kmnc, d->kmns};
+  const double** extra_dst[3] = {&v.mma_image_bs, &v.mma_image_kc, &v.mma_image_ks};
+  for (int x = 0; x < 3; ++x) {
+    if (!extra_tab[x]) continue;
+    std::vector<double> ximg((size_t)(d->ns + 4) * RS, 0.0);
+    fill_mma_rows<2, 4>(d, RS, ximg, extra_tab[x], x != 1);
+    double* dev_x = nullptr;
+    rc = upload(ximg.data(), ximg.size(), &dev_x);
+    if (rc != GC_OK) return rc;
+    f->allocs.push_back(dev_x);
+    *extra_dst[x] = dev_x;
+  }
   f->mma_smem = smem;
   const void* fn = mma_fn(f);
   GC_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, kBinnedSmemCap));
@@ -465,6 +486,9 @@ int gc_field_create(const gc_field_desc* d, gc_field** out) {
   if (!all_finite(d->bmnc, (size_t)d->ns * d->nh) || !all_finite(d->G, d->ns) || !all_finite(d->I, d->ns) ||
       !all_finite(d->iota, d->ns))
     return fail(GC_EINVAL, "gc_field_create: non-finite value in an equilibrium table");
+  for (const double* x : {d->bmns, d->kmnc, d->kmns})
+    if (x && !all_finite(x, (size_t)d->ns * d->nh))
+      return fail(GC_EINVAL, "gc_field_create: non-finite value in bmns, kmnc or kmns");
   int M = 0, N = 0;
   for (int k = 0; k < d->nh; ++k) {
     if (d->xm[k] < 0) return fail(GC_EINVAL, "gc_field_create: xm < 0");
@@ -495,7 +519,11 @@ int gc_field_create(const gc_field_desc* d, gc_field** out) {
     if (rc == GC_OK && *devp) f->allocs.push_back((void*)*devp);
   };
   int *xm, *xn, *mm, *mn;
-  double *bmnc, *G, *I, *iota, *om, *ph, *phihat;
+  double *bmnc, *G, *I, *iota, *om, *ph, *phihat, *bmns = nullptr, *kmnc = nullptr, *kmns = nullptr;
+  f->extra = d->bmns || d->kmnc || d->kmns;
+  if (d->bmns) up(d->bmns, (size_t)d->ns * d->nh, &bmns);
+  if (d->kmnc) up(d->kmnc, (size_t)d->ns * d->nh, &kmnc);
+  if (d->kmns) up(d->kmns, (size_t)d->ns * d->nh, &kmns);
   up(d->xm, d->nh, &xm); up(d->xn, d->nh, &xn); up(d->bmnc, (size_t)d->ns * d->nh, &bmnc);
   up(d->G, d->ns, &G); up(d->I, d->ns, &I); up(d->iota, d->ns, &iota);
   up(d->mode_m, d->nk, &mm); up(d->mode_n, d->nk, &mn); up(d->mode_omega, d->nk, &om);
@@ -507,6 +535,7 @@ int gc_field_create(const gc_field_desc* d, gc_field** out) {
   if (rc == GC_OK) {
     v.xm = xm; v.xn = xn; v.bmnc = bmnc; v.G = G; v.I = I; v.iota = iota;
     v.mode_m = mm; v.mode_n = mn; v.omega = om; v.inv_omega = iom; v.phase = ph; v.phihat = phihat;
+    v.bmns = bmns; v.kmnc = kmnc; v.kmns = kmns;
     rc = pack_rows(f, d);
   }
   if (rc == GC_OK) rc = pack_tile_images(f, d);
@@ -548,9 +577,9 @@ int gc_field_create(const gc_field_desc* d, gc_field** out) {
 int gc_set_kernel(gc_field* f, int32_t kernel) {
   if (!f) return fail(GC_EINVAL, "gc_set_kernel: NULL field");
   if (kernel == GC_KERNEL_WARP && !f->warp_ok)
-    return fail(GC_EINVAL, "gc_set_kernel: field does not fit the warp kernel (max|xn| <= 16, max xm <= 28)");
+    return fail(GC_EINVAL, "gc_set_kernel: field does not fit the warp kernel (max|xn| <= 16, max xm <= 28, no bmns / kmnc / kmns)");
   if (kernel == GC_KERNEL_TILE && !f->tile_ok)
-    return fail(GC_EINVAL, "gc_set_kernel: field does not fit the tile kernel (max|xn| <= 16, window <= 110 KB)");
+    return fail(GC_EINVAL, "gc_set_kernel: field does not fit the tile kernel (max|xn| <= 16, window <= 110 KB, no bmns / kmnc / kmns)");
   if (kernel == GC_KERNEL_MMA && !f->mma_ok)
     return fail(GC_EINVAL, "gc_set_kernel: field does not fit the mma kernel (max|xn| <= 16, max xm <= 16)");
   if (kernel != GC_KERNEL_AUTO && kernel != GC_KERNEL_WARP && kernel != GC_KERNEL_GENERIC && kernel != GC_KERNEL_TILE &&
@@ -614,6 +643,17 @@ int gc_field_eval(const gc_field* f, int64_t n, const double* s, const double* t
   if (!s || !th || !ze || !B) return fail(GC_EINVAL, "gc_field_eval: NULL array");
   const int tb = 128;
   gc::field_eval_kernel<<<(unsigned)((n + tb - 1) / tb), tb, 0, (cudaStream_t)stream>>>(f->dev, n, s, th, ze, B, dB);
+  GC_CUDA(cudaGetLastError());
+  return GC_OK;
+}
+
+int gc_kcov_eval(const gc_field* f, int64_t n, const double* s, const double* th, const double* ze, double* K,
+                 double* dK, void* stream) {
+  if (!f || n < 0) return fail(GC_EINVAL, "gc_kcov_eval: NULL field or n < 0");
+  if (n == 0) return GC_OK;
+  if (!s || !th || !ze || !K) return fail(GC_EINVAL, "gc_kcov_eval: NULL array");
+  const int tb = 128;
+  gc::kcov_eval_kernel<<<(unsigned)((n + tb - 1) / tb), tb, 0, (cudaStream_t)stream>>>(f->dev, n, s, th, ze, K, dK);
   GC_CUDA(cudaGetLastError());
   return GC_OK;
 }

@@ -19,23 +19,40 @@ __device__ __forceinline__ void interp4(const double* tab, int stride, int i0, c
   d = fma(dw[3], t3, fma(dw[2], t2, fma(dw[1], t1, dw[0] * t0)));
 }
 
-__device__ inline void eval_B_generic(const FieldDev& f, int i0, const double w[4], const double dw[4],
-                                      double th, double ze, double out[4]) {
+// One Fourier series X = sum_k [ xc_k(s) cos(a_k) + xs_k(s) sin(a_k) ], a_k = m_k theta - n_k nfp zeta, with its
+// derivatives in s, theta, zeta; either table may be nullptr (NEXT-4: the sin table of B, both tables of K).
+__device__ inline void eval_series_generic(const FieldDev& f, const double* tabc, const double* tabs, int i0,
+                                           const double w[4], const double dw[4], double th, double ze, double out[4]) {
   const double thr = reduce_2pi(th);
   const double phr = reduce_2pi((double)f.nfp * ze);
   double B = 0.0, Bs = 0.0, Bth = 0.0, Bze = 0.0;
   for (int k = 0; k < f.nh; ++k) {
-    double b, bs;
-    interp4(f.bmnc + k, f.nh, i0, w, dw, b, bs);
     const double m = (double)__ldg(f.xm + k), n = (double)__ldg(f.xn + k);
     double sn, cs;
     sincos_poly(fma(m, thr, -n * phr), sn, cs);
-    B = fma(b, cs, B);
-    Bs = fma(bs, cs, Bs);
-    Bth = fma(-m * b, sn, Bth);
-    Bze = fma(n * (double)f.nfp * b, sn, Bze);
+    if (tabc) {
+      double b, bs;
+      interp4(tabc + k, f.nh, i0, w, dw, b, bs);
+      B = fma(b, cs, B);
+      Bs = fma(bs, cs, Bs);
+      Bth = fma(-m * b, sn, Bth);
+      Bze = fma(n * (double)f.nfp * b, sn, Bze);
+    }
+    if (tabs) {
+      double b, bs;
+      interp4(tabs + k, f.nh, i0, w, dw, b, bs);
+      B = fma(b, sn, B);
+      Bs = fma(bs, sn, Bs);
+      Bth = fma(m * b, cs, Bth);
+      Bze = fma(-n * (double)f.nfp * b, cs, Bze);
+    }
   }
   out[0] = B; out[1] = Bs; out[2] = Bth; out[3] = Bze;
+}
+
+__device__ inline void eval_B_generic(const FieldDev& f, int i0, const double w[4], const double dw[4],
+                                      double th, double ze, double out[4]) {
+  eval_series_generic(f, f.bmnc, f.bmns, i0, w, dw, th, ze, out);
 }
 
 // out = Phi, Phi_psi, Phi_th, Phi_ze, al, al_psi, al_th, al_ze, al_t
@@ -100,6 +117,36 @@ __device__ __forceinline__ void gc_algebra(double mass, double charge, double mu
   dy[3] = mvdot / mass;
 }
 
+// O4 with the covariant radial component K kept (NEXT-4).  The Euler-Lagrange equations of
+//   L = q [ rho_c K psidot + (psi + rho_c I) thetadot + (rho_c G - chi) zetadot ] - H,   H = m v^2 / 2 + mu B + q Phi,
+// are  sum_j w_ij zdot_j = R_i  (z = psi, theta, zeta, v) with the antisymmetric w_ij = d_i A*_j - d_j A*_i and
+// R_i = d_i H / q + d_t A*_i; a 4 x 4 antisymmetric matrix is inverted in closed form through its Pfaffian:
+//   w^-1 = [[0, -w34, w24, -w23], [w34, 0, -w14, w13], [-w24, w14, 0, -w12], [w23, -w13, w12, 0]] / Pf,
+//   Pf = w12 w34 - w13 w24 + w14 w23.   fk = K, K_s (unused), K_theta, K_zeta.  For K = 0 this is gc_algebra.
+__device__ __forceinline__ void gc_algebra_general(double mass, double charge, double mu, double inv_psi0, double v,
+                                                   const double fb[4], const double fk[4], const Profiles& p,
+                                                   const double pt[9], double dy[4]) {
+  const double B = fb[0], B_psi = fb[1] * inv_psi0, B_th = fb[2], B_ze = fb[3];
+  const double K = fk[0], K_th = fk[2], K_ze = fk[3];
+  const double G = p.G, Gp = p.Gs * inv_psi0, I = p.I, Ip = p.Is * inv_psi0;
+  const double al = pt[4], al_t = pt[8];
+  const double invB = 1.0 / B, invq = 1.0 / charge;
+  const double rv = mass * invB * invq;                    // d rho_c / d v
+  const double rho = rv * v, rho_c = rho + al;
+  const double r_psi = fma(-rho * invB, B_psi, pt[5]), r_th = fma(-rho * invB, B_th, pt[6]),
+               r_ze = fma(-rho * invB, B_ze, pt[7]);
+  const double w12 = 1.0 + r_psi * I + rho_c * Ip - r_th * K - rho_c * K_th;
+  const double w13 = r_psi * G + rho_c * Gp - p.io - r_ze * K - rho_c * K_ze;
+  const double w14 = -rv * K, w23 = r_th * G - r_ze * I, w24 = -rv * I, w34 = -rv * G;
+  const double R1 = fma(mu * invq, B_psi, pt[1]) + al_t * K, R2 = fma(mu * invq, B_th, pt[2]) + al_t * I,
+               R3 = fma(mu * invq, B_ze, pt[3]) + al_t * G, R4 = mass * v * invq;
+  const double invPf = 1.0 / (w12 * w34 - w13 * w24 + w14 * w23);
+  dy[0] = (-w34 * R2 + w24 * R3 - w23 * R4) * invPf * inv_psi0;
+  dy[1] = (w34 * R1 - w14 * R3 + w13 * R4) * invPf;
+  dy[2] = (-w24 * R1 + w14 * R2 - w12 * R4) * invPf;
+  dy[3] = (w23 * R1 - w13 * R2 + w12 * R3) * invPf;
+}
+
 // y = (s, theta, zeta, u = v_par / v_ref); dy in the same scaled variables.
 __device__ inline void rhs_generic(const FieldDev& f, double mass, double charge, double mu, double v_ref,
                                    double inv_v_ref, double t, const double y[4], double dy[4]) {
@@ -117,7 +164,13 @@ __device__ inline void rhs_generic(const FieldDev& f, double mass, double charge
 #pragma unroll
     for (int i = 0; i < 9; ++i) pt[i] = 0.0;
   }
-  gc_algebra(mass, charge, mu, f.inv_psi0, y[3] * v_ref, fb, p, pt, dy);
+  if (f.kmnc || f.kmns) {
+    double fk[4];
+    eval_series_generic(f, f.kmnc, f.kmns, i0, w, dw, y[1], y[2], fk);
+    gc_algebra_general(mass, charge, mu, f.inv_psi0, y[3] * v_ref, fb, fk, p, pt, dy);
+  } else {
+    gc_algebra(mass, charge, mu, f.inv_psi0, y[3] * v_ref, fb, p, pt, dy);
+  }
   dy[3] *= inv_v_ref;
 }
 
@@ -487,6 +540,18 @@ __global__ void field_eval_kernel(FieldDev f, long long n, const double* s, cons
   eval_B_generic(f, i0, w, dw, th[i], ze[i], out);
   B[i] = out[0];
   if (dB) { dB[i] = out[1]; dB[n + i] = out[2]; dB[2 * n + i] = out[3]; }
+}
+
+__global__ void kcov_eval_kernel(FieldDev f, long long n, const double* s, const double* th, const double* ze,
+                                 double* K, double* dK) {
+  const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int i0;
+  double w[4], dw[4], out[4] = {0.0, 0.0, 0.0, 0.0};
+  lagrange_weights(f.ns, s[i], i0, w, dw);
+  if (f.kmnc || f.kmns) eval_series_generic(f, f.kmnc, f.kmns, i0, w, dw, th[i], ze[i], out);
+  K[i] = out[0];
+  if (dK) { dK[i] = out[1]; dK[n + i] = out[2]; dK[2 * n + i] = out[3]; }
 }
 
 __global__ void pert_eval_kernel(FieldDev f, long long n, const double* s, const double* th, const double* ze,

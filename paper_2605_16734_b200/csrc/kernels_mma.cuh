@@ -40,6 +40,8 @@
 #pragma once
 #include <cooperative_groups.h>
 
+#include <type_traits>
+
 #include "device_math.cuh"
 #include "field.cuh"
 #include "kernels_generic.cuh"
@@ -108,7 +110,10 @@ __device__ __forceinline__ void cmul(double a, double b, double c, double d, dou
 // zero, the four stencil weights, zero), off_f = row of its first stencil node in this pass (kMmaNone when it does
 // not take part: weight 0 on every row).  Issues the DMMA and accumulates this lane's share of B, B_s, B_theta,
 // B_zeta / nfp in o[].
-template <int MT, int KS, class Ld>
+// SIN (NEXT-4): the image holds the coefficients of a sin series, b sin(m th - n ph): the caller passes (c_m, s_m)
+// rotated by a quarter period, (s_m, -c_m), which turns the cos sweep into the sin sweep for every m >= 1; only the
+// m = 0 row differs: b(0, n) sin(-n ph) = -b S_n, zeta-derivative -n nfp b C_n.
+template <int MT, int KS, class Ld, bool SIN = false>
 __device__ __forceinline__ void mma_sweep(const double* base, int RS, int r_lo, int r_hi, int off_f,
                                           const double2* wsrc, int lane, int q,
                                           const double (&AC)[KS], const double (&AS)[KS], const double (&AnC)[KS],
@@ -156,12 +161,17 @@ __device__ __forceinline__ void mma_sweep(const double* base, int RS, int r_lo, 
       T3 = fma(s1, QC1, T3); T3 = fma(-c1, PS1, T3);
     }
     // m = 0: b(0,n) C_n and its zeta-derivative, n = 4 j + q + 1 on this lane; n = 0 on lane q = 0
-    double x = (q == 0) ? Ld::ld1(row + R::kM0) : 0.0, xs = 0.0;
+    double x = (!SIN && q == 0) ? Ld::ld1(row + R::kM0) : 0.0, xs = 0.0;
 #pragma unroll
     for (int j = 0; j < KS; ++j) {
       const double b0 = Ld::ld1(row + R::kM0 + 1 + 4 * j + q);
-      x = fma(b0, AC[j], x);
-      xs = fma(b0, AnS[j], xs);
+      if constexpr (SIN) {
+        x = fma(-b0, AS[j], x);
+        xs = fma(b0, AnC[j], xs);
+      } else {
+        x = fma(b0, AC[j], x);
+        xs = fma(b0, AnS[j], xs);
+      }
     }
     T1 += x;
     T3 -= xs;
@@ -174,7 +184,7 @@ __device__ __forceinline__ void mma_sweep(const double* base, int RS, int r_lo, 
 
 // Right-hand side of one lane = one particle (same contract as rhs_tile); must be called by all 32 lanes of a warp.
 // win = shared-memory copy of image rows cell .. cell+7 (node rows cell-2 .. cell+5).
-template <int MT, int KS, bool MODES>
+template <int MT, int KS, bool MODES, bool EXTRA = false>
 __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, double* ext, int cell, bool active,
                                         double mass, double charge, double mu, double v_ref, double inv_v_ref,
                                         double t, const double (&y)[4], double (&dy)[4]) {
@@ -202,6 +212,7 @@ __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, do
   sincos_poly(thr, s1, c1);
   sincos_poly(phr, S1, C1);
   double fb[4] = {0.0, 0.0, 0.0, 0.0};
+  double fk[4] = {0.0, 0.0, 0.0, 0.0};                                  // EXTRA: the K series
   const unsigned onmask = __ballot_sync(0xffffffffu, active);
 #pragma unroll 1
   for (int G = 0; G < 4; ++G) {
@@ -262,11 +273,46 @@ __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, do
                              cm, sm, o);
       pend &= ~__ballot_sync(0xffffffffu, mine);
     }
+    // ---- NEXT-4: the sin series of B and the two series of K, same rows, images read through L1 -------------------
+    double ok[4] = {0.0, 0.0, 0.0, 0.0};
+    if constexpr (EXTRA) {
+      const int off_w = __shfl_sync(0xffffffffu, inwin ? off : kMmaNone, src);
+      const unsigned pend0 = __ballot_sync(0xffffffffu, ingrp && outside);
+      double cr[2 * MT], sr[2 * MT];                                    // (c_m, s_m) rotated by a quarter period
+#pragma unroll
+      for (int k = 0; k < 2 * MT; ++k) { cr[k] = sm[k]; sr[k] = -cm[k]; }
+      auto series = [&](const double* image, auto sin_tag, const double (&c_)[2 * MT], const double (&s_)[2 * MT],
+                        double (&acc)[4]) {
+        constexpr bool SINP = decltype(sin_tag)::value;
+        if (r_hi >= 0)
+          mma_sweep<MT, KS, LdG, SINP>(image + (size_t)cell * RS, RS, r_lo, r_hi, off_w, wsrc, lane, q, AC, AS, AnC,
+                                       AnS, c_, s_, acc);
+        unsigned pd = pend0;
+        while (pd) {
+          const int i0L = __shfl_sync(0xffffffffu, i0, __ffs(pd) - 1);
+          const bool mine = ingrp && outside && i0 == i0L;
+          const int off_f = __shfl_sync(0xffffffffu, mine ? 0 : kMmaNone, src);
+          mma_sweep<MT, KS, LdG, SINP>(image + (size_t)(i0L + 2) * RS, RS, 0, 3, off_f, wsrc, lane, q, AC, AS, AnC,
+                                       AnS, c_, s_, acc);
+          pd &= ~__ballot_sync(0xffffffffu, mine);
+        }
+      };
+      if (f.mma_image_bs) series(f.mma_image_bs, std::true_type{}, cr, sr, o);
+      if (f.mma_image_kc) series(f.mma_image_kc, std::false_type{}, cm, sm, ok);
+      if (f.mma_image_ks) series(f.mma_image_ks, std::true_type{}, cr, sr, ok);
+    }
     // ---- back to the particle lanes: lane 8 G + g takes the quad sum of fragment lanes 4 g .. 4 g + 3 ---------------
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
       const double v = __shfl_sync(0xffffffffu, quad_sum(o[k]), 4 * (lane & 7));
       if (ingrp) fb[k] = v;
+    }
+    if constexpr (EXTRA) {
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const double v = __shfl_sync(0xffffffffu, quad_sum(ok[k]), 4 * (lane & 7));
+        if (ingrp) fk[k] = v;
+      }
     }
   }
   // ---- particle role: profiles, perturbation, guiding-centre algebra ------------------------------------------------
@@ -318,13 +364,18 @@ __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, do
       pt[5] *= f.inv_psi0;
     }
     fb[3] *= (double)f.nfp;
-    gc_algebra(mass, charge, mu, f.inv_psi0, y[3] * v_ref, fb, pr, pt, dy);
+    if (EXTRA && (f.mma_image_kc || f.mma_image_ks)) {
+      fk[3] *= (double)f.nfp;
+      gc_algebra_general(mass, charge, mu, f.inv_psi0, y[3] * v_ref, fb, fk, pr, pt, dy);
+    } else {
+      gc_algebra(mass, charge, mu, f.inv_psi0, y[3] * v_ref, fb, pr, pt, dy);
+    }
     dy[3] *= inv_v_ref;
   }
 }
 
 // The table engine of trace_mma_kernel.
-template <int MT, int KS, bool MODES>
+template <int MT, int KS, bool MODES, bool EXTRA = false>
 struct MmaEngine {
   static constexpr bool kStageWindow = true;
   static __device__ __forceinline__ int win_doubles(const FieldDev& f) { return kMmaWinRows * f.mma_RS; }
@@ -335,14 +386,14 @@ struct MmaEngine {
   static __device__ __forceinline__ void rhs(const FieldDev& f, const double* win, double* ext, int cell, bool active,
                                              double mass, double charge, double mu, double v_ref, double inv_v_ref,
                                              double t, const double (&y)[4], double (&dy)[4]) {
-    rhs_mma<MT, KS, MODES>(f, win, ext, cell, active, mass, charge, mu, v_ref, inv_v_ref, t, y, dy);
+    rhs_mma<MT, KS, MODES, EXTRA>(f, win, ext, cell, active, mass, charge, mu, v_ref, inv_v_ref, t, y, dy);
   }
 };
 
-template <int MT, int KS, bool MODES, bool SAMPLE>
+template <int MT, int KS, bool MODES, bool SAMPLE, bool EXTRA = false>
 __global__ void __launch_bounds__(kMmaThreads, kMmaBlocksPerSm)
 trace_mma_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_out) {
-  trace_binned_body<MmaEngine<MT, KS, MODES>, kMmaThreads, kMmaCap, SAMPLE>(f, p, sc, mode, rhs_out);
+  trace_binned_body<MmaEngine<MT, KS, MODES, EXTRA>, kMmaThreads, kMmaCap, SAMPLE>(f, p, sc, mode, rhs_out);
 }
 
 }  // namespace gc

@@ -23,7 +23,7 @@ ST_TMAX, ST_LOST, ST_AXIS, ST_MAXSTEPS, ST_NONFINITE = 0, 1, 2, 3, 4
 
 EXPORTS = ["gc_field_create", "gc_field_destroy", "gc_field_eval", "gc_pert_eval", "gc_rhs_eval", "gc_trace",
            "gc_trace_host", "gc_set_kernel", "gc_set_option", "gc_kernel_info", "gc_last_error",
-           "gc_trace_sampled", "gc_pzeta_eval", "gc_birkhoff"]
+           "gc_trace_sampled", "gc_pzeta_eval", "gc_birkhoff", "gc_kcov_eval"]
 
 
 class GcError(RuntimeError):
@@ -38,7 +38,8 @@ class gc_field_desc(C.Structure):
                 ("G", C.c_void_p), ("I", C.c_void_p), ("iota", C.c_void_p),
                 ("psi0", C.c_double), ("nk", C.c_int32),
                 ("mode_m", C.c_void_p), ("mode_n", C.c_void_p),
-                ("mode_omega", C.c_void_p), ("mode_phase", C.c_void_p), ("phihat", C.c_void_p)]
+                ("mode_omega", C.c_void_p), ("mode_phase", C.c_void_p), ("phihat", C.c_void_p),
+                ("bmns", C.c_void_p), ("kmnc", C.c_void_p), ("kmns", C.c_void_p)]
 
 
 class gc_trace_params(C.Structure):
@@ -64,6 +65,7 @@ def load_library():
         L.gc_field_create.argtypes = [C.POINTER(gc_field_desc), C.POINTER(vp)]
         L.gc_field_destroy.argtypes = [vp]
         L.gc_field_eval.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp]
+        L.gc_kcov_eval.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp]
         L.gc_pert_eval.argtypes = [vp, i64, vp, vp, vp, dbl, vp, vp]
         L.gc_rhs_eval.argtypes = [vp, dbl, dbl, dbl, i64, vp, vp, vp, vp]
         L.gc_trace.argtypes = [vp, C.POINTER(gc_trace_params), i64] + [vp] * 15
@@ -146,11 +148,16 @@ class Field:
                  mode_phase=np.ascontiguousarray(fld.mode_phase, np.float64),
                  phihat=np.ascontiguousarray(fld.phihat, np.float64))
         ns, nh, nk = int(fld.ns), int(k["xm"].shape[0]), int(k["mode_m"].shape[0])
-        if k["bmnc"].shape != (ns, nh) or (nk and k["phihat"].shape != (ns, nk)):
+        for name in ("bmns", "kmnc", "kmns"):                  # NEXT-4 tables: None = absent
+            a = getattr(fld, name, None)
+            k[name] = None if a is None else np.ascontiguousarray(a, np.float64)
+        if k["bmnc"].shape != (ns, nh) or (nk and k["phihat"].shape != (ns, nk)) or \
+                any(k[nm] is not None and k[nm].shape != (ns, nh) for nm in ("bmns", "kmnc", "kmns")):
             raise ValueError("table shapes do not match ns, nh, nk")
         d = gc_field_desc(ns, int(fld.nfp), nh, _hp(k["xm"]), _hp(k["xn"]), _hp(k["bmnc"]), _hp(k["G"]),
                           _hp(k["I"]), _hp(k["iota"]), float(fld.psi0), nk, _hp(k["mode_m"]),
-                          _hp(k["mode_n"]), _hp(k["mode_omega"]), _hp(k["mode_phase"]), _hp(k["phihat"]))
+                          _hp(k["mode_n"]), _hp(k["mode_omega"]), _hp(k["mode_phase"]), _hp(k["phihat"]),
+                          _hp(k["bmns"]), _hp(k["kmnc"]), _hp(k["kmns"]))
         h = C.c_void_p(None)
         _check(L.gc_field_create(C.byref(d), C.byref(h)))
         self._h = h
@@ -190,6 +197,14 @@ class Field:
         _check(load_library().gc_field_eval(self._h, n, _dp(s), _dp(th), _dp(ze), _dp(B), _dp(dB),
                                             _stream_ptr(torch)))
         return B, dB
+
+    def kcov_eval(self, s, th, ze, derivs=True):
+        torch = _torch()
+        n = s.numel()
+        K = torch.empty(n, dtype=torch.float64, device=s.device)
+        dK = torch.empty((3, n), dtype=torch.float64, device=s.device) if derivs else None
+        _check(load_library().gc_kcov_eval(self._h, n, _dp(s), _dp(th), _dp(ze), _dp(K), _dp(dK), _stream_ptr(torch)))
+        return K, dK
 
     def pert_eval(self, s, th, ze, t):
         torch = _torch()

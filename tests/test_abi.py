@@ -61,7 +61,7 @@ def test_struct_layouts_match_the_header():
     from paper_2605_16734_b200 import gcorbit
     # gc_trace_params: 11 doubles + 3 int64; gc_field_desc: pointers and int32 with natural alignment
     assert C.sizeof(gcorbit.gc_trace_params) == 11 * 8 + 3 * 8
-    assert C.sizeof(gcorbit.gc_field_desc) == 16 + 6 * 8 + 8 + 8 + 5 * 8
+    assert C.sizeof(gcorbit.gc_field_desc) == 16 + 6 * 8 + 8 + 8 + 5 * 8 + 3 * 8          # + bmns, kmnc, kmns (NEXT-4)
     assert gcorbit.gc_field_desc.psi0.offset == 64 and gcorbit.gc_field_desc.nk.offset == 72
 
 

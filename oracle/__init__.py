@@ -176,6 +176,26 @@ class OracleField:
             out[i] = self.eval_B(a, b, c)
         return out
 
+    # ---- NEXT-2: local tricubic interpolant of B on an (s, theta, zeta) grid ----------------------------
+    def set_grid(self, ngs: int, nth: int, nze: int):
+        """Tabulate B by the direct sum and evaluate it from now on as a tensor-product cubic Lagrange
+        interpolant (reading A27); (0, 0, 0) switches back to the direct sum."""
+        if _load().oracle_field_set_grid(self._h, C.c_int32(ngs), C.c_int32(nth), C.c_int32(nze)) != 0:
+            raise ValueError("oracle_field_set_grid: each grid size must be >= 4 (or all 0)")
+        self.grid_shape = (ngs, nth, nze) if ngs else None
+
+    def grid(self) -> np.ndarray:
+        L = _load()
+        L.oracle_field_grid.restype = C.POINTER(C.c_double)
+        L.oracle_field_grid.argtypes = [C.c_void_p]
+        ptr = L.oracle_field_grid(self._h)
+        return np.ctypeslib.as_array(ptr, shape=self.grid_shape).copy()
+
+    def eval_B_sum(self, s, th, ze):
+        out = np.zeros(4)
+        _load().oracle_eval_B_sum(self._h, C.c_double(s), C.c_double(th), C.c_double(ze), _p(out))
+        return out
+
     def eval_K(self, s, th, ze):
         out = np.zeros(4)
         _load().oracle_eval_K(self._h, C.c_double(s), C.c_double(th), C.c_double(ze), _p(out))

@@ -19,6 +19,9 @@ struct oracle_field {
   double *bmnc, *G, *I, *iota, *mode_omega, *mode_phase, *phihat;
   double *bmns, *kmnc, *kmns;          /* NEXT-4: NULL = absent */
   double psi0;
+  /* NEXT-2: node values of B on the (s, theta, zeta) grid, [ngs][nth][nze]; NULL = the direct harmonic sum */
+  int32_t ngs, nth, nze;
+  double *grid;
 };
 
 static void *dup_mem(const void *src, size_t bytes) {
@@ -55,7 +58,7 @@ void oracle_field_destroy(oracle_field *f) {
   if (!f) return;
   free(f->xm); free(f->xn); free(f->bmnc); free(f->G); free(f->I); free(f->iota);
   free(f->mode_m); free(f->mode_n); free(f->mode_omega); free(f->mode_phase); free(f->phihat);
-  free(f->bmns); free(f->kmnc); free(f->kmns);
+  free(f->bmns); free(f->kmnc); free(f->kmns); free(f->grid);
   free(f);
 }
 
@@ -132,8 +135,85 @@ static void eval_series(const oracle_field *f, const double *tabc, const double 
   out[0] = X; out[1] = Xs; out[2] = Xth; out[3] = Xze;
 }
 
-void oracle_eval_B(const oracle_field *f, double s, double th, double ze, double out[4]) {
+void oracle_eval_B_sum(const oracle_field *f, double s, double th, double ze, double out[4]) {
   eval_series(f, f->bmnc, f->bmns, s, th, ze, out);
+}
+
+/* ---- NEXT-2 ("CUDA kernels implement field interpolation", "local
+ * tricubics"; reading A27 of DESIGN.md): B as a local tricubic interpolant of its own node values.
+ * Grid: s_i = i/(ngs-1), theta_j = 2 pi j/nth, zeta_k = (2 pi/nfp) k/nze (one field period; both angles periodic).
+ * Node values come from the direct sum O2.  Evaluation: tensor product of the cubic Lagrange weights of O1 in each
+ * direction; the radial stencil is clamped as in O1, an angular stencil is the four nodes c-1 .. c+2 around the
+ * cell c = floor(u), u = angle * (nodes per radian), taken modulo the period. */
+static const double ORACLE_TWO_PI = 6.283185307179586476925286766559;
+
+int oracle_field_set_grid(oracle_field *f, int32_t ngs, int32_t nth, int32_t nze) {
+  if (!f) return -1;
+  free(f->grid); f->grid = NULL; f->ngs = f->nth = f->nze = 0;
+  if (ngs == 0 && nth == 0 && nze == 0) return 0;                 /* back to the direct sum */
+  if (ngs < 4 || nth < 4 || nze < 4) return -1;
+  double *g = (double *)malloc(sizeof(double) * (size_t)ngs * nth * nze);
+  if (!g) return -1;
+#pragma omp parallel for collapse(2) schedule(static)
+  for (int i = 0; i < ngs; ++i)
+    for (int j = 0; j < nth; ++j)
+      for (int k = 0; k < nze; ++k) {
+        double s = (double)i / (double)(ngs - 1);
+        double th = ORACLE_TWO_PI * (double)j / (double)nth;
+        double ze = ORACLE_TWO_PI * (double)k / ((double)nze * (double)f->nfp);
+        double out[4];
+        oracle_eval_B_sum(f, s, th, ze, out);
+        g[((size_t)i * nth + j) * nze + k] = out[0];
+      }
+  f->grid = g; f->ngs = ngs; f->nth = nth; f->nze = nze;
+  return 0;
+}
+
+const double *oracle_field_grid(const oracle_field *f) { return f->grid; }
+
+/* cubic Lagrange weights on a periodic uniform grid of `nodes` points per `period`: first node j0 (before the
+ * modulo), weights w[4], d/d(angle) weights dw[4].  x = u - j0 lies in [1, 2): the stencil is always centred. */
+static void periodic_weights(int32_t nodes, double nodes_per_radian, double angle, int64_t *j0_out,
+                             double w[4], double dw[4]) {
+  double u = angle * nodes_per_radian;
+  double c = floor(u);
+  double x = u - (c - 1.0);
+  w[0] = -(x - 1.0) * (x - 2.0) * (x - 3.0) / 6.0;
+  w[1] = x * (x - 2.0) * (x - 3.0) / 2.0;
+  w[2] = -x * (x - 1.0) * (x - 3.0) / 2.0;
+  w[3] = x * (x - 1.0) * (x - 2.0) / 6.0;
+  dw[0] = -((x - 2.0) * (x - 3.0) + (x - 1.0) * (x - 3.0) + (x - 1.0) * (x - 2.0)) / 6.0 * nodes_per_radian;
+  dw[1] = ((x - 2.0) * (x - 3.0) + x * (x - 3.0) + x * (x - 2.0)) / 2.0 * nodes_per_radian;
+  dw[2] = -((x - 1.0) * (x - 3.0) + x * (x - 3.0) + x * (x - 1.0)) / 2.0 * nodes_per_radian;
+  dw[3] = ((x - 1.0) * (x - 2.0) + x * (x - 2.0) + x * (x - 1.0)) / 6.0 * nodes_per_radian;
+  double r = fmod(c - 1.0, (double)nodes);           /* exact: both are integers below 2^53 */
+  if (r < 0.0) r += (double)nodes;
+  *j0_out = (int64_t)r;
+}
+
+void oracle_eval_B_grid(const oracle_field *f, double s, double th, double ze, double out[4]) {
+  int32_t i0; double ws[4], dws[4], wt[4], dwt[4], wz[4], dwz[4];
+  int64_t j0, k0;
+  oracle_lagrange(f->ngs, s, &i0, ws, dws);
+  periodic_weights(f->nth, (double)f->nth / ORACLE_TWO_PI, th, &j0, wt, dwt);
+  periodic_weights(f->nze, (double)f->nze * (double)f->nfp / ORACLE_TWO_PI, ze, &k0, wz, dwz);
+  double B = 0.0, Bs = 0.0, Bt = 0.0, Bz = 0.0;
+  for (int a = 0; a < 4; ++a)
+    for (int b = 0; b < 4; ++b)
+      for (int c = 0; c < 4; ++c) {
+        int64_t j = (j0 + b) % f->nth, k = (k0 + c) % f->nze;
+        double v = f->grid[((size_t)(i0 + a) * f->nth + j) * f->nze + k];
+        B += ws[a] * wt[b] * wz[c] * v;
+        Bs += dws[a] * wt[b] * wz[c] * v;
+        Bt += ws[a] * dwt[b] * wz[c] * v;
+        Bz += ws[a] * wt[b] * dwz[c] * v;
+      }
+  out[0] = B; out[1] = Bs; out[2] = Bt; out[3] = Bz;
+}
+
+void oracle_eval_B(const oracle_field *f, double s, double th, double ze, double out[4]) {
+  if (f->grid) oracle_eval_B_grid(f, s, th, ze, out);
+  else oracle_eval_B_sum(f, s, th, ze, out);
 }
 
 /* NEXT-4: the covariant radial component K(s, theta, zeta) of B = G grad zeta + I grad theta + K grad psi. */

@@ -68,6 +68,17 @@ void oracle_lagrange(int32_t ns, double s, int32_t *i0, double w[4], double dw[4
 
 /* O2: out = {B, dB/ds, dB/dtheta, dB/dzeta}. */
 void oracle_eval_B(const oracle_field *f, double s, double th, double ze, double out[4]);
+/* The direct sum O2 whatever oracle_field_set_grid says. */
+void oracle_eval_B_sum(const oracle_field *f, double s, double th, double ze, double out[4]);
+/* NEXT-2 (reading A27): replace the direct sum by a local tricubic interpolant.
+ * oracle_field_set_grid tabulates B (direct sum O2) at s_i = i/(ngs-1), theta_j = 2 pi j/nth,
+ * zeta_k = (2 pi/nfp) k/nze (each count >= 4; 0,0,0 switches back to the direct sum) and from then on oracle_eval_B,
+ * and with it oracle_rhs, oracle_trace and oracle_pzeta, evaluate B and its three derivatives as the tensor-product
+ * cubic Lagrange interpolant of those node values (radial stencil as O1, angular stencils periodic and centred).
+ * Fields with K tables are rejected by the CUDA path; the oracle interpolates B only.  Returns 0, -1 on bad sizes. */
+int oracle_field_set_grid(oracle_field *f, int32_t ngs, int32_t nth, int32_t nze);
+const double *oracle_field_grid(const oracle_field *f);           /* [ngs][nth][nze] or NULL */
+void oracle_eval_B_grid(const oracle_field *f, double s, double th, double ze, double out[4]);
 /* NEXT-4: covariant radial component, out = {K, dK/ds, dK/dtheta, dK/dzeta} (all zero without K tables). */
 void oracle_eval_K(const oracle_field *f, double s, double th, double ze, double out[4]);
 /* O1 on profiles: out = {G, dG/ds, I, dI/ds, iota, diota/ds}. */

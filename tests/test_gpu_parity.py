@@ -208,26 +208,37 @@ def test_full_size_launch_sampled(cases, config, n_full, seg):
                       h_in=o1.h[alive], t0=seg, t_max=2 * seg)
         y_ref, st_ref, t_ref = o1.y.copy(), o1.status.copy(), o1.t.copy()
         y_ref[:, alive], st_ref[alive], t_ref[alive] = o2.y, o2.status, o2.t
+        two_segments.counts = (o1.n_acc.copy(), o1.n_rej.copy())
+        two_segments.counts[0][alive] += o2.n_acc
+        two_segments.counts[1][alive] += o2.n_rej
         return y_ref, st_ref, t_ref
 
     y_ref, st_ref, t_ref = two_segments(Q)
+    acc_ref, rej_ref = two_segments.counts
     # the oracle's own conditioning on these particles (gpu_common): theta0 moved by ~1 ulp
     spread, tspread = np.zeros(len(idx)), np.zeros(len(idx))
-    for eps in (1e-15, -1e-15):
-        Qp = W.Particles(Q.s, Q.theta * (1.0 + eps), Q.zeta, Q.pitch, Q.speed)
+    for a, b in [(1e-15, 0.0), (-1e-15, 0.0), (0.0, 1e-15), (0.0, -1e-15)]:     # as gpu_common.oracle_conditioning
+        Qp = W.Particles(Q.s, Q.theta * (1.0 + a), Q.zeta * (1.0 + b), Q.pitch, Q.speed)
         y2, st2, t2 = two_segments(Qp)
         assert np.array_equal(st2, st_ref)
         spread = np.maximum(spread, rel_diff(y2, y_ref, spec.v_ref))
         tspread = np.maximum(tspread, np.abs(t2 - t_ref) / t_ref)
     assert np.array_equal(status[idx], st_ref)
     rel = rel_diff(st.y.cpu().numpy()[:, idx], y_ref, spec.v_ref)
-    assert np.median(rel) < 1e-11 and (rel <= np.maximum(SAME_RTOL, COND_FACTOR * spread)).all(), rel.max()
+    # DESIGN.md section 5 ("Controller decisions"), the rule assert_trace_parity applies: a particle on the oracle's
+    # step sequence is held to max(1e-9, 10 x the oracle's own spread); an accept/reject decision taken at
+    # err = 1 +- 1e-13 may flip, the two step sequences then differ and the results agree to the truncation error
+    # only (FLIP_RTOL); at most 5 % of the sampled particles may do that
+    same = (st.n_acc.cpu().numpy()[idx] == acc_ref) & (st.n_rej.cpu().numpy()[idx] == rej_ref)
+    assert same.mean() >= 0.95, same.mean()
+    tol = np.where(same, np.maximum(SAME_RTOL, COND_FACTOR * spread), FLIP_RTOL)
+    assert np.median(rel) < 1e-11 and (rel <= tol).all(), (rel.max(), np.nonzero(rel > tol)[0])
     relt = np.abs(st.t.cpu().numpy()[idx] - t_ref) / t_ref
-    assert (relt <= np.maximum(SAME_RTOL, COND_FACTOR * tspread)).all(), relt.max()
+    assert (relt <= np.where(same, np.maximum(SAME_RTOL, COND_FACTOR * tspread), FLIP_RTOL)).all(), relt.max()
     from gpu_common import record_info
     record_info("full_size_sampled", label=f"config {config} mma, {n_full} particles, 2 x {seg:g} s", particles=len(idx),
                 max_rel=float(rel.max()), median_rel=float(np.median(rel)), within=float((rel <= SAME_RTOL).mean()),
-                max_rel_t=float(relt.max()), waves=-(-n_full // (1 << 18)))
+                max_rel_t=float(relt.max()), same_frac=float(same.mean()), waves=-(-n_full // (1 << 18)))
 
 
 @pytest.mark.parametrize("kernel", ["tile", "mma"])

@@ -49,6 +49,11 @@ class _Params(C.Structure):
                 ("section", C.c_int64), ("refine_loss", C.c_int64)]
 
 
+class _SymParams(C.Structure):
+    _fields_ = [("mass", C.c_double), ("charge", C.c_double), ("t0", C.c_double), ("dt", C.c_double),
+                ("nsteps", C.c_int64), ("s_loss", C.c_double), ("s_min", C.c_double), ("newton_tol", C.c_double)]
+
+
 def _load():
     global _lib
     if _lib is None:
@@ -126,6 +131,17 @@ class TraceResult:
     poincare_count: int = 0
     traj: np.ndarray | None = None          # [n][cap][5]
     traj_count: np.ndarray | None = None
+
+
+@dataclass
+class SymplecticResult:
+    y: np.ndarray          # [4][n]: s, theta, zeta, v_par (m/s)
+    t: np.ndarray          # [n]
+    status: np.ndarray     # [n] int32: 0 all steps done, 1 lost, 2 axis, 4 Newton failure / non-finite
+    n_steps: np.ndarray
+    n_iter: np.ndarray
+    samples: np.ndarray | None = None       # [4][nsamp][n]
+    sample_end: np.ndarray | None = None
 
 
 class OracleField:
@@ -305,6 +321,53 @@ class OracleField:
         for idx in np.ndindex(s.shape):
             out[idx] = L.oracle_pzeta(self._h, mass, charge, _p(chi_nodes), s[idx], th[idx], ze[idx], vpar[idx], t[idx])
         return out
+
+    # ---- NEXT-3: symplectic explicit-implicit Euler (static fields, K = 0) ---------------------------------------
+    def symplectic_step(self, mass, charge, mu, chi_nodes, h, z, newton_tol=1e-13):
+        """One step on z = (s, theta, zeta, p_zeta); returns (z_new, Newton iterations)."""
+        chi_nodes, z = _f64(chi_nodes), _f64(z).copy()
+        it = C.c_int32(0)
+        L = _load()
+        L.oracle_symplectic_step.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_void_p, C.c_double,
+                                             C.c_double, C.c_void_p, C.c_void_p]
+        rc = L.oracle_symplectic_step(self._h, mass, charge, mu, _p(chi_nodes), h, newton_tol, _p(z), C.byref(it))
+        if rc != 0:
+            raise ArithmeticError("oracle_symplectic_step: Newton did not converge")
+        return z, int(it.value)
+
+    def symplectic_pzeta(self, mass, charge, chi_nodes, s, th, ze, vpar):
+        chi_nodes = _f64(chi_nodes)
+        L = _load()
+        L.oracle_symplectic_pzeta.restype = C.c_double
+        L.oracle_symplectic_pzeta.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_void_p] + [C.c_double] * 4
+        return L.oracle_symplectic_pzeta(self._h, mass, charge, _p(chi_nodes), s, th, ze, vpar)
+
+    def symplectic_vpar(self, mass, charge, chi_nodes, s, th, ze, pz):
+        chi_nodes = _f64(chi_nodes)
+        L = _load()
+        L.oracle_symplectic_vpar.restype = C.c_double
+        L.oracle_symplectic_vpar.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_void_p] + [C.c_double] * 4
+        return L.oracle_symplectic_vpar(self._h, mass, charge, _p(chi_nodes), s, th, ze, pz)
+
+    def trace_symplectic(self, mass, charge, s0, th0, ze0, vpar0, mu, chi_nodes, dt, nsteps, t0=0.0, s_loss=1.0,
+                         s_min=1e-3, newton_tol=1e-13, sample_stride=0, nsamp=0):
+        """n particles, nsteps fixed steps each; returns a SymplecticResult."""
+        s0, th0, ze0, vpar0, mu, chi_nodes = map(_f64, (s0, th0, ze0, vpar0, mu, chi_nodes))
+        n = s0.shape[0]
+        p = _SymParams(mass, charge, t0, dt, int(nsteps), s_loss, s_min, newton_tol)
+        y, t = np.zeros((4, n)), np.zeros(n)
+        status, steps, iters = (np.zeros(n, np.int32) for _ in range(3))
+        samples = np.full((4, int(nsamp), n), np.nan) if nsamp else None
+        send = np.zeros(n, np.int32) if nsamp else None
+        L = _load()
+        L.oracle_trace_symplectic.argtypes = [C.c_void_p, C.c_void_p, C.c_int64] + [C.c_void_p] * 11 + \
+            [C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
+        rc = L.oracle_trace_symplectic(self._h, C.byref(p), n, _p(s0), _p(th0), _p(ze0), _p(vpar0), _p(mu),
+                                       _p(chi_nodes), _p(y), _p(t), _p(status), _p(steps), _p(iters),
+                                       int(sample_stride), int(nsamp), _p(samples), _p(send))
+        if rc != 0:
+            raise ValueError("oracle_trace_symplectic: bad arguments")
+        return SymplecticResult(y, t, status, steps, iters, samples, send)
 
     def rk4(self, mass, charge, v_ref, s0, th0, ze0, vpar0, mu, t0, h, nsteps):
         s0, th0, ze0, vpar0, mu = map(_f64, (s0, th0, ze0, vpar0, mu))

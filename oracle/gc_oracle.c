@@ -714,6 +714,178 @@ double oracle_pzeta(const oracle_field *f, double mass, double charge, const dou
   return charge * ((rho + pt[4]) * pr[0] - chi);
 }
 
+/* ---- NEXT-3 ("A symplectic integrator for non-canonical guiding-center orbits uses the
+ * explicit-implicit Euler scheme of (Albert et al., 2020)"; Fig. 1 left; reading A28 of DESIGN.md).
+ *
+ * Albert et al. 2020 is not in the container; the scheme is restated from what the sentence fixes.  For a static field
+ * with K = 0 and no perturbation the guiding-centre Lagrangian of O4,
+ *     L = q (psi + rho I) thetadot + q (rho G - chi) zetadot - H,     rho = m v_par / (q B),  H = m v_par^2 / 2 + mu B,
+ * is already of the form p_theta thetadot + p_zeta zetadot - H with the canonical momenta
+ *     p_theta = q (psi0 s + rho I(s)),     p_zeta = q (rho G(s) - chi(s)),
+ * so (theta, zeta, p_theta, p_zeta) are canonical coordinates and s is a parameter fixed by them ("non-canonical":
+ * the state carried is z = (s, theta, zeta, p_zeta)).  With rho(s, p_zeta) = (p_zeta / q + chi(s)) / G(s),
+ *     H(s, theta, zeta, p_zeta) = (q rho B)^2 / (2 m) + mu B,          p_theta(s, p_zeta) = q (psi0 s + rho I),
+ * the symplectic ("explicit-implicit") Euler step of size h, implicit in the momenta and explicit in the angles, is
+ *     p_theta(s', p_zeta') - p_theta(s, p_zeta) + h dH/dtheta = 0        (1)   derivatives of H at constant s, p_zeta
+ *     p_zeta' - p_zeta                          + h dH/dzeta  = 0        (2)   taken at (s', theta, zeta, p_zeta')
+ *     theta' = theta + h (dH/ds) / (dp_theta/ds)                          (3)
+ *     zeta'  = zeta  + h [ dH/dp_zeta - (dH/ds) (dp_theta/dp_zeta) / (dp_theta/ds) ]          (4)
+ * (the chain rule through s(theta, zeta, p_theta, p_zeta) turns the canonical dK/dp_theta, dK/dp_zeta, dK/dtheta,
+ * dK/dzeta of K = H(s(..), ..) into these; p_theta does not depend on the angles here).  (1), (2) are solved for
+ * (s', p_zeta') by Newton's method on the scaled unknowns x = (s, p_zeta / (q psi0)) with a central-difference
+ * Jacobian (step 1e-6), started from the old values, until max |dx_i| <= newton_tol max(1, |x_i|); at most 50
+ * iterations, failure or a non-finite value ends the particle with status 4.  chi(s) is supplied at the radial
+ * nodes (as for oracle_pzeta) and interpolated by O1, and d chi / d s of THAT interpolant is what the scheme uses
+ * where the equations of motion have psi0 iota: the map is then exactly symplectic within a radial cell.
+ * Stop rules after every step as O7: s >= s_loss -> 1, s <= s_min -> 2; nsteps steps done -> 0. */
+typedef struct {
+  const oracle_field *f;
+  const double *chi_nodes;
+  double mass, charge, mu;
+} sym_ctx;
+
+/* H and p_theta with their first partial derivatives at (s, theta, zeta, p_zeta). */
+static void sym_eval(const sym_ctx *c, double s, double th, double ze, double pz,
+                     double *H, double dH[4] /* d/ds, d/dtheta, d/dzeta, d/dp_zeta */,
+                     double *ptheta, double *dpth_ds, double *dpth_dpz, double *vpar) {
+  const oracle_field *f = c->f;
+  const double q = c->charge, m = c->mass;
+  double fb[4], pr[6];
+  oracle_eval_B(f, s, th, ze, fb);
+  oracle_eval_profiles(f, s, pr);
+  int32_t i0; double w[4], dw[4], chi, chi_s;
+  oracle_lagrange(f->ns, s, &i0, w, dw);
+  interp(c->chi_nodes, 1, i0, w, dw, &chi, &chi_s);
+  const double B = fb[0], Bs = fb[1], Bth = fb[2], Bze = fb[3];
+  const double G = pr[0], Gs = pr[1], I = pr[2], Is = pr[3];
+  const double rho = (pz / q + chi) / G;
+  const double rho_s = (chi_s - rho * Gs) / G;
+  const double rho_pz = 1.0 / (q * G);
+  const double e = q * q * rho * rho * B / m + c->mu;        /* dH/dB */
+  *H = q * q * rho * rho * B * B / (2.0 * m) + c->mu * B;
+  dH[0] = q * q * rho * rho_s * B * B / m + e * Bs;
+  dH[1] = e * Bth;
+  dH[2] = e * Bze;
+  dH[3] = q * q * rho * rho_pz * B * B / m;
+  *ptheta = q * (f->psi0 * s + rho * I);
+  *dpth_ds = q * (f->psi0 + rho_s * I + rho * Is);
+  *dpth_dpz = q * rho_pz * I;
+  *vpar = q * rho * B / m;
+}
+
+/* residuals of (1), (2) in units of q psi0 at the scaled unknowns x = (s, p_zeta / (q psi0)) */
+static void sym_residual(const sym_ctx *c, double th, double ze, double pth_old, double pz_old, double h,
+                         const double x[2], double F[2]) {
+  const double unit = c->charge * c->f->psi0;
+  double H, dH[4], pth, d1, d2, v;
+  sym_eval(c, x[0], th, ze, x[1] * unit, &H, dH, &pth, &d1, &d2, &v);
+  F[0] = (pth - pth_old + h * dH[1]) / unit;
+  F[1] = (x[1] * unit - pz_old + h * dH[2]) / unit;
+}
+
+int oracle_symplectic_step(const oracle_field *f, double mass, double charge, double mu, const double *chi_nodes,
+                           double h, double newton_tol, double z[4] /* s, theta, zeta, p_zeta: in and out */,
+                           int32_t *iterations) {
+  sym_ctx c = {f, chi_nodes, mass, charge, mu};
+  const double unit = charge * f->psi0;
+  double H, dH[4], pth_old, d1, d2, v;
+  sym_eval(&c, z[0], z[1], z[2], z[3], &H, dH, &pth_old, &d1, &d2, &v);
+  double x[2] = {z[0], z[3] / unit};
+  int ok = 0, it = 0;
+  for (it = 1; it <= 50; ++it) {
+    double F[2], J[2][2];
+    sym_residual(&c, z[1], z[2], pth_old, z[3], h, x, F);
+    for (int j = 0; j < 2; ++j) {
+      const double e = 1e-6;
+      double xp[2] = {x[0], x[1]}, xm[2] = {x[0], x[1]}, Fp[2], Fm[2];
+      xp[j] += e; xm[j] -= e;
+      sym_residual(&c, z[1], z[2], pth_old, z[3], h, xp, Fp);
+      sym_residual(&c, z[1], z[2], pth_old, z[3], h, xm, Fm);
+      J[0][j] = (Fp[0] - Fm[0]) / (2.0 * e);
+      J[1][j] = (Fp[1] - Fm[1]) / (2.0 * e);
+    }
+    const double det = J[0][0] * J[1][1] - J[0][1] * J[1][0];
+    const double dx0 = -(J[1][1] * F[0] - J[0][1] * F[1]) / det;
+    const double dx1 = -(-J[1][0] * F[0] + J[0][0] * F[1]) / det;
+    if (!isfinite(dx0) || !isfinite(dx1)) break;
+    x[0] += dx0; x[1] += dx1;
+    if (fabs(dx0) <= newton_tol * fmax(1.0, fabs(x[0])) && fabs(dx1) <= newton_tol * fmax(1.0, fabs(x[1]))) {
+      ok = 1;
+      break;
+    }
+  }
+  if (iterations) *iterations = it;
+  if (!ok) return -1;
+  sym_eval(&c, x[0], z[1], z[2], x[1] * unit, &H, dH, &pth_old, &d1, &d2, &v);   /* partials at (s', theta, zeta, p_zeta') */
+  z[1] = z[1] + h * dH[0] / d1;
+  z[2] = z[2] + h * (dH[3] - dH[0] * d2 / d1);
+  z[0] = x[0];
+  z[3] = x[1] * unit;
+  return 0;
+}
+
+/* p_zeta of a state given as (s, theta, zeta, v_par) and back (static field: no alpha). */
+double oracle_symplectic_pzeta(const oracle_field *f, double mass, double charge, const double *chi_nodes,
+                               double s, double th, double ze, double vpar) {
+  return oracle_pzeta(f, mass, charge, chi_nodes, s, th, ze, vpar, 0.0);
+}
+
+double oracle_symplectic_vpar(const oracle_field *f, double mass, double charge, const double *chi_nodes,
+                              double s, double th, double ze, double pz) {
+  sym_ctx c = {f, chi_nodes, mass, charge, 0.0};
+  double H, dH[4], pth, d1, d2, v;
+  sym_eval(&c, s, th, ze, pz, &H, dH, &pth, &d1, &d2, &v);
+  return v;
+}
+
+int oracle_trace_symplectic(const oracle_field *f, const oracle_symplectic_params *p, int64_t n,
+                            const double *s0, const double *th0, const double *ze0, const double *vpar0,
+                            const double *mu, const double *chi_nodes,
+                            double *y_out, double *t_out, int32_t *status, int32_t *n_steps, int32_t *n_iter,
+                            int64_t sample_stride, int64_t nsamp, double *samples, int32_t *sample_end) {
+  if (!f || !p || n < 0 || !chi_nodes || f->nk > 0 || f->kmnc || f->kmns || !(p->dt > 0.0) || p->nsteps < 0 ||
+      !(p->newton_tol > 0.0) || (nsamp > 0 && (sample_stride < 1 || !samples || !sample_end)))
+    return -1;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int64_t i = 0; i < n; ++i) {
+    double z[4] = {s0[i], th0[i], ze0[i], 0.0};
+    z[3] = oracle_symplectic_pzeta(f, p->mass, p->charge, chi_nodes, z[0], z[1], z[2], vpar0[i]);
+    double vpar = vpar0[i];
+    int32_t st = 0, steps = 0, iters = 0;
+    int64_t js = 0;
+    if (!isfinite(z[0]) || !isfinite(z[1]) || !isfinite(z[2]) || !isfinite(z[3])) st = 4;
+    if (nsamp > 0 && st == 0) {                                /* sample 0 is the initial state */
+      samples[(0 * nsamp + 0) * n + i] = z[0]; samples[(1 * nsamp + 0) * n + i] = z[1];
+      samples[(2 * nsamp + 0) * n + i] = z[2]; samples[(3 * nsamp + 0) * n + i] = vpar;
+      js = 1;
+    }
+    for (int64_t k = 0; k < p->nsteps && st == 0; ++k) {
+      int32_t it = 0;
+      int rc = oracle_symplectic_step(f, p->mass, p->charge, mu[i], chi_nodes, p->dt, p->newton_tol, z, &it);
+      iters += it;
+      if (rc != 0 || !isfinite(z[0]) || !isfinite(z[1]) || !isfinite(z[2]) || !isfinite(z[3])) { st = 4; break; }
+      ++steps;
+      if (nsamp > 0 && js < nsamp && (k + 1) % sample_stride == 0) {     /* state after every sample_stride-th step */
+        samples[(0 * nsamp + js) * n + i] = z[0]; samples[(1 * nsamp + js) * n + i] = z[1];
+        samples[(2 * nsamp + js) * n + i] = z[2];
+        samples[(3 * nsamp + js) * n + i] =
+            oracle_symplectic_vpar(f, p->mass, p->charge, chi_nodes, z[0], z[1], z[2], z[3]);
+        ++js;
+      }
+      if (z[0] >= p->s_loss) st = 1;
+      else if (z[0] <= p->s_min) st = 2;
+    }
+    if (steps > 0) vpar = oracle_symplectic_vpar(f, p->mass, p->charge, chi_nodes, z[0], z[1], z[2], z[3]);
+    y_out[0 * n + i] = z[0]; y_out[1 * n + i] = z[1]; y_out[2 * n + i] = z[2]; y_out[3 * n + i] = vpar;
+    t_out[i] = p->t0 + (double)steps * p->dt;
+    status[i] = st;
+    if (n_steps) n_steps[i] = steps;
+    if (n_iter) n_iter[i] = iters;
+    if (nsamp > 0) sample_end[i] = (int32_t)js;
+  }
+  return 0;
+}
+
 /* ---- check (d): classical RK4 at fixed step -------------------------------------------------------- */
 void oracle_rk4(const oracle_field *f, double mass, double charge, double v_ref, int64_t n,
                 const double *s0, const double *th0, const double *ze0, const double *vpar0,

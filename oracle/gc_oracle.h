@@ -147,6 +147,35 @@ int oracle_trace_sampled(const oracle_field *f, const oracle_trace_params *p, in
 double oracle_pzeta(const oracle_field *f, double mass, double charge, const double *chi_nodes,
                     double s, double th, double ze, double vpar, double t);
 
+/* ---- NEXT-3: the symplectic explicit-implicit Euler integrator for static fields
+ * with K = 0 (reading A28; the scheme is written out above oracle_symplectic_step in gc_oracle.c).  State
+ * z = (s, theta, zeta, p_zeta); chi_nodes [ns] = chi at the radial nodes (d chi / d psi = iota), interpolated by O1. */
+typedef struct {
+  double mass, charge;
+  double t0, dt;               /* fixed step, s                                             */
+  int64_t nsteps;              /* steps per particle                                        */
+  double s_loss, s_min;        /* stop rules of O7                                          */
+  double newton_tol;           /* relative size of the last Newton update, e.g. 1e-13       */
+} oracle_symplectic_params;
+
+/* One step of size h on z = (s, theta, zeta, p_zeta); returns 0, -1 if Newton did not converge. */
+int oracle_symplectic_step(const oracle_field *f, double mass, double charge, double mu, const double *chi_nodes,
+                           double h, double newton_tol, double z[4], int32_t *iterations);
+double oracle_symplectic_pzeta(const oracle_field *f, double mass, double charge, const double *chi_nodes,
+                               double s, double th, double ze, double vpar);
+double oracle_symplectic_vpar(const oracle_field *f, double mass, double charge, const double *chi_nodes,
+                              double s, double th, double ze, double pz);
+/* n particles, nsteps steps each (OpenMP over particles).  y_out [4][n] = s, theta, zeta, v_par (m/s); t_out [n];
+ * status 0 all steps done, 1 lost, 2 axis, 4 Newton failure / non-finite; n_steps, n_iter [n] or NULL (steps taken,
+ * Newton iterations in total).  samples [4][nsamp][n] (or nsamp = 0): sample 0 = the initial state, sample j = the
+ * state after step j * sample_stride; sample_end [n] = samples written.  Returns 0, -1 on bad arguments (among them:
+ * a field with modes or K tables). */
+int oracle_trace_symplectic(const oracle_field *f, const oracle_symplectic_params *p, int64_t n,
+                            const double *s0, const double *th0, const double *ze0, const double *vpar0,
+                            const double *mu, const double *chi_nodes,
+                            double *y_out, double *t_out, int32_t *status, int32_t *n_steps, int32_t *n_iter,
+                            int64_t sample_stride, int64_t nsamp, double *samples, int32_t *sample_end);
+
 /* Check (d): classical fixed-step RK4, nsteps steps of size h from t0; y_out [4][n]. */
 void oracle_rk4(const oracle_field *f, double mass, double charge, double v_ref, int64_t n,
                 const double *s0, const double *th0, const double *ze0, const double *vpar0,

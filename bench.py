@@ -69,6 +69,12 @@ def parse_args():
                     "post-processing time to config")
     ap.add_argument("--slots", type=int, default=0, help="GC_OPT_WAVE_PARTICLES: record slots of the binned kernels "
                     "(0 = the library's default, 2^18)")
+    ap.add_argument("--grid", default="", help="NEXT-2: NGSxNTHxNZE -- trace on the 3-D tricubic interpolant of B "
+                    "(gc_field_set_grid) instead of the direct harmonic sum; not the default line")
+    ap.add_argument("--symplectic", type=float, default=0.0, metavar="DT", help="NEXT-3: advance every segment with the "
+                    "symplectic explicit-implicit Euler integrator at the fixed step DT seconds (gc_trace_symplectic) "
+                    "instead of Dormand-Prince; a particle-step is then one symplectic step; static configs only; "
+                    "not the default line")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
@@ -245,6 +251,8 @@ def run_cuda(args):
         GF.set_kernel({"warp": G.GC_KERNEL_WARP, "generic": G.GC_KERNEL_GENERIC, "tile": G.GC_KERNEL_TILE, "mma": G.GC_KERNEL_MMA}[args.kernel])
     if args.slots:
         GF.set_option(G.GC_OPT_WAVE_PARTICLES, args.slots)
+    if args.grid:
+        GF.set_grid(*[int(x) for x in args.grid.lower().split("x")])
     kinfo = GF.kernel_info(n)
     kinfo["record_slots"] = args.slots if args.slots else "default"
     T = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device=dev)
@@ -263,7 +271,19 @@ def run_cuda(args):
 
     # warm-up: the first W segments of the trace
     S = args.samples
-    if S > 0:
+    if args.symplectic > 0.0:
+        s_n = np.arange(fld.ns) / (fld.ns - 1)
+        chi = T(fld.psi0 * np.concatenate([[0.0], np.cumsum(0.5 * (fld.iota[1:] + fld.iota[:-1]) * np.diff(s_n))]))
+        nst = max(1, int(round(seg / args.symplectic)))
+
+        def resume(state, t0, t1):
+            y = state.y
+            return GF.trace_symplectic(spec.mass, spec.charge, y[0], y[1], y[2], y[3], mu, chi, args.symplectic, nst,
+                                       t0=t0, out=state, flags=G.GC_TRACE_RESUME)
+        state = GF.trace_symplectic(spec.mass, spec.charge, s, th, ze, vpar, mu, chi, args.symplectic, nst)
+        state.n_acc, state.n_rej = state.n_steps, torch.zeros_like(state.n_steps)
+        info["symplectic"] = {"dt": args.symplectic, "steps_per_segment": nst}
+    elif S > 0:
         nsamp_total = S * (max(Wu, 1) + K) + 1
         sdt = seg / S
 
@@ -332,7 +352,7 @@ def run_cuda(args):
 
     # ---- e2e: the same segments through gc_trace_host, pinned host buffers, copies inside the timed region
     e2e = None
-    if not args.no_e2e and S == 0:
+    if not args.no_e2e and S == 0 and not args.symplectic:
         Ke = K                                                 # as many calls as timed steps: dilutes host-side stalls
         pin = lambda t: t.detach().cpu().pin_memory()
         hy, ht, hs, hh, hmu = pin(state.y), pin(state.t), pin(state.status), pin(state.h), pin(mu)
@@ -390,7 +410,8 @@ def run_cuda(args):
     # capture): DRAM bytes per launch and executed FP64 flop per particle-step.  Any other workload: null.
     traffic = executed = cap_src = None
     default_launch = (args.config == DEFAULT_CONFIG and args.particles is None and args.segment == 2e-5 and
-                      kinfo["kernel"] == "mma" and args.samples == 0 and args.slots == 0)
+                      kinfo["kernel"] == "mma" and args.samples == 0 and args.slots == 0 and not args.grid and
+                      not args.symplectic)
     tp = os.path.join(ROOT, "profiles", "ncu_constants.json.txt")
     if os.path.exists(tp) and default_launch:
         try:
@@ -416,6 +437,35 @@ def run_cuda(args):
                 "frac_of_probe": achieved / (probe_flops / 1e12),
                 "flop_per_particle_step": fstep, "flop_per_particle_step_min": fstep_min,
                 "particle_steps_per_launch": attempts / K}
+    if args.symplectic > 0.0 or args.grid:
+        # other formulations of the path (NEXT-2, NEXT-3): field evaluations per particle-step instead of the
+        # Dormand-Prince count of 6
+        evals = 6.0
+        if args.symplectic > 0.0:
+            evals = float(state.n_iter.sum(dtype=torch.int64).item()) / max(attempts_of(state), 1)
+            info["symplectic"]["field_evaluations_per_step"] = evals
+        if args.grid:
+            # gather-bound: 64 node values of 8 bytes per field evaluation come through the L1 data pipe from a table
+            # that lives in L2; nominal pipe width 128 bytes per SM and cycle
+            sms = torch.cuda.get_device_properties(dev).multi_processor_count
+            gbytes = evals * 64.0 * 8.0
+            peak_l1 = sms * 128.0 * peak_nominal * 1e12 / (sms * FP64_LANES_PER_SM * 2) / 1e9   # same clock as the ALU peak
+            roofline = {"bound": "l1", "achieved": rate * gbytes / 1e9, "peak": peak_l1, "unit": "GB/s",
+                        "frac": rate * gbytes / 1e9 / peak_l1, "traffic": None,
+                        "model": f"{gbytes:.0f} gathered bytes per particle-step ({evals:.2f} evaluations of the "
+                                 "tricubic interpolant x 64 nodes x 8 B) against sms x 128 B x 1.965 GHz of L1 data "
+                                 "pipe; the table is read from L2, not HBM",
+                        "fp64_frac": rate * (evals * 700.0 + 250.0) / 1e12 / peak_nominal,
+                        "kernel": "trace_symplectic_kernel<true>" if args.symplectic > 0.0 else "trace_lane_kernel<true>",
+                        "launch_ms_avg": kernel_ms / K, "particle_steps_per_launch": attempts / K}
+        else:
+            f_eval = (fstep - 250.0) / 6.0
+            roofline.update({"flop_per_particle_step": evals * f_eval, "achieved": rate * evals * f_eval / 1e12,
+                             "frac": rate * evals * f_eval / 1e12 / peak_nominal, "frac_min_formulation": None,
+                             "frac_executed": None, "kernel": "trace_symplectic_kernel<false>",
+                             "flop_model": "survey count of one field evaluation (28 flop per harmonic) x measured "
+                                           "evaluations per symplectic step; this kernel evaluates the harmonic sum "
+                                           "with one sincos per harmonic (generic engine)"})
     cpu = None
     if not args.no_cpu_baseline:
         cpu = oracle_sample(fld, spec, P, seg, args.cpu_seconds)

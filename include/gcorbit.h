@@ -104,10 +104,12 @@ enum { GC_ST_TMAX = 0, GC_ST_LOST = 1, GC_ST_AXIS = 2, GC_ST_MAXSTEPS = 3, GC_ST
  *   GC_KERNEL_WARP    one warp per particle, stencil window in registers; the kernel for small ensembles
  *                     (needs max |xn| <= 16, max xm <= 28)
  *   GC_KERNEL_GENERIC one thread per particle, tables read from global memory; any field
+ *   GC_KERNEL_GRID    one lane per particle, atomic particle queue, B from the 3-D interpolant of gc_field_set_grid;
+ *                     reported by gc_kernel_info while a grid is set, not selectable through gc_set_kernel
  *   GC_KERNEL_AUTO    per call: MMA (else TILE) when the field fits it and n >= GC_TILE_MIN_PARTICLES, else WARP
  *                     when the field fits it, else GENERIC.
  * All four implement the same equations and controller; their results differ at rounding level only. */
-enum { GC_KERNEL_AUTO = 0, GC_KERNEL_GENERIC = 1, GC_KERNEL_WARP = 2, GC_KERNEL_TILE = 3, GC_KERNEL_MMA = 4 };
+enum { GC_KERNEL_AUTO = 0, GC_KERNEL_GENERIC = 1, GC_KERNEL_WARP = 2, GC_KERNEL_TILE = 3, GC_KERNEL_MMA = 4, GC_KERNEL_GRID = 5 };
 enum { GC_TILE_MIN_PARTICLES = 4096 };
 
 /* Copies the tables to the device, checks them (finite values, xm >= 0, omega != 0) and builds the packed layouts of
@@ -116,6 +118,19 @@ enum { GC_TILE_MIN_PARTICLES = 4096 };
  * failure. */
 int gc_field_create(const gc_field_desc* desc, gc_field** out);
 int gc_field_destroy(gc_field* f);
+
+/* ---- NEXT-2 of SURVEY.md section 8(f): the 3-D local-interpolant field ("CUDA kernels implement field interpolation
+ * and trajectory integration on GPU" PAPER.md:48; "local tricubics" PAPER.md:80,111; reading A27 of DESIGN.md).
+ * Tabulates B (direct sum O2) at s_i = i/(ngs-1), theta_j = 2 pi j/nth, zeta_k = (2 pi/nfp) k/nze (one field period;
+ * every count >= 4) on the device, asynchronously on `stream`, and from then on every call on this field --
+ * gc_field_eval, gc_rhs_eval, gc_trace, gc_trace_sampled, gc_trace_host, gc_pzeta_eval -- evaluates B and its three
+ * derivatives as the tensor-product cubic Lagrange interpolant of those node values (radial stencil clamped as in
+ * O1, angular stencils periodic and centred on the cell); profiles and the perturbation keep their radial tables.
+ * Traces then run on GC_KERNEL_GRID whatever gc_set_kernel says.  (0, 0, 0) drops the grid and returns to the direct
+ * sum.  The table takes 32 ngs (nth + 3) nze bytes of device memory (every node stored with its three
+ * zeta neighbours so that a stencil row is one 32-byte load), owned by the field.  GC_EINVAL for
+ * a count in 1..3 or a field with kmnc / kmns; calls must not overlap traces that still run on this field. */
+int gc_field_set_grid(gc_field* f, int32_t ngs, int32_t nth, int32_t nze, void* stream);
 
 /* O2 at n points.  DEVICE pointers.  B [n]; dB [3][n] = dB/ds, dB/dtheta, dB/dzeta, or NULL.
  * Asynchronous on `stream` (a cudaStream_t, NULL = default stream).  Used to compute mu and by tests. */
@@ -206,6 +221,41 @@ int gc_pzeta_eval(const gc_field* f, double mass, double charge, int64_t n, cons
  * -log10(|WB_1 - WB_2| / max(|WB_1|, |WB_2|)) capped at 16 (NaN for series with fewer than 4 samples). */
 int gc_birkhoff(int64_t n, int64_t nsamp, const double* series, int64_t j_first, const int32_t* sample_end,
                 double* out, void* stream);
+
+/* ---- NEXT-3 of SURVEY.md section 8(f): the symplectic integrator ("A symplectic integrator for
+ * non-canonical guiding-center orbits uses the explicit-implicit Euler scheme of (Albert et al., 2020)"; PAPER.md:60-62,
+ * Fig. 1 left: "the symplectic algorithm exhibits a stable moving time average of the energy").  Reading A28 of
+ * static fields with K = 0 (GC_EINVAL for a field with modes or kmnc / kmns); canonical momenta
+ * p_theta = q (psi0 s + rho I), p_zeta = q (rho G - chi), rho = m v_par / (q B); state (s, theta, zeta, p_zeta); one
+ * step of size dt solves  p_theta' - p_theta + dt dH/dtheta = 0,  p_zeta' - p_zeta + dt dH/dzeta = 0  for
+ * (s', p_zeta') at the old angles (to a last update below newton_tol max(1, |x|) of x = (s, p_zeta / (q psi0)),
+ * status 4 after max_iter iterations) and then advances the angles explicitly with the derivatives of H at the new
+ * (s', p_zeta').  Works on the direct harmonic sum and on the 3-D interpolant of gc_field_set_grid alike. */
+typedef struct {
+  double mass, charge;        /* kg, C                                                              */
+  double t0, dt;              /* s; fixed step dt > 0                                               */
+  int64_t nsteps;             /* steps per particle and call                                        */
+  double s_loss, s_min;       /* stop rules of O7, checked after every step                         */
+  double newton_tol;          /* e.g. 1e-13                                                         */
+  int64_t max_iter;           /* e.g. 50                                                            */
+  int64_t flags;              /* 0 or GC_TRACE_RESUME (skip particles whose status is not 0; counters add up) */
+} gc_symplectic_params;
+
+/* DEVICE pointers, asynchronous on `stream`.
+ *   in : s0, th0, ze0, vpar0 (m/s), mu (J/T) [n] (may alias the rows of y_out as in gc_trace);
+ *        chi_nodes [ns]: chi at the radial nodes, d chi / d psi = iota, interpolated like every profile (O1); the
+ *        integrator takes d chi / d s from THAT interpolant where the equations of motion have psi0 iota
+ *   out: y_out [4][n] = s, theta, zeta, v_par (m/s); t_out [n] = t0 + steps dt; status [n]: GC_ST_TMAX (all steps
+ *        done), GC_ST_LOST, GC_ST_AXIS, GC_ST_NONFINITE (iteration failed or a non-finite value: the state before
+ *        the failed step is reported); n_steps, n_iter [n] or NULL: steps taken, iterations in total
+ *   samples [4][nsamp][n] or nsamp = 0: sample 0 = the initial state, sample j = the state after step
+ *        j * sample_stride; sample_end [n] = samples written (under GC_TRACE_RESUME the count continues from
+ *        sample_end; nsteps should then be a multiple of sample_stride). */
+int gc_trace_symplectic(const gc_field* f, const gc_symplectic_params* params, int64_t n,
+                        const double* s0, const double* th0, const double* ze0, const double* vpar0,
+                        const double* mu, const double* chi_nodes,
+                        double* y_out, double* t_out, int32_t* status, int32_t* n_steps, int32_t* n_iter,
+                        int64_t sample_stride, int64_t nsamp, double* samples, int32_t* sample_end, void* stream);
 
 /* Kernel choice (GC_KERNEL_*) for later gc_trace / gc_rhs_eval calls on this field (default AUTO); GC_EINVAL
  * if the field does not fit the requested kernel. */

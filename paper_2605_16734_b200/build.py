@@ -12,7 +12,7 @@ SO = os.path.join(_HERE, "libgcorbit.so")
 PROBES_SO = os.path.join(_HERE, "libgcprobes.so")
 SOURCES = ["gcorbit_api.cu"]
 PROBE_SOURCES = ["fp64_probes.cu"]
-HEADERS = ["device_math.cuh", "field.cuh", "kernels_generic.cuh", "kernels_warp.cuh", "kernels_tile.cuh", "kernels_mma.cuh",
+HEADERS = ["device_math.cuh", "field.cuh", "kernels_generic.cuh", "kernels_grid.cuh", "kernels_lane.cuh", "kernels_symplectic.cuh", "kernels_warp.cuh", "kernels_tile.cuh", "kernels_mma.cuh",
            os.path.join("..", "..", "include", "gcorbit.h")]
 
 

@@ -43,6 +43,12 @@ struct FieldDev {
   const double* mma_image_bs;
   const double* mma_image_kc;
   const double* mma_image_ks;
+  // NEXT-2 (kernels_grid.cuh): node values of B on the (s, theta, zeta) grid over one field period in the gather
+  // layout grid[ngs][nth + 3][nze][4] (entry k = nodes k .. k+3 mod nze; three theta rows repeated); nullptr = the
+  // direct harmonic sum.  th_scale = nth / 2 pi, ze_scale = nze nfp / 2 pi (nodes per radian).
+  const double* grid;
+  int ngs, nth, nze;
+  double th_scale, ze_scale, inv_nth, inv_nze;
 };
 
 // Integrator parameters as the kernels see them (gc_trace_params + derived values).

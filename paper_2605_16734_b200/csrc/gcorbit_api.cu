@@ -14,6 +14,8 @@
 
 namespace gc { constexpr int GC_ST_NONFINITE_ = 4; }
 #include "kernels_generic.cuh"
+#include "kernels_lane.cuh"
+#include "kernels_symplectic.cuh"
 #include "kernels_warp.cuh"
 #include "kernels_tile.cuh"
 #include "kernels_mma.cuh"
@@ -77,6 +79,7 @@ struct gc_field {
   bool extra = false;               // NEXT-4 tables present (bmns, kmnc or kmns): mma or generic kernel only
   int mma_smem = 0;                 // dynamic shared memory of the mma kernel
   int mma_blocks_per_sm = 0;
+  double* grid = nullptr;           // NEXT-2: node values of the 3-D interpolant (gc_field_set_grid), else nullptr
 };
 
 namespace {
@@ -217,6 +220,7 @@ const void* mma_fn_t(const gc_field* f) {
 const void* mma_fn(const gc_field* f, bool sample = false) { return sample ? mma_fn_t<true>(f) : mma_fn_t<false>(f); }
 
 int resolve_kernel(const gc_field* f, int64_t n) {
+  if (f->dev.grid) return GC_KERNEL_GRID;                  // the field IS the interpolant while a grid is set
   if (f->kernel != GC_KERNEL_AUTO) return f->kernel;
   if (f->mma_ok && n >= GC_TILE_MIN_PARTICLES) return GC_KERNEL_MMA;
   if (f->tile_ok && n >= GC_TILE_MIN_PARTICLES) return GC_KERNEL_TILE;
@@ -438,6 +442,33 @@ int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, c
   return GC_OK;
 }
 
+// One launch of the lane kernel (generic field or 3-D interpolant): persistent grid, atomic particle queue.
+long long lane_blocks(const gc_field* f, long long n, bool grid) {
+  int per_sm = 0;
+  const void* fn = grid ? (const void*)gc::trace_lane_kernel<true> : (const void*)gc::trace_lane_kernel<false>;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, gc::kLaneThreads, gc::kLaneSmemBytes) != cudaSuccess || per_sm < 1)
+    per_sm = 1;
+  long long blocks = (n + gc::kLaneThreads - 1) / gc::kLaneThreads;
+  const long long cap = (long long)f->sm_count * per_sm;
+  if (blocks > cap) blocks = cap;
+  return blocks < 1 ? 1 : blocks;
+}
+
+int launch_lane(const gc_field* f, gc::TraceDev& t, bool grid, cudaStream_t st) {
+  unsigned long long* counter = nullptr;
+  GC_CUDA(cudaMallocFromPoolAsync((void**)&counter, sizeof(unsigned long long), f->pool, st));
+  GC_CUDA(cudaMemsetAsync(counter, 0, sizeof(unsigned long long), st));
+  t.work_counter = counter;
+  const unsigned blocks = (unsigned)lane_blocks(f, t.n, grid);
+  if (grid) gc::trace_lane_kernel<true><<<blocks, gc::kLaneThreads, gc::kLaneSmemBytes, st>>>(f->dev, t);
+  else gc::trace_lane_kernel<false><<<blocks, gc::kLaneThreads, gc::kLaneSmemBytes, st>>>(f->dev, t);
+  const cudaError_t le = cudaGetLastError();
+  const cudaError_t fe = cudaFreeAsync(counter, st);          // also on a failed launch
+  GC_CUDA(le);
+  GC_CUDA(fe);
+  return GC_OK;
+}
+
 int build_trace_dev(const gc_field* f, const gc_trace_params* p, int64_t n, gc::TraceDev* t) {
   if (!f || !p) return fail(GC_EINVAL, "gc_trace: NULL field or params");
   if (n < 0 || n > 0x7fffffffLL) return fail(GC_EINVAL, "gc_trace: n < 0 or n >= 2^31");
@@ -464,6 +495,7 @@ const char* gc_last_error(void) { return g_last_error.c_str(); }
 int gc_field_destroy(gc_field* f) {
   if (!f) return GC_OK;
   for (void* p : f->allocs) cudaFree(p);
+  if (f->grid) cudaFree(f->grid);
   if (f->host_slab) cudaFree(f->host_slab);
   if (f->host_stream) cudaStreamDestroy(f->host_stream);
   if (f->pool) cudaMemPoolDestroy(f->pool);                // waits for nothing: callers synchronise before destroying
@@ -606,6 +638,46 @@ int gc_set_option(gc_field* f, int32_t option, int64_t value) {
   }
 }
 
+int gc_field_set_grid(gc_field* f, int32_t ngs, int32_t nth, int32_t nze, void* stream) {
+  if (!f) return fail(GC_EINVAL, "gc_field_set_grid: NULL field");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (f->grid) {                                             // drop the old interpolant first
+    GC_CUDA(cudaStreamSynchronize(st));
+    cudaFree(f->grid);
+    f->grid = nullptr;
+    f->dev.grid = nullptr;
+    f->dev.ngs = f->dev.nth = f->dev.nze = 0;
+  }
+  if (ngs == 0 && nth == 0 && nze == 0) return GC_OK;        // back to the direct harmonic sum
+  if (ngs < 4 || nth < 4 || nze < 4) return fail(GC_EINVAL, "gc_field_set_grid: every node count must be >= 4 (or all 0)");
+  if (f->dev.kmnc || f->dev.kmns)
+    return fail(GC_EINVAL, "gc_field_set_grid: fields with a covariant radial component K are traced by the direct sum only");
+  const size_t nodes = (size_t)ngs * (size_t)nth * (size_t)nze;
+  const size_t total = (size_t)ngs * (size_t)(nth + 3) * (size_t)nze * 4;
+  if (total > ((size_t)1 << 33)) return fail(GC_EINVAL, "gc_field_set_grid: table larger than 64 GiB");
+  double *g = nullptr, *plain = nullptr;
+  GC_CUDA(cudaMalloc((void**)&g, total * sizeof(double)));
+  if (cudaMallocAsync((void**)&plain, nodes * sizeof(double), st) != cudaSuccess) {
+    cudaFree(g);
+    return fail(GC_ENOMEM, "gc_field_set_grid: device allocation failed");
+  }
+  const int tb = 256;
+  gc::grid_build_kernel<<<(unsigned)((nodes + tb - 1) / tb), tb, 0, st>>>(f->dev, ngs, nth, nze, plain);
+  gc::grid_pack_kernel<<<(unsigned)((total / 4 + tb - 1) / tb), tb, 0, st>>>(ngs, nth, nze, plain, g);
+  const cudaError_t le = cudaGetLastError();
+  cudaFreeAsync(plain, st);
+  if (le != cudaSuccess) { cudaFree(g); GC_CUDA(le); }
+  constexpr double kTwoPi = 6.283185307179586476925286766559;
+  f->grid = g;
+  f->dev.grid = g;
+  f->dev.ngs = ngs; f->dev.nth = nth; f->dev.nze = nze;
+  f->dev.th_scale = (double)nth / kTwoPi;
+  f->dev.ze_scale = (double)nze * (double)f->dev.nfp / kTwoPi;
+  f->dev.inv_nth = 1.0 / (double)nth;
+  f->dev.inv_nze = 1.0 / (double)nze;
+  return GC_OK;
+}
+
 int gc_kernel_info(const gc_field* f, int64_t n, int32_t* kernel, int32_t* blocks, int32_t* threads, int32_t* smem,
                    int32_t* regs) {
   if (!f) return fail(GC_EINVAL, "gc_kernel_info: NULL field");
@@ -625,8 +697,10 @@ int gc_kernel_info(const gc_field* f, int64_t n, int32_t* kernel, int32_t* block
     GC_CUDA(cudaFuncGetAttributes(&at, w->trace_fn));
     b = f->sm_count; t = gc::kWarpsPerBlock * 32; s = w->smem_bytes;
   } else {
-    GC_CUDA(cudaFuncGetAttributes(&at, (const void*)gc::trace_generic_kernel));
-    b = f->sm_count * 4; t = 128; s = 0;
+    const bool grid = k == GC_KERNEL_GRID;
+    GC_CUDA(cudaFuncGetAttributes(&at, grid ? (const void*)gc::trace_lane_kernel<true>
+                                            : (const void*)gc::trace_lane_kernel<false>));
+    b = (int)lane_blocks(f, n, grid); t = gc::kLaneThreads; s = gc::kLaneSmemBytes;
   }
   if (kernel) *kernel = k;
   if (blocks) *blocks = b;
@@ -744,10 +818,7 @@ int trace_common(const gc_field* f, const gc_trace_params* params, int64_t n, co
     GC_CUDA(le);
     GC_CUDA(fe);
   } else {
-    long long blocks = (n + 127) / 128;
-    if (blocks > (long long)f->sm_count * 16) blocks = (long long)f->sm_count * 16;
-    gc::trace_generic_kernel<<<(unsigned)blocks, 128, 0, st>>>(f->dev, t);
-    GC_CUDA(cudaGetLastError());
+    return launch_lane(f, t, kern == GC_KERNEL_GRID, st);
   }
   return GC_OK;
 }
@@ -772,6 +843,39 @@ int gc_trace_sampled(const gc_field* f, const gc_trace_params* params, int64_t n
     return fail(GC_EINVAL, "gc_trace_sampled: records no Poincare crossings (poincare_capacity must be 0)");
   return trace_common(f, params, n, s0, th0, ze0, vpar0, mu, h_inout, y_out, t_out, status, n_acc, n_rej, n_forced,
                       nullptr, nullptr, sample_t0, sample_dt, nsamp, samples, sample_end, stream);
+}
+
+int gc_trace_symplectic(const gc_field* f, const gc_symplectic_params* p, int64_t n, const double* s0,
+                        const double* th0, const double* ze0, const double* vpar0, const double* mu,
+                        const double* chi_nodes, double* y_out, double* t_out, int32_t* status, int32_t* n_steps,
+                        int32_t* n_iter, int64_t sample_stride, int64_t nsamp, double* samples, int32_t* sample_end,
+                        void* stream) {
+  if (!f || !p) return fail(GC_EINVAL, "gc_trace_symplectic: NULL field or params");
+  if (f->dev.nk > 0 || f->dev.kmnc || f->dev.kmns)
+    return fail(GC_EINVAL, "gc_trace_symplectic: static fields with K = 0 only (no modes, no kmnc / kmns)");
+  if (n < 0 || n > 0x7fffffffLL) return fail(GC_EINVAL, "gc_trace_symplectic: n < 0 or n >= 2^31");
+  if (!(p->mass > 0.0) || p->charge == 0.0 || !(p->dt > 0.0) || !std::isfinite(p->t0) || p->nsteps < 0 ||
+      !(p->newton_tol > 0.0) || p->max_iter < 1 || p->max_iter > 1000 || (p->flags & ~(int64_t)GC_TRACE_RESUME) != 0)
+    return fail(GC_EINVAL, "gc_trace_symplectic: invalid integrator specification");
+  if (nsamp < 0 || (nsamp > 0 && (sample_stride < 1 || !samples || !sample_end)))
+    return fail(GC_EINVAL, "gc_trace_symplectic: nsamp > 0 needs sample_stride >= 1, samples and sample_end");
+  if (n == 0) return GC_OK;
+  if (!s0 || !th0 || !ze0 || !vpar0 || !mu || !chi_nodes || !y_out || !t_out || !status)
+    return fail(GC_EINVAL, "gc_trace_symplectic: NULL particle array or chi_nodes");
+  gc::SymplecticDev d{};
+  d.mass = p->mass; d.charge = p->charge; d.t0 = p->t0; d.dt = p->dt; d.s_loss = p->s_loss; d.s_min = p->s_min;
+  d.tol = p->newton_tol; d.nsteps = p->nsteps; d.n = n; d.sample_stride = sample_stride > 0 ? sample_stride : 1;
+  d.nsamp = nsamp; d.max_iter = (int)p->max_iter; d.resume = (p->flags & GC_TRACE_RESUME) ? 1 : 0;
+  d.s0 = s0; d.th0 = th0; d.ze0 = ze0; d.vpar0 = vpar0; d.mu = mu; d.chi = chi_nodes;
+  d.y_out = y_out; d.t_out = t_out; d.status = status; d.n_steps = n_steps; d.n_iter = n_iter;
+  d.samples = samples; d.sample_end = sample_end;
+  const int tb = 128;
+  long long blocks = (n + tb - 1) / tb;
+  if (blocks > (long long)f->sm_count * 16) blocks = (long long)f->sm_count * 16;
+  if (f->dev.grid) gc::trace_symplectic_kernel<true><<<(unsigned)blocks, tb, 0, (cudaStream_t)stream>>>(f->dev, d);
+  else gc::trace_symplectic_kernel<false><<<(unsigned)blocks, tb, 0, (cudaStream_t)stream>>>(f->dev, d);
+  GC_CUDA(cudaGetLastError());
+  return GC_OK;
 }
 
 int gc_pzeta_eval(const gc_field* f, double mass, double charge, int64_t n, const double* y, const double* t,

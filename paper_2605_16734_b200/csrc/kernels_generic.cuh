@@ -5,6 +5,7 @@
 #pragma once
 #include "device_math.cuh"
 #include "field.cuh"
+#include "kernels_grid.cuh"
 
 namespace gc {
 
@@ -174,6 +175,27 @@ __device__ inline void rhs_generic(const FieldDev& f, double mass, double charge
   dy[3] *= inv_v_ref;
 }
 
+// The same with B from the tricubic interpolant (NEXT-2); profiles and perturbation from the radial tables as always.
+__device__ inline void rhs_grid(const FieldDev& f, double mass, double charge, double mu, double v_ref,
+                                double inv_v_ref, double t, const double y[4], double dy[4]) {
+  int i0;
+  double w[4], dw[4], fb[4], pt[9];
+  lagrange_weights(f.ns, y[0], i0, w, dw);
+  Profiles p;
+  interp4(f.G, 1, i0, w, dw, p.G, p.Gs);
+  interp4(f.I, 1, i0, w, dw, p.I, p.Is);
+  interp4(f.iota, 1, i0, w, dw, p.io, p.ios);
+  eval_B_grid(f, y[0], y[1], y[2], fb);
+  if (f.nk > 0) {
+    eval_pert_generic(f, i0, w, dw, p, y[1], y[2], t, pt);
+  } else {
+#pragma unroll
+    for (int i = 0; i < 9; ++i) pt[i] = 0.0;
+  }
+  gc_algebra(mass, charge, mu, f.inv_psi0, y[3] * v_ref, fb, p, pt, dy);
+  dy[3] *= inv_v_ref;
+}
+
 // ---- O8: Poincare records from the continuous extension of an accepted step ------------------------------
 // r1..r5 are the dense-output coefficients of components s, theta, zeta (index 0..2).
 struct Dense3 { double r1[3], r2[3], r3[3], r4[3], r5[3]; };
@@ -306,177 +328,6 @@ __device__ inline double loss_root(double y0, double yn0, double hk1, double hk7
   return tau;
 }
 
-// ---- generic trace: one thread per particle ----------------------------------------------------------------
-__global__ void __launch_bounds__(128) trace_generic_kernel(FieldDev f, TraceDev p) {
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < p.n;
-       i += (long long)gridDim.x * blockDim.x) {
-    if (p.resume && p.status[i] != 0) continue;            // finished in an earlier segment
-    const double mu = p.mu[i];
-    double y[4] = {p.s0[i], p.th0[i], p.ze0[i], p.vpar0[i] * p.inv_v_ref};
-    double t = p.t0;
-    double h = (p.h_inout && p.h_inout[i] > 0.0) ? p.h_inout[i] : p.h0;
-    if (h < p.h_min) h = p.h_min;
-    double k[7][4], yn[4], ys[4];
-    long long attempts = 0;
-    int n_acc = 0, n_rej = 0, n_forced = 0, st = -1;
-    bool prev_rejected = false;
-    long long jn = 0;
-    if (p.nsamp > 0) {
-      jn = first_sample_index(p, t);
-      if (jn < p.nsamp && sample_time(p, jn) == t) {         // a sample on t0 is the initial state
-#pragma unroll
-        for (int c = 0; c < 4; ++c) p.samples[((long long)c * p.nsamp + jn) * p.n + i] = c == 3 ? p.vpar0[i] : y[c];
-        ++jn;
-      }
-    }
-    rhs_generic(f, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, t, y, k[0]);
-    if (!finite4(y[0], y[1], y[2], y[3]) || !finite4(k[0][0], k[0][1], k[0][2], k[0][3])) st = GC_ST_NONFINITE_;
-    else if (!(t < p.t_max)) st = 0;
-    while (st < 0) {
-      double h_try = h;
-      bool clipped = false;
-      if (t + h_try >= p.t_max) { h_try = p.t_max - t; clipped = true; }
-      if (!(t + h_try > t)) { st = GC_ST_NONFINITE_; break; }
-      const bool forced = prev_rejected && p.h_min > 0.0 && h == p.h_min;
-#pragma unroll
-      for (int c = 0; c < 4; ++c) ys[c] = fma(h_try * dp::a21, k[0][c], y[c]);
-      rhs_generic(f, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, fma(dp::c2, h_try, t), ys, k[1]);
-#pragma unroll
-      for (int c = 0; c < 4; ++c) ys[c] = fma(h_try, fma(dp::a32, k[1][c], dp::a31 * k[0][c]), y[c]);
-      rhs_generic(f, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, fma(dp::c3, h_try, t), ys, k[2]);
-#pragma unroll
-      for (int c = 0; c < 4; ++c)
-        ys[c] = fma(h_try, fma(dp::a43, k[2][c], fma(dp::a42, k[1][c], dp::a41 * k[0][c])), y[c]);
-      rhs_generic(f, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, fma(dp::c4, h_try, t), ys, k[3]);
-#pragma unroll
-      for (int c = 0; c < 4; ++c)
-        ys[c] = fma(h_try, fma(dp::a54, k[3][c], fma(dp::a53, k[2][c], fma(dp::a52, k[1][c], dp::a51 * k[0][c]))),
-                    y[c]);
-      rhs_generic(f, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, fma(dp::c5, h_try, t), ys, k[4]);
-#pragma unroll
-      for (int c = 0; c < 4; ++c)
-        ys[c] = fma(h_try, fma(dp::a65, k[4][c], fma(dp::a64, k[3][c], fma(dp::a63, k[2][c],
-                    fma(dp::a62, k[1][c], dp::a61 * k[0][c])))), y[c]);
-      rhs_generic(f, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, t + h_try, ys, k[5]);
-#pragma unroll
-      for (int c = 0; c < 4; ++c)
-        yn[c] = fma(h_try, fma(dp::a76, k[5][c], fma(dp::a75, k[4][c], fma(dp::a74, k[3][c],
-                    fma(dp::a73, k[2][c], dp::a71 * k[0][c])))), y[c]);
-      rhs_generic(f, p.mass, p.charge, mu, p.v_ref, p.inv_v_ref, t + h_try, yn, k[6]);
-      ++attempts;
-      double acc = 0.0;
-#pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        const double delta = h_try * fma(dp::e7, k[6][c], fma(dp::e6, k[5][c], fma(dp::e5, k[4][c],
-                                 fma(dp::e4, k[3][c], fma(dp::e3, k[2][c], dp::e1 * k[0][c])))));
-        const double sk = fma(p.rtol, fmax(fabs(y[c]), fabs(yn[c])), p.atol);
-        const double r = delta / sk;
-        acc = fma(r, r, acc);
-      }
-      const double err = sqrt(acc * 0.25);
-      const bool finite = finite4(yn[0], yn[1], yn[2], yn[3]) &&
-                          finite4(k[6][0], k[6][1], k[6][2], k[6][3]) && isfinite(err);
-      bool accept;
-      if (forced) {
-        if (!finite) { st = GC_ST_NONFINITE_; break; }
-        accept = true;
-      } else {
-        accept = finite && err <= 1.0;
-      }
-      if (accept) {
-        const double sc = scale_after_accept(err);
-        const double h_next = prev_rejected ? h_try * fmin(sc, 1.0) : h_try * sc;
-        if (p.poincare_capacity > 0 && p.section == 1) {              // O8b: bounce section
-          if (bounce_crossed(y[3], yn[3])) {
-            double hk1[4], hk7[4], hd[4];
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-              hk1[c] = h_try * k[0][c]; hk7[c] = h_try * k[6][c];
-              hd[c] = h_try * fma(dp::d7, k[6][c], fma(dp::d6, k[5][c], fma(dp::d5, k[4][c],
-                                fma(dp::d4, k[3][c], fma(dp::d3, k[2][c], dp::d1 * k[0][c])))));
-            }
-            bounce_emit(y, yn, hk1, hk7, hd, i, t, h_try, p.poincare, p.poincare_capacity, p.poincare_count);
-          }
-        } else if (p.poincare_capacity > 0 && floor(y[2] / 6.283185307179586476925286766559) !=
-                                                  floor(yn[2] / 6.283185307179586476925286766559)) {
-          Dense3 d;
-#pragma unroll
-          for (int c = 0; c < 3; ++c) {
-            d.r1[c] = y[c];
-            d.r2[c] = yn[c] - y[c];
-            d.r3[c] = h_try * k[0][c] - d.r2[c];
-            d.r4[c] = d.r2[c] - h_try * k[6][c] - d.r3[c];
-            d.r5[c] = h_try * fma(dp::d7, k[6][c], fma(dp::d6, k[5][c], fma(dp::d5, k[4][c],
-                                  fma(dp::d4, k[3][c], fma(dp::d3, k[2][c], dp::d1 * k[0][c])))));
-          }
-          poincare_emit(d, i, t, h_try, y[2], yn[2], p.poincare, p.poincare_capacity, p.poincare_count);
-        }
-        const double t_new = clipped ? p.t_max : t + h_try;
-        if (p.nsamp > 0 && jn < p.nsamp && sample_time(p, jn) <= t_new) {       // O9
-          double hd[4];
-#pragma unroll
-          for (int c = 0; c < 4; ++c)
-            hd[c] = h_try * fma(dp::d7, k[6][c], fma(dp::d6, k[5][c], fma(dp::d5, k[4][c],
-                              fma(dp::d4, k[3][c], fma(dp::d3, k[2][c], dp::d1 * k[0][c])))));
-          while (jn < p.nsamp) {
-            const double tj = sample_time(p, jn);
-            if (tj > t_new) break;
-            const double tau = (tj - t) / h_try;
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-              const double v = dense_component(y[c], yn[c], h_try * k[0][c], h_try * k[6][c], hd[c], tau);
-              p.samples[((long long)c * p.nsamp + jn) * p.n + i] = c == 3 ? v * p.v_ref : v;
-            }
-            ++jn;
-          }
-        }
-        const bool lost_now = yn[0] >= p.s_loss;
-        double t_rep = t_new;
-        if (lost_now && p.refine_loss && y[0] < p.s_loss) {            // O7b
-          double hd[4];
-#pragma unroll
-          for (int c = 0; c < 4; ++c)
-            hd[c] = h_try * fma(dp::d7, k[6][c], fma(dp::d6, k[5][c], fma(dp::d5, k[4][c],
-                              fma(dp::d4, k[3][c], fma(dp::d3, k[2][c], dp::d1 * k[0][c])))));
-          const double tau = loss_root(y[0], yn[0], h_try * k[0][0], h_try * k[6][0], hd[0], p.s_loss);
-#pragma unroll
-          for (int c = 0; c < 4; ++c) yn[c] = dense_component(y[c], yn[c], h_try * k[0][c], h_try * k[6][c], hd[c], tau);
-          t_rep = fma(tau, h_try, t);
-        }
-        t = lost_now ? t_rep : t_new;
-#pragma unroll
-        for (int c = 0; c < 4; ++c) { y[c] = yn[c]; k[0][c] = k[6][c]; }
-        ++n_acc;
-        if (forced) ++n_forced;
-        prev_rejected = false;
-        if (!clipped) h = h_next;
-        if (h < p.h_min) h = p.h_min;
-        if (lost_now) st = 1;
-        else if (y[0] <= p.s_min) st = 2;
-        else if (clipped) st = 0;
-        else if (attempts >= p.max_steps) st = 3;
-      } else {
-        ++n_rej;
-        h = h_try * scale_after_reject(err);
-        if (h < p.h_min) h = p.h_min;
-        prev_rejected = true;
-        if (attempts >= p.max_steps) st = 3;
-      }
-    }
-    p.y_out[0 * p.n + i] = y[0];
-    p.y_out[1 * p.n + i] = y[1];
-    p.y_out[2 * p.n + i] = y[2];
-    p.y_out[3 * p.n + i] = y[3] * p.v_ref;
-    p.t_out[i] = t;
-    p.status[i] = st;
-    if (p.h_inout) p.h_inout[i] = h;
-    if (p.n_acc) p.n_acc[i] = (p.resume ? p.n_acc[i] : 0) + n_acc;
-    if (p.n_rej) p.n_rej[i] = (p.resume ? p.n_rej[i] : 0) + n_rej;
-    if (p.n_forced) p.n_forced[i] = (p.resume ? p.n_forced[i] : 0) + n_forced;
-    if (p.nsamp > 0 && p.sample_end) p.sample_end[i] = (int)jn;
-  }
-}
-
 // ---- A17: P_zeta = q ((rho + alpha) G - chi) at n states and times ----------------------------------------------
 __global__ void pzeta_eval_kernel(FieldDev f, double mass, double charge, long long n, const double* y,
                                   const double* t, const double* chi_nodes, double* out) {
@@ -490,7 +341,8 @@ __global__ void pzeta_eval_kernel(FieldDev f, double mass, double charge, long l
   interp4(f.G, 1, i0, w, dw, p.G, p.Gs);
   interp4(f.I, 1, i0, w, dw, p.I, p.Is);
   interp4(f.iota, 1, i0, w, dw, p.io, p.ios);
-  eval_B_generic(f, i0, w, dw, th, ze, fb);
+  if (f.grid) eval_B_grid(f, s, th, ze, fb);
+  else eval_B_generic(f, i0, w, dw, th, ze, fb);
   double al = 0.0;
   if (f.nk > 0) {
     eval_pert_generic(f, i0, w, dw, p, th, ze, t ? t[i] : 0.0, pt);
@@ -536,10 +388,47 @@ __global__ void field_eval_kernel(FieldDev f, long long n, const double* s, cons
   if (i >= n) return;
   int i0;
   double w[4], dw[4], out[4];
-  lagrange_weights(f.ns, s[i], i0, w, dw);
-  eval_B_generic(f, i0, w, dw, th[i], ze[i], out);
+  if (f.grid) {
+    eval_B_grid(f, s[i], th[i], ze[i], out);               // NEXT-2: the field is the interpolant
+  } else {
+    lagrange_weights(f.ns, s[i], i0, w, dw);
+    eval_B_generic(f, i0, w, dw, th[i], ze[i], out);
+  }
   B[i] = out[0];
   if (dB) { dB[i] = out[1]; dB[n + i] = out[2]; dB[2 * n + i] = out[3]; }
+}
+
+// NEXT-2 setup, step 1: node values of B (direct sum O2), plain[ngs][nth][nze].  One thread per node.
+__global__ void grid_build_kernel(FieldDev f, int ngs, int nth, int nze, double* plain) {
+  constexpr double kTwoPi = 6.283185307179586476925286766559;
+  const long long total = (long long)ngs * nth * nze;
+  const long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (e >= total) return;
+  const int k = (int)(e % nze);
+  const int j = (int)((e / nze) % nth);
+  const int i = (int)(e / ((long long)nze * nth));
+  const double s = (double)i / (double)(ngs - 1);
+  const double th = kTwoPi * (double)j / (double)nth;
+  const double ze = kTwoPi * (double)k / ((double)nze * (double)f.nfp);
+  int i0;
+  double w[4], dw[4], out[4];
+  lagrange_weights(f.ns, s, i0, w, dw);
+  eval_B_generic(f, i0, w, dw, th, ze, out);
+  plain[e] = out[0];
+}
+
+// Step 2: the gather layout of kernels_grid.cuh, grid[ngs][nth + 3][nze][4]: entry (i, jp, k) = nodes k .. k+3 (mod
+// nze) of row (i, jp mod nth).  One thread per entry.
+__global__ void grid_pack_kernel(int ngs, int nth, int nze, const double* plain, double* grid) {
+  const long long total = (long long)ngs * (nth + 3) * nze;
+  const long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (e >= total) return;
+  const int k = (int)(e % nze);
+  const int jp = (int)((e / nze) % (nth + 3));
+  const int i = (int)(e / ((long long)nze * (nth + 3)));
+  const double* row = plain + ((long long)i * nth + jp % nth) * nze;
+#pragma unroll
+  for (int c = 0; c < 4; ++c) grid[e * 4 + c] = row[(k + c) % nze];
 }
 
 __global__ void kcov_eval_kernel(FieldDev f, long long n, const double* s, const double* th, const double* ze,
@@ -579,7 +468,8 @@ __global__ void rhs_eval_generic_kernel(FieldDev f, double mass, double charge, 
   if (i >= n) return;
   const double yy[4] = {y[i], y[n + i], y[2 * n + i], y[3 * n + i]};
   double dy[4];
-  rhs_generic(f, mass, charge, mu[i], 1.0, 1.0, t, yy, dy);
+  if (f.grid) rhs_grid(f, mass, charge, mu[i], 1.0, 1.0, t, yy, dy);
+  else rhs_generic(f, mass, charge, mu[i], 1.0, 1.0, t, yy, dy);
   for (int c = 0; c < 4; ++c) dydt[c * n + i] = dy[c];
 }
 

@@ -16,14 +16,14 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 SO_PATH = os.path.join(_HERE, "libgcorbit.so")
 
 GC_OK, GC_EINVAL, GC_ENOMEM, GC_ECUDA = 0, -1, -2, -3
-GC_KERNEL_AUTO, GC_KERNEL_GENERIC, GC_KERNEL_WARP, GC_KERNEL_TILE, GC_KERNEL_MMA = 0, 1, 2, 3, 4
+GC_KERNEL_AUTO, GC_KERNEL_GENERIC, GC_KERNEL_WARP, GC_KERNEL_TILE, GC_KERNEL_MMA, GC_KERNEL_GRID = 0, 1, 2, 3, 4, 5
 GC_TILE_MIN_PARTICLES = 4096
 GC_OPT_WAVE_PARTICLES, GC_OPT_CHUNK_ATTEMPTS = 1, 2
 ST_TMAX, ST_LOST, ST_AXIS, ST_MAXSTEPS, ST_NONFINITE = 0, 1, 2, 3, 4
 
 EXPORTS = ["gc_field_create", "gc_field_destroy", "gc_field_eval", "gc_pert_eval", "gc_rhs_eval", "gc_trace",
            "gc_trace_host", "gc_set_kernel", "gc_set_option", "gc_kernel_info", "gc_last_error",
-           "gc_trace_sampled", "gc_pzeta_eval", "gc_birkhoff", "gc_kcov_eval"]
+           "gc_trace_sampled", "gc_pzeta_eval", "gc_birkhoff", "gc_kcov_eval", "gc_field_set_grid", "gc_trace_symplectic"]
 
 
 class GcError(RuntimeError):
@@ -74,6 +74,8 @@ def load_library():
         L.gc_pzeta_eval.argtypes = [vp, dbl, dbl, i64, vp, vp, vp, vp, vp]
         L.gc_birkhoff.argtypes = [i64, i64, vp, i64, vp, vp, vp]
         L.gc_set_kernel.argtypes = [vp, i32]
+        L.gc_field_set_grid.argtypes = [vp, i32, i32, i32, vp]
+        L.gc_trace_symplectic.argtypes = [vp, C.POINTER(gc_symplectic_params), i64] + [vp] * 11 + [i64, i64, vp, vp, vp]
         L.gc_set_option.argtypes = [vp, i32, i64]
         L.gc_kernel_info.argtypes = [vp, C.c_int64] + [C.POINTER(i32)] * 5
         for name in EXPORTS:
@@ -134,6 +136,23 @@ class TraceResult:
     sample_end: object = None     # [n] int32
 
 
+class gc_symplectic_params(C.Structure):
+    _fields_ = [("mass", C.c_double), ("charge", C.c_double), ("t0", C.c_double), ("dt", C.c_double),
+                ("nsteps", C.c_int64), ("s_loss", C.c_double), ("s_min", C.c_double), ("newton_tol", C.c_double),
+                ("max_iter", C.c_int64), ("flags", C.c_int64)]
+
+
+@dataclass
+class SymplecticResult:
+    y: object            # [4][n]: s, theta, zeta, v_par (m/s)
+    t: object            # [n]
+    status: object       # [n] int32
+    n_steps: object
+    n_iter: object
+    samples: object = None        # [4][nsamp][n]
+    sample_end: object = None
+
+
 class Field:
     """gc_field_create / gc_field_destroy.  ``fld`` carries host numpy tables (workloads.Field layout)."""
 
@@ -181,11 +200,17 @@ class Field:
     def set_option(self, option: int, value: int):
         _check(load_library().gc_set_option(self._h, int(option), int(value)))
 
+    def set_grid(self, ngs: int, nth: int, nze: int):
+        """gc_field_set_grid (NEXT-2): B becomes the tricubic interpolant of its node values; (0, 0, 0) drops it."""
+        torch = _torch()
+        _check(load_library().gc_field_set_grid(self._h, int(ngs), int(nth), int(nze), _stream_ptr(torch)))
+
     def kernel_info(self, n: int = 1 << 20) -> dict:
         """Kernel and launch geometry gc_trace uses for an ensemble of n particles."""
         v = [C.c_int32(0) for _ in range(5)]
         _check(load_library().gc_kernel_info(self._h, int(n), *[C.byref(x) for x in v]))
-        return dict(kernel={GC_KERNEL_GENERIC: "generic", GC_KERNEL_WARP: "warp", GC_KERNEL_TILE: "tile", GC_KERNEL_MMA: "mma"}[v[0].value],
+        return dict(kernel={GC_KERNEL_GENERIC: "generic", GC_KERNEL_WARP: "warp", GC_KERNEL_TILE: "tile", GC_KERNEL_MMA: "mma",
+                            GC_KERNEL_GRID: "grid"}[v[0].value],
                     blocks=v[1].value, threads=v[2].value, smem_bytes=v[3].value, regs=v[4].value)
 
     # ---- gc_field_eval / gc_pert_eval / gc_rhs_eval (device tensors in, device tensors out) ------------------
@@ -282,6 +307,30 @@ class Field:
         out = torch.empty(n, dtype=torch.float64, device=y.device)
         _check(load_library().gc_pzeta_eval(self._h, float(mass), float(charge), n, _dp(y), _dp(t), _dp(chi_nodes),
                                             _dp(out), _stream_ptr(torch)))
+        return out
+
+    def trace_symplectic(self, mass, charge, s0, th0, ze0, vpar0, mu, chi_nodes, dt, nsteps, t0=0.0, s_loss=1.0,
+                         s_min=1e-3, newton_tol=1e-13, max_iter=50, sample_stride=0, nsamp=0, out=None, flags=0):
+        """gc_trace_symplectic (NEXT-3).  Returns a SymplecticResult of device tensors; ``out`` may carry the result
+        of a previous call (buffers reused; with GC_TRACE_RESUME the call continues it in place)."""
+        torch = _torch()
+        n = s0.numel()
+        dev = s0.device
+        if out is None:
+            out = SymplecticResult(torch.empty((4, n), dtype=torch.float64, device=dev),
+                                   torch.empty(n, dtype=torch.float64, device=dev),
+                                   torch.zeros(n, dtype=torch.int32, device=dev),
+                                   torch.zeros(n, dtype=torch.int32, device=dev),
+                                   torch.zeros(n, dtype=torch.int32, device=dev),
+                                   torch.full((4, int(nsamp), n), float("nan"), dtype=torch.float64, device=dev)
+                                   if nsamp else None,
+                                   torch.zeros(n, dtype=torch.int32, device=dev) if nsamp else None)
+        p = gc_symplectic_params(float(mass), float(charge), float(t0), float(dt), int(nsteps), float(s_loss),
+                                 float(s_min), float(newton_tol), int(max_iter), int(flags))
+        _check(load_library().gc_trace_symplectic(
+            self._h, C.byref(p), C.c_int64(n), _dp(s0), _dp(th0), _dp(ze0), _dp(vpar0), _dp(mu), _dp(chi_nodes),
+            _dp(out.y), _dp(out.t), _dp(out.status), _dp(out.n_steps), _dp(out.n_iter), C.c_int64(int(sample_stride)),
+            C.c_int64(int(nsamp)), _dp(out.samples), _dp(out.sample_end), _stream_ptr(torch)))
         return out
 
     def trace_resume(self, spec, state: TraceResult, mu, t0, t_max, poincare_capacity=0) -> TraceResult:

@@ -1,0 +1,355 @@
+"""-m gpu: NEXT-2 of SURVEY.md section 8(f) on the device -- B as a local tricubic interpolant of its own node values
+(gc_field_set_grid, kernels_grid.cuh, the lane kernel) against the oracle's interpolant (oracle_field_set_grid;
+PAPER.md:48,80,111; reading A27), element by element through the C ABI."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+from gpu_common import (gpu_trace, make_case, oracle_conditioning, record_info, rel_diff,
+                        sort_poincare, to_dev, COND_FACTOR, FLIP_RTOL, SAME_RTOL)
+
+pytestmark = pytest.mark.gpu
+
+# node counts per config: deliberately not powers of two and not multiples of four on config 0
+GRIDS = {0: (37, 29, 23), 1: (101, 64, 48), 2: (101, 64, 48), 3: (101, 64, 48), 4: (101, 64, 48)}
+
+
+@pytest.fixture(scope="module")
+def gcases():
+    cache = {}
+
+    def get(config, n):
+        if (config, n) not in cache:
+            fld, spec, P, OF, GF, mu = make_case(config, n)
+            OF.set_grid(*GRIDS[config])
+            GF.set_grid(*GRIDS[config])
+            from paper_2605_16734_b200 import workloads as W
+            mu = W.mu_from(P, OF.eval_B_many(P.s, P.theta, P.zeta)[:, 0])   # mu from the interpolated B, both sides
+            cache[(config, n)] = (fld, spec, P, OF, GF, mu)
+        return cache[(config, n)]
+    return get
+
+
+def test_set_grid_selects_the_grid_kernel_and_can_be_dropped(gcases):
+    from paper_2605_16734_b200 import gcorbit as G, workloads as W
+    fld = W.make_field(1)
+    GF = G.Field(fld)
+    assert GF.kernel_info(100_000)["kernel"] == "mma"
+    GF.set_grid(21, 16, 12)
+    info = GF.kernel_info(100_000)
+    assert info["kernel"] == "grid" and info["threads"] == 128 and info["blocks"] >= 148
+    assert GF.kernel_info(5)["kernel"] == "grid"
+    GF.set_grid(0, 0, 0)
+    assert GF.kernel_info(100_000)["kernel"] == "mma"
+    for bad in [(3, 16, 16), (16, 3, 16), (16, 16, 2), (0, 16, 16), (-4, 16, 16)]:
+        with pytest.raises(G.GcError) as e:
+            GF.set_grid(*bad)
+        assert e.value.code == G.GC_EINVAL
+    assert GF.kernel_info(100_000)["kernel"] == "mma"
+
+
+def test_set_grid_rejects_fields_with_K():
+    import dataclasses
+    from paper_2605_16734_b200 import gcorbit as G, workloads as W
+    fld = W.make_field(0)
+    fld = dataclasses.replace(fld, kmnc=1e-3 * np.ones_like(fld.bmnc))
+    GF = G.Field(fld)
+    with pytest.raises(G.GcError) as e:
+        GF.set_grid(16, 16, 16)
+    assert e.value.code == G.GC_EINVAL
+
+
+@pytest.mark.parametrize("config", [0, 1])
+def test_grid_nodes_and_field_eval_match_oracle(gcases, config):
+    import torch
+    fld, spec, P, OF, GF, mu = gcases(config, 400)
+    ngs, nth, nze = GRIDS[config]
+    # (1) the node values: evaluating the interpolant AT a node returns that node (weights 0, 1, 0, 0)
+    V = OF.grid()
+    rng = np.random.default_rng(5)
+    ii, jj, kk = rng.integers(0, ngs, 300), rng.integers(0, nth, 300), rng.integers(0, nze, 300)
+    s = ii / (ngs - 1.0)
+    th = 2.0 * np.pi * jj / nth
+    ze = 2.0 * np.pi * kk / (nze * fld.nfp)
+    B, _ = GF.field_eval(to_dev(s), to_dev(th), to_dev(ze))
+    torch.cuda.synchronize()
+    assert np.abs(B.cpu().numpy() / V[ii, jj, kk] - 1.0).max() < 1e-13
+    # (2) random points, with s outside [0, 1], negative and large unwrapped angles, a cell that wraps the period
+    s = P.s.copy(); th = P.theta.copy(); ze = P.zeta.copy()
+    s[:4] = [-0.01, 0.0, 1.0, 1.02]
+    th[4:8] += 5.0e3
+    ze[8:12] -= 2.0e4
+    th[12:16] = [-1e-9, 2 * np.pi - 1e-9, 2 * np.pi, -3.0]
+    ze[16:20] = [-1e-9, 2 * np.pi / fld.nfp - 1e-9, 2 * np.pi / fld.nfp, -0.7]
+    B, dB = GF.field_eval(to_dev(s), to_dev(th), to_dev(ze))
+    torch.cuda.synchronize()
+    ref = OF.eval_B_many(s, th, ze)
+    B, dB = B.cpu().numpy(), dB.cpu().numpy()
+    assert np.abs(B / ref[:, 0] - 1.0).max() < 1e-13
+    for c in range(3):
+        assert np.abs(dB[c] - ref[:, 1 + c]).max() <= 1e-11 * np.abs(ref[:, 1 + c]).max(), c
+    # the interpolant is not the direct sum: the two differ by the interpolation error (else the test tests nothing)
+    direct = np.array([OF.eval_B_sum(s[i], th[i], ze[i])[0] for i in range(20, 60)])
+    assert 1e-9 < np.abs(B[20:60] / direct - 1.0).max() < 5e-2
+
+
+@pytest.mark.parametrize("config", [0, 2, 4])
+def test_grid_rhs_matches_oracle(gcases, config):
+    import torch
+    fld, spec, P, OF, GF, mu = gcases(config, 256)
+    t = 3.3e-5
+    y = np.stack([P.s, P.theta + 50.0, P.zeta - 30.0, P.vpar])
+    got = GF.rhs_eval(spec.mass, spec.charge, t, to_dev(y), to_dev(mu))
+    torch.cuda.synchronize()
+    got = got.cpu().numpy()
+    ref = np.array([OF.rhs(spec.mass, spec.charge, mu[i], 1.0, t, y[:, i]) for i in range(P.n)]).T
+    for c in range(4):
+        scale = np.maximum(np.abs(ref[c]), 1e-6 * np.abs(ref[c]).max())
+        assert (np.abs(got[c] - ref[c]) / scale).max() < 1e-9, (c, (np.abs(got[c] - ref[c]) / scale).max())
+
+
+# ---- traces -------------------------------------------------------------------------------------------------------
+# The tricubic Lagrange interpolant is C0: its derivatives jump at every cell face in all three directions.  At
+# rtol 1e-9 the controller then rejects more attempts than it accepts (oracle, config 0: 1340 rejected against 1118
+# accepted per 1e-5 s) and the step-size sequence becomes an ill-conditioned function of the state: the error norm
+# divides a defect of the size of a derivative jump by rtol |y|, so a 1e-15 change of theta0 moves the ORACLE's own
+# end state by 1e-9 (median) to 1e-6 after 1e-6 s even where the (accepted, rejected) counts stay the same (measured
+# with the oracle alone).  No implementation can match the oracle more closely than the oracle
+# matches itself, so the trace tests are: (A) ONE attempted step from a given step size, where no sequence exists yet,
+# at rounding level; (B) short horizons with each particle's tolerance taken from the oracle's own spread (the rule of
+# gpu_common for the direct sum) and ensemble quantiles bounded by the oracle's; (C) a full-size launch sampled.
+GRID_FLIP_RTOL = 1e-4          # a flipped decision: oracle against itself reaches 5e-6 at 1e-6 s
+
+
+def test_grid_single_attempt_matches_oracle_at_rounding_level(gcases):
+    """max_steps = 1: every particle makes exactly one Dormand-Prince attempt with its own given step size (1e-9 ..
+    1e-7 s, so some are accepted and some rejected); final state, decision and next proposal against the oracle."""
+    import dataclasses
+    import torch
+    for config in (0, 2, 4):
+        fld, spec, P, OF, GF, mu = gcases(config, 256)
+        one = dataclasses.replace(spec, max_steps=1)
+        h0 = 10.0 ** np.random.default_rng(3).uniform(-9.0, -7.0, P.n)
+        h = to_dev(h0.copy())
+        r = GF.trace(one, to_dev(P.s), to_dev(P.theta), to_dev(P.zeta), to_dev(P.vpar), to_dev(mu), h_inout=h,
+                     t_max=1e-3)
+        torch.cuda.synchronize()
+        o = OF.trace(one, P.s, P.theta, P.zeta, P.vpar, mu, h_in=h0, t_max=1e-3)
+        assert np.array_equal(r.status.cpu().numpy(), o.status) and (o.status == 3).all()
+        assert np.array_equal(r.n_acc.cpu().numpy(), o.n_acc) and np.array_equal(r.n_rej.cpu().numpy(), o.n_rej)
+        assert 0 < o.n_acc.sum() < P.n                                   # both branches taken
+        rel = rel_diff(r.y.cpu().numpy(), o.y, spec.v_ref)
+        assert rel.max() < 1e-12, rel.max()
+        assert np.array_equal(r.t.cpu().numpy(), o.t)
+        # next proposal h 0.9 err^(-1/5): err is a sum that cancels to h^6 divided by rtol |y|; at h = 1e-9 it is
+        # mostly rounding noise of the stage values, so the proposals agree to 1e-8 (median) .. 6e-6 only
+        assert np.abs(r.h.cpu().numpy() / o.h - 1.0).max() < 1e-4
+        record_info("grid_single_attempt", label=f"config {config} grid {GRIDS[config]}", particles=P.n,
+                    max_rel=float(rel.max()), accepted=int(o.n_acc.sum()),
+                    max_rel_h_next=float(np.abs(r.h.cpu().numpy() / o.h - 1.0).max()))
+
+
+def _grid_parity(r, o, cond, spec, label, min_same):
+    """The rule of gpu_common.assert_trace_parity adapted to a field on which the oracle is ill-conditioned everywhere:
+    each particle on the oracle's step sequence is held to max(1e-9, 10 x its own oracle spread); the spread is the
+    maximum of only four oracle reruns, so in a large ensemble a few particles exceed ten times it by chance -- at most
+    1 % may, and they stay below the flip bound like every other particle; and the ensemble of device-against-oracle
+    differences must look like the ensemble of oracle-against-oracle differences (median and 95 % quantile)."""
+    spread, tspread, stable = cond
+    stg = r.status.cpu().numpy()
+    bad = np.nonzero((stg != o.status) & stable)[0]
+    assert bad.size == 0, f"{label}: status differs at {bad[:8]}"
+    same = (r.n_acc.cpu().numpy() == o.n_acc) & (r.n_rej.cpu().numpy() == o.n_rej)
+    assert same.mean() >= min_same, f"{label}: only {same.mean() * 100:.1f} % on the oracle's step sequence"
+    rel = rel_diff(r.y.cpu().numpy(), o.y, spec.v_ref)
+    over = same & stable & (rel > np.maximum(SAME_RTOL, COND_FACTOR * spread))
+    assert over.sum() <= max(0, int(0.01 * len(rel))), f"{label}: {over.sum()} of {len(rel)} beyond 10 x oracle spread"
+    assert rel[stable].max() <= GRID_FLIP_RTOL, f"{label}: max rel diff {rel[stable].max():.3e}"
+    if same.any():
+        assert np.array_equal(r.n_forced.cpu().numpy()[same], o.n_forced[same])
+    med, med_o = float(np.median(rel)), float(np.median(spread))
+    q95, q95_o = float(np.quantile(rel, 0.95)), float(np.quantile(spread, 0.95))
+    assert med <= max(1e-11, 3.0 * med_o), (label, med, med_o)
+    assert q95 <= max(1e-9, 3.0 * q95_o), (label, q95, q95_o)
+    info = dict(same_frac=float(same.mean()), max_rel=float(rel[stable].max()), median_rel=med,
+                oracle_median_spread=med_o, q95_rel=q95, oracle_q95_spread=q95_o, beyond_10x_spread=int(over.sum()),
+                within_1e9=float((rel <= SAME_RTOL).mean()))
+    record_info("grid_trace_parity", label=label, particles=len(rel), **info)
+    return info
+
+
+def test_grid_trace_config0_short_horizon(gcases):
+    """All 512 particles of BASELINE.json configs[0] on the interpolated field, 3e-7 s (36 accepted + 40 rejected
+    attempts per particle at rtol 1e-9)."""
+    fld, spec, P, OF, GF, mu = gcases(0, None)
+    T = 3e-7
+    r = gpu_trace(GF, spec, P, mu, t_max=T)
+    o = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=T)
+    cond = oracle_conditioning(OF, spec, P, mu, o, t_max=T)
+    print(_grid_parity(r, o, cond, spec, "config 0 grid 3e-7 s", min_same=0.85))
+
+
+@pytest.mark.parametrize("config,n,t_max", [(1, 296, 3e-7), (2, 256, 3e-7), (3, 301, 1e-6), (4, 256, 5e-7)])
+def test_grid_trace_subsamples(gcases, config, n, t_max):
+    fld, spec, P, OF, GF, mu = gcases(config, n)
+    cap = 4096 if config == 4 else 0
+    r = gpu_trace(GF, spec, P, mu, t_max=t_max, poincare_capacity=cap)
+    o = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=t_max, poincare_capacity=cap)
+    cond = oracle_conditioning(OF, spec, P, mu, o, t_max=t_max)
+    info = _grid_parity(r, o, cond, spec, f"config {config} grid {t_max:g} s", min_same=0.85)
+    print(f"config {config} grid: {info}")
+    if cap:
+        # O8 records of the particles on the oracle's step sequence
+        same = (r.n_acc.cpu().numpy() == o.n_acc) & (r.n_rej.cpu().numpy() == o.n_rej)
+        a, b = sort_poincare(r.poincare.cpu().numpy()), sort_poincare(o.poincare)
+        a, b = a[same[a[:, 0].astype(int)]], b[same[b[:, 0].astype(int)]]
+        assert len(b) > 0 and np.array_equal(a[:, 0], b[:, 0])
+        assert np.abs(a[:, 1] - b[:, 1]).max() <= 1e-6 * t_max
+        assert np.abs(a[:, 2] - b[:, 2]).max() <= 1e-7
+
+
+def test_grid_trace_config0_full_horizon_is_statistically_the_oracle(gcases):
+    """BASELINE.json configs[0] in full (512 alphas, 1e-4 s, rtol 1e-9) on the coarse grid: step sequences have long
+    diverged (the oracle's own runs under a 1-ulp change share 0.4 % of them), so what is compared is what is unique:
+    the loss fraction within the Monte Carlo standard error, the distribution of the end radius (two-sample KS), the
+    work done, and the spread itself, which must not exceed the oracle's own."""
+    from scipy.stats import ks_2samp
+    fld, spec, P, OF, GF, mu = gcases(0, None)
+    r = gpu_trace(GF, spec, P, mu)
+    o = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu)
+    o2 = OF.trace(spec, P.s, P.theta * (1.0 + 1e-15), P.zeta, P.vpar, mu)
+    st = r.status.cpu().numpy()
+    assert set(np.unique(st)) <= {0, 1} and set(np.unique(o.status)) <= {0, 1}
+    f_dev, f_orc = float((st == 1).mean()), float((o.status == 1).mean())
+    assert abs(f_dev - f_orc) <= 2.0 * np.sqrt(2.0 * max(f_orc, 1.0 / P.n) * (1.0 - f_orc) / P.n)
+    y = r.y.cpu().numpy()
+    both = (st == 0) & (o.status == 0) & (o2.status == 0)
+    assert ks_2samp(y[0][st == 0], o.y[0][o.status == 0]).pvalue > 0.01
+    d_dev, d_orc = np.abs(y[0] - o.y[0])[both], np.abs(o2.y[0] - o.y[0])[both]
+    assert np.median(d_dev) <= 3.0 * np.median(d_orc) + 1e-12
+    assert np.quantile(d_dev, 0.95) <= 3.0 * np.quantile(d_orc, 0.95) + 1e-12
+    att = (r.n_acc + r.n_rej).sum().item() / float((o.n_acc + o.n_rej).sum())
+    assert abs(att - 1.0) < 0.03                                         # same work, statistically
+    record_info("grid_full_horizon", label="config 0 grid 1e-4 s", lost_device=f_dev, lost_oracle=f_orc,
+                median_ds_device=float(np.median(d_dev)), median_ds_oracle_self=float(np.median(d_orc)),
+                attempts_ratio=att)
+
+
+@pytest.mark.parametrize("n", [1, 7, 33, 148 * 8 * 4 + 3])
+def test_grid_trace_ragged_sizes(gcases, n):
+    fld, spec, P, OF, GF, mu = gcases(0, 148 * 8 * 4 + 3)
+    Q = P.head(n)
+    r = gpu_trace(GF, spec, Q, mu[:n], t_max=2e-7)
+    o = OF.trace(spec, Q.s, Q.theta, Q.zeta, Q.vpar, mu[:n], t_max=2e-7)
+    cond = oracle_conditioning(OF, spec, Q, mu[:n], o, t_max=2e-7)
+    _grid_parity(r, o, cond, spec, f"grid n={n}", min_same=0.0 if n < 100 else 0.85)
+
+
+def test_grid_trace_empty_and_resume_segments(gcases):
+    import torch
+    from paper_2605_16734_b200 import gcorbit as G
+    fld, spec, P, OF, GF, mu = gcases(0, 200)
+    e = P.head(0)
+    r = gpu_trace(GF, spec, e, mu[:0], t_max=1e-6)
+    assert r.y.shape[1] == 0
+    # two segments in place (GC_TRACE_RESUME) against the oracle run with the same segments (A24)
+    seg = 1.5e-7
+    s, th, ze, vp, mud = (to_dev(x) for x in (P.s, P.theta, P.zeta, P.vpar, mu))
+    h = torch.zeros(P.n, dtype=torch.float64, device="cuda:0")
+    st = GF.trace(spec, s, th, ze, vp, mud, h_inout=h, t0=0.0, t_max=seg)
+    GF.trace_resume(spec, st, mud, t0=seg, t_max=2 * seg)
+    torch.cuda.synchronize()
+    o1 = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu, t0=0.0, t_max=seg)
+    alive = o1.status == 0
+    o2 = OF.trace(spec, o1.y[0, alive], o1.y[1, alive], o1.y[2, alive], o1.y[3, alive], mu[alive], h_in=o1.h[alive],
+                  t0=seg, t_max=2 * seg)
+    y_ref, st_ref = o1.y.copy(), o1.status.copy()
+    y_ref[:, alive], st_ref[alive] = o2.y, o2.status
+    assert np.array_equal(st.status.cpu().numpy(), st_ref)
+    n_ref = o1.n_acc.copy(); n_ref[alive] += o2.n_acc
+    same = st.n_acc.cpu().numpy() == n_ref
+    rel = rel_diff(st.y.cpu().numpy(), y_ref, spec.v_ref)
+    assert same.mean() >= 0.85 and np.median(rel) < 1e-9 and rel[same].max() < 1e-6 and rel.max() < GRID_FLIP_RTOL
+
+
+def test_grid_samples_and_pzeta_match_oracle(gcases):
+    """NEXT-1 on the interpolated field: uniform-time samples (gc_trace_sampled) and P_zeta at the samples."""
+    import torch
+    fld, spec, P, OF, GF, mu = gcases(0, 64)
+    nsamp, t_max = 33, 3e-7
+    dt = t_max / (nsamp - 1)
+    r = GF.trace_sampled(spec, to_dev(P.s), to_dev(P.theta), to_dev(P.zeta), to_dev(P.vpar), to_dev(mu), 0.0, dt,
+                         nsamp, t_max=t_max)
+    torch.cuda.synchronize()
+    o = OF.trace_sampled(spec, P.s, P.theta, P.zeta, P.vpar, mu, 0.0, dt, nsamp, t_max=t_max)
+    assert np.array_equal(r.sample_end.cpu().numpy(), o.nsampled)
+    same = (r.n_acc.cpu().numpy() == o.n_acc) & (r.n_rej.cpu().numpy() == o.n_rej)
+    assert same.mean() >= 0.85
+    S, So = r.samples.cpu().numpy(), o.samples
+    floor = np.array([1.0, 1.0, 1.0, spec.v_ref])[:, None, None]
+    ok = np.arange(nsamp)[:, None] < o.nsampled[None, :]
+    rel = (np.abs(S - So) / np.maximum(np.abs(So), floor)).max(axis=0)
+    assert np.median(rel[ok & same[None, :]]) < 1e-10 and rel[ok & same[None, :]].max() < 1e-6
+    s_n = np.arange(fld.ns) / (fld.ns - 1)
+    chi = fld.psi0 * np.concatenate([[0.0], np.cumsum(0.5 * (fld.iota[1:] + fld.iota[:-1]) * np.diff(s_n))])
+    y = So[:, :, same][:, :8, :].reshape(4, -1)
+    pz = GF.pzeta_eval(spec.mass, spec.charge, to_dev(y), None, to_dev(chi))
+    torch.cuda.synchronize()
+    ref = np.array([OF.pzeta(spec.mass, spec.charge, chi, *y[:, i], 0.0) for i in range(y.shape[1])])
+    assert np.abs(pz.cpu().numpy() / ref - 1.0).max() < 1e-12
+
+
+@pytest.mark.parametrize("config,seg", [(3, 5e-7)])
+def test_grid_full_size_launch_sampled(config, seg):
+    """BASELINE.json configs[3] at FULL size (10^6 particles) on the grid the bench uses (101 x 128 x 128), two
+    resumed segments; 48 sampled particles (and a few lost ones) one by one against the oracle's interpolant."""
+    import torch
+    import oracle
+    from paper_2605_16734_b200 import gcorbit as G, workloads as W
+    fld, spec = W.make_field(config), W.make_spec(config)
+    OF, GF = oracle.OracleField(fld), G.Field(fld)
+    OF.set_grid(101, 128, 128)
+    GF.set_grid(101, 128, 128)
+    P = W.make_particles(config)
+    assert GF.kernel_info(P.n)["kernel"] == "grid"
+    s, th, ze, vp = (to_dev(x) for x in (P.s, P.theta, P.zeta, P.vpar))
+    B, _ = GF.field_eval(s, th, ze, derivs=False)
+    mu_d = to_dev(0.5 * spec.mass * P.vperp2()) / B
+    h = torch.zeros(P.n, dtype=torch.float64, device="cuda:0")
+    st = GF.trace(spec, s, th, ze, vp, mu_d, h_inout=h, t0=0.0, t_max=seg)
+    GF.trace_resume(spec, st, mu_d, t0=seg, t_max=2 * seg)
+    torch.cuda.synchronize()
+    status = st.status.cpu().numpy()
+    assert set(np.unique(status)) <= {0, 1, 2}
+    assert (st.t.cpu().numpy()[status == 0] == 2 * seg).all()
+    idx = np.random.default_rng(7).choice(P.n, 48, replace=False)
+    idx = np.union1d(idx, np.nonzero(status == 1)[0][:8])
+    mu = mu_d.cpu().numpy()
+    Q = W.Particles(P.s[idx], P.theta[idx], P.zeta[idx], P.pitch[idx], P.speed[idx])
+
+    def two_segments(Qp):
+        o1 = OF.trace(spec, Qp.s, Qp.theta, Qp.zeta, Qp.vpar, mu[idx], t0=0.0, t_max=seg)
+        alive = o1.status == 0
+        o2 = OF.trace(spec, o1.y[0, alive], o1.y[1, alive], o1.y[2, alive], o1.y[3, alive], mu[idx][alive],
+                      h_in=o1.h[alive], t0=seg, t_max=2 * seg)
+        y_ref, st_ref = o1.y.copy(), o1.status.copy()
+        y_ref[:, alive], st_ref[alive] = o2.y, o2.status
+        acc, rej = o1.n_acc.copy(), o1.n_rej.copy()
+        acc[alive] += o2.n_acc
+        rej[alive] += o2.n_rej
+        return y_ref, st_ref, acc, rej
+
+    y_ref, st_ref, acc_ref, rej_ref = two_segments(Q)
+    spread = np.zeros(len(idx))
+    for a, b in [(1e-15, 0.0), (-1e-15, 0.0), (0.0, 1e-15), (0.0, -1e-15)]:
+        y2, st2, _, _ = two_segments(W.Particles(Q.s, Q.theta * (1.0 + a), Q.zeta * (1.0 + b), Q.pitch, Q.speed))
+        spread = np.maximum(spread, rel_diff(y2, y_ref, spec.v_ref))
+    assert np.array_equal(status[idx], st_ref)
+    same = (st.n_acc.cpu().numpy()[idx] == acc_ref) & (st.n_rej.cpu().numpy()[idx] == rej_ref)
+    rel = rel_diff(st.y.cpu().numpy()[:, idx], y_ref, spec.v_ref)
+    tol = np.where(same, np.maximum(SAME_RTOL, COND_FACTOR * spread), GRID_FLIP_RTOL)
+    assert same.mean() >= 0.9 and np.median(rel) < 1e-10 and (rel <= tol).all(), (same.mean(), rel.max())
+    record_info("full_size_sampled", label=f"config {config} grid 101x128x128, {P.n} particles, 2 x {seg:g} s",
+                particles=len(idx), max_rel=float(rel.max()), median_rel=float(np.median(rel)),
+                within=float((rel <= SAME_RTOL).mean()), same_frac=float(same.mean()))

@@ -25,6 +25,16 @@ struct FieldDev {
   const double* bmns;
   const double* kmnc;
   const double* kmns;
+  // the same four tables with the row stride padded to nhp = roundup4(nh) (zero fill) and 32-byte aligned rows, so the
+  // lane kernel and the point evaluations read FOUR consecutive harmonics of a node row with one 256-bit load
+  // (nullptr = absent); xmp / xnp are xm / xn padded with (0, 0) harmonics
+  const double* bmnc4;
+  const double* bmns4;
+  const double* kmnc4;
+  const double* kmns4;
+  const int* xmp;
+  const int* xnp;
+  int nhp;
   // packed by-node layout of the warp kernel (kernels_warp.cuh): rows[node][it][lane]
   const double* rows;
   int M, N;              // max xm, max |xn|

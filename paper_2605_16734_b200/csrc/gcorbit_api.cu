@@ -4,6 +4,7 @@
 
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdio>
@@ -564,7 +565,28 @@ int gc_field_create(const gc_field_desc* d, gc_field** out) {
   double* iom = nullptr;
   up(inv_om.data(), d->nk, &iom);
   up(d->mode_phase, d->nk, &ph); up(d->phihat, (size_t)d->ns * d->nk, &phihat);
+  // node rows padded to a multiple of four harmonics (field.cuh)
+  double *bmnc4 = nullptr, *bmns4 = nullptr, *kmnc4 = nullptr, *kmns4 = nullptr;
+  int *xmp = nullptr, *xnp = nullptr;
+  const int nhp = (d->nh + 3) & ~3;
+  {
+    std::vector<double> pk((size_t)d->ns * nhp);
+    auto pad = [&](const double* tab, double** devp) {
+      if (!tab) return;
+      std::fill(pk.begin(), pk.end(), 0.0);
+      for (int i = 0; i < d->ns; ++i)
+        std::memcpy(&pk[(size_t)i * nhp], tab + (size_t)i * d->nh, sizeof(double) * d->nh);
+      up(pk.data(), pk.size(), devp);
+    };
+    pad(d->bmnc, &bmnc4); pad(d->bmns, &bmns4); pad(d->kmnc, &kmnc4); pad(d->kmns, &kmns4);
+    std::vector<int> im(nhp, 0), in(nhp, 0);
+    std::memcpy(im.data(), d->xm, sizeof(int) * d->nh);
+    std::memcpy(in.data(), d->xn, sizeof(int) * d->nh);
+    up(im.data(), im.size(), &xmp);
+    up(in.data(), in.size(), &xnp);
+  }
   if (rc == GC_OK) {
+    v.bmnc4 = bmnc4; v.bmns4 = bmns4; v.kmnc4 = kmnc4; v.kmns4 = kmns4; v.xmp = xmp; v.xnp = xnp; v.nhp = nhp;
     v.xm = xm; v.xn = xn; v.bmnc = bmnc; v.G = G; v.I = I; v.iota = iota;
     v.mode_m = mm; v.mode_n = mn; v.omega = om; v.inv_omega = iom; v.phase = ph; v.phihat = phihat;
     v.bmns = bmns; v.kmnc = kmnc; v.kmns = kmns;

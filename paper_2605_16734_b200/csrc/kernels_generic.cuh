@@ -22,30 +22,92 @@ __device__ __forceinline__ void interp4(const double* tab, int stride, int i0, c
 
 // One Fourier series X = sum_k [ xc_k(s) cos(a_k) + xs_k(s) sin(a_k) ], a_k = m_k theta - n_k nfp zeta, with its
 // derivatives in s, theta, zeta; either table may be nullptr (NEXT-4: the sin table of B, both tables of K).
+// The harmonic list comes in the caller's order, so the trig factors are looked up by (m, n): cos / sin (m theta) and
+// cos / sin (n nfp zeta) are built once per call by angle-addition recurrences from ONE sincos each (north_star piece
+// 2) into small per-thread tables, and cos(a_k) = c_m C_n + s_m S_n, sin(a_k) = s_m C_n - c_m S_n cost two FMA each
+// instead of a 40-instruction sincos per harmonic.  Fields with max m or max |n| above kGenericTrigMax keep one sincos
+// per harmonic.
+constexpr int kGenericTrigMax = 32;
+
 __device__ inline void eval_series_generic(const FieldDev& f, const double* tabc, const double* tabs, int i0,
-                                           const double w[4], const double dw[4], double th, double ze, double out[4]) {
+                                           const double w[4], const double dw[4], double th, double ze, double out[4],
+                                           const double* tabc4 = nullptr, const double* tabs4 = nullptr) {
   const double thr = reduce_2pi(th);
   const double phr = reduce_2pi((double)f.nfp * ze);
   double B = 0.0, Bs = 0.0, Bth = 0.0, Bze = 0.0;
-  for (int k = 0; k < f.nh; ++k) {
-    const double m = (double)__ldg(f.xm + k), n = (double)__ldg(f.xn + k);
-    double sn, cs;
-    sincos_poly(fma(m, thr, -n * phr), sn, cs);
-    if (tabc) {
-      double b, bs;
-      interp4(tabc + k, f.nh, i0, w, dw, b, bs);
-      B = fma(b, cs, B);
-      Bs = fma(bs, cs, Bs);
-      Bth = fma(-m * b, sn, Bth);
-      Bze = fma(n * (double)f.nfp * b, sn, Bze);
+  const bool tables = f.M <= kGenericTrigMax && f.N <= kGenericTrigMax;
+  double cm[kGenericTrigMax + 1], sm[kGenericTrigMax + 1], cn[kGenericTrigMax + 1], sn_[kGenericTrigMax + 1];
+  if (tables) {
+    double s1, c1;
+    sincos_poly(thr, s1, c1);
+    cm[0] = 1.0; sm[0] = 0.0;
+    for (int m = 1; m <= f.M; ++m) {
+      cm[m] = fma(cm[m - 1], c1, -sm[m - 1] * s1);
+      sm[m] = fma(sm[m - 1], c1, cm[m - 1] * s1);
     }
-    if (tabs) {
-      double b, bs;
-      interp4(tabs + k, f.nh, i0, w, dw, b, bs);
-      B = fma(b, sn, B);
-      Bs = fma(bs, sn, Bs);
-      Bth = fma(m * b, cs, Bth);
-      Bze = fma(-n * (double)f.nfp * b, cs, Bze);
+    sincos_poly(phr, s1, c1);
+    cn[0] = 1.0; sn_[0] = 0.0;
+    for (int n = 1; n <= f.N; ++n) {
+      cn[n] = fma(cn[n - 1], c1, -sn_[n - 1] * s1);
+      sn_[n] = fma(sn_[n - 1], c1, cn[n - 1] * s1);
+    }
+  }
+  // four harmonics per pass: one 256-bit load per stencil row and table (rows padded to nhp, field.cuh)
+  const bool vec = tables && (!tabc || tabc4) && (!tabs || tabs4);
+  const int nloop = vec ? f.nhp : f.nh;
+  for (int k0 = 0; k0 < nloop; k0 += vec ? 4 : 1) {
+    double bc[4], bcs[4], bsn[4], bss[4];
+    if (vec) {
+#pragma unroll
+      for (int e = 0; e < 4; ++e) bc[e] = bcs[e] = bsn[e] = bss[e] = 0.0;
+#pragma unroll
+      for (int a = 0; a < 4; ++a) {
+        double t[4];
+        if (tabc) {
+          ldg256(tabc4 + (size_t)(i0 + a) * f.nhp + k0, t[0], t[1], t[2], t[3]);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) { bc[e] = fma(w[a], t[e], bc[e]); bcs[e] = fma(dw[a], t[e], bcs[e]); }
+        }
+        if (tabs) {
+          ldg256(tabs4 + (size_t)(i0 + a) * f.nhp + k0, t[0], t[1], t[2], t[3]);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) { bsn[e] = fma(w[a], t[e], bsn[e]); bss[e] = fma(dw[a], t[e], bss[e]); }
+        }
+      }
+    }
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      if (!vec && e > 0) break;
+      const int k = k0 + e;
+      const int mi = __ldg((vec ? f.xmp : f.xm) + k), ni = __ldg((vec ? f.xnp : f.xn) + k);
+      const double m = (double)mi, n = (double)ni;
+      double sn, cs;
+      if (tables) {
+        const int na = ni < 0 ? -ni : ni;
+        const double Sn = ni < 0 ? -sn_[na] : sn_[na];              // sin(n phi) is odd in n
+        cs = fma(cm[mi], cn[na], sm[mi] * Sn);                      // cos(m theta - n phi)
+        sn = fma(sm[mi], cn[na], -cm[mi] * Sn);                     // sin(m theta - n phi)
+      } else {
+        sincos_poly(fma(m, thr, -n * phr), sn, cs);
+      }
+      if (tabc) {
+        double b, bs;
+        if (vec) { b = bc[e]; bs = bcs[e]; }
+        else interp4(tabc + k, f.nh, i0, w, dw, b, bs);
+        B = fma(b, cs, B);
+        Bs = fma(bs, cs, Bs);
+        Bth = fma(-m * b, sn, Bth);
+        Bze = fma(n * (double)f.nfp * b, sn, Bze);
+      }
+      if (tabs) {
+        double b, bs;
+        if (vec) { b = bsn[e]; bs = bss[e]; }
+        else interp4(tabs + k, f.nh, i0, w, dw, b, bs);
+        B = fma(b, sn, B);
+        Bs = fma(bs, sn, Bs);
+        Bth = fma(m * b, cs, Bth);
+        Bze = fma(-n * (double)f.nfp * b, cs, Bze);
+      }
     }
   }
   out[0] = B; out[1] = Bs; out[2] = Bth; out[3] = Bze;
@@ -53,7 +115,7 @@ __device__ inline void eval_series_generic(const FieldDev& f, const double* tabc
 
 __device__ inline void eval_B_generic(const FieldDev& f, int i0, const double w[4], const double dw[4],
                                       double th, double ze, double out[4]) {
-  eval_series_generic(f, f.bmnc, f.bmns, i0, w, dw, th, ze, out);
+  eval_series_generic(f, f.bmnc, f.bmns, i0, w, dw, th, ze, out, f.bmnc4, f.bmns4);
 }
 
 // out = Phi, Phi_psi, Phi_th, Phi_ze, al, al_psi, al_th, al_ze, al_t
@@ -167,7 +229,7 @@ __device__ inline void rhs_generic(const FieldDev& f, double mass, double charge
   }
   if (f.kmnc || f.kmns) {
     double fk[4];
-    eval_series_generic(f, f.kmnc, f.kmns, i0, w, dw, y[1], y[2], fk);
+    eval_series_generic(f, f.kmnc, f.kmns, i0, w, dw, y[1], y[2], fk, f.kmnc4, f.kmns4);
     gc_algebra_general(mass, charge, mu, f.inv_psi0, y[3] * v_ref, fb, fk, p, pt, dy);
   } else {
     gc_algebra(mass, charge, mu, f.inv_psi0, y[3] * v_ref, fb, p, pt, dy);
@@ -438,7 +500,7 @@ __global__ void kcov_eval_kernel(FieldDev f, long long n, const double* s, const
   int i0;
   double w[4], dw[4], out[4] = {0.0, 0.0, 0.0, 0.0};
   lagrange_weights(f.ns, s[i], i0, w, dw);
-  if (f.kmnc || f.kmns) eval_series_generic(f, f.kmnc, f.kmns, i0, w, dw, th[i], ze[i], out);
+  if (f.kmnc || f.kmns) eval_series_generic(f, f.kmnc, f.kmns, i0, w, dw, th[i], ze[i], out, f.kmnc4, f.kmns4);
   K[i] = out[0];
   if (dK) { dK[i] = out[1]; dK[n + i] = out[2]; dK[2 * n + i] = out[3]; }
 }

@@ -106,11 +106,13 @@ enum { GC_ST_TMAX = 0, GC_ST_LOST = 1, GC_ST_AXIS = 2, GC_ST_MAXSTEPS = 3, GC_ST
  *   GC_KERNEL_GENERIC one thread per particle, tables read from global memory; any field
  *   GC_KERNEL_GRID    one lane per particle, atomic particle queue, B from the 3-D interpolant of gc_field_set_grid;
  *                     reported by gc_kernel_info while a grid is set, not selectable through gc_set_kernel
- *   GC_KERNEL_AUTO    per call: MMA (else TILE) when the field fits it and n >= GC_TILE_MIN_PARTICLES, else WARP
+ *   GC_KERNEL_AUTO    per call: MMA (else TILE) when the field fits it and n >= GC_TILE_MIN_PARTICLES (measured
+ *                     switch-over, profiles/r2_ensemble_size_sweep.md; GC_TILE_MIN_PARTICLES_SMALL for fields with
+ *                     max xm, max |xn| <= 8, whose warp kernel saturates earlier), else WARP
  *                     when the field fits it, else GENERIC.
  * All four implement the same equations and controller; their results differ at rounding level only. */
 enum { GC_KERNEL_AUTO = 0, GC_KERNEL_GENERIC = 1, GC_KERNEL_WARP = 2, GC_KERNEL_TILE = 3, GC_KERNEL_MMA = 4, GC_KERNEL_GRID = 5 };
-enum { GC_TILE_MIN_PARTICLES = 4096 };
+enum { GC_TILE_MIN_PARTICLES = 3072, GC_TILE_MIN_PARTICLES_SMALL = 2048 };
 
 /* Copies the tables to the device, checks them (finite values, xm >= 0, omega != 0) and builds the packed layouts of
  * every trace kernel the field fits: the by-node lane rows of the warp kernel, the per-cell window images of the

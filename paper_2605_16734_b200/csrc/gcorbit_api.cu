@@ -223,8 +223,10 @@ const void* mma_fn(const gc_field* f, bool sample = false) { return sample ? mma
 int resolve_kernel(const gc_field* f, int64_t n) {
   if (f->dev.grid) return GC_KERNEL_GRID;                  // the field IS the interpolant while a grid is set
   if (f->kernel != GC_KERNEL_AUTO) return f->kernel;
-  if (f->mma_ok && n >= GC_TILE_MIN_PARTICLES) return GC_KERNEL_MMA;
-  if (f->tile_ok && n >= GC_TILE_MIN_PARTICLES) return GC_KERNEL_TILE;
+  // switch-over measured on B200 (profiles/r2_ensemble_size_sweep.md): the warp kernel wins below it
+  const int64_t nmin = (f->dev.M <= 8 && f->dev.N <= 8) ? GC_TILE_MIN_PARTICLES_SMALL : GC_TILE_MIN_PARTICLES;
+  if (f->mma_ok && n >= nmin) return GC_KERNEL_MMA;
+  if (f->tile_ok && n >= nmin) return GC_KERNEL_TILE;
   return f->warp_ok ? GC_KERNEL_WARP : GC_KERNEL_GENERIC;
 }
 

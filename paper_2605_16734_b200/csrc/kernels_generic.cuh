@@ -180,6 +180,34 @@ __device__ __forceinline__ void gc_algebra(double mass, double charge, double mu
   dy[3] = mvdot / mass;
 }
 
+// The same with 1 / mass and 1 / charge given (the warp kernel: its right-hand side is one warp's dependent chain,
+// where each of the three FP64 divisions by mass and charge costs ~200 cycles of latency; rounding-level difference).
+__device__ __forceinline__ void gc_algebra_r(double mass, double charge, double inv_mass, double inv_charge, double mu,
+                                             double inv_psi0, double v, const double fb[4], const Profiles& p,
+                                             const double pt[9], double dy[4]) {
+  const double B = fb[0], B_psi = fb[1] * inv_psi0, B_th = fb[2], B_ze = fb[3];
+  const double G = p.G, Gp = p.Gs * inv_psi0, I = p.I, Ip = p.Is * inv_psi0;
+  const double Phi_psi = pt[1], Phi_th = pt[2], Phi_ze = pt[3];
+  const double al = pt[4], al_psi = pt[5], al_th = pt[6], al_ze = pt[7], al_t = pt[8];
+  const double invB = 1.0 / B;
+  const double rho_c = mass * v * invB * inv_charge + al;
+  const double Fq = (mass * v * v * invB + mu) * inv_charge;
+  const double a = 1.0 + rho_c * Ip + al_psi * I;
+  const double b = p.io - rho_c * Gp - al_psi * G;
+  const double invD = 1.0 / (a * G + b * I);
+  const double C = al_th * G - al_ze * I;
+  const double h_psi = fma(Fq, B_psi, Phi_psi), h_th = fma(Fq, B_th, Phi_th), h_ze = fma(Fq, B_ze, Phi_ze);
+  const double vB = v * B;
+  const double Lam = a * B_ze + b * B_th + C * B_psi;
+  dy[0] = (I * h_ze - G * h_th + C * vB) * invD * inv_psi0;
+  dy[1] = (b * vB + G * h_psi) * invD;
+  dy[2] = (a * vB - I * h_psi) * invD;
+  const double mvdot = (-mu * B * Lam - charge * B * (a * Phi_ze + b * Phi_th + C * Phi_psi)
+                        + mass * v * invB * (B_psi * (I * Phi_ze - G * Phi_th) + Phi_psi * (G * B_th - I * B_ze)))
+                           * invD - charge * B * al_t;
+  dy[3] = mvdot * inv_mass;
+}
+
 // O4 with the covariant radial component K kept (NEXT-4).  The Euler-Lagrange equations of
 //   L = q [ rho_c K psidot + (psi + rho_c I) thetadot + (rho_c G - chi) zetadot ] - H,   H = m v^2 / 2 + mu B + q Phi,
 // are  sum_j w_ij zdot_j = R_i  (z = psi, theta, zeta, v) with the antisymmetric w_ij = d_i A*_j - d_j A*_i and

@@ -112,6 +112,7 @@ struct WarpRhs {
   static constexpr int NIT = NIT_MAIN + NX;
   RowWindow<NIT, NREG> win;
   int cur_i0;
+  double inv_mass, inv_charge;        // set once per kernel by the caller (loop-invariant reciprocals)
 
   // Warp-cooperative right-hand side.  All arguments and results are warp-uniform.
   __device__ __forceinline__ void operator()(const FieldDev& f, WarpScratch& sc, const LaneRole& role,
@@ -266,7 +267,7 @@ struct WarpRhs {
       for (int q = 0; q < 9; ++q) pt[q] = 0.0;
     }
     const double fb[4] = {pv[0], pv[1], pv[2], pv[3]};
-    gc_algebra(mass, charge, mu, f.inv_psi0, u * v_ref, fb, pr, pt, dy);
+    gc_algebra_r(mass, charge, inv_mass, inv_charge, mu, f.inv_psi0, u * v_ref, fb, pr, pt, dy);
     dy[3] *= inv_v_ref;
   }
 
@@ -325,6 +326,8 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, 1) trace_warp_kernel(Fiel
   const LaneRole role = make_role(f, lane);
   WarpRhs<NIT_MAIN, NX, MODES, NREG> rhs;
   rhs.win.sm = warp_window_smem<NIT_MAIN, NX, MODES, NREG>(warp, lane);
+  rhs.inv_mass = 1.0 / p.mass;
+  rhs.inv_charge = 1.0 / p.charge;
   const int comp = lane & 3;
   constexpr double kTwoPi = 6.283185307179586476925286766559;
 
@@ -496,6 +499,8 @@ rhs_eval_warp_kernel(FieldDev f, double mass, double charge, double t, long long
   WarpRhs<NIT_MAIN, NX, MODES, NREG> rhs;
   rhs.win.sm = warp_window_smem<NIT_MAIN, NX, MODES, NREG>(warp, lane);
   rhs.cur_i0 = -1000;
+  rhs.inv_mass = 1.0 / mass;
+  rhs.inv_charge = 1.0 / charge;
   for (long long i = (long long)blockIdx.x * kWarpsPerBlock + warp; i < n;
        i += (long long)gridDim.x * kWarpsPerBlock) {
     double dy[4];

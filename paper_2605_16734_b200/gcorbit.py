@@ -17,7 +17,7 @@ SO_PATH = os.path.join(_HERE, "libgcorbit.so")
 
 GC_OK, GC_EINVAL, GC_ENOMEM, GC_ECUDA = 0, -1, -2, -3
 GC_KERNEL_AUTO, GC_KERNEL_GENERIC, GC_KERNEL_WARP, GC_KERNEL_TILE, GC_KERNEL_MMA, GC_KERNEL_GRID = 0, 1, 2, 3, 4, 5
-GC_TILE_MIN_PARTICLES = 4096
+GC_TILE_MIN_PARTICLES, GC_TILE_MIN_PARTICLES_SMALL = 3072, 2048
 GC_OPT_WAVE_PARTICLES, GC_OPT_CHUNK_ATTEMPTS = 1, 2
 ST_TMAX, ST_LOST, ST_AXIS, ST_MAXSTEPS, ST_NONFINITE = 0, 1, 2, 3, 4
 

@@ -7,6 +7,7 @@ this package.  It shares nothing with ``paper_2605_16734_b200/csrc``.
 from __future__ import annotations
 
 import ctypes as C
+import math
 import os
 import subprocess
 from dataclasses import dataclass
@@ -427,3 +428,50 @@ def birkhoff_digits(f):
     d = abs(a - b)
     digits = 16.0 if (d == 0.0 or scale == 0.0) else min(16.0, -np.log10(d / scale))
     return a, b, float(digits)
+
+
+# ---- orbit classification, characteristic frequencies, J_par from uniform-time samples -------------------------------
+# "Given trajectory data, transport diagnostics include Poincare plots, characteristic orbit frequencies,
+# weighted Birkhoff averaging (Duignan & Meiss, 2023), and orbit classification".  The paper prints no definition;
+# reading A30 of DESIGN.md section 12, written out here on ONE particle's series sampled every dt:
+#   * a reversal is a pair of consecutive samples with (v_j < 0) != (v_{j+1} < 0); its time is the zero of the straight
+#     line through the two samples, tau = t_j + dt v_j / (v_j - v_{j+1});
+#   * class 0 = passing (no reversal), 1 = trapped (at least one);
+#   * omega_theta, omega_zeta = (angle_last - angle_first) / (t_last - t_first): the mean poloidal and toroidal rates;
+#   * bounce frequency: with R >= 3 reversals, P = (R - 1) // 2 full periods lie between reversal 0 and reversal 2 P:
+#     omega_b = 2 pi P / (tau_{2P} - tau_0); 0 otherwise;
+#   * J_par of period p = m * integral of v_par^2 dt from tau_{2p} to tau_{2p+2} (dl = v_par dt along the orbit), by the
+#     trapezoid rule on the samples in between, with v_par = 0 at both ends; reported: the mean over the P periods and
+#     (max - min) / mean ("J_par and its variation").
+def orbit_diagnostics(theta, zeta, vpar, dt: float, mass: float) -> dict:
+    """theta, zeta, vpar: the valid samples of one particle (1-D arrays of equal length >= 2)."""
+    theta, zeta, vpar = (np.asarray(a, float) for a in (theta, zeta, vpar))
+    c = vpar.shape[0]
+    nan = float("nan")
+    if c < 2:
+        return dict(orbit_class=nan, reversals=0, omega_theta=nan, omega_zeta=nan, omega_bounce=nan, j_par=nan,
+                    j_par_variation=nan)
+    T = (c - 1) * dt
+    taus, idx = [], []
+    for j in range(c - 1):
+        if (vpar[j] < 0.0) != (vpar[j + 1] < 0.0):
+            taus.append(j * dt + dt * vpar[j] / (vpar[j] - vpar[j + 1]))
+            idx.append(j)
+    R = len(taus)
+    P = (R - 1) // 2 if R >= 3 else 0
+    omega_b, jmean, jvar = 0.0, nan, nan
+    if P > 0:
+        omega_b = 2.0 * math.pi * P / (taus[2 * P] - taus[0])
+        J = []
+        for p in range(P):
+            a, b = 2 * p, 2 * p + 2
+            ja, jb = idx[a] + 1, idx[b]                       # first and last sample inside the period
+            acc = 0.5 * vpar[ja] ** 2 * (ja * dt - taus[a])    # from the reversal (v = 0) to the first sample
+            for j in range(ja, jb):
+                acc += 0.5 * (vpar[j] ** 2 + vpar[j + 1] ** 2) * dt
+            acc += 0.5 * vpar[jb] ** 2 * (taus[b] - jb * dt)   # from the last sample to the reversal
+            J.append(mass * acc)
+        jmean = sum(J) / P
+        jvar = (max(J) - min(J)) / jmean
+    return dict(orbit_class=1.0 if R >= 1 else 0.0, reversals=R, omega_theta=(theta[-1] - theta[0]) / T,
+                omega_zeta=(zeta[-1] - zeta[0]) / T, omega_bounce=omega_b, j_par=jmean, j_par_variation=jvar)

@@ -224,6 +224,20 @@ int gc_pzeta_eval(const gc_field* f, double mass, double charge, int64_t n, cons
 int gc_birkhoff(int64_t n, int64_t nsamp, const double* series, int64_t j_first, const int32_t* sample_end,
                 double* out, void* stream);
 
+/* Orbit classification, characteristic frequencies and J_par of n particles from their uniform-time samples
+ * ("Given trajectory data, transport diagnostics include ... characteristic orbit frequencies ... and orbit
+ * classification"; reading A30 of DESIGN.md section 12).  DEVICE pointers.  samples [4][nsamp][n] as written by
+ * gc_trace_sampled or gc_trace_symplectic (s, theta, zeta, v_par); the valid samples of particle i are
+ * j_first <= j < (sample_end ? sample_end[i] : nsamp), taken sample_dt apart.  A reversal is a pair of consecutive
+ * samples with different signs of v_par, located by the straight line through them.  out [7][n]:
+ *   0 class: 0 passing (no reversal), 1 trapped;  1 number of reversals;
+ *   2, 3 omega_theta, omega_zeta = (last - first angle) / elapsed time, rad/s;
+ *   4 omega_bounce = 2 pi P / (time between reversal 0 and reversal 2 P), P = (reversals - 1) / 2 full periods, 0 if P = 0;
+ *   5 J_par = mass * integral of v_par^2 dt over a full period (trapezoid rule, v_par = 0 at both ends), mean over the
+ *     P periods, J s;  6 (max - min) / mean of it.   NaN where undefined (fewer than 2 samples; 5, 6 for P = 0). */
+int gc_orbit_diagnostics(int64_t n, int64_t nsamp, const double* samples, int64_t j_first, const int32_t* sample_end,
+                         double sample_dt, double mass, double* out, void* stream);
+
 /* ---- NEXT-3 of SURVEY.md section 8(f): the symplectic integrator ("A symplectic integrator for
  * non-canonical guiding-center orbits uses the explicit-implicit Euler scheme of (Albert et al., 2020)"; PAPER.md:60-62,
  * Fig. 1 left: "the symplectic algorithm exhibits a stable moving time average of the energy").  Reading A28 of

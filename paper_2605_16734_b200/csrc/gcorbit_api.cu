@@ -926,6 +926,19 @@ int gc_birkhoff(int64_t n, int64_t nsamp, const double* series, int64_t j_first,
   return GC_OK;
 }
 
+int gc_orbit_diagnostics(int64_t n, int64_t nsamp, const double* samples, int64_t j_first, const int32_t* sample_end,
+                         double sample_dt, double mass, double* out, void* stream) {
+  if (n < 0 || nsamp < 0 || j_first < 0) return fail(GC_EINVAL, "gc_orbit_diagnostics: negative size");
+  if (!(sample_dt > 0.0) || !(mass > 0.0)) return fail(GC_EINVAL, "gc_orbit_diagnostics: sample_dt and mass must be > 0");
+  if (n == 0) return GC_OK;
+  if (!samples || !out) return fail(GC_EINVAL, "gc_orbit_diagnostics: NULL array");
+  const int tb = 128;
+  gc::orbit_diag_kernel<<<(unsigned)((n + tb - 1) / tb), tb, 0, (cudaStream_t)stream>>>(n, nsamp, samples, j_first,
+                                                                                       sample_end, sample_dt, mass, out);
+  GC_CUDA(cudaGetLastError());
+  return GC_OK;
+}
+
 int gc_trace_host(gc_field* f, const gc_trace_params* params, int64_t n, const double* s0,
                   const double* th0, const double* ze0, const double* vpar0, const double* mu, double* h_inout,
                   double* y_out, double* t_out, int32_t* status, int32_t* n_acc, int32_t* n_rej,

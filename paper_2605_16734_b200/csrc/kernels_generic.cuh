@@ -472,6 +472,79 @@ __global__ void birkhoff_kernel(long long n, long long nsamp, const double* seri
   out[2 * n + i] = (d == 0.0 || scale == 0.0) ? 16.0 : fmin(16.0, -log10(d / scale));
 }
 
+// ---- A30: orbit classification, characteristic frequencies, J_par of n series of uniform-time samples -----------------
+// samples [4][nsamp][n] (gc_trace_sampled / gc_trace_symplectic layout); out [7][n] = class (0 passing, 1 trapped),
+// reversals of v_par, omega_theta, omega_zeta, omega_bounce, mean J_par over the full bounce periods, (max - min) / mean.
+__global__ void orbit_diag_kernel(long long n, long long nsamp, const double* samples, long long j_first,
+                                  const int* sample_end, double dt, double mass, double* out) {
+  const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  long long end = sample_end ? (long long)sample_end[i] : nsamp;
+  if (end > nsamp) end = nsamp;
+  const long long c = end - j_first;
+  const double nan = __longlong_as_double(0x7ff8000000000000LL);
+  if (j_first < 0 || c < 2) {
+    out[i] = nan; out[n + i] = 0.0;
+#pragma unroll
+    for (int q = 2; q < 7; ++q) out[q * n + i] = nan;
+    return;
+  }
+  const double* th = samples + (1 * nsamp + j_first) * n + i;
+  const double* ze = samples + (2 * nsamp + j_first) * n + i;
+  const double* vp = samples + (3 * nsamp + j_first) * n + i;
+  // pass 1: count the reversals and find the first one
+  long long R = 0;
+  double v0 = vp[0];
+  for (long long j = 0; j + 1 < c; ++j) {
+    const double v1 = vp[(j + 1) * n];
+    if ((v0 < 0.0) != (v1 < 0.0)) ++R;
+    v0 = v1;
+  }
+  const long long P = R >= 3 ? (R - 1) / 2 : 0;
+  double omega_b = 0.0, jmean = nan, jvar = nan;
+  if (P > 0) {
+    // pass 2: walk the reversals 0 .. 2 P; between reversal 2 p and 2 p + 2 integrate m v^2 dt by the trapezoid rule
+    long long r = -1;                    // index of the last reversal seen
+    double tau0 = 0.0, tau_last = 0.0, acc = 0.0, jsum = 0.0, jmin = 0.0, jmax = 0.0;
+    v0 = vp[0];
+    for (long long j = 0; j + 1 < c && r < 2 * P; ++j) {
+      const double v1 = vp[(j + 1) * n];
+      if ((v0 < 0.0) != (v1 < 0.0)) {
+        const double tau = (double)j * dt + dt * v0 / (v0 - v1);
+        ++r;
+        if (r == 0) {
+          tau0 = tau;
+          acc = 0.5 * v1 * v1 * ((double)(j + 1) * dt - tau);                  // reversal -> first sample of the period
+        } else if (r & 1) {
+          acc += 0.5 * (v0 * v0 + v1 * v1) * dt;                                // the reversal in the middle of a period
+        } else {
+          acc += 0.5 * v0 * v0 * (tau - (double)j * dt);                        // last sample of the period -> reversal
+          const double J = mass * acc;
+          jsum += J;
+          jmin = r == 2 ? J : fmin(jmin, J);
+          jmax = r == 2 ? J : fmax(jmax, J);
+          acc = 0.5 * v1 * v1 * ((double)(j + 1) * dt - tau);
+        }
+        tau_last = tau;
+      } else if (r >= 0) {
+        acc += 0.5 * (v0 * v0 + v1 * v1) * dt;
+      }
+      v0 = v1;
+    }
+    omega_b = 6.283185307179586476925286766559 * (double)P / (tau_last - tau0);
+    jmean = jsum / (double)P;
+    jvar = (jmax - jmin) / jmean;
+  }
+  const double T = (double)(c - 1) * dt;
+  out[i] = R >= 1 ? 1.0 : 0.0;
+  out[n + i] = (double)R;
+  out[2 * n + i] = (th[(c - 1) * n] - th[0]) / T;
+  out[3 * n + i] = (ze[(c - 1) * n] - ze[0]) / T;
+  out[4 * n + i] = omega_b;
+  out[5 * n + i] = jmean;
+  out[6 * n + i] = jvar;
+}
+
 __global__ void field_eval_kernel(FieldDev f, long long n, const double* s, const double* th, const double* ze,
                                   double* B, double* dB) {
   const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;

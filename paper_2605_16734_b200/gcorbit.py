@@ -23,7 +23,7 @@ ST_TMAX, ST_LOST, ST_AXIS, ST_MAXSTEPS, ST_NONFINITE = 0, 1, 2, 3, 4
 
 EXPORTS = ["gc_field_create", "gc_field_destroy", "gc_field_eval", "gc_pert_eval", "gc_rhs_eval", "gc_trace",
            "gc_trace_host", "gc_set_kernel", "gc_set_option", "gc_kernel_info", "gc_last_error",
-           "gc_trace_sampled", "gc_pzeta_eval", "gc_birkhoff", "gc_kcov_eval", "gc_field_set_grid", "gc_trace_symplectic"]
+           "gc_trace_sampled", "gc_pzeta_eval", "gc_birkhoff", "gc_kcov_eval", "gc_field_set_grid", "gc_trace_symplectic", "gc_orbit_diagnostics"]
 
 
 class GcError(RuntimeError):
@@ -74,6 +74,7 @@ def load_library():
         L.gc_pzeta_eval.argtypes = [vp, dbl, dbl, i64, vp, vp, vp, vp, vp]
         L.gc_birkhoff.argtypes = [i64, i64, vp, i64, vp, vp, vp]
         L.gc_set_kernel.argtypes = [vp, i32]
+        L.gc_orbit_diagnostics.argtypes = [i64, i64, vp, i64, vp, dbl, dbl, vp, vp]
         L.gc_field_set_grid.argtypes = [vp, i32, i32, i32, vp]
         L.gc_trace_symplectic.argtypes = [vp, C.POINTER(gc_symplectic_params), i64] + [vp] * 11 + [i64, i64, vp, vp, vp]
         L.gc_set_option.argtypes = [vp, i32, i64]
@@ -134,6 +135,18 @@ class TraceResult:
     poincare_count: int = 0
     samples: object = None        # [4][nsamp][n] (gc_trace_sampled)
     sample_end: object = None     # [n] int32
+
+
+def orbit_diagnostics(samples, j_first, sample_end, sample_dt, mass):
+    """gc_orbit_diagnostics: samples [4][nsamp][n] device tensor -> out [7][n] (class, reversals, omega_theta,
+    omega_zeta, omega_bounce, J_par, J_par variation)."""
+    torch = _torch()
+    _, nsamp, n = samples.shape
+    assert samples.is_contiguous()
+    out = torch.empty((7, n), dtype=torch.float64, device=samples.device)
+    _check(load_library().gc_orbit_diagnostics(n, nsamp, _dp(samples), int(j_first), _dp(sample_end), float(sample_dt),
+                                               float(mass), _dp(out), _stream_ptr(torch)))
+    return out
 
 
 class gc_symplectic_params(C.Structure):

@@ -208,6 +208,24 @@ class OracleField:
         ptr = L.oracle_field_grid(self._h)
         return np.ctypeslib.as_array(ptr, shape=self.grid_shape).copy()
 
+    def set_grid_hermite(self, ngs: int, nth: int, nze: int):
+        """Second reading of NEXT-2 (A31): the C1 tricubic Hermite interpolant on the same node grid."""
+        if _load().oracle_field_set_grid_hermite(self._h, C.c_int32(ngs), C.c_int32(nth), C.c_int32(nze)) != 0:
+            raise ValueError("oracle_field_set_grid_hermite: each grid size must be >= 2 (or all 0)")
+        self.grid_shape = (ngs, nth, nze) if ngs else None
+
+    def grid8(self) -> np.ndarray:
+        L = _load()
+        L.oracle_field_grid8.restype = C.POINTER(C.c_double)
+        L.oracle_field_grid8.argtypes = [C.c_void_p]
+        ptr = L.oracle_field_grid8(self._h)
+        return np.ctypeslib.as_array(ptr, shape=self.grid_shape + (8,)).copy()
+
+    def eval_B_mixed(self, s, th, ze):
+        out = np.zeros(8)
+        _load().oracle_eval_B_mixed(self._h, C.c_double(s), C.c_double(th), C.c_double(ze), _p(out))
+        return out
+
     def eval_B_sum(self, s, th, ze):
         out = np.zeros(4)
         _load().oracle_eval_B_sum(self._h, C.c_double(s), C.c_double(th), C.c_double(ze), _p(out))

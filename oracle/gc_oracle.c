@@ -22,6 +22,9 @@ struct oracle_field {
   /* NEXT-2: node values of B on the (s, theta, zeta) grid, [ngs][nth][nze]; NULL = the direct harmonic sum */
   int32_t ngs, nth, nze;
   double *grid;
+  /* the Hermite variant (reading A31): per node the 8 values f, f_s, f_th, f_ze, f_s_th, f_s_ze, f_th_ze, f_s_th_ze,
+     [ngs][nth][nze][8]; NULL unless oracle_field_set_grid_hermite was called */
+  double *grid8;
 };
 
 static void *dup_mem(const void *src, size_t bytes) {
@@ -58,7 +61,7 @@ void oracle_field_destroy(oracle_field *f) {
   if (!f) return;
   free(f->xm); free(f->xn); free(f->bmnc); free(f->G); free(f->I); free(f->iota);
   free(f->mode_m); free(f->mode_n); free(f->mode_omega); free(f->mode_phase); free(f->phihat);
-  free(f->bmns); free(f->kmnc); free(f->kmns); free(f->grid);
+  free(f->bmns); free(f->kmnc); free(f->kmns); free(f->grid); free(f->grid8);
   free(f);
 }
 
@@ -150,6 +153,7 @@ static const double ORACLE_TWO_PI = 6.283185307179586476925286766559;
 int oracle_field_set_grid(oracle_field *f, int32_t ngs, int32_t nth, int32_t nze) {
   if (!f) return -1;
   free(f->grid); f->grid = NULL; f->ngs = f->nth = f->nze = 0;
+  free(f->grid8); f->grid8 = NULL;
   if (ngs == 0 && nth == 0 && nze == 0) return 0;                 /* back to the direct sum */
   if (ngs < 4 || nth < 4 || nze < 4) return -1;
   double *g = (double *)malloc(sizeof(double) * (size_t)ngs * nth * nze);
@@ -211,7 +215,120 @@ void oracle_eval_B_grid(const oracle_field *f, double s, double th, double ze, d
   out[0] = B; out[1] = Bs; out[2] = Bt; out[3] = Bz;
 }
 
+/* ---- NEXT-2, second reading (A31 of DESIGN.md): "local tricubics" as the C1 tricubic HERMITE
+ * interpolant.  Every node carries the value of B and its seven first and mixed derivatives
+ *     f, f_s, f_th, f_ze, f_s_th, f_s_ze, f_th_ze, f_s_th_ze
+ * (direct sum O2 and its term-by-term derivatives; the s-derivatives are those of the radial Lagrange interpolant of
+ * O1 on the stencil that O1 picks AT the node).  In the cell [s_i, s_i+1] x [th_j, th_j+1] x [ze_k, ze_k+1] with
+ * local coordinates x, y, z in [0, 1) the interpolant is the tensor product of the 1-D cubic Hermite basis
+ *     h00 = 1 - 3x^2 + 2x^3 (value at 0)   h10 = 3x^2 - 2x^3 (value at 1)
+ *     h01 = x - 2x^2 + x^3  (slope at 0)   h11 = -x^2 + x^3  (slope at 1)        slopes scaled by the cell width:
+ *     f = sum over corners (a, b, c) and derivative orders (p, q, r) in {0,1}^3 of
+ *         D[corner][p q r] (ds)^p (dth)^q (dze)^r  h_{a p}(x) h_{b q}(y) h_{c r}(z)
+ * and its derivatives are the derivatives of that polynomial.  Value and gradient are continuous across cell faces
+ * (C1), unlike the Lagrange variant above.  Radial cell: i = clamp(floor(s (ngs-1)), 0, ngs-2) (extrapolates outside
+ * [0, 1] like O1); angular cells periodic. */
+static void eval_series_mixed(const oracle_field *f, double s, double th, double ze, double out[8]) {
+  int32_t i0; double w[4], dw[4];
+  oracle_lagrange(f->ns, s, &i0, w, dw);
+  for (int q = 0; q < 8; ++q) out[q] = 0.0;
+  for (int k = 0; k < f->nh; ++k) {
+    double m = (double)f->xm[k], nn = (double)f->xn[k] * (double)f->nfp;
+    double ang = m * th - nn * ze;
+    double c = cos(ang), sn = sin(ang);
+    for (int pass = 0; pass < 2; ++pass) {
+      const double *tab = pass == 0 ? f->bmnc : f->bmns;
+      if (!tab) continue;
+      double b, bs;
+      interp(tab + k, f->nh, i0, w, dw, &b, &bs);
+      /* pass 0: b cos(ang); pass 1: b sin(ang).  d/dth: -m sin | m cos; d/dze: nn sin | -nn cos;
+         d2/dth dze: m nn cos | m nn sin */
+      double v = pass == 0 ? c : sn;
+      double vth = pass == 0 ? -m * sn : m * c;
+      double vze = pass == 0 ? nn * sn : -nn * c;
+      double vtz = pass == 0 ? m * nn * c : m * nn * sn;
+      out[0] += b * v;   out[1] += bs * v;
+      out[2] += b * vth; out[3] += b * vze;
+      out[4] += bs * vth; out[5] += bs * vze;
+      out[6] += b * vtz; out[7] += bs * vtz;
+    }
+  }
+}
+
+void oracle_eval_B_mixed(const oracle_field *f, double s, double th, double ze, double out[8]) {
+  eval_series_mixed(f, s, th, ze, out);
+}
+
+int oracle_field_set_grid_hermite(oracle_field *f, int32_t ngs, int32_t nth, int32_t nze) {
+  if (!f) return -1;
+  free(f->grid); f->grid = NULL; free(f->grid8); f->grid8 = NULL; f->ngs = f->nth = f->nze = 0;
+  if (ngs == 0 && nth == 0 && nze == 0) return 0;
+  if (ngs < 2 || nth < 2 || nze < 2) return -1;
+  double *g = (double *)malloc(sizeof(double) * 8 * (size_t)ngs * nth * nze);
+  if (!g) return -1;
+#pragma omp parallel for collapse(2) schedule(static)
+  for (int i = 0; i < ngs; ++i)
+    for (int j = 0; j < nth; ++j)
+      for (int k = 0; k < nze; ++k) {
+        double s = (double)i / (double)(ngs - 1);
+        double th = ORACLE_TWO_PI * (double)j / (double)nth;
+        double ze = ORACLE_TWO_PI * (double)k / ((double)nze * (double)f->nfp);
+        eval_series_mixed(f, s, th, ze, g + 8 * (((size_t)i * nth + j) * nze + k));
+      }
+  f->grid8 = g; f->ngs = ngs; f->nth = nth; f->nze = nze;
+  return 0;
+}
+
+const double *oracle_field_grid8(const oracle_field *f) { return f->grid8; }
+
+/* 1-D cubic Hermite basis and its x-derivative: h[corner][order] */
+static void hermite_basis(double x, double h[2][2], double dh[2][2]) {
+  h[0][0] = 1.0 - 3.0 * x * x + 2.0 * x * x * x;  dh[0][0] = -6.0 * x + 6.0 * x * x;
+  h[1][0] = 3.0 * x * x - 2.0 * x * x * x;        dh[1][0] = 6.0 * x - 6.0 * x * x;
+  h[0][1] = x - 2.0 * x * x + x * x * x;          dh[0][1] = 1.0 - 4.0 * x + 3.0 * x * x;
+  h[1][1] = -x * x + x * x * x;                   dh[1][1] = -2.0 * x + 3.0 * x * x;
+}
+
+void oracle_eval_B_hermite(const oracle_field *f, double s, double th, double ze, double out[4]) {
+  const double ds = 1.0 / (double)(f->ngs - 1);
+  const double dth = ORACLE_TWO_PI / (double)f->nth;
+  const double dze = ORACLE_TWO_PI / ((double)f->nze * (double)f->nfp);
+  double us = s * (double)(f->ngs - 1), cs = floor(us);
+  if (!(cs >= 0.0)) cs = 0.0;                                     /* also NaN */
+  if (cs > (double)(f->ngs - 2)) cs = (double)(f->ngs - 2);
+  const int64_t ci = (int64_t)cs;
+  const double x = us - cs;
+  double ut = th * ((double)f->nth / ORACLE_TWO_PI), ct = floor(ut), y = ut - ct;
+  double uz = ze * ((double)f->nze * (double)f->nfp / ORACLE_TWO_PI), cz = floor(uz), z = uz - cz;
+  double rj = fmod(ct, (double)f->nth); if (rj < 0.0) rj += (double)f->nth;
+  double rk = fmod(cz, (double)f->nze); if (rk < 0.0) rk += (double)f->nze;
+  const int64_t cj = (int64_t)rj, ck = (int64_t)rk;
+  double hs[2][2], dhs[2][2], ht[2][2], dht[2][2], hz[2][2], dhz[2][2];
+  hermite_basis(x, hs, dhs); hermite_basis(y, ht, dht); hermite_basis(z, hz, dhz);
+  const double sc[2][3] = {{1.0, 1.0, 1.0}, {ds, dth, dze}};     /* slope scaling by the cell widths */
+  double B = 0.0, Bs = 0.0, Bt = 0.0, Bz = 0.0;
+  for (int a = 0; a < 2; ++a)
+    for (int b = 0; b < 2; ++b)
+      for (int c = 0; c < 2; ++c) {
+        const int64_t i = ci + a, j = (cj + b) % f->nth, k = (ck + c) % f->nze;
+        const double *D = f->grid8 + 8 * (((size_t)i * f->nth + j) * f->nze + k);
+        /* D index by derivative orders (p, q, r): f 0, f_s 1, f_th 2, f_ze 3, f_s_th 4, f_s_ze 5, f_th_ze 6, all 7 */
+        static const int idx[2][2][2] = {{{0, 3}, {2, 6}}, {{1, 5}, {4, 7}}};
+        for (int p = 0; p < 2; ++p)
+          for (int q = 0; q < 2; ++q)
+            for (int r = 0; r < 2; ++r) {
+              const double v = D[idx[p][q][r]] * sc[p][0] * sc[q][1] * sc[r][2];
+              B += v * hs[a][p] * ht[b][q] * hz[c][r];
+              Bs += v * dhs[a][p] * ht[b][q] * hz[c][r] / ds;
+              Bt += v * hs[a][p] * dht[b][q] * hz[c][r] / dth;
+              Bz += v * hs[a][p] * ht[b][q] * dhz[c][r] / dze;
+            }
+      }
+  out[0] = B; out[1] = Bs; out[2] = Bt; out[3] = Bz;
+}
+
 void oracle_eval_B(const oracle_field *f, double s, double th, double ze, double out[4]) {
+  if (f->grid8) { oracle_eval_B_hermite(f, s, th, ze, out); return; }
   if (f->grid) oracle_eval_B_grid(f, s, th, ze, out);
   else oracle_eval_B_sum(f, s, th, ze, out);
 }

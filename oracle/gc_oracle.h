@@ -79,6 +79,15 @@ void oracle_eval_B_sum(const oracle_field *f, double s, double th, double ze, do
 int oracle_field_set_grid(oracle_field *f, int32_t ngs, int32_t nth, int32_t nze);
 const double *oracle_field_grid(const oracle_field *f);           /* [ngs][nth][nze] or NULL */
 void oracle_eval_B_grid(const oracle_field *f, double s, double th, double ze, double out[4]);
+/* NEXT-2, second reading (A31): the C1 tricubic Hermite interpolant.  oracle_field_set_grid_hermite tabulates B and
+ * its seven first and mixed derivatives (f, f_s, f_th, f_ze, f_s_th, f_s_ze, f_th_ze, f_s_th_ze; direct sum, term by
+ * term) on the same node grid (each count >= 2; 0,0,0 switches back) and from then on oracle_eval_B evaluates the
+ * tensor-product cubic Hermite interpolant of the cell that holds the point.  Drops a Lagrange grid and vice versa. */
+int oracle_field_set_grid_hermite(oracle_field *f, int32_t ngs, int32_t nth, int32_t nze);
+const double *oracle_field_grid8(const oracle_field *f);          /* [ngs][nth][nze][8] or NULL */
+void oracle_eval_B_hermite(const oracle_field *f, double s, double th, double ze, double out[4]);
+/* The direct sum with its mixed derivatives: out = {f, f_s, f_th, f_ze, f_s_th, f_s_ze, f_th_ze, f_s_th_ze}. */
+void oracle_eval_B_mixed(const oracle_field *f, double s, double th, double ze, double out[8]);
 /* NEXT-4: covariant radial component, out = {K, dK/ds, dK/dtheta, dK/dzeta} (all zero without K tables). */
 void oracle_eval_K(const oracle_field *f, double s, double th, double ze, double out[4]);
 /* O1 on profiles: out = {G, dG/ds, I, dI/ds, iota, diota/ds}. */

@@ -69,7 +69,7 @@ def parse_args():
                     "post-processing time to config")
     ap.add_argument("--slots", type=int, default=0, help="GC_OPT_WAVE_PARTICLES: record slots of the binned kernels "
                     "(0 = the library's default, 2^18)")
-    ap.add_argument("--grid", default="", help="NEXT-2: NGSxNTHxNZE -- trace on the 3-D tricubic interpolant of B "
+    ap.add_argument("--grid", default="", help="NEXT-2: NGSxNTHxNZE[:hermite] -- trace on the 3-D tricubic interpolant of B "
                     "(gc_field_set_grid) instead of the direct harmonic sum; not the default line")
     ap.add_argument("--symplectic", type=float, default=0.0, metavar="DT", help="NEXT-3: advance every segment with the "
                     "symplectic explicit-implicit Euler integrator at the fixed step DT seconds (gc_trace_symplectic) "
@@ -252,7 +252,9 @@ def run_cuda(args):
     if args.slots:
         GF.set_option(G.GC_OPT_WAVE_PARTICLES, args.slots)
     if args.grid:
-        GF.set_grid(*[int(x) for x in args.grid.lower().split("x")])
+        gspec = args.grid.lower().split(":")
+        GF.set_grid(*[int(x) for x in gspec[0].split("x")],
+                    kind=G.GC_GRID_HERMITE if len(gspec) > 1 and gspec[1].startswith("h") else G.GC_GRID_LAGRANGE)
     kinfo = GF.kernel_info(n)
     kinfo["record_slots"] = args.slots if args.slots else "default"
     T = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device=dev)

@@ -122,17 +122,23 @@ int gc_field_create(const gc_field_desc* desc, gc_field** out);
 int gc_field_destroy(gc_field* f);
 
 /* ---- NEXT-2 of SURVEY.md section 8(f): the 3-D local-interpolant field ("CUDA kernels implement field interpolation
- * and trajectory integration on GPU" PAPER.md:48; "local tricubics" PAPER.md:80,111; reading A27 of DESIGN.md).
- * Tabulates B (direct sum O2) at s_i = i/(ngs-1), theta_j = 2 pi j/nth, zeta_k = (2 pi/nfp) k/nze (one field period;
- * every count >= 4) on the device, asynchronously on `stream`, and from then on every call on this field --
- * gc_field_eval, gc_rhs_eval, gc_trace, gc_trace_sampled, gc_trace_host, gc_pzeta_eval -- evaluates B and its three
- * derivatives as the tensor-product cubic Lagrange interpolant of those node values (radial stencil clamped as in
- * O1, angular stencils periodic and centred on the cell); profiles and the perturbation keep their radial tables.
+ * and trajectory integration on GPU" PAPER.md:48; "local tricubics" PAPER.md:80,111; readings A27, A31 of DESIGN.md).
+ * Tabulates B (direct sum O2) at s_i = i/(ngs-1), theta_j = 2 pi j/nth, zeta_k = (2 pi/nfp) k/nze (one field period)
+ * on the device, asynchronously on `stream`, and from then on every call on this field -- gc_field_eval, gc_rhs_eval,
+ * gc_trace, gc_trace_sampled, gc_trace_host, gc_trace_symplectic, gc_pzeta_eval -- evaluates B and its three
+ * derivatives from a local tricubic interpolant; profiles and the perturbation keep their radial tables.
+ *   GC_GRID_LAGRANGE  tensor product of 4-point cubic Lagrange polynomials through the node VALUES (radial stencil
+ *                     clamped as in O1, angular stencils periodic and centred on the cell); continuous, gradient jumps
+ *                     at the cell faces (C0); every count >= 4; 32 ngs (nth + 3) nze bytes of device memory
+ *   GC_GRID_HERMITE   tensor product of cubic Hermite polynomials through the node values AND node derivatives (f, f_s,
+ *                     f_theta, f_zeta and the four mixed ones, term by term from the harmonic sum); value and gradient
+ *                     continuous (C1): an adaptive integrator needs several times fewer steps on it; every count >= 2;
+ *                     64 ngs (nth + 1) (nze + 1) bytes
  * Traces then run on GC_KERNEL_GRID whatever gc_set_kernel says.  (0, 0, 0) drops the grid and returns to the direct
- * sum.  The table takes 32 ngs (nth + 3) nze bytes of device memory (every node stored with its three
- * zeta neighbours so that a stencil row is one 32-byte load), owned by the field.  GC_EINVAL for
- * a count in 1..3 or a field with kmnc / kmns; calls must not overlap traces that still run on this field. */
-int gc_field_set_grid(gc_field* f, int32_t ngs, int32_t nth, int32_t nze, void* stream);
+ * sum.  The table is owned by the field.  GC_EINVAL for a count below the minimum, an unknown kind or a field with
+ * kmnc / kmns; calls must not overlap traces that still run on this field. */
+enum { GC_GRID_LAGRANGE = 0, GC_GRID_HERMITE = 1 };
+int gc_field_set_grid(gc_field* f, int32_t ngs, int32_t nth, int32_t nze, int32_t kind, void* stream);
 
 /* O2 at n points.  DEVICE pointers.  B [n]; dB [3][n] = dB/ds, dB/dtheta, dB/dzeta, or NULL.
  * Asynchronous on `stream` (a cudaStream_t, NULL = default stream).  Used to compute mu and by tests. */

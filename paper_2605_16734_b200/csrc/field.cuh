@@ -56,7 +56,12 @@ struct FieldDev {
   // NEXT-2 (kernels_grid.cuh): node values of B on the (s, theta, zeta) grid over one field period in the gather
   // layout grid[ngs][nth + 3][nze][4] (entry k = nodes k .. k+3 mod nze; three theta rows repeated); nullptr = the
   // direct harmonic sum.  th_scale = nth / 2 pi, ze_scale = nze nfp / 2 pi (nodes per radian).
+  // grid_kind 1: the Lagrange gather layout above.  grid_kind 2 (reading A31, C1 tricubic Hermite): grid[ngs][nth + 1]
+  // [nze + 1][8], per node (f, f_ze, f_th, f_th_ze, f_s, f_s_ze, f_s_th, f_s_th_ze) pre-multiplied by the cell widths of
+  // the differentiated directions (64 bytes = two 256-bit loads), one periodic image appended in both angles.
   const double* grid;
+  int grid_kind;
+  double inv_ds, inv_dth, inv_dze;   // 1 / cell width in s, theta, zeta (Hermite: derivative outputs)
   int ngs, nth, nze;
   double th_scale, ze_scale, inv_nth, inv_nze;
 };

@@ -446,9 +446,14 @@ int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, c
 }
 
 // One launch of the lane kernel (generic field or 3-D interpolant): persistent grid, atomic particle queue.
-long long lane_blocks(const gc_field* f, long long n, bool grid) {
+const void* lane_fn(int kind) {       // 0 direct sum, 1 Lagrange interpolant, 2 Hermite interpolant
+  return kind == 2 ? (const void*)gc::trace_lane_kernel<2>
+                   : kind == 1 ? (const void*)gc::trace_lane_kernel<1> : (const void*)gc::trace_lane_kernel<0>;
+}
+
+long long lane_blocks(const gc_field* f, long long n, int kind) {
   int per_sm = 0;
-  const void* fn = grid ? (const void*)gc::trace_lane_kernel<true> : (const void*)gc::trace_lane_kernel<false>;
+  const void* fn = lane_fn(kind);
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, gc::kLaneThreads, gc::kLaneSmemBytes) != cudaSuccess || per_sm < 1)
     per_sm = 1;
   long long blocks = (n + gc::kLaneThreads - 1) / gc::kLaneThreads;
@@ -457,14 +462,15 @@ long long lane_blocks(const gc_field* f, long long n, bool grid) {
   return blocks < 1 ? 1 : blocks;
 }
 
-int launch_lane(const gc_field* f, gc::TraceDev& t, bool grid, cudaStream_t st) {
+int launch_lane(const gc_field* f, gc::TraceDev& t, int kind, cudaStream_t st) {
   unsigned long long* counter = nullptr;
   GC_CUDA(cudaMallocFromPoolAsync((void**)&counter, sizeof(unsigned long long), f->pool, st));
   GC_CUDA(cudaMemsetAsync(counter, 0, sizeof(unsigned long long), st));
   t.work_counter = counter;
-  const unsigned blocks = (unsigned)lane_blocks(f, t.n, grid);
-  if (grid) gc::trace_lane_kernel<true><<<blocks, gc::kLaneThreads, gc::kLaneSmemBytes, st>>>(f->dev, t);
-  else gc::trace_lane_kernel<false><<<blocks, gc::kLaneThreads, gc::kLaneSmemBytes, st>>>(f->dev, t);
+  const unsigned blocks = (unsigned)lane_blocks(f, t.n, kind);
+  if (kind == 2) gc::trace_lane_kernel<2><<<blocks, gc::kLaneThreads, gc::kLaneSmemBytes, st>>>(f->dev, t);
+  else if (kind == 1) gc::trace_lane_kernel<1><<<blocks, gc::kLaneThreads, gc::kLaneSmemBytes, st>>>(f->dev, t);
+  else gc::trace_lane_kernel<0><<<blocks, gc::kLaneThreads, gc::kLaneSmemBytes, st>>>(f->dev, t);
   const cudaError_t le = cudaGetLastError();
   const cudaError_t fe = cudaFreeAsync(counter, st);          // also on a failed launch
   GC_CUDA(le);
@@ -662,7 +668,7 @@ int gc_set_option(gc_field* f, int32_t option, int64_t value) {
   }
 }
 
-int gc_field_set_grid(gc_field* f, int32_t ngs, int32_t nth, int32_t nze, void* stream) {
+int gc_field_set_grid(gc_field* f, int32_t ngs, int32_t nth, int32_t nze, int32_t kind, void* stream) {
   if (!f) return fail(GC_EINVAL, "gc_field_set_grid: NULL field");
   cudaStream_t st = (cudaStream_t)stream;
   if (f->grid) {                                             // drop the old interpolant first
@@ -670,35 +676,53 @@ int gc_field_set_grid(gc_field* f, int32_t ngs, int32_t nth, int32_t nze, void* 
     cudaFree(f->grid);
     f->grid = nullptr;
     f->dev.grid = nullptr;
+    f->dev.grid_kind = 0;
     f->dev.ngs = f->dev.nth = f->dev.nze = 0;
   }
   if (ngs == 0 && nth == 0 && nze == 0) return GC_OK;        // back to the direct harmonic sum
-  if (ngs < 4 || nth < 4 || nze < 4) return fail(GC_EINVAL, "gc_field_set_grid: every node count must be >= 4 (or all 0)");
+  if (kind != GC_GRID_LAGRANGE && kind != GC_GRID_HERMITE) return fail(GC_EINVAL, "gc_field_set_grid: unknown kind");
+  const int nmin = kind == GC_GRID_HERMITE ? 2 : 4;
+  if (ngs < nmin || nth < nmin || nze < nmin)
+    return fail(GC_EINVAL, "gc_field_set_grid: every node count must be >= 4 (Lagrange) / >= 2 (Hermite), or all 0");
   if (f->dev.kmnc || f->dev.kmns)
     return fail(GC_EINVAL, "gc_field_set_grid: fields with a covariant radial component K are traced by the direct sum only");
-  const size_t nodes = (size_t)ngs * (size_t)nth * (size_t)nze;
-  const size_t total = (size_t)ngs * (size_t)(nth + 3) * (size_t)nze * 4;
-  if (total > ((size_t)1 << 33)) return fail(GC_EINVAL, "gc_field_set_grid: table larger than 64 GiB");
-  double *g = nullptr, *plain = nullptr;
-  GC_CUDA(cudaMalloc((void**)&g, total * sizeof(double)));
-  if (cudaMallocAsync((void**)&plain, nodes * sizeof(double), st) != cudaSuccess) {
-    cudaFree(g);
-    return fail(GC_ENOMEM, "gc_field_set_grid: device allocation failed");
-  }
-  const int tb = 256;
-  gc::grid_build_kernel<<<(unsigned)((nodes + tb - 1) / tb), tb, 0, st>>>(f->dev, ngs, nth, nze, plain);
-  gc::grid_pack_kernel<<<(unsigned)((total / 4 + tb - 1) / tb), tb, 0, st>>>(ngs, nth, nze, plain, g);
-  const cudaError_t le = cudaGetLastError();
-  cudaFreeAsync(plain, st);
-  if (le != cudaSuccess) { cudaFree(g); GC_CUDA(le); }
   constexpr double kTwoPi = 6.283185307179586476925286766559;
+  const int tb = 256;
+  double* g = nullptr;
+  if (kind == GC_GRID_HERMITE) {
+    const size_t entries = (size_t)ngs * (size_t)(nth + 1) * (size_t)(nze + 1);
+    if (entries * 8 > ((size_t)1 << 33)) return fail(GC_EINVAL, "gc_field_set_grid: table larger than 64 GiB");
+    GC_CUDA(cudaMalloc((void**)&g, entries * 8 * sizeof(double)));
+    gc::grid8_build_kernel<<<(unsigned)((entries + tb - 1) / tb), tb, 0, st>>>(f->dev, ngs, nth, nze, g);
+    const cudaError_t le = cudaGetLastError();
+    if (le != cudaSuccess) { cudaFree(g); GC_CUDA(le); }
+  } else {
+    const size_t nodes = (size_t)ngs * (size_t)nth * (size_t)nze;
+    const size_t total = (size_t)ngs * (size_t)(nth + 3) * (size_t)nze * 4;
+    if (total > ((size_t)1 << 33)) return fail(GC_EINVAL, "gc_field_set_grid: table larger than 64 GiB");
+    double* plain = nullptr;
+    GC_CUDA(cudaMalloc((void**)&g, total * sizeof(double)));
+    if (cudaMallocAsync((void**)&plain, nodes * sizeof(double), st) != cudaSuccess) {
+      cudaFree(g);
+      return fail(GC_ENOMEM, "gc_field_set_grid: device allocation failed");
+    }
+    gc::grid_build_kernel<<<(unsigned)((nodes + tb - 1) / tb), tb, 0, st>>>(f->dev, ngs, nth, nze, plain);
+    gc::grid_pack_kernel<<<(unsigned)((total / 4 + tb - 1) / tb), tb, 0, st>>>(ngs, nth, nze, plain, g);
+    const cudaError_t le = cudaGetLastError();
+    cudaFreeAsync(plain, st);
+    if (le != cudaSuccess) { cudaFree(g); GC_CUDA(le); }
+  }
   f->grid = g;
   f->dev.grid = g;
+  f->dev.grid_kind = kind == GC_GRID_HERMITE ? 2 : 1;
   f->dev.ngs = ngs; f->dev.nth = nth; f->dev.nze = nze;
   f->dev.th_scale = (double)nth / kTwoPi;
   f->dev.ze_scale = (double)nze * (double)f->dev.nfp / kTwoPi;
   f->dev.inv_nth = 1.0 / (double)nth;
   f->dev.inv_nze = 1.0 / (double)nze;
+  f->dev.inv_ds = (double)(ngs - 1);
+  f->dev.inv_dth = f->dev.th_scale;
+  f->dev.inv_dze = f->dev.ze_scale;
   return GC_OK;
 }
 
@@ -721,10 +745,9 @@ int gc_kernel_info(const gc_field* f, int64_t n, int32_t* kernel, int32_t* block
     GC_CUDA(cudaFuncGetAttributes(&at, w->trace_fn));
     b = f->sm_count; t = gc::kWarpsPerBlock * 32; s = w->smem_bytes;
   } else {
-    const bool grid = k == GC_KERNEL_GRID;
-    GC_CUDA(cudaFuncGetAttributes(&at, grid ? (const void*)gc::trace_lane_kernel<true>
-                                            : (const void*)gc::trace_lane_kernel<false>));
-    b = (int)lane_blocks(f, n, grid); t = gc::kLaneThreads; s = gc::kLaneSmemBytes;
+    const int kind = k == GC_KERNEL_GRID ? f->dev.grid_kind : 0;
+    GC_CUDA(cudaFuncGetAttributes(&at, lane_fn(kind)));
+    b = (int)lane_blocks(f, n, kind); t = gc::kLaneThreads; s = gc::kLaneSmemBytes;
   }
   if (kernel) *kernel = k;
   if (blocks) *blocks = b;
@@ -842,7 +865,7 @@ int trace_common(const gc_field* f, const gc_trace_params* params, int64_t n, co
     GC_CUDA(le);
     GC_CUDA(fe);
   } else {
-    return launch_lane(f, t, kern == GC_KERNEL_GRID, st);
+    return launch_lane(f, t, kern == GC_KERNEL_GRID ? f->dev.grid_kind : 0, st);
   }
   return GC_OK;
 }
@@ -896,8 +919,10 @@ int gc_trace_symplectic(const gc_field* f, const gc_symplectic_params* p, int64_
   const int tb = 128;
   long long blocks = (n + tb - 1) / tb;
   if (blocks > (long long)f->sm_count * 16) blocks = (long long)f->sm_count * 16;
-  if (f->dev.grid) gc::trace_symplectic_kernel<true><<<(unsigned)blocks, tb, 0, (cudaStream_t)stream>>>(f->dev, d);
-  else gc::trace_symplectic_kernel<false><<<(unsigned)blocks, tb, 0, (cudaStream_t)stream>>>(f->dev, d);
+  if (f->dev.grid && f->dev.grid_kind == 2)
+    gc::trace_symplectic_kernel<2><<<(unsigned)blocks, tb, 0, (cudaStream_t)stream>>>(f->dev, d);
+  else if (f->dev.grid) gc::trace_symplectic_kernel<1><<<(unsigned)blocks, tb, 0, (cudaStream_t)stream>>>(f->dev, d);
+  else gc::trace_symplectic_kernel<0><<<(unsigned)blocks, tb, 0, (cudaStream_t)stream>>>(f->dev, d);
   GC_CUDA(cudaGetLastError());
   return GC_OK;
 }

@@ -265,7 +265,9 @@ __device__ inline void rhs_generic(const FieldDev& f, double mass, double charge
   dy[3] *= inv_v_ref;
 }
 
-// The same with B from the tricubic interpolant (NEXT-2); profiles and perturbation from the radial tables as always.
+// The same with B from a tricubic interpolant (NEXT-2; KIND 1 Lagrange, 2 Hermite); profiles and perturbation from the
+// radial tables as always.
+template <int KIND>
 __device__ inline void rhs_grid(const FieldDev& f, double mass, double charge, double mu, double v_ref,
                                 double inv_v_ref, double t, const double y[4], double dy[4]) {
   int i0;
@@ -275,7 +277,7 @@ __device__ inline void rhs_grid(const FieldDev& f, double mass, double charge, d
   interp4(f.G, 1, i0, w, dw, p.G, p.Gs);
   interp4(f.I, 1, i0, w, dw, p.I, p.Is);
   interp4(f.iota, 1, i0, w, dw, p.io, p.ios);
-  eval_B_grid(f, y[0], y[1], y[2], fb);
+  eval_B_interp<KIND>(f, y[0], y[1], y[2], fb);
   if (f.nk > 0) {
     eval_pert_generic(f, i0, w, dw, p, y[1], y[2], t, pt);
   } else {
@@ -431,7 +433,7 @@ __global__ void pzeta_eval_kernel(FieldDev f, double mass, double charge, long l
   interp4(f.G, 1, i0, w, dw, p.G, p.Gs);
   interp4(f.I, 1, i0, w, dw, p.I, p.Is);
   interp4(f.iota, 1, i0, w, dw, p.io, p.ios);
-  if (f.grid) eval_B_grid(f, s, th, ze, fb);
+  if (f.grid) eval_B_interp_rt(f, s, th, ze, fb);
   else eval_B_generic(f, i0, w, dw, th, ze, fb);
   double al = 0.0;
   if (f.nk > 0) {
@@ -552,7 +554,7 @@ __global__ void field_eval_kernel(FieldDev f, long long n, const double* s, cons
   int i0;
   double w[4], dw[4], out[4];
   if (f.grid) {
-    eval_B_grid(f, s[i], th[i], ze[i], out);               // NEXT-2: the field is the interpolant
+    eval_B_interp_rt(f, s[i], th[i], ze[i], out);          // NEXT-2: the field is the interpolant
   } else {
     lagrange_weights(f.ns, s[i], i0, w, dw);
     eval_B_generic(f, i0, w, dw, th[i], ze[i], out);
@@ -594,6 +596,52 @@ __global__ void grid_pack_kernel(int ngs, int nth, int nze, const double* plain,
   for (int c = 0; c < 4; ++c) grid[e * 4 + c] = row[(k + c) % nze];
 }
 
+// Setup of the Hermite variant (A31): per node the direct sum and its seven first and mixed derivatives, term by term,
+// pre-multiplied by the cell widths of the differentiated directions, in the layout of field.cuh:
+// grid[ngs][nth + 1][nze + 1][8] = (f, f_ze, f_th, f_th_ze, f_s, f_s_ze, f_s_th, f_s_th_ze).  One thread per entry.
+__global__ void grid8_build_kernel(FieldDev f, int ngs, int nth, int nze, double* grid) {
+  constexpr double kTwoPi = 6.283185307179586476925286766559;
+  const long long total = (long long)ngs * (nth + 1) * (nze + 1);
+  const long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (e >= total) return;
+  const int kp = (int)(e % (nze + 1));
+  const int jp = (int)((e / (nze + 1)) % (nth + 1));
+  const int i = (int)(e / ((long long)(nze + 1) * (nth + 1)));
+  const int j = jp % nth, k = kp % nze;
+  const double s = (double)i / (double)(ngs - 1);
+  const double th = kTwoPi * (double)j / (double)nth;
+  const double ze = kTwoPi * (double)k / ((double)nze * (double)f.nfp);
+  const double ds = 1.0 / (double)(ngs - 1), dth = kTwoPi / (double)nth, dze = kTwoPi / ((double)nze * (double)f.nfp);
+  int i0;
+  double w[4], dw[4];
+  lagrange_weights(f.ns, s, i0, w, dw);
+  const double thr = reduce_2pi(th), phr = reduce_2pi((double)f.nfp * ze);
+  double o[8] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};     // f, f_s, f_th, f_ze, f_s_th, f_s_ze, f_th_ze, f_s_th_ze
+  for (int h = 0; h < f.nh; ++h) {
+    const double m = (double)__ldg(f.xm + h), nn = (double)__ldg(f.xn + h) * (double)f.nfp;
+    double sn, cs;
+    sincos_poly(fma(m, thr, -(double)__ldg(f.xn + h) * phr), sn, cs);
+#pragma unroll
+    for (int pass = 0; pass < 2; ++pass) {
+      const double* tab = pass == 0 ? f.bmnc : f.bmns;
+      if (!tab) continue;
+      double b, bs;
+      interp4(tab + h, f.nh, i0, w, dw, b, bs);
+      const double v = pass == 0 ? cs : sn;
+      const double vth = pass == 0 ? -m * sn : m * cs;
+      const double vze = pass == 0 ? nn * sn : -nn * cs;
+      const double vtz = pass == 0 ? m * nn * cs : m * nn * sn;
+      o[0] = fma(b, v, o[0]);     o[1] = fma(bs, v, o[1]);
+      o[2] = fma(b, vth, o[2]);   o[3] = fma(b, vze, o[3]);
+      o[4] = fma(bs, vth, o[4]);  o[5] = fma(bs, vze, o[5]);
+      o[6] = fma(b, vtz, o[6]);   o[7] = fma(bs, vtz, o[7]);
+    }
+  }
+  double* g = grid + e * 8;
+  g[0] = o[0];            g[1] = o[3] * dze;        g[2] = o[2] * dth;       g[3] = o[6] * dth * dze;
+  g[4] = o[1] * ds;       g[5] = o[5] * ds * dze;   g[6] = o[4] * ds * dth;  g[7] = o[7] * ds * dth * dze;
+}
+
 __global__ void kcov_eval_kernel(FieldDev f, long long n, const double* s, const double* th, const double* ze,
                                  double* K, double* dK) {
   const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
@@ -631,7 +679,8 @@ __global__ void rhs_eval_generic_kernel(FieldDev f, double mass, double charge, 
   if (i >= n) return;
   const double yy[4] = {y[i], y[n + i], y[2 * n + i], y[3 * n + i]};
   double dy[4];
-  if (f.grid) rhs_grid(f, mass, charge, mu[i], 1.0, 1.0, t, yy, dy);
+  if (f.grid && f.grid_kind == 2) rhs_grid<2>(f, mass, charge, mu[i], 1.0, 1.0, t, yy, dy);
+  else if (f.grid) rhs_grid<1>(f, mass, charge, mu[i], 1.0, 1.0, t, yy, dy);
   else rhs_generic(f, mass, charge, mu[i], 1.0, 1.0, t, yy, dy);
   for (int c = 0; c < 4; ++c) dydt[c * n + i] = dy[c];
 }

@@ -81,4 +81,90 @@ __device__ __forceinline__ void eval_B_grid(const FieldDev& f, double s, double 
   out[0] = B; out[1] = Bs; out[2] = Bt; out[3] = Bz;
 }
 
+// ---- reading A31: the C1 tricubic Hermite interpolant --------------------------------------------------------------
+// 1-D cubic Hermite basis on [0, 1] and its derivative: h[corner][order] (value / slope at corner 0 / 1).
+__device__ __forceinline__ void hermite_basis(double x, double (&h)[2][2], double (&dh)[2][2]) {
+  const double x2 = x * x, x3 = x2 * x;
+  h[0][0] = fma(2.0, x3, fma(-3.0, x2, 1.0));  dh[0][0] = 6.0 * (x2 - x);
+  h[1][0] = fma(-2.0, x3, 3.0 * x2);           dh[1][0] = 6.0 * (x - x2);
+  h[0][1] = x3 - 2.0 * x2 + x;                 dh[0][1] = fma(3.0, x2, fma(-4.0, x, 1.0));
+  h[1][1] = x3 - x2;                           dh[1][1] = fma(3.0, x2, -2.0 * x);
+}
+
+// cell index in [0, nodes) and local coordinate of a periodic direction; the decision floor(u) on the same product as
+// the oracle
+__device__ __forceinline__ void periodic_cell(int nodes, double inv_nodes, double npr, double angle, int& c, double& x) {
+  const double u = angle * npr, fl = floor(u);
+  x = u - fl;
+  const double nd = (double)nodes;
+  double r = fma(-floor(fl * inv_nodes), nd, fl);
+  if (r < 0.0) r += nd;
+  if (r >= nd) r -= nd;
+  c = (r >= 0.0 && r < nd) ? (int)r : 0;
+}
+
+// out = B, dB/ds, dB/dtheta, dB/dzeta from the 8 corner nodes (64 doubles, 16 x 256-bit loads) of the cell.
+__device__ __forceinline__ void eval_B_hermite(const FieldDev& f, double s, double th, double ze, double out[4]) {
+  const double us = s * (double)(f.ngs - 1);
+  double cs = floor(us);
+  if (!(cs >= 0.0)) cs = 0.0;                                  // also NaN
+  if (cs > (double)(f.ngs - 2)) cs = (double)(f.ngs - 2);
+  const int ci = (int)cs;
+  const double x = us - cs;
+  int cj, ck;
+  double y, z;
+  periodic_cell(f.nth, f.inv_nth, f.th_scale, th, cj, y);
+  periodic_cell(f.nze, f.inv_nze, f.ze_scale, ze, ck, z);
+  double hs[2][2], dhs[2][2], ht[2][2], dht[2][2], hz[2][2], dhz[2][2];
+  hermite_basis(x, hs, dhs);
+  hermite_basis(y, ht, dht);
+  hermite_basis(z, hz, dhz);
+  const size_t rs = (size_t)(f.nze + 1) * 8, ps = (size_t)(f.nth + 1) * rs;
+  const double* base = f.grid + (size_t)ci * ps + (size_t)cj * rs + (size_t)ck * 8;
+  double B = 0.0, Bs = 0.0, Bt = 0.0, Bz = 0.0;
+#pragma unroll
+  for (int a = 0; a < 2; ++a) {
+    double w[2] = {0.0, 0.0}, wt[2] = {0.0, 0.0}, wz[2] = {0.0, 0.0};      // by s-order p
+#pragma unroll
+    for (int b = 0; b < 2; ++b) {
+      const double* nd0 = base + a * ps + b * rs;                           // node (a, b, 0); (a, b, 1) follows it
+#pragma unroll
+      for (int p = 0; p < 2; ++p) {
+        double d0[4], d1[4];                                                // (q, r) = (0,0) (0,1) (1,0) (1,1)
+        ldg256(nd0 + 4 * p, d0[0], d0[1], d0[2], d0[3]);
+        ldg256(nd0 + 8 + 4 * p, d1[0], d1[1], d1[2], d1[3]);
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+          const double v = fma(hz[1][1], d1[2 * q + 1], fma(hz[1][0], d1[2 * q], fma(hz[0][1], d0[2 * q + 1],
+                               hz[0][0] * d0[2 * q])));
+          const double vz = fma(dhz[1][1], d1[2 * q + 1], fma(dhz[1][0], d1[2 * q], fma(dhz[0][1], d0[2 * q + 1],
+                                dhz[0][0] * d0[2 * q])));
+          w[p] = fma(ht[b][q], v, w[p]);
+          wt[p] = fma(dht[b][q], v, wt[p]);
+          wz[p] = fma(ht[b][q], vz, wz[p]);
+        }
+      }
+    }
+#pragma unroll
+    for (int p = 0; p < 2; ++p) {
+      B = fma(hs[a][p], w[p], B);
+      Bs = fma(dhs[a][p], w[p], Bs);
+      Bt = fma(hs[a][p], wt[p], Bt);
+      Bz = fma(hs[a][p], wz[p], Bz);
+    }
+  }
+  out[0] = B; out[1] = Bs * f.inv_ds; out[2] = Bt * f.inv_dth; out[3] = Bz * f.inv_dze;
+}
+
+// B from whichever interpolant the field carries (grid_kind 1 or 2).
+template <int KIND>
+__device__ __forceinline__ void eval_B_interp(const FieldDev& f, double s, double th, double ze, double out[4]) {
+  if (KIND == 2) eval_B_hermite(f, s, th, ze, out);
+  else eval_B_grid(f, s, th, ze, out);
+}
+__device__ __forceinline__ void eval_B_interp_rt(const FieldDev& f, double s, double th, double ze, double out[4]) {
+  if (f.grid_kind == 2) eval_B_hermite(f, s, th, ze, out);
+  else eval_B_grid(f, s, th, ze, out);
+}
+
 }  // namespace gc

@@ -17,13 +17,13 @@ constexpr int kLaneThreads = 128;
 #define GC_LANE_MIN_BLOCKS 2
 #endif
 
-// O4 at one state: GRID = false: direct harmonic sum from the caller's tables (rhs_generic); GRID = true: B and its
-// derivatives from the tricubic interpolant, profiles and perturbation from the radial tables as always.
-template <bool GRID>
+// O4 at one state: GRID = 0: direct harmonic sum from the caller's tables (rhs_generic); GRID = 1 / 2: B and its
+// derivatives from the tricubic Lagrange / Hermite interpolant, profiles and perturbation from the radial tables.
+template <int GRID>
 __device__ __forceinline__ void rhs_lane(const FieldDev& f, double mass, double charge, double mu, double v_ref,
                                          double inv_v_ref, double t, const double y[4], double dy[4]) {
-  if (!GRID) rhs_generic(f, mass, charge, mu, v_ref, inv_v_ref, t, y, dy);
-  else rhs_grid(f, mass, charge, mu, v_ref, inv_v_ref, t, y, dy);
+  if (GRID == 0) rhs_generic(f, mass, charge, mu, v_ref, inv_v_ref, t, y, dy);
+  else rhs_grid<GRID>(f, mass, charge, mu, v_ref, inv_v_ref, t, y, dy);
 }
 
 // Dormand-Prince coefficients by stage for the stage loop: row r holds a_{r+2, 1..6} (O5); c_2 .. c_7.
@@ -49,7 +49,7 @@ __device__ __forceinline__ double dense_hd(const double* kbuf, int c, double h) 
                  fma(dp::d4, GC_K(3, c), fma(dp::d3, GC_K(2, c), dp::d1 * GC_K(0, c))))));
 }
 
-template <bool GRID>
+template <int GRID>
 __global__ void __launch_bounds__(kLaneThreads, GC_LANE_MIN_BLOCKS) trace_lane_kernel(FieldDev f, TraceDev p) {
   extern __shared__ double kbuf[];
   constexpr unsigned kFull = 0xffffffffu;

@@ -36,7 +36,7 @@ struct SymPoint {          // everything of one evaluation at (s, theta, zeta, p
   double B, Bs, Bth, Bze, G, Gs, I, Is, rho, rho_s, pth, D, dpth_dpz;
 };
 
-template <bool GRID>
+template <int GRID>
 __device__ __forceinline__ void sym_eval(const FieldDev& f, const double* chi_nodes, double q, double s, double th,
                                          double ze, double pz, bool with_field, SymPoint& e) {
   int i0;
@@ -53,13 +53,13 @@ __device__ __forceinline__ void sym_eval(const FieldDev& f, const double* chi_no
   e.dpth_dpz = e.I * invG;
   if (with_field) {
     double fb[4];
-    if (GRID) eval_B_grid(f, s, th, ze, fb);
+    if (GRID) eval_B_interp<GRID>(f, s, th, ze, fb);
     else eval_B_generic(f, i0, w, dw, th, ze, fb);
     e.B = fb[0]; e.Bs = fb[1]; e.Bth = fb[2]; e.Bze = fb[3];
   }
 }
 
-template <bool GRID>
+template <int GRID>
 __global__ void __launch_bounds__(128) trace_symplectic_kernel(FieldDev f, SymplecticDev p) {
   for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < p.n;
        i += (long long)gridDim.x * blockDim.x) {
@@ -73,7 +73,7 @@ __global__ void __launch_bounds__(128) trace_symplectic_kernel(FieldDev f, Sympl
       int i0;
       double w[4], dw[4], fb[4], G, Gs, chi, chi_s;
       lagrange_weights(f.ns, s, i0, w, dw);
-      if (GRID) eval_B_grid(f, s, th, ze, fb);
+      if (GRID) eval_B_interp<GRID>(f, s, th, ze, fb);
       else eval_B_generic(f, i0, w, dw, th, ze, fb);
       interp4(f.G, 1, i0, w, dw, G, Gs);
       interp4(p.chi, 1, i0, w, dw, chi, chi_s);
@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(128) trace_symplectic_kernel(FieldDev f, Sympl
         int i0;
         double w[4], dw[4], fb[4];
         lagrange_weights(f.ns, s, i0, w, dw);
-        if (GRID) eval_B_grid(f, s, th, ze, fb);
+        if (GRID) eval_B_interp<GRID>(f, s, th, ze, fb);
         else eval_B_generic(f, i0, w, dw, th, ze, fb);
         p.samples[(0 * p.nsamp + js) * p.n + i] = s;  p.samples[(1 * p.nsamp + js) * p.n + i] = th;
         p.samples[(2 * p.nsamp + js) * p.n + i] = ze; p.samples[(3 * p.nsamp + js) * p.n + i] = q * e.rho * fb[0] / m;
@@ -143,7 +143,7 @@ __global__ void __launch_bounds__(128) trace_symplectic_kernel(FieldDev f, Sympl
       double w[4], dw[4], fb[4];
       sym_eval<GRID>(f, p.chi, q, s, th, ze, pz, false, e);     // rho at the reported state (a failed step moved e)
       lagrange_weights(f.ns, s, i0, w, dw);
-      if (GRID) eval_B_grid(f, s, th, ze, fb);
+      if (GRID) eval_B_interp<GRID>(f, s, th, ze, fb);
       else eval_B_generic(f, i0, w, dw, th, ze, fb);
       vpar = q * e.rho * fb[0] / m;
     }

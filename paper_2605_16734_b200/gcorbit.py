@@ -19,6 +19,7 @@ GC_OK, GC_EINVAL, GC_ENOMEM, GC_ECUDA = 0, -1, -2, -3
 GC_KERNEL_AUTO, GC_KERNEL_GENERIC, GC_KERNEL_WARP, GC_KERNEL_TILE, GC_KERNEL_MMA, GC_KERNEL_GRID = 0, 1, 2, 3, 4, 5
 GC_TILE_MIN_PARTICLES, GC_TILE_MIN_PARTICLES_SMALL = 3072, 2048
 GC_OPT_WAVE_PARTICLES, GC_OPT_CHUNK_ATTEMPTS = 1, 2
+GC_GRID_LAGRANGE, GC_GRID_HERMITE = 0, 1
 ST_TMAX, ST_LOST, ST_AXIS, ST_MAXSTEPS, ST_NONFINITE = 0, 1, 2, 3, 4
 
 EXPORTS = ["gc_field_create", "gc_field_destroy", "gc_field_eval", "gc_pert_eval", "gc_rhs_eval", "gc_trace",
@@ -75,7 +76,7 @@ def load_library():
         L.gc_birkhoff.argtypes = [i64, i64, vp, i64, vp, vp, vp]
         L.gc_set_kernel.argtypes = [vp, i32]
         L.gc_orbit_diagnostics.argtypes = [i64, i64, vp, i64, vp, dbl, dbl, vp, vp]
-        L.gc_field_set_grid.argtypes = [vp, i32, i32, i32, vp]
+        L.gc_field_set_grid.argtypes = [vp, i32, i32, i32, i32, vp]
         L.gc_trace_symplectic.argtypes = [vp, C.POINTER(gc_symplectic_params), i64] + [vp] * 11 + [i64, i64, vp, vp, vp]
         L.gc_set_option.argtypes = [vp, i32, i64]
         L.gc_kernel_info.argtypes = [vp, C.c_int64] + [C.POINTER(i32)] * 5
@@ -213,10 +214,11 @@ class Field:
     def set_option(self, option: int, value: int):
         _check(load_library().gc_set_option(self._h, int(option), int(value)))
 
-    def set_grid(self, ngs: int, nth: int, nze: int):
-        """gc_field_set_grid (NEXT-2): B becomes the tricubic interpolant of its node values; (0, 0, 0) drops it."""
+    def set_grid(self, ngs: int, nth: int, nze: int, kind: int = 0):
+        """gc_field_set_grid (NEXT-2): B becomes a tricubic interpolant of its node values (kind GC_GRID_LAGRANGE) or
+        of its node values and derivatives (GC_GRID_HERMITE); (0, 0, 0) drops it."""
         torch = _torch()
-        _check(load_library().gc_field_set_grid(self._h, int(ngs), int(nth), int(nze), _stream_ptr(torch)))
+        _check(load_library().gc_field_set_grid(self._h, int(ngs), int(nth), int(nze), int(kind), _stream_ptr(torch)))
 
     def kernel_info(self, n: int = 1 << 20) -> dict:
         """Kernel and launch geometry gc_trace uses for an ensemble of n particles."""

@@ -32,14 +32,18 @@ def _run_both(fld, spec, P, OF, GF, mu, dt, nsteps, **kw):
     return r, o
 
 
-@pytest.mark.parametrize("grid", [None, (51, 40, 36)])
+@pytest.mark.parametrize("grid", [None, ("lagrange", (51, 40, 36)), ("hermite", (51, 40, 36))])
 @pytest.mark.parametrize("config,n,dt,nsteps", [(0, 300, 1e-8, 600), (1, 200, 2e-8, 250), (3, 257, 4e-8, 150)])
 def test_symplectic_trace_matches_oracle(config, n, dt, nsteps, grid):
     fld, spec, P, OF, GF, mu = make_case(config, n)
     if grid:
-        OF.set_grid(*grid)
-        GF.set_grid(*grid)
-        from paper_2605_16734_b200 import workloads as W
+        from paper_2605_16734_b200 import gcorbit as G, workloads as W
+        if grid[0] == "hermite":
+            OF.set_grid_hermite(*grid[1])
+            GF.set_grid(*grid[1], kind=G.GC_GRID_HERMITE)
+        else:
+            OF.set_grid(*grid[1])
+            GF.set_grid(*grid[1])
         mu = W.mu_from(P, OF.eval_B_many(P.s, P.theta, P.zeta)[:, 0])
     r, o = _run_both(fld, spec, P, OF, GF, mu, dt, nsteps)
     assert np.array_equal(r.status.cpu().numpy(), o.status)
@@ -48,7 +52,7 @@ def test_symplectic_trace_matches_oracle(config, n, dt, nsteps, grid):
     ok = o.status != 4
     rel = rel_diff(r.y.cpu().numpy()[:, ok], o.y[:, ok], spec.v_ref)
     it = r.n_iter.cpu().numpy() / np.maximum(o.n_steps, 1)
-    record_info("symplectic_parity", label=f"config {config} {'grid' if grid else 'sum'} dt={dt:g} x {nsteps}",
+    record_info("symplectic_parity", label=f"config {config} {grid[0] + ' grid' if grid else 'sum'} dt={dt:g} x {nsteps}",
                 particles=int(ok.sum()), max_rel=float(rel.max()), median_rel=float(np.median(rel)),
                 iterations_per_step=float(it.mean()), oracle_iterations_per_step=float((o.n_iter / np.maximum(o.n_steps, 1)).mean()))
     assert rel.max() < 1e-9 and np.median(rel) < 1e-11, (rel.max(), np.median(rel))

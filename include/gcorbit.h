@@ -252,7 +252,9 @@ int gc_orbit_diagnostics(int64_t n, int64_t nsamp, const double* samples, int64_
  * step of size dt solves  p_theta' - p_theta + dt dH/dtheta = 0,  p_zeta' - p_zeta + dt dH/dzeta = 0  for
  * (s', p_zeta') at the old angles (to a last update below newton_tol max(1, |x|) of x = (s, p_zeta / (q psi0)),
  * status 4 after max_iter iterations) and then advances the angles explicitly with the derivatives of H at the new
- * (s', p_zeta').  Works on the direct harmonic sum and on the 3-D interpolant of gc_field_set_grid alike. */
+ * (s', p_zeta').  Works on the direct harmonic sum (ensembles of at least GC_TILE_MIN_PARTICLES on the cell-binned mma
+ * engine, one pass per field evaluation; smaller ones, sampled ones and GC_KERNEL_GENERIC on the lane kernel) and on
+ * the 3-D interpolants of gc_field_set_grid. */
 typedef struct {
   double mass, charge;        /* kg, C                                                              */
   double t0, dt;              /* s; fixed step dt > 0                                               */

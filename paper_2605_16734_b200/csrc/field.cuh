@@ -87,6 +87,12 @@ struct TraceDev {
   long long nsamp;
   double* samples;
   int* sample_end;
+  // the symplectic integrator inside the cell-binned body (trace_mma_symplectic_kernel): fixed step, steps per call,
+  // tolerance and cap of the quasi-Newton iteration, chi at the radial nodes; n_acc / n_rej receive steps / iterations
+  double sym_dt, sym_tol;
+  long long sym_nsteps;
+  int sym_max_iter;
+  const double* chi;
 };
 
 }  // namespace gc

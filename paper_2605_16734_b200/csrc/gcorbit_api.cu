@@ -219,6 +219,11 @@ const void* mma_fn_t(const gc_field* f) {
   return modes ? (const void*)gc::trace_mma_kernel<2, 4, true, SAMPLE> : (const void*)gc::trace_mma_kernel<2, 4, false, SAMPLE>;
 }
 const void* mma_fn(const gc_field* f, bool sample = false) { return sample ? mma_fn_t<true>(f) : mma_fn_t<false>(f); }
+// the symplectic integrator on the mma engine (static fields without NEXT-4 tables)
+const void* mma_sym_fn(const gc_field* f) {
+  return f->dev.mma_MT == 1 ? (const void*)gc::trace_mma_symplectic_kernel<1, 2>
+                            : (const void*)gc::trace_mma_symplectic_kernel<2, 4>;
+}
 
 int resolve_kernel(const gc_field* f, int64_t n) {
   if (f->dev.grid) return GC_KERNEL_GRID;                  // the field IS the interpolant while a grid is set
@@ -362,6 +367,7 @@ int pack_mma_image(gc_field* f, const gc_field_desc* d) {
   const void* fn = mma_fn(f);
   GC_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, kBinnedSmemCap));
   GC_CUDA(cudaFuncSetAttribute(mma_fn(f, true), cudaFuncAttributeMaxDynamicSharedMemorySize, kBinnedSmemCap));
+  if (!f->extra) GC_CUDA(cudaFuncSetAttribute(mma_sym_fn(f), cudaFuncAttributeMaxDynamicSharedMemorySize, kBinnedSmemCap));
   int per_sm = 0, per_sm_diag = 0;                         // the plain and the diagnostics build share one grid size
   GC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, gc::kMmaThreads, (size_t)smem));
   GC_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_diag, mma_fn(f, true), gc::kMmaThreads, (size_t)smem));
@@ -404,7 +410,8 @@ long long wave_size(const gc_field* f, long long n) {
 }
 
 // One cooperative launch of the tile or mma kernel (mode 0 trace, mode 1 right-hand side only) with its scratch.
-int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, cudaStream_t st, bool mma = false) {
+int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, cudaStream_t st, bool mma = false,
+                bool symplectic = false) {
   const int ncell = f->dev.ns - 3;
   const size_t n = (size_t)t.n;
   const long long wave = wave_size(f, (long long)n);
@@ -435,8 +442,8 @@ int launch_tile(const gc_field* f, gc::TraceDev& t, int mode, double* rhs_out, c
   void* args[] = {(void*)&fd, (void*)&t, (void*)&sc, (void*)&mode, (void*)&rhs_out};
   const bool sample = mode == 0 && (t.nsamp > 0 || t.section != 0 || t.refine_loss != 0);   // the diagnostics build of the kernel
   const cudaError_t le =
-      mma ? cudaLaunchCooperativeKernel(mma_fn(f, sample), dim3((unsigned)blocks), dim3(gc::kMmaThreads), args,
-                                        (size_t)f->mma_smem, st)
+      mma ? cudaLaunchCooperativeKernel(symplectic ? mma_sym_fn(f) : mma_fn(f, sample), dim3((unsigned)blocks),
+                                        dim3(gc::kMmaThreads), args, (size_t)f->mma_smem, st)
           : cudaLaunchCooperativeKernel(tile_fn(f, sample), dim3((unsigned)blocks), dim3(gc::kTileThreads), args,
                                         (size_t)f->tile_smem, st);
   const cudaError_t fe = cudaFreeAsync(slab, st);           // also on a failed launch: the scratch must not leak
@@ -909,6 +916,22 @@ int gc_trace_symplectic(const gc_field* f, const gc_symplectic_params* p, int64_
   if (n == 0) return GC_OK;
   if (!s0 || !th0 || !ze0 || !vpar0 || !mu || !chi_nodes || !y_out || !t_out || !status)
     return fail(GC_EINVAL, "gc_trace_symplectic: NULL particle array or chi_nodes");
+  // large ensembles on the direct sum: the cell-binned mma engine (one pass = one field evaluation per lane)
+  {
+    const int64_t nmin = (f->dev.M <= 8 && f->dev.N <= 8) ? GC_TILE_MIN_PARTICLES_SMALL : GC_TILE_MIN_PARTICLES;
+    if (!f->dev.grid && f->mma_ok && !f->extra && f->mma_blocks_per_sm > 0 && n >= nmin && nsamp == 0 &&
+        p->nsteps >= 1 && f->kernel != GC_KERNEL_GENERIC) {
+      gc::TraceDev t{};
+      t.mass = p->mass; t.charge = p->charge; t.t0 = p->t0; t.t_max = p->t0; t.v_ref = 1.0; t.inv_v_ref = 1.0;
+      t.s_loss = p->s_loss; t.s_min = p->s_min; t.max_steps = 1; t.n = n;
+      t.resume = (p->flags & GC_TRACE_RESUME) ? 1 : 0;
+      t.s0 = s0; t.th0 = th0; t.ze0 = ze0; t.vpar0 = vpar0; t.mu = mu;
+      t.y_out = y_out; t.t_out = t_out; t.status = status; t.n_acc = n_steps; t.n_rej = n_iter;
+      t.sym_dt = p->dt; t.sym_tol = p->newton_tol; t.sym_nsteps = p->nsteps; t.sym_max_iter = (int)p->max_iter;
+      t.chi = chi_nodes;
+      return launch_tile(f, t, 0, nullptr, (cudaStream_t)stream, true, true);
+    }
+  }
   gc::SymplecticDev d{};
   d.mass = p->mass; d.charge = p->charge; d.t0 = p->t0; d.dt = p->dt; d.s_loss = p->s_loss; d.s_min = p->s_min;
   d.tol = p->newton_tol; d.nsteps = p->nsteps; d.n = n; d.sample_stride = sample_stride > 0 ? sample_stride : 1;

@@ -124,6 +124,7 @@ __device__ inline void eval_pert_generic(const FieldDev& f, int i0, const double
   double Phi = 0, Phi_s = 0, Phi_th = 0, Phi_ze = 0, al = 0, al_s = 0, al_th = 0, al_ze = 0, al_t = 0;
   const double thr = reduce_2pi(th), zer = reduce_2pi(ze);
   const double GI = p.G + p.io * p.I, GI_s = p.Gs + p.ios * p.I + p.io * p.Is;
+  const double invGI = 1.0 / GI, gig = GI_s * invGI;          // one division per evaluation, not one per mode
   for (int k = 0; k < f.nk; ++k) {
     double ph, ph_s;
     interp4(f.phihat + k, f.nk, i0, w, dw, ph, ph_s);
@@ -133,10 +134,10 @@ __device__ inline void eval_pert_generic(const FieldDev& f, int i0, const double
     double sn, cs;
     sincos_poly(fma(m, thr, fma(-n, zer, wt + __ldg(f.phase + k))), sn, cs);
     // alpha_hat = -Phi_hat (iota m - n) / (omega (G + iota I))    (O3)
-    const double inv = 1.0 / (om * GI);
+    const double inv = __ldg(f.inv_omega + k) * invGI;         // 1 / (omega (G + iota I))
     const double N = fma(p.io, m, -n);
     const double ah = -ph * N * inv;
-    const double ah_s = -(ph_s * N + ph * p.ios * m) * inv + ph * N * inv * (GI_s / GI);
+    const double ah_s = -(ph_s * N + ph * p.ios * m) * inv + ph * N * inv * gig;
     Phi = fma(ph, sn, Phi);
     Phi_s = fma(ph_s, sn, Phi_s);
     Phi_th = fma(m * ph, cs, Phi_th);

@@ -184,10 +184,12 @@ __device__ __forceinline__ void mma_sweep(const double* base, int RS, int r_lo, 
 
 // Right-hand side of one lane = one particle (same contract as rhs_tile); must be called by all 32 lanes of a warp.
 // win = shared-memory copy of image rows cell .. cell+7 (node rows cell-2 .. cell+5).
-template <int MT, int KS, bool MODES, bool EXTRA = false>
+// FIELD_ONLY (the symplectic integrator, NEXT-3): stop after the sums and the profiles and hand out B, B_s, B_theta,
+// B_zeta in dy[0..3] and G, G_s, I, I_s, iota, iota_s in *prof_out instead of the guiding-centre algebra.
+template <int MT, int KS, bool MODES, bool EXTRA = false, bool FIELD_ONLY = false>
 __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, double* ext, int cell, bool active,
                                         double mass, double charge, double mu, double v_ref, double inv_v_ref,
-                                        double t, const double (&y)[4], double (&dy)[4]) {
+                                        double t, const double (&y)[4], double (&dy)[4], Profiles* prof_out = nullptr) {
   using R = MmaRow<MT, KS>;
   const int lane = threadIdx.x & 31, q = lane & 3;
   const int RS = f.mma_RS;
@@ -329,6 +331,10 @@ __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, do
 #pragma unroll
     for (int a = 0; a < 4; ++a) v[a] = prow[(size_t)a * RS + R::kProf + 2];
     pr.io = dot4(w, v); pr.ios = dot4(dw, v);
+    if constexpr (FIELD_ONLY) {
+      dy[0] = fb[0]; dy[1] = fb[1]; dy[2] = fb[2]; dy[3] = fb[3] * (double)f.nfp;
+      *prof_out = pr;
+    } else {
     double pt[9];
 #pragma unroll
     for (int k = 0; k < 9; ++k) pt[k] = 0.0;
@@ -371,6 +377,7 @@ __device__ __forceinline__ void rhs_mma(const FieldDev& f, const double* win, do
       gc_algebra(mass, charge, mu, f.inv_psi0, y[3] * v_ref, fb, pr, pt, dy);
     }
     dy[3] *= inv_v_ref;
+    }
   }
 }
 
@@ -388,12 +395,27 @@ struct MmaEngine {
                                              double t, const double (&y)[4], double (&dy)[4]) {
     rhs_mma<MT, KS, MODES, EXTRA>(f, win, ext, cell, active, mass, charge, mu, v_ref, inv_v_ref, t, y, dy);
   }
+  // B, B_s, B_theta, B_zeta and the profiles at (s, theta, zeta); must be called by all 32 lanes of a warp.
+  static __device__ __forceinline__ void field(const FieldDev& f, const double* win, double* ext, int cell, bool active,
+                                               double s, double th, double ze, double (&fb)[4], Profiles& pr) {
+    const double y[4] = {s, th, ze, 0.0};
+    rhs_mma<MT, KS, false, false, true>(f, win, ext, cell, active, 1.0, 1.0, 0.0, 1.0, 1.0, 0.0, y, fb, &pr);
+  }
 };
 
 template <int MT, int KS, bool MODES, bool SAMPLE, bool EXTRA = false>
 __global__ void __launch_bounds__(kMmaThreads, kMmaBlocksPerSm)
 trace_mma_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_out) {
   trace_binned_body<MmaEngine<MT, KS, MODES, EXTRA>, kMmaThreads, kMmaCap, SAMPLE>(f, p, sc, mode, rhs_out);
+}
+
+// NEXT-3 on the direct harmonic sum: the symplectic explicit-implicit Euler integrator inside the same cell-binned
+// persistent body (binning, tiles, record slots, DMMA sweep); every pass of a lane is one evaluation of the field, i.e.
+// one quasi-Newton iteration of its current step (kernels_symplectic.cuh has the scheme).
+template <int MT, int KS>
+__global__ void __launch_bounds__(kMmaThreads, kMmaBlocksPerSm)
+trace_mma_symplectic_kernel(FieldDev f, TraceDev p, TileScratch sc, int mode, double* rhs_out) {
+  trace_binned_body<MmaEngine<MT, KS, false, false>, kMmaThreads, kMmaCap, false, 1>(f, p, sc, mode, rhs_out);
 }
 
 }  // namespace gc

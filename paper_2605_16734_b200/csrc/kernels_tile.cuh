@@ -65,7 +65,7 @@ struct TileScratch {
   int* ctrl;        // [0] tile counter, [1] tiles past their first chunk, [2] tiles this epoch, [3] running, [4] input exhausted
 };
 
-enum { kFlagPrevRejected = 1, kFlagHaveK1 = 2 };
+enum { kFlagPrevRejected = 1, kFlagHaveK1 = 2, kFlagFresh = 4, kFlagFinal = 8 };   // 4, 8: symplectic passes
 enum { kStRunning = -1, kStSkip = -2, kStEmpty = -3 };   // slot states below 0; >= 0: finished, not yet flushed
 
 __constant__ double cDpA[7][6] = {
@@ -308,7 +308,13 @@ struct TileEngine {
 // mode 0: trace.  mode 1: right-hand side only (gc_rhs_eval): k1 of every particle goes to rhs_out[4][n].
 // THREADS = particles per tile = threads per block; CAP = attempted steps per lane per chunk; SAMPLE = record the
 // uniform-time samples of gc_trace_sampled (O9; a separate instantiation, so that gc_trace pays nothing for it).
-template <class Eng, int THREADS, int CAP, bool SAMPLE>
+// INTEG = 1: the symplectic explicit-implicit Euler integrator (NEXT-3) instead of Dormand-Prince: a pass of a lane is
+// one field evaluation = one quasi-Newton iteration of its current step.  Lane state in the same record: y = (s, theta,
+// zeta, p_zeta / (q psi0)) at the start of the step (v_par until the first pass has turned it into p_zeta), the k1 slot
+// = (p_theta at the start of the step, iterate s, iterate p_zeta / (q psi0), v_par at the start of the step), n_acc =
+// steps, n_rej = iterations, n_forced = iterations of the current step, `attempts` = the status the particle will
+// report once its final pass has evaluated B at the end point (v_par = q rho B / m needs it).
+template <class Eng, int THREADS, int CAP, bool SAMPLE, int INTEG = 0>
 __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const TraceDev& p, const TileScratch& sc, int mode,
                                                   double* rhs_out) {
   cgx::grid_group grid = cgx::this_grid();
@@ -361,9 +367,9 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
       }
     }
     stcg4(r, make_double4(y0, y1, y2, y3));
-    stcg4(r + 4, make_double4(0.0, 0.0, 0.0, 0.0));
+    stcg4(r + 4, INTEG == 1 ? make_double4(0.0, y0, 0.0, y3) : make_double4(0.0, 0.0, 0.0, 0.0));
     stcg4(r + 8, make_double4(t, h, mu, __longlong_as_double(0LL)));
-    __stcg(reinterpret_cast<int4*>(r + 12), make_int4(kStRunning, 0, 0, 0));
+    __stcg(reinterpret_cast<int4*>(r + 12), make_int4(kStRunning, INTEG == 1 ? (int)kFlagFresh : 0, 0, 0));
     __stcg(reinterpret_cast<int4*>(r + 12) + 1, make_int4(0, bin, jn0, (int)i));
     atomicAdd(sc.cnt + bin, 1);
   };
@@ -525,6 +531,82 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
             int done = 0;
             if ((tid & 31) == 0) done = *reinterpret_cast<const volatile int*>(sc.ctrl + 1);
             if (__shfl_sync(0xffffffffu, done, 0) >= ntiles) break;
+          }
+          if constexpr (INTEG == 1) {
+            // ---- one symplectic pass: the field at the current iterate (kernels_symplectic.cuh has the scheme) ------
+            const double q = p.charge, unit = q * f.psi0, inv_unit = 1.0 / unit;
+            const double x0 = kb(0, 1);
+            double fb[4];
+            Profiles pr;
+            Eng::field(f, win, ext, cell, running, x0, y[1], y[2], fb, pr);
+            if (running) {
+              int i0c;
+              double wc[4], dwc[4], chi, chi_s;
+              lagrange_weights(f.ns, x0, i0c, wc, dwc);
+              interp4(p.chi, 1, i0c, wc, dwc, chi, chi_s);
+              const double invG = 1.0 / pr.G;
+              double x1 = kb(0, 2);
+              if (flags & kFlagFresh) {                        // v_par -> p_zeta = q (rho G - chi), rho = m v_par / (q B)
+                x1 = (p.mass * y[3] / (q * fb[0]) * pr.G - chi) * q * inv_unit;
+                y[3] = x1;
+                flags &= ~kFlagFresh;
+                if (!finite4(y[0], y[1], y[2], x1)) { st = GC_ST_NONFINITE_; y[3] = kb(0, 3); running = false; }
+              }
+              const double rho = (x1 * unit / q + chi) * invG;
+              const double vpar_here = q * rho * fb[0] / p.mass;
+              if (running && (flags & kFlagFinal)) {             // the end point: report v_par and stop
+                y[3] = vpar_here;
+                st = (int)attempts;
+                running = false;
+              }
+              if (running) {
+                const double rho_s = (chi_s - rho * pr.Gs) * invG;
+                const double pth = q * fma(rho, pr.I, f.psi0 * x0);
+                const double D = q * (f.psi0 + rho_s * pr.I + rho * pr.Is);
+                const double dpth_dpz = pr.I * invG;
+                if (n_forced == 0) { kb(0, 0) = pth; kb(0, 3) = vpar_here; }      // a step starts at this point
+                const double qr = q * rho;
+                const double dHdB = fma(qr * qr / p.mass, fb[0], mu);
+                const double F1 = pth - kb(0, 0) + p.sym_dt * dHdB * fb[2];
+                const double F2 = (x1 - y[3]) * unit + p.sym_dt * dHdB * fb[3];
+                const double dpz = -F2;
+                const double ds = -(F1 + dpth_dpz * dpz) / D;
+                const double dx1 = dpz * inv_unit;
+                ++n_forced;
+                ++n_rej;
+                if (!isfinite(ds) || !isfinite(dx1)) {
+                  st = GC_ST_NONFINITE_; y[3] = kb(0, 3); running = false;
+                } else {
+                  const double xn0 = x0 + ds, xn1 = x1 + dx1;
+                  kb(0, 1) = xn0; kb(0, 2) = xn1;
+                  if (fabs(ds) <= p.sym_tol * fmax(1.0, fabs(xn0)) && fabs(dx1) <= p.sym_tol * fmax(1.0, fabs(xn1))) {
+                    const double H_s = qr * q * rho_s * fb[0] * fb[0] / p.mass + dHdB * fb[1];
+                    const double H_pz = qr * fb[0] * fb[0] / (p.mass * pr.G);
+                    y[1] = fma(p.sym_dt, H_s / D, y[1]);
+                    y[2] = fma(p.sym_dt, H_pz - H_s * dpth_dpz / D, y[2]);
+                    y[0] = xn0;
+                    y[3] = xn1;
+                    n_forced = 0;
+                    if (!finite4(y[0], y[1], y[2], y[3])) {
+                      st = GC_ST_NONFINITE_; running = false;          // (cannot be told from the oracle's case)
+                    } else {
+                      ++n_acc;
+                      t = __dadd_rn(p.t0, __dmul_rn((double)n_acc, p.sym_dt));
+                      int stop = -1;
+                      if (y[0] >= p.s_loss) stop = 1;
+                      else if (y[0] <= p.s_min) stop = 2;
+                      else if ((long long)n_acc >= p.sym_nsteps) stop = 0;
+                      if (stop >= 0) { flags |= kFlagFinal; attempts = stop; }
+                      const int hc = home_cell(f.ns, y[0]);
+                      if (hc < cell - 1 || hc > cell + 1) running = false;   // parked until the next binning
+                    }
+                  } else if (n_forced >= p.sym_max_iter) {
+                    st = GC_ST_NONFINITE_; y[3] = kb(0, 3); running = false;  // the state before the failed step
+                  }
+                }
+              }
+            }
+            continue;
           }
           // stage 0 gives k1 to lanes that do not carry one yet (first epoch; gc_rhs_eval)
           const bool do_k1 = __any_sync(0xffffffffu, running && !(flags & kFlagHaveK1));

@@ -151,3 +151,51 @@ def test_symplectic_energy_is_bounded_while_dormand_prince_drifts_on_the_device(
     record_info("symplectic_energy", label=f"config-0 smooth field, {int(keep.sum())} particles, 4e-4 s",
                 sym_amp_max=float(amp_s.max()), sym_drift_median=float(np.median(drift_s)),
                 dp5_rtol1e6_drift_median=float(np.median(drift_d)))
+
+
+@pytest.mark.parametrize("config,n,dt,nsteps", [(0, 2048 + 37, 1e-8, 300), (1, 3072 + 5, 2e-8, 100)])
+def test_symplectic_on_the_mma_engine_matches_oracle_and_the_lane_kernel(config, n, dt, nsteps):
+    """Ensembles of at least GC_TILE_MIN_PARTICLES(_SMALL) on the direct sum run through the cell-binned mma engine
+    (trace_mma_symplectic_kernel: one pass of a lane = one field evaluation = one quasi-Newton iteration); smaller ones
+    and GC_KERNEL_GENERIC through the lane kernel.  Both against the oracle, with stop surfaces close enough that all
+    three exits occur."""
+    import torch
+    from paper_2605_16734_b200 import gcorbit as G
+    fld, spec, P, OF, GF, mu = make_case(config, n)
+    lo, hi = float(np.quantile(P.s, 0.02)), float(np.quantile(P.s, 0.98))
+    kw = dict(s_loss=hi + 2e-4, s_min=max(lo - 2e-4, 1e-3))
+    if config == 0:                                          # every particle starts on s = 0.25
+        kw = dict(s_loss=0.2515, s_min=0.2485)
+    r, o = _run_both(fld, spec, P, OF, GF, mu, dt, nsteps, **kw)
+    GF.set_kernel(G.GC_KERNEL_GENERIC)
+    g = GF.trace_symplectic(spec.mass, spec.charge, to_dev(P.s), to_dev(P.theta), to_dev(P.zeta), to_dev(P.vpar),
+                            to_dev(mu), to_dev(_chi(fld)), dt, nsteps, **kw)
+    GF.set_kernel(G.GC_KERNEL_AUTO)
+    torch.cuda.synchronize()
+    st = r.status.cpu().numpy()
+    assert np.array_equal(st, o.status) and np.array_equal(g.status.cpu().numpy(), o.status)
+    assert (st == 0).any() and ((st == 1).any() or (st == 2).any())
+    assert np.array_equal(r.n_steps.cpu().numpy(), o.n_steps) and np.array_equal(g.n_steps.cpu().numpy(), o.n_steps)
+    assert np.allclose(r.t.cpu().numpy(), o.t, rtol=1e-15, atol=0)
+    rel = rel_diff(r.y.cpu().numpy(), o.y, spec.v_ref)
+    relg = rel_diff(g.y.cpu().numpy(), o.y, spec.v_ref)
+    it = r.n_iter.cpu().numpy().sum() / max(o.n_steps.sum(), 1)
+    record_info("symplectic_parity", label=f"config {config} sum, mma engine, {n} particles dt={dt:g} x {nsteps}",
+                particles=n, max_rel=float(rel.max()), median_rel=float(np.median(rel)), iterations_per_step=float(it),
+                oracle_iterations_per_step=float(o.n_iter.sum() / max(o.n_steps.sum(), 1)))
+    assert rel.max() < 1e-9 and np.median(rel) < 1e-11, (rel.max(), np.median(rel))
+    assert relg.max() < 1e-9
+    # the two device paths iterate alike (the final pass of the binned path counts as one more evaluation per particle)
+    assert abs(it - g.n_iter.cpu().numpy().sum() / max(o.n_steps.sum(), 1)) < 0.1
+    # two resumed halves on the mma engine against one call
+    a = [to_dev(x) for x in (P.s, P.theta, P.zeta, P.vpar, mu)]
+    chi = to_dev(_chi(fld))
+    h = nsteps // 2
+    two = GF.trace_symplectic(spec.mass, spec.charge, *a, chi, dt, h, **kw)
+    y = two.y
+    GF.trace_symplectic(spec.mass, spec.charge, y[0], y[1], y[2], y[3], a[4], chi, dt, nsteps - h, t0=h * dt, out=two,
+                        flags=G.GC_TRACE_RESUME, **kw)
+    torch.cuda.synchronize()
+    assert np.array_equal(two.status.cpu().numpy(), o.status)
+    assert np.array_equal(two.n_steps.cpu().numpy(), o.n_steps)
+    assert rel_diff(two.y.cpu().numpy(), o.y, spec.v_ref).max() < 1e-9

@@ -12,7 +12,8 @@
 //     zeta'  = zeta  + h [dH/dp_zeta - (dH/ds) (dp_theta/dp_zeta) / (dp_theta/ds)]
 // The 2 x 2 system is solved by a quasi-Newton iteration whose Jacobian is the h = 0 part of the exact one,
 // [[dp_theta/ds, dp_theta/dp_zeta], [0, 1]]: every iteration costs ONE evaluation of B and its derivatives (no second
-// derivatives of the field), the error shrinks by h |d(dH/dtheta)/ds| / (dp_theta/ds) ~ 1e-3 per iteration, and the
+// derivatives of the field), the error shrinks by h |d(dH/dtheta)/ds| / (dp_theta/ds) ~ 1e-3 per iteration, it starts
+// from the linear extrapolation of the previous step, and the
 // iteration stops when the update of (s, p_zeta / (q psi0)) is below newton_tol max(1, |x|) -- the root the oracle's
 // Newton iteration converges to.  The partial derivatives of the last evaluation (within newton_tol of the root) feed
 // the explicit half.  One lane per particle; every particle takes the same number of steps, so there is no queue.
@@ -91,9 +92,12 @@ __global__ void __launch_bounds__(128) trace_symplectic_kernel(FieldDev f, Sympl
     }
     sym_eval<GRID>(f, p.chi, q, s, th, ze, pz, false, e);
     double pth_old = e.pth;
+    double ds_prev = 0.0, dx1_prev = 0.0;                      // increments of the last step: the predictor
     for (long long k = 0; k < p.nsteps && st == 0; ++k) {
       const double pz_old = pz;
-      double x0 = s, x1 = pz * inv_unit;
+      // start the iteration from the linear extrapolation of the last step (error O(h^2) instead of O(h): one to two
+      // iterations fewer; the root it converges to is the same)
+      double x0 = s + ds_prev, x1 = pz * inv_unit + dx1_prev;
       bool ok = false;
       int it = 0;
       double H_s = 0.0, H_pz = 0.0;
@@ -118,6 +122,8 @@ __global__ void __launch_bounds__(128) trace_symplectic_kernel(FieldDev f, Sympl
       // explicit half with the partial derivatives of the last evaluation (within tol of the root)
       th = fma(p.dt, H_s / e.D, th);
       ze = fma(p.dt, H_pz - H_s * e.dpth_dpz / e.D, ze);
+      ds_prev = x0 - s;
+      dx1_prev = x1 - pz * inv_unit;
       s = x0;
       pz = x1 * unit;
       if (!finite4(s, th, ze, pz)) { st = GC_ST_NONFINITE_; break; }

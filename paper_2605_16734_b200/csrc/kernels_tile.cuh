@@ -313,7 +313,7 @@ struct TileEngine {
 // zeta, p_zeta / (q psi0)) at the start of the step (v_par until the first pass has turned it into p_zeta), the k1 slot
 // = (p_theta at the start of the step, iterate s, iterate p_zeta / (q psi0), v_par at the start of the step), n_acc =
 // steps, n_rej = iterations, n_forced = iterations of the current step, `attempts` = the status the particle will
-// report once its final pass has evaluated B at the end point (v_par = q rho B / m needs it).
+// report once its final pass has evaluated B at the reported point (v_par = q rho B / m needs it).
 template <class Eng, int THREADS, int CAP, bool SAMPLE, int INTEG = 0>
 __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const TraceDev& p, const TileScratch& sc, int mode,
                                                   double* rhs_out) {
@@ -367,7 +367,7 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
       }
     }
     stcg4(r, make_double4(y0, y1, y2, y3));
-    stcg4(r + 4, INTEG == 1 ? make_double4(0.0, y0, 0.0, y3) : make_double4(0.0, 0.0, 0.0, 0.0));
+    stcg4(r + 4, INTEG == 1 ? make_double4(0.0, y0, 0.0, 0.0) : make_double4(0.0, 0.0, 0.0, 0.0));
     stcg4(r + 8, make_double4(t, h, mu, __longlong_as_double(0LL)));
     __stcg(reinterpret_cast<int4*>(r + 12), make_int4(kStRunning, INTEG == 1 ? (int)kFlagFresh : 0, 0, 0));
     __stcg(reinterpret_cast<int4*>(r + 12) + 1, make_int4(0, bin, jn0, (int)i));
@@ -534,6 +534,8 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
           }
           if constexpr (INTEG == 1) {
             // ---- one symplectic pass: the field at the current iterate (kernels_symplectic.cuh has the scheme) ------
+            // k1 slot: (p_theta at the start of the step, iterate s, iterate p_zeta / (q psi0), increment of s over the
+            // last step); h = increment of p_zeta / (q psi0) over the last step (the predictor of the next one)
             const double q = p.charge, unit = q * f.psi0, inv_unit = 1.0 / unit;
             const double x0 = kb(0, 1);
             double fb[4];
@@ -548,23 +550,30 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
               double x1 = kb(0, 2);
               if (flags & kFlagFresh) {                        // v_par -> p_zeta = q (rho G - chi), rho = m v_par / (q B)
                 x1 = (p.mass * y[3] / (q * fb[0]) * pr.G - chi) * q * inv_unit;
-                y[3] = x1;
                 flags &= ~kFlagFresh;
-                if (!finite4(y[0], y[1], y[2], x1)) { st = GC_ST_NONFINITE_; y[3] = kb(0, 3); running = false; }
+                if (!finite4(y[0], y[1], y[2], x1)) { st = GC_ST_NONFINITE_; running = false; }   // y[3] is still v_par
+                else y[3] = x1;
               }
               const double rho = (x1 * unit / q + chi) * invG;
-              const double vpar_here = q * rho * fb[0] / p.mass;
-              if (running && (flags & kFlagFinal)) {             // the end point: report v_par and stop
-                y[3] = vpar_here;
+              if (running && (flags & kFlagFinal)) {             // the reported point: v_par = q rho B / m, then stop
+                y[3] = q * rho * fb[0] / p.mass;
                 st = (int)attempts;
                 running = false;
               }
               if (running) {
+                if (n_forced == 0) {                             // a step starts: p_theta at its start point (profiles only)
+                  int i0s;
+                  double ws[4], dws[4], Gs_, dG_, Is_, dI_, chis_, dchis_;
+                  lagrange_weights(f.ns, y[0], i0s, ws, dws);
+                  interp4(f.G, 1, i0s, ws, dws, Gs_, dG_);
+                  interp4(f.I, 1, i0s, ws, dws, Is_, dI_);
+                  interp4(p.chi, 1, i0s, ws, dws, chis_, dchis_);
+                  kb(0, 0) = q * fma((y[3] * unit / q + chis_) / Gs_, Is_, f.psi0 * y[0]);
+                }
                 const double rho_s = (chi_s - rho * pr.Gs) * invG;
                 const double pth = q * fma(rho, pr.I, f.psi0 * x0);
                 const double D = q * (f.psi0 + rho_s * pr.I + rho * pr.Is);
                 const double dpth_dpz = pr.I * invG;
-                if (n_forced == 0) { kb(0, 0) = pth; kb(0, 3) = vpar_here; }      // a step starts at this point
                 const double qr = q * rho;
                 const double dHdB = fma(qr * qr / p.mass, fb[0], mu);
                 const double F1 = pth - kb(0, 0) + p.sym_dt * dHdB * fb[2];
@@ -574,35 +583,45 @@ __device__ __forceinline__ void trace_binned_body(const FieldDev& f, const Trace
                 const double dx1 = dpz * inv_unit;
                 ++n_forced;
                 ++n_rej;
-                if (!isfinite(ds) || !isfinite(dx1)) {
-                  st = GC_ST_NONFINITE_; y[3] = kb(0, 3); running = false;
-                } else {
+                bool failed = !isfinite(ds) || !isfinite(dx1);
+                if (!failed) {
                   const double xn0 = x0 + ds, xn1 = x1 + dx1;
                   kb(0, 1) = xn0; kb(0, 2) = xn1;
                   if (fabs(ds) <= p.sym_tol * fmax(1.0, fabs(xn0)) && fabs(dx1) <= p.sym_tol * fmax(1.0, fabs(xn1))) {
                     const double H_s = qr * q * rho_s * fb[0] * fb[0] / p.mass + dHdB * fb[1];
                     const double H_pz = qr * fb[0] * fb[0] / (p.mass * pr.G);
-                    y[1] = fma(p.sym_dt, H_s / D, y[1]);
-                    y[2] = fma(p.sym_dt, H_pz - H_s * dpth_dpz / D, y[2]);
-                    y[0] = xn0;
-                    y[3] = xn1;
-                    n_forced = 0;
-                    if (!finite4(y[0], y[1], y[2], y[3])) {
-                      st = GC_ST_NONFINITE_; running = false;          // (cannot be told from the oracle's case)
+                    const double th_new = fma(p.sym_dt, H_s / D, y[1]);
+                    const double ze_new = fma(p.sym_dt, H_pz - H_s * dpth_dpz / D, y[2]);
+                    if (!finite4(xn0, th_new, ze_new, xn1)) {
+                      failed = true;
                     } else {
+                      kb(0, 3) = xn0 - y[0];                     // the predictor of the next step
+                      h = xn1 - y[3];
+                      y[0] = xn0; y[1] = th_new; y[2] = ze_new; y[3] = xn1;
+                      n_forced = 0;
                       ++n_acc;
                       t = __dadd_rn(p.t0, __dmul_rn((double)n_acc, p.sym_dt));
                       int stop = -1;
                       if (y[0] >= p.s_loss) stop = 1;
                       else if (y[0] <= p.s_min) stop = 2;
                       else if ((long long)n_acc >= p.sym_nsteps) stop = 0;
-                      if (stop >= 0) { flags |= kFlagFinal; attempts = stop; }
+                      if (stop >= 0) {
+                        flags |= kFlagFinal; attempts = stop;     // next pass: B at the end point
+                      } else {
+                        kb(0, 1) = y[0] + kb(0, 3);              // start the next step from the extrapolation
+                        kb(0, 2) = y[3] + h;
+                      }
                       const int hc = home_cell(f.ns, y[0]);
                       if (hc < cell - 1 || hc > cell + 1) running = false;   // parked until the next binning
                     }
                   } else if (n_forced >= p.sym_max_iter) {
-                    st = GC_ST_NONFINITE_; y[3] = kb(0, 3); running = false;  // the state before the failed step
+                    failed = true;
                   }
+                }
+                if (failed) {                                    // report the state before the failed step: one more
+                  flags |= kFlagFinal; attempts = GC_ST_NONFINITE_;   // pass at that point for its v_par
+                  kb(0, 1) = y[0]; kb(0, 2) = y[3];
+                  n_forced = 0;
                 }
               }
             }

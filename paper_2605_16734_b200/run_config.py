@@ -3,6 +3,7 @@ loss fraction versus time, status counts, attempted steps, device time, energy c
 (static fields) and, for config 4, the number of Poincare records.
 
     python -m paper_2605_16734_b200.run_config --config 1 [--segments 100] [--particles N] [--t-max T]
+                                               [--grid NGSxNTHxNZE[:hermite]]     (NEXT-2: trace on the interpolant)
 
 The horizon is cut into equal segments traced in place with GC_TRACE_RESUME (A24: the last step of each
 segment is clipped to the segment end).  Everything runs in the CUDA kernels behind the C ABI; there is no CPU path.
@@ -23,6 +24,8 @@ def main():
     ap.add_argument("--particles", type=int, default=None)
     ap.add_argument("--t-max", type=float, default=None, help="horizon in seconds (default: the config's)")
     ap.add_argument("--poincare-per-particle", type=int, default=8, help="config 4: record capacity per particle")
+    ap.add_argument("--grid", default="", help="NGSxNTHxNZE[:hermite]: trace on the 3-D tricubic interpolant of B; mu and the "
+                    "energy check still use the direct sum at the start and end points")
     args = ap.parse_args()
 
     import torch
@@ -40,6 +43,10 @@ def main():
     B0, _ = GF.field_eval(s, th, ze, derivs=False)
     mu = T(0.5 * spec.mass * P.vperp2()) / B0
     E0 = 0.5 * spec.mass * vpar ** 2 + mu * B0
+    if args.grid:
+        gspec = args.grid.lower().split(":")
+        GF.set_grid(*[int(x) for x in gspec[0].split("x")],
+                    kind=G.GC_GRID_HERMITE if len(gspec) > 1 and gspec[1].startswith("h") else G.GC_GRID_LAGRANGE)
     h = torch.zeros(n, dtype=torch.float64, device=dev)
     cap = args.poincare_per_particle * n if args.config == 4 else 0
     stream = torch.cuda.current_stream()
@@ -71,7 +78,7 @@ def main():
 
     st = state.status.cpu().numpy()
     attempts = int(state.n_acc.sum(dtype=torch.int64).item() + state.n_rej.sum(dtype=torch.int64).item())
-    out = {"config": args.config, "particles": n, "t_max": t_max, "segments": args.segments,
+    out = {"config": args.config, "particles": n, "t_max": t_max, "segments": args.segments, "grid": args.grid or None,
            "kernel": GF.kernel_info(n), "attempted_steps": attempts,
            "accepted_fraction": float(state.n_acc.sum(dtype=torch.int64).item()) / max(attempts, 1),
            "forced_min_steps": int(state.n_forced.sum(dtype=torch.int64).item()),
@@ -90,6 +97,8 @@ def main():
     if fld.nk == 0:                                            # static field: energy of the survivors is conserved
         surv = state.status == G.ST_TMAX
         y = state.y
+        if args.grid:
+            GF.set_grid(0, 0, 0)                               # energy with the direct sum at both ends
         B1, _ = GF.field_eval(y[0].contiguous(), y[1].contiguous(), y[2].contiguous(), derivs=False)
         E1 = 0.5 * spec.mass * y[3] ** 2 + mu * B1
         rel = ((E1 - E0) / E0).abs()[surv]

@@ -299,6 +299,45 @@ int gc_set_option(gc_field* f, int32_t option, int64_t value);
 int gc_kernel_info(const gc_field* f, int64_t n, int32_t* kernel, int32_t* blocks, int32_t* threads_per_block,
                    int32_t* smem_bytes, int32_t* regs_per_thread);
 
+/* ---- gc_trace for callers that must not allocate device memory.
+ *
+ * Who needs it.  gc_trace borrows its per-call work area (one 128-byte record per particle plus the index arrays of the
+ * cell binning) from a stream-ordered memory pool, and the first call of a given size makes that pool ask the driver for
+ * memory.  Some programs that embed this library cannot afford that once they are up: a long-running service that gave
+ * the whole GPU to its own arena at start-up and treats every later driver allocation as a budget violation (or simply
+ * has none left to give); a control or acquisition loop with a deadline, for which the unbounded latency and the
+ * device-wide synchronisation an allocation or a release can cause are not acceptable; a plug-in whose host forbids the
+ * CUDA allocation calls outside its own allocator.  For them gc_trace_noalloc traces with the work area in a fixed
+ * array that is part of the library image: GC_NOALLOC_SCRATCH_BYTES (5 MiB) of device memory on every GPU that loads
+ * libgcorbit.so, held until the process exits whether or not this function is ever called.
+ *
+ * What it does.  The arguments, the results and the asynchronous behaviour on `stream` are those of gc_trace with
+ * GC_KERNEL_MMA selected (same kernel, same launch geometry; only the address of the work area differs).  It never
+ * calls cudaMalloc, cudaFree, their stream-ordered forms or any library routine that allocates; inputs and outputs
+ * remain the caller's device buffers.
+ *
+ * Limits.  n <= GC_NOALLOC_MAX_PARTICLES (32768; one record slot per particle) and the binning arrays of the field must
+ * fit the rest of the array (they do up to several thousand radial nodes): beyond either the call returns GC_EINVAL and
+ * gc_last_error() says which limit and by how much -- trace a larger ensemble as consecutive slices.  The field must fit
+ * the mma kernel (max |xn| <= 16, max xm <= 16) and must not have a 3-D interpolant set; GC_EINVAL otherwise.
+ *
+ * Set-up.  The first call on each GPU looks up the device address of the array (one cudaGetSymbolAddress, with that
+ * GPU current) and remembers it; make that first call during start-up, before any stream capture.  Call with the
+ * field's GPU current, as for every other entry point.
+ *
+ * Sharing.  There is ONE array per GPU and every call uses it.  A call clears the counters it needs at zero itself (in
+ * stream order), so what the previous call left behind never matters; but two calls that can run on the GPU at the same
+ * time -- different streams, or different host threads on different streams, also through different fields -- would
+ * overwrite each other's records and return garbage.  Issue all gc_trace_noalloc calls on one stream, or order them
+ * with events.  gc_trace itself is not affected and may run next to it. */
+enum { GC_NOALLOC_MAX_PARTICLES = 32768, GC_NOALLOC_SCRATCH_BYTES = 5 * 1024 * 1024 };
+int gc_trace_noalloc(const gc_field* f, const gc_trace_params* params, int64_t n,
+                     const double* s0, const double* th0, const double* ze0, const double* vpar0,
+                     const double* mu, double* h_inout,
+                     double* y_out, double* t_out, int32_t* status,
+                     int32_t* n_acc, int32_t* n_rej, int32_t* n_forced,
+                     double* poincare, int64_t* poincare_count, void* stream);
+
 /* Thread-local text of the last nonzero return ("" if none). */
 const char* gc_last_error(void);
 

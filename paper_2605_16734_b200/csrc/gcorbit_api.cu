@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1066,6 +1067,110 @@ int gc_trace_host(gc_field* f, const gc_trace_params* params, int64_t n, const d
   GC_H(cudaStreamSynchronize(st));
 #undef GC_H
   cleanup();
+  return GC_OK;
+}
+
+}  // extern "C"
+
+// ---- gc_trace_noalloc: the mma trace with its work area in a fixed array of the library image (include/gcorbit.h) ----
+// For callers that may not allocate device memory once they run (a host application that owns the whole GPU through
+// its own arena, a loop with a deadline, a plug-in whose host forbids the CUDA allocation calls).  Nothing above this
+// line is changed by it; the carve-up of the work area below repeats launch_tile's on purpose.
+namespace {
+
+// The work area.  It exists once per GPU that loads the library and lives until the process ends.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[GC_NOALLOC_SCRATCH_BYTES];
+
+// In host code the name g_noalloc_scratch is only a handle for the runtime, not an address the GPU understands: the
+// device address has to be asked for, per GPU, with that GPU current.
+constexpr int kNoAllocMaxDevices = 64;
+std::mutex g_noalloc_mutex;
+unsigned char* g_noalloc_addr[kNoAllocMaxDevices] = {};
+
+int noalloc_scratch(unsigned char** out) {
+  int dev = -1;
+  GC_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kNoAllocMaxDevices) return fail(GC_EINVAL, "gc_trace_noalloc: device ordinal out of range");
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_addr[dev]) {                               // first call on this GPU: the set-up step
+    void* p = nullptr;
+    GC_CUDA(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+    if (!p) return fail(GC_ECUDA, "gc_trace_noalloc: cudaGetSymbolAddress returned no address");
+    g_noalloc_addr[dev] = static_cast<unsigned char*>(p);
+  }
+  *out = g_noalloc_addr[dev];
+  return GC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int gc_trace_noalloc(const gc_field* f, const gc_trace_params* params, int64_t n, const double* s0, const double* th0,
+                     const double* ze0, const double* vpar0, const double* mu, double* h_inout, double* y_out,
+                     double* t_out, int32_t* status, int32_t* n_acc, int32_t* n_rej, int32_t* n_forced,
+                     double* poincare, int64_t* poincare_count, void* stream) {
+  gc::TraceDev t{};
+  int rc = build_trace_dev(f, params, n, &t);
+  if (rc != GC_OK) return rc;
+  if (n > GC_NOALLOC_MAX_PARTICLES)
+    return fail(GC_EINVAL, "gc_trace_noalloc: n = " + std::to_string((long long)n) + " particles, the fixed work area holds " +
+                               std::to_string((int)GC_NOALLOC_MAX_PARTICLES) + " (GC_NOALLOC_MAX_PARTICLES); trace the ensemble in slices");
+  if (!f->mma_ok) return fail(GC_EINVAL, "gc_trace_noalloc: the field does not fit the mma kernel (max |xn| <= 16, max xm <= 16)");
+  if (f->dev.grid) return fail(GC_EINVAL, "gc_trace_noalloc: the field has a 3-D interpolant set (gc_field_set_grid)");
+  // the same carve-up as launch_tile: records, then order | cnt | cursor | start | tstart | ctrl | next
+  const int ncell = f->dev.ns - 3;
+  const size_t wn = (size_t)(n > 0 ? n : 1);                // one record slot per particle
+  const size_t rec_bytes = wn * gc::kRecDoubles * sizeof(double);
+  const size_t nbin = (size_t)ncell * gc::kSubBins;
+  const size_t order_count = (wn + 1) & ~(size_t)1;
+  const size_t zero_count = 2 * nbin + (size_t)2 * (ncell + 1) + 8 + 4;
+  const size_t need = rec_bytes + (order_count + zero_count) * sizeof(int);
+  if (need > (size_t)GC_NOALLOC_SCRATCH_BYTES)
+    return fail(GC_EINVAL, "gc_trace_noalloc: " + std::to_string(need) + " bytes of work area needed for n = " +
+                               std::to_string((long long)n) + " and ns = " + std::to_string(f->dev.ns) + ", the fixed array has " +
+                               std::to_string((int)GC_NOALLOC_SCRATCH_BYTES) + " (GC_NOALLOC_SCRATCH_BYTES)");
+  if (n == 0) return GC_OK;
+  if (!s0 || !th0 || !ze0 || !vpar0 || !mu || !y_out || !t_out || !status)
+    return fail(GC_EINVAL, "gc_trace_noalloc: NULL particle array");
+  if (params->poincare_capacity > 0 && (!poincare || !poincare_count))
+    return fail(GC_EINVAL, "gc_trace_noalloc: poincare_capacity > 0 needs poincare and poincare_count");
+  unsigned char* slab = nullptr;
+  rc = noalloc_scratch(&slab);
+  if (rc != GC_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  t.s0 = s0; t.th0 = th0; t.ze0 = ze0; t.vpar0 = vpar0; t.mu = mu; t.h_inout = h_inout;
+  t.y_out = y_out; t.t_out = t_out; t.status = status; t.n_acc = n_acc; t.n_rej = n_rej; t.n_forced = n_forced;
+  t.poincare = poincare;
+  t.poincare_count = reinterpret_cast<unsigned long long*>(poincare_count);
+  if (!poincare || !poincare_count) t.poincare_capacity = 0;
+  if (poincare_count) GC_CUDA(cudaMemsetAsync(poincare_count, 0, sizeof(int64_t), st));
+  gc::TileScratch sc{};
+  sc.slots = (long long)wn;
+  sc.chunk = f->chunk_attempts;
+  sc.rec = reinterpret_cast<double*>(slab);
+  int* ip = reinterpret_cast<int*>(slab + rec_bytes);
+  sc.order = ip; ip += order_count;
+  sc.cnt = ip; ip += nbin;
+  sc.cursor = ip; ip += nbin;
+  sc.start = ip; ip += ncell + 1;
+  sc.tstart = ip; ip += ncell + 1;
+  sc.ctrl = ip; ip += 8;
+  ip += ((reinterpret_cast<uintptr_t>(ip) & 7) ? 1 : 0);   // the 64-bit input cursor
+  sc.next = reinterpret_cast<unsigned long long*>(ip);
+  // the array keeps what the last call left in it: the bin counts, cursors, offsets, control words and the input
+  // cursor must start at zero (records and `order` are written by the kernel before it reads them)
+  GC_CUDA(cudaMemsetAsync(sc.cnt, 0, zero_count * sizeof(int), st));
+  int per_tile = 0;
+  const long long blocks = tile_geometry(f, (long long)wn, true, &per_tile);
+  sc.tile_size = per_tile;
+  gc::FieldDev fd = f->dev;
+  int mode = 0;
+  double* rhs_out = nullptr;
+  void* args[] = {(void*)&fd, (void*)&t, (void*)&sc, (void*)&mode, (void*)&rhs_out};
+  const bool sample = t.section != 0 || t.refine_loss != 0;   // the diagnostics build of the kernel, as in launch_tile
+  GC_CUDA(cudaLaunchCooperativeKernel(mma_fn(f, sample), dim3((unsigned)blocks), dim3(gc::kMmaThreads), args,
+                                      (size_t)f->mma_smem, st));
   return GC_OK;
 }
 

@@ -24,7 +24,8 @@ ST_TMAX, ST_LOST, ST_AXIS, ST_MAXSTEPS, ST_NONFINITE = 0, 1, 2, 3, 4
 
 EXPORTS = ["gc_field_create", "gc_field_destroy", "gc_field_eval", "gc_pert_eval", "gc_rhs_eval", "gc_trace",
            "gc_trace_host", "gc_set_kernel", "gc_set_option", "gc_kernel_info", "gc_last_error",
-           "gc_trace_sampled", "gc_pzeta_eval", "gc_birkhoff", "gc_kcov_eval", "gc_field_set_grid", "gc_trace_symplectic", "gc_orbit_diagnostics"]
+           "gc_trace_sampled", "gc_pzeta_eval", "gc_birkhoff", "gc_kcov_eval", "gc_field_set_grid", "gc_trace_symplectic", "gc_orbit_diagnostics",
+           "gc_trace_noalloc"]
 
 
 class GcError(RuntimeError):
@@ -70,6 +71,7 @@ def load_library():
         L.gc_pert_eval.argtypes = [vp, i64, vp, vp, vp, dbl, vp, vp]
         L.gc_rhs_eval.argtypes = [vp, dbl, dbl, dbl, i64, vp, vp, vp, vp]
         L.gc_trace.argtypes = [vp, C.POINTER(gc_trace_params), i64] + [vp] * 15
+        L.gc_trace_noalloc.argtypes = [vp, C.POINTER(gc_trace_params), i64] + [vp] * 15
         L.gc_trace_host.argtypes = [vp, C.POINTER(gc_trace_params), i64] + [vp] * 14
         L.gc_trace_sampled.argtypes = [vp, C.POINTER(gc_trace_params), i64] + [vp] * 12 + [dbl, dbl, i64, vp, vp, vp]
         L.gc_pzeta_eval.argtypes = [vp, dbl, dbl, i64, vp, vp, vp, vp, vp]
@@ -111,6 +113,7 @@ def _stream_ptr(torch):
     return C.c_void_p(torch.cuda.current_stream().cuda_stream)
 
 
+NOALLOC_MAX_PARTICLES = 32768      # GC_NOALLOC_MAX_PARTICLES of include/gcorbit.h
 GC_TRACE_RESUME = 1
 GC_TRACE_SECTION_VPAR = 2
 GC_TRACE_REFINE_LOSS = 4
@@ -290,6 +293,30 @@ class Field:
                                        _dp(out.poincare) if poincare_capacity else None, _dp(cnt),
                                        _stream_ptr(torch)))
         out._count_tensor = cnt
+        return out
+
+    # ---- gc_trace_noalloc (device tensors) -------------------------------------------------------------------
+    def trace_noalloc(self, spec, s0, th0, ze0, vpar0, mu, out: TraceResult, h_inout=None, t0=None, t_max=None,
+                      flags=0, poincare_count=None) -> TraceResult:
+        """gc_trace for hosts that must not allocate on the GPU while they run (a service whose own arena owns the
+        device, a loop with a deadline, a plug-in under a foreign allocator): the library works in a fixed 5 MiB
+        array inside its own image instead of pool memory.  At most ``NOALLOC_MAX_PARTICLES`` particles per call;
+        calls share the one array, so keep them on one stream.  Nothing is allocated here either: ``out`` must
+        carry every output buffer (y, t, status; counters and poincare if wanted), and Poincare records need the
+        caller's one-element int64 ``poincare_count`` tensor.  Asynchronous on torch's current stream."""
+        torch = _torch()
+        n = s0.numel()
+        for x in (s0, th0, ze0, vpar0, mu):
+            assert x.dtype == torch.float64 and x.is_cuda and x.is_contiguous() and x.numel() == n
+        cap = 0 if out.poincare is None or poincare_count is None else out.poincare.shape[0]
+        p = make_params(spec, t0, t_max, cap, flags)
+        out.h = h_inout
+        _check(load_library().gc_trace_noalloc(self._h, C.byref(p), n, _dp(s0), _dp(th0), _dp(ze0), _dp(vpar0),
+                                               _dp(mu), _dp(h_inout), _dp(out.y), _dp(out.t), _dp(out.status),
+                                               _dp(out.n_acc), _dp(out.n_rej), _dp(out.n_forced),
+                                               _dp(out.poincare) if cap else None,
+                                               _dp(poincare_count) if cap else None, _stream_ptr(torch)))
+        out._count_tensor = poincare_count if cap else None
         return out
 
     # ---- NEXT-1: gc_trace_sampled / gc_pzeta_eval / gc_birkhoff ----------------------------------------------------

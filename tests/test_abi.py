@@ -97,6 +97,7 @@ def test_argument_validation_needs_no_device(lib):
     assert b"non-finite" in lib.gc_last_error()
     assert lib.gc_field_destroy(None) == G.GC_OK
     assert lib.gc_trace(None, None, 0, *([None] * 15)) == G.GC_EINVAL
+    assert lib.gc_trace_noalloc(None, None, 0, *([None] * 15)) == G.GC_EINVAL
     assert lib.gc_field_eval(None, 0, None, None, None, None, None, None) == G.GC_EINVAL
 
 

@@ -122,6 +122,48 @@ def test_no_growth_on_the_step_after_a_rejection():
     assert n_rej >= 10
 
 
+def test_clipped_last_step_hands_on_the_unclipped_proposal():
+    """O6: "the step that would pass t_max is clipped to land on it; the unclipped h_next is
+    kept for h_inout", so that a horizon cut into segments continues with the step size the controller had reached,
+    not with one derived from the short clipped step.  Built by hand: take the attempt record up to an accepted
+    attempt k (no rejection before it), whose proposal is h_k = h_used scale_accept(err_k); put t_max 0.05 h_k behind
+    t_k, so attempt k + 1 is clipped to 0.05 h_k.  The call must end on t_max and return h_k -- not
+    0.05 h_k scale_accept(err of the clipped step), at most half of h_k whatever the growth cap, the value the reading "every accepted step updates h" gives
+    (mutation `if (!clipped) h = h_next` -> `h = h_next` of trace_impl).  The next segment then starts with a full
+    step h_k."""
+    F, s, th, ze, v, mu = _one_particle()
+    spec = W.make_spec(0)
+    spec.t_max = 1e-3
+    rec = _attempt_record(F, spec, s, th, ze, v, mu, 40)
+    k = next(j for j in range(20, 40) if rec[j][0] and rec[j - 1][0])      # accepted, and so was the one before it
+    t_b, y_b, h_used = rec[k - 1][1], rec[k - 1][6], rec[k - 1][5]
+    err_k, _ = _err_of_attempt(F, spec, t_b, y_b, mu[0], h_used)
+    h_k = h_used * oracle.scale_accept(err_k)                               # the proposal after attempt k, by hand
+    t_k, y_k = rec[k][1], rec[k][6]
+    assert t_k == t_b + h_used and math.isclose(rec[k][5], h_k, rel_tol=1e-7)
+    spec.max_steps = 10 ** 9
+    spec.t_max = t_k + 0.05 * h_k
+    a = F.trace(spec, s, th, ze, v, mu, traj_capacity=64)
+    assert a.status[0] == 0 and a.t[0] == spec.t_max and a.n_acc[0] + a.n_rej[0] == k + 2   # attempts are 0-based in rec
+    h_clip = spec.t_max - t_k
+    err_c, _ = _err_of_attempt(F, spec, t_k, y_k, mu[0], h_clip)
+    h_wrong = h_clip * oracle.scale_accept(err_c)                           # what the other reading would hand on
+    assert err_c <= 1.0 and h_wrong < 0.6 * h_k    # premise: the two readings differ
+    assert math.isclose(a.h[0], h_k, rel_tol=1e-7)
+    assert a.h[0] == rec[k][5]                                              # exactly the proposal before the clip
+    # the second segment takes its first step with that h: the accepted step sequence of the two-segment run
+    # continues t_k + 0.05 h_k -> + h_k (err of that attempt, recomputed here, is below one)
+    T2 = spec.t_max + 5.0 * h_k
+    y_a = np.array([a.y[0, 0], a.y[1, 0], a.y[2, 0], a.y[3, 0] / VREF])
+    err_n, _ = _err_of_attempt(F, spec, a.t[0], y_a, mu[0], a.h[0])
+    assert err_n <= 1.0
+    b = F.trace(spec, a.y[0], a.y[1], a.y[2], a.y[3], mu, h_in=a.h, t0=a.t[0], t_max=T2, traj_capacity=64)
+    assert b.traj[0, 0, 0] == a.t[0] + h_k
+    # and the whole two-segment run stays on the single call's error level
+    full = F.trace(spec, s, th, ze, v, mu, t_max=T2)
+    assert np.abs(b.y[:3, 0] - full.y[:3, 0]).max() < 1e-9 and abs(b.y[3, 0] - full.y[3, 0]) < 1e-9 * VREF
+
+
 def test_step_underflow_ends_the_particle_with_status_4():
     """A23: with h_min = 0 a step so small that t + h == t in floating point can never advance the particle; it ends
     with status 4 (non-finite / stalled) instead of looping for ever: zero attempts, state untouched."""

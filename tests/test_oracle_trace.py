@@ -77,6 +77,44 @@ def test_axis_stop_and_stop_order():
     assert r.status[0] == 1 and r.n_acc[0] == 1
 
 
+def test_axis_stop_at_closed_form_time_and_start_at_or_below_s_min():
+    """O7 / A7: a particle stops with status 2 on the first accepted step that ends at s <= s_min (the radial
+    coordinate is singular on the axis), checked after the loss test and before the t_max test.  Inward E x B drift
+    in closed form: psi(t) = psi0 s0 - (2 A / omega) (sin(phi0 + omega t) - sin(phi0)) reaches psi0 s_min at t*; the
+    stopping step must straddle t*, i.e. the step before it ends above s_min (a stop rule that waits for s < 0, or
+    any later s, would take further steps below s_min first)."""
+    A, om = 8.0e3, TWO_PI * 1e3
+    fld = _exb_drift_field(A, om)
+    F = oracle.OracleField(fld)
+    spec = W.make_spec(0)
+    spec.t_max, spec.s_min = 1e-4, 0.05
+    v0 = np.array([0.7, -0.6]) * VREF
+    mu = 0.5 * M * (VREF ** 2 - v0 ** 2) / 5.7
+    s0, th0, ze0 = np.array([0.1, 0.12]), np.array([0.1, 0.1]), np.array([0.2, -0.3])
+    r = F.trace(spec, s0, th0, ze0, v0, mu, traj_capacity=5000)
+    phi0 = 2 * th0 - ze0
+    assert list(r.status) == [2, 2]
+    for i in range(2):
+        t_star = (math.asin(math.sin(phi0[i]) + om * fld.psi0 * (s0[i] - spec.s_min) / (2 * A)) - phi0[i]) / om
+        assert 0.0 < t_star < spec.t_max
+        tr = r.traj[i, :r.traj_count[i]]
+        assert len(tr) >= 3 and tr[-1, 0] == r.t[i] and tr[-1, 1] == r.y[0, i] <= spec.s_min
+        assert tr[-2, 1] > spec.s_min                              # the step before the stop ended above s_min
+        assert tr[-2, 0] <= t_star * (1 + 1e-9) and r.t[i] >= t_star * (1 - 1e-9)
+        s_exact = s0[i] - (2 * A / om) * (math.sin(phi0[i] + om * r.t[i]) - math.sin(phi0[i])) / fld.psi0
+        assert abs(r.y[0, i] - s_exact) < 1e-9 and r.y[0, i] > 0.0   # stopped at s_min, well before s = 0
+    # a start at or below s_min stops after its first accepted step (here s stays positive: only s <= s_min says stop);
+    # a start just above it does not; a start at s_loss is lost, and loss is tested before the axis
+    spec.s_min = 1e-3
+    fld0 = _b00_field()
+    F0 = oracle.OracleField(fld0)
+    v1 = np.full(4, 0.7 * VREF)
+    mu1 = 0.5 * M * (VREF ** 2 - v1 ** 2) / 5.7
+    r = F0.trace(spec, [5e-4, 1e-3, 2e-3, 1.0], [0.1] * 4, [0.2] * 4, v1, mu1, t_max=2e-6)
+    assert list(r.status) == [2, 2, 0, 1] and list(r.n_acc[[0, 1, 3]]) == [1, 1, 1] and r.n_acc[2] > 1
+    assert np.all(r.y[0, :2] > 0.0) and r.t[2] == 2e-6 and np.all(r.t[[0, 1, 3]] < 2e-6)
+
+
 def test_t_max_landing_max_steps_and_start_beyond_t_max():
     F = oracle.OracleField(W.make_field(0))
     P = W.make_particles(0).head(16)

@@ -10,8 +10,8 @@ Calls ONLY oracle/ and the seeded input recipes (paper_2605_16734_b200/workloads
 Size as SURVEY.md section 8(d) asks: 2048 particles per config traced to 1e-3 s (150-400 loss events each), about
 5-10 minutes per config on 16 host threads.  Ensemble: workloads.make_particles(config, 2048) (its own seeded draw
 of that size), mu from the oracle's B at the start point; config 1 keeps its h_min = 1e-12.  Config 0 (512 particles
-on s = 0.25, 1e-4 s) loses nothing inside its horizon and is compared particle by particle instead
-(tests/test_gpu_parity.py).  Columns: status, t_out [s], s_out, attempted steps.
+on s = 0.25, 1e-4 s; the oracle loses 40 of them inside that horizon) is too small for statistics and is
+compared particle by particle, status included, instead (tests/test_gpu_parity.py).  Columns: status, t_out [s], s_out, attempted steps.
 """
 from __future__ import annotations
 

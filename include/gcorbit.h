@@ -124,9 +124,11 @@ int gc_field_destroy(gc_field* f);
 /* ---- NEXT-2 of SURVEY.md section 8(f): the 3-D local-interpolant field ("CUDA kernels implement field interpolation
  * and trajectory integration on GPU" PAPER.md:48; "local tricubics" PAPER.md:80,111; readings A27, A31 of DESIGN.md).
  * Tabulates B (direct sum O2) at s_i = i/(ngs-1), theta_j = 2 pi j/nth, zeta_k = (2 pi/nfp) k/nze (one field period)
- * on the device, asynchronously on `stream`, and from then on every call on this field -- gc_field_eval, gc_rhs_eval,
- * gc_trace, gc_trace_sampled, gc_trace_host, gc_trace_symplectic, gc_pzeta_eval -- evaluates B and its three
- * derivatives from a local tricubic interpolant; profiles and the perturbation keep their radial tables.
+ * on the device (the kernels run on `stream`; this is a set-up call and returns only when the table is complete, so
+ * that calls on any other stream, gc_trace_host's own included, never see a half-built table), and from then on every
+ * call on this field -- gc_field_eval, gc_rhs_eval, gc_trace, gc_trace_sampled, gc_trace_host, gc_trace_symplectic,
+ * gc_pzeta_eval -- evaluates B and its three derivatives from a local tricubic interpolant; profiles and the
+ * perturbation keep their radial tables.
  *   GC_GRID_LAGRANGE  tensor product of 4-point cubic Lagrange polynomials through the node VALUES (radial stencil
  *                     clamped as in O1, angular stencils periodic and centred on the cell); continuous, gradient jumps
  *                     at the cell faces (C0); every count >= 4; 32 ngs (nth + 3) nze bytes of device memory
@@ -136,7 +138,8 @@ int gc_field_destroy(gc_field* f);
  *                     64 ngs (nth + 1) (nze + 1) bytes
  * Traces then run on GC_KERNEL_GRID whatever gc_set_kernel says.  (0, 0, 0) drops the grid and returns to the direct
  * sum.  The table is owned by the field.  GC_EINVAL for a count below the minimum, an unknown kind or a field with
- * kmnc / kmns; calls must not overlap traces that still run on this field. */
+ * kmnc / kmns -- a refused call leaves the field as it was, interpolant included; calls must not overlap traces that
+ * still run on this field. */
 enum { GC_GRID_LAGRANGE = 0, GC_GRID_HERMITE = 1 };
 int gc_field_set_grid(gc_field* f, int32_t ngs, int32_t nth, int32_t nze, int32_t kind, void* stream);
 
@@ -254,7 +257,13 @@ int gc_orbit_diagnostics(int64_t n, int64_t nsamp, const double* samples, int64_
  * status 4 after max_iter iterations) and then advances the angles explicitly with the derivatives of H at the new
  * (s', p_zeta').  Works on the direct harmonic sum (ensembles of at least GC_TILE_MIN_PARTICLES on the cell-binned mma
  * engine, one pass per field evaluation; smaller ones, sampled ones and GC_KERNEL_GENERIC on the lane kernel) and on
- * the 3-D interpolants of gc_field_set_grid. */
+ * the 3-D interpolants of gc_field_set_grid.
+ * The 2 x 2 system is solved by a quasi-Newton iteration that keeps the Jacobian of the dt = 0 part of the equations
+ * (one field evaluation per iteration, started from the linear extrapolation of the last step).  It contracts like
+ * dt times the gradient scale of H: for steps well below the bounce and drift times -- the regime of the method, a few
+ * percent of a transit time, where it takes 4 to 6 iterations -- it reaches newton_tol; for a dt of the order of the
+ * transit time it does not converge where a full Newton iteration still would, and the particle ends with status
+ * GC_ST_NONFINITE after max_iter iterations.  Reduce dt then; raising max_iter does not help. */
 typedef struct {
   double mass, charge;        /* kg, C                                                              */
   double t0, dt;              /* s; fixed step dt > 0                                               */

@@ -668,7 +668,9 @@ int gc_set_option(gc_field* f, int32_t option, int64_t value) {
       f->wave_particles = value;
       return GC_OK;
     case GC_OPT_CHUNK_ATTEMPTS:
-      if (value > 64) return fail(GC_EINVAL, "gc_set_option: at most 64 attempts per chunk");
+      if (value > (gc::kMmaCap > gc::kTileCap ? gc::kMmaCap : gc::kTileCap))   // the kernels' compiled maximum
+        return fail(GC_EINVAL, "gc_set_option: at most " + std::to_string(gc::kMmaCap > gc::kTileCap ? gc::kMmaCap : gc::kTileCap) +
+                                   " attempts per chunk (the kernels' compiled maximum)");
       f->chunk_attempts = (int)value;
       return GC_OK;
     default:
@@ -679,7 +681,20 @@ int gc_set_option(gc_field* f, int32_t option, int64_t value) {
 int gc_field_set_grid(gc_field* f, int32_t ngs, int32_t nth, int32_t nze, int32_t kind, void* stream) {
   if (!f) return fail(GC_EINVAL, "gc_field_set_grid: NULL field");
   cudaStream_t st = (cudaStream_t)stream;
-  if (f->grid) {                                             // drop the old interpolant first
+  // every argument is checked before the interpolant in use is touched: a refused call changes nothing
+  const bool drop = ngs == 0 && nth == 0 && nze == 0;        // back to the direct harmonic sum
+  if (!drop) {
+    if (kind != GC_GRID_LAGRANGE && kind != GC_GRID_HERMITE) return fail(GC_EINVAL, "gc_field_set_grid: unknown kind");
+    const int nmin = kind == GC_GRID_HERMITE ? 2 : 4;
+    if (ngs < nmin || nth < nmin || nze < nmin)
+      return fail(GC_EINVAL, "gc_field_set_grid: every node count must be >= 4 (Lagrange) / >= 2 (Hermite), or all 0");
+    if (f->dev.kmnc || f->dev.kmns)
+      return fail(GC_EINVAL, "gc_field_set_grid: fields with a covariant radial component K are traced by the direct sum only");
+    const size_t doubles = kind == GC_GRID_HERMITE ? (size_t)ngs * (size_t)(nth + 1) * (size_t)(nze + 1) * 8
+                                                   : (size_t)ngs * (size_t)(nth + 3) * (size_t)nze * 4;
+    if (doubles > ((size_t)1 << 33)) return fail(GC_EINVAL, "gc_field_set_grid: table larger than 64 GiB");
+  }
+  if (f->grid) {                                             // drop the old interpolant
     GC_CUDA(cudaStreamSynchronize(st));
     cudaFree(f->grid);
     f->grid = nullptr;
@@ -687,19 +702,12 @@ int gc_field_set_grid(gc_field* f, int32_t ngs, int32_t nth, int32_t nze, int32_
     f->dev.grid_kind = 0;
     f->dev.ngs = f->dev.nth = f->dev.nze = 0;
   }
-  if (ngs == 0 && nth == 0 && nze == 0) return GC_OK;        // back to the direct harmonic sum
-  if (kind != GC_GRID_LAGRANGE && kind != GC_GRID_HERMITE) return fail(GC_EINVAL, "gc_field_set_grid: unknown kind");
-  const int nmin = kind == GC_GRID_HERMITE ? 2 : 4;
-  if (ngs < nmin || nth < nmin || nze < nmin)
-    return fail(GC_EINVAL, "gc_field_set_grid: every node count must be >= 4 (Lagrange) / >= 2 (Hermite), or all 0");
-  if (f->dev.kmnc || f->dev.kmns)
-    return fail(GC_EINVAL, "gc_field_set_grid: fields with a covariant radial component K are traced by the direct sum only");
+  if (drop) return GC_OK;
   constexpr double kTwoPi = 6.283185307179586476925286766559;
   const int tb = 256;
   double* g = nullptr;
   if (kind == GC_GRID_HERMITE) {
     const size_t entries = (size_t)ngs * (size_t)(nth + 1) * (size_t)(nze + 1);
-    if (entries * 8 > ((size_t)1 << 33)) return fail(GC_EINVAL, "gc_field_set_grid: table larger than 64 GiB");
     GC_CUDA(cudaMalloc((void**)&g, entries * 8 * sizeof(double)));
     gc::grid8_build_kernel<<<(unsigned)((entries + tb - 1) / tb), tb, 0, st>>>(f->dev, ngs, nth, nze, g);
     const cudaError_t le = cudaGetLastError();
@@ -707,7 +715,6 @@ int gc_field_set_grid(gc_field* f, int32_t ngs, int32_t nth, int32_t nze, int32_
   } else {
     const size_t nodes = (size_t)ngs * (size_t)nth * (size_t)nze;
     const size_t total = (size_t)ngs * (size_t)(nth + 3) * (size_t)nze * 4;
-    if (total > ((size_t)1 << 33)) return fail(GC_EINVAL, "gc_field_set_grid: table larger than 64 GiB");
     double* plain = nullptr;
     GC_CUDA(cudaMalloc((void**)&g, total * sizeof(double)));
     if (cudaMallocAsync((void**)&plain, nodes * sizeof(double), st) != cudaSuccess) {
@@ -720,6 +727,11 @@ int gc_field_set_grid(gc_field* f, int32_t ngs, int32_t nth, int32_t nze, int32_
     cudaFreeAsync(plain, st);
     if (le != cudaSuccess) { cudaFree(g); GC_CUDA(le); }
   }
+  // A set-up call: the table is published only once it is complete.  Traces may run on any stream (gc_trace_host
+  // uses a stream of the field's own that is ordered against nothing), so the build is waited for here instead of
+  // leaving every later call to order itself against `st`.
+  const cudaError_t se = cudaStreamSynchronize(st);
+  if (se != cudaSuccess) { cudaFree(g); GC_CUDA(se); }
   f->grid = g;
   f->dev.grid = g;
   f->dev.grid_kind = kind == GC_GRID_HERMITE ? 2 : 1;

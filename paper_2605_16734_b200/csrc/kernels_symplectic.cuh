@@ -120,13 +120,17 @@ __global__ void __launch_bounds__(128) trace_symplectic_kernel(FieldDev f, Sympl
       iters += it;
       if (!ok) { st = GC_ST_NONFINITE_; break; }
       // explicit half with the partial derivatives of the last evaluation (within tol of the root)
-      th = fma(p.dt, H_s / e.D, th);
-      ze = fma(p.dt, H_pz - H_s * e.dpth_dpz / e.D, ze);
+      const double th_new = fma(p.dt, H_s / e.D, th);
+      const double ze_new = fma(p.dt, H_pz - H_s * e.dpth_dpz / e.D, ze);
+      // a step that ends on a non-finite value is not committed: the state before it is reported (gcorbit.h), as
+      // trace_mma_symplectic_kernel does, so the result does not depend on which engine the ensemble size selects
+      if (!finite4(x0, th_new, ze_new, x1 * unit)) { st = GC_ST_NONFINITE_; break; }
+      th = th_new;
+      ze = ze_new;
       ds_prev = x0 - s;
       dx1_prev = x1 - pz * inv_unit;
       s = x0;
       pz = x1 * unit;
-      if (!finite4(s, th, ze, pz)) { st = GC_ST_NONFINITE_; break; }
       ++steps;
       sym_eval<GRID>(f, p.chi, q, s, th, ze, pz, false, e);     // profiles at the new point: p_theta of the next step
       pth_old = e.pth;

@@ -431,3 +431,18 @@ def test_trace_host_refuses_overlapping_calls_on_one_field(case0):
     assert err.code == G.GC_EINVAL and "another gc_trace_host call" in str(err)
     again = GF.trace_host(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=1e-6)      # and the field is usable afterwards
     assert (again.status == 0).all()
+
+
+def test_chunk_option_beyond_the_compiled_maximum_is_refused(case0):
+    """GC_OPT_CHUNK_ATTEMPTS: gcorbit.h promises GC_EINVAL for a value out of range; the kernels are compiled for at
+    most 8 attempted steps per chunk, and a larger value used to be clamped silently."""
+    from paper_2605_16734_b200 import gcorbit as G
+    fld, spec, P, OF, GF, mu = case0
+    for ok in (0, 1, 8):
+        GF.set_option(G.GC_OPT_CHUNK_ATTEMPTS, ok)
+    for bad in (9, 64, 1000):
+        with pytest.raises(G.GcError) as e:
+            GF.set_option(G.GC_OPT_CHUNK_ATTEMPTS, bad)
+        assert e.value.code == G.GC_EINVAL
+    GF.set_option(G.GC_OPT_CHUNK_ATTEMPTS, 0)
+

@@ -68,6 +68,41 @@ def test_set_grid_selects_the_grid_kernel_and_can_be_dropped(gcases):
     assert GF.kernel_info(100_000)["kernel"] == "mma"
 
 
+def test_set_grid_then_trace_host_at_once_and_refused_calls_change_nothing():
+    """gc_field_set_grid is a set-up call: when it returns the table is complete, so a gc_trace_host issued straight
+    after it (it runs on the field's own non-blocking stream, ordered against nothing) reads the finished table; and
+    a refused call (unknown kind, a count below the minimum) leaves the interpolant in use where it was."""
+    import torch
+    from paper_2605_16734_b200 import gcorbit as G, workloads as W
+    fld, spec, P, OF, GF, mu = make_case(1, 96)
+    grid = (101, 96, 80)                                      # a table large enough that its build takes a while
+    OF.set_grid_hermite(*grid)
+    mu = W.mu_from(P, OF.eval_B_many(P.s, P.theta, P.zeta)[:, 0])
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        GF.set_grid(*grid, kind=G.GC_GRID_HERMITE)
+        r = GF.trace_host(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=3e-7)
+    # the same trace by gc_trace once everything has certainly finished: a table read half-built would differ
+    torch.cuda.synchronize()
+    d = gpu_trace(GF, spec, P, mu, t_max=3e-7)
+    assert np.array_equal(r.y, d.y.cpu().numpy()) and np.array_equal(r.status, d.status.cpu().numpy())
+    assert np.array_equal(r.n_acc, d.n_acc.cpu().numpy()) and np.array_equal(r.n_rej, d.n_rej.cpu().numpy())
+    # and against the oracle on the same interpolant (on this C1 field the controller is ill-conditioned in the oracle
+    # itself, see _grid_parity: the flipped-decision bound is the one that holds for every particle)
+    o = OF.trace(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=3e-7)
+    assert np.array_equal(r.status, o.status)
+    assert rel_diff(r.y, o.y, spec.v_ref).max() <= GRID_FLIP_RTOL
+    for bad in [dict(kind=7), dict(kind=G.GC_GRID_HERMITE, counts=(1, 16, 16)), dict(kind=G.GC_GRID_LAGRANGE, counts=(16, 3, 16))]:
+        with pytest.raises(G.GcError) as e:
+            GF.set_grid(*bad.get("counts", grid), kind=bad["kind"])
+        assert e.value.code == G.GC_EINVAL
+        assert GF.kernel_info(100_000)["kernel"] == "grid"   # still on the interpolant set above
+    r2 = GF.trace_host(spec, P.s, P.theta, P.zeta, P.vpar, mu, t_max=3e-7)
+    assert np.array_equal(r2.y, r.y) and np.array_equal(r2.status, r.status)
+    GF.set_grid(0, 0, 0)
+    assert GF.kernel_info(100_000)["kernel"] == "mma"
+
+
 def test_set_grid_rejects_fields_with_K():
     import dataclasses
     from paper_2605_16734_b200 import gcorbit as G, workloads as W

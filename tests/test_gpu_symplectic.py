@@ -199,3 +199,41 @@ def test_symplectic_on_the_mma_engine_matches_oracle_and_the_lane_kernel(config,
     assert np.array_equal(two.status.cpu().numpy(), o.status)
     assert np.array_equal(two.n_steps.cpu().numpy(), o.n_steps)
     assert rel_diff(two.y.cpu().numpy(), o.y, spec.v_ref).max() < 1e-9
+
+
+def test_symplectic_mma_engine_streams_through_few_record_slots():
+    """The streaming case of the mma symplectic engine: 4096 record slots (GC_OPT_WAVE_PARTICLES) for 20 011 particles,
+    so that slots are handed from finished particles to waiting ones inside one launch, in two resumed halves.  The
+    result must not depend on the number of slots (bit for bit against one slot per particle) and a sample of the
+    particles is checked against the oracle."""
+    import torch
+    from paper_2605_16734_b200 import gcorbit as G
+    n, dt, nsteps = 20011, 2e-8, 60
+    fld, spec, P, OF, GF, mu = make_case(1, n)
+    lo, hi = float(np.quantile(P.s, 0.02)), float(np.quantile(P.s, 0.98))
+    kw = dict(s_loss=hi + 2e-4, s_min=max(lo - 2e-4, 1e-3))
+    a = [to_dev(x) for x in (P.s, P.theta, P.zeta, P.vpar, mu)]
+    chi = to_dev(_chi(fld))
+    one = GF.trace_symplectic(spec.mass, spec.charge, *a, chi, dt, nsteps, **kw)       # a slot per particle, one call
+    GF.set_option(G.GC_OPT_WAVE_PARTICLES, 4096)
+    h = nsteps // 2
+    two = GF.trace_symplectic(spec.mass, spec.charge, *a, chi, dt, h, **kw)
+    y = two.y
+    GF.trace_symplectic(spec.mass, spec.charge, y[0], y[1], y[2], y[3], a[4], chi, dt, nsteps - h, t0=h * dt, out=two,
+                        flags=G.GC_TRACE_RESUME, **kw)
+    streamed = GF.trace_symplectic(spec.mass, spec.charge, *a, chi, dt, nsteps, **kw)  # 4096 slots, one call
+    GF.set_option(G.GC_OPT_WAVE_PARTICLES, 0)
+    torch.cuda.synchronize()
+    assert torch.equal(streamed.status, one.status) and torch.equal(streamed.n_steps, one.n_steps)
+    assert torch.equal(streamed.y, one.y) and torch.equal(streamed.t, one.t)
+    assert torch.equal(two.status, one.status) and torch.equal(two.n_steps, one.n_steps)
+    assert rel_diff(two.y.cpu().numpy(), one.y.cpu().numpy(), spec.v_ref).max() < 1e-12   # v_par -> p_zeta -> v_par at the hand-over
+    st = one.status.cpu().numpy()
+    assert (st == 0).any() and ((st == 1).any() or (st == 2).any())
+    idx = np.random.default_rng(11).choice(n, 96, replace=False)
+    idx = np.union1d(idx, np.nonzero(st != 0)[0][:16])
+    o = OF.trace_symplectic(spec.mass, spec.charge, P.s[idx], P.theta[idx], P.zeta[idx], P.vpar[idx], mu[idx], _chi(fld),
+                            dt, nsteps, **kw)
+    assert np.array_equal(st[idx], o.status) and np.array_equal(one.n_steps.cpu().numpy()[idx], o.n_steps)
+    assert rel_diff(streamed.y.cpu().numpy()[:, idx], o.y, spec.v_ref).max() < 1e-9
+

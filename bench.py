@@ -251,10 +251,12 @@ def run_cuda(args):
         GF.set_kernel({"warp": G.GC_KERNEL_WARP, "generic": G.GC_KERNEL_GENERIC, "tile": G.GC_KERNEL_TILE, "mma": G.GC_KERNEL_MMA}[args.kernel])
     if args.slots:
         GF.set_option(G.GC_OPT_WAVE_PARTICLES, args.slots)
+    grid_kind = 0                                              # template argument of the lane kernels: 1 Lagrange, 2 Hermite
     if args.grid:
         gspec = args.grid.lower().split(":")
+        grid_kind = 2 if len(gspec) > 1 and gspec[1].startswith("h") else 1
         GF.set_grid(*[int(x) for x in gspec[0].split("x")],
-                    kind=G.GC_GRID_HERMITE if len(gspec) > 1 and gspec[1].startswith("h") else G.GC_GRID_LAGRANGE)
+                    kind=G.GC_GRID_HERMITE if grid_kind == 2 else G.GC_GRID_LAGRANGE)
     kinfo = GF.kernel_info(n)
     kinfo["record_slots"] = args.slots if args.slots else "default"
     T = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=torch.float64, device=dev)
@@ -401,36 +403,50 @@ def run_cuda(args):
                     "(DESIGN.md section 6; the file holds no FP64 figure, so the ALU peak is derived)")
     except Exception:
         pass
-    from paper_2605_16734_b200 import probes
+    from bench_probes import probes
     probe_flops, _ = probes.dfma()
     dmma_flops, mixed_flops = probes.dmma()
     lds_distinct, lds_paired = probes.lds128()
     fstep, fstep_min = info["flop_per_particle_step"], info["flop_per_particle_step_min"]
     rate = attempts / (kernel_ms * 1e-3)                            # this rank's kernel, particle-steps/s
     achieved = rate * fstep / 1e12
-    # constants of ONE ncu --set full capture of the default launch (profiles/ncu_constants.json.txt names the
-    # capture): DRAM bytes per launch and executed FP64 flop per particle-step.  Any other workload: null.
-    traffic = executed = cap_src = None
-    default_launch = (args.config == DEFAULT_CONFIG and args.particles is None and args.segment == 2e-5 and
-                      kinfo["kernel"] == "mma" and args.samples == 0 and args.slots == 0 and not args.grid and
-                      not args.symplectic)
+    # constants of ncu --set full captures of the standard launches (profiles/ncu_constants.json.txt names each
+    # capture): DRAM bytes per launch and executed FP64 flop per particle-step, per config.  They are used only when
+    # the kernel sources are the ones that were profiled (hash stored beside them); any other workload or build: null.
+    traffic = executed = cap_src = cap_stale = None
+    std_launch = (args.particles is None and args.segment == 2e-5 and kinfo["kernel"] == "mma" and
+                  args.samples == 0 and args.slots == 0 and not args.grid and not args.symplectic)
     tp = os.path.join(ROOT, "profiles", "ncu_constants.json.txt")
-    if os.path.exists(tp) and default_launch:
+    if os.path.exists(tp) and std_launch:
         try:
             with open(tp) as fh:
                 c = json.load(fh).get(f"config{args.config}", {})
-            traffic, executed, cap_src = c.get("dram_bytes_per_launch"), c.get("executed_flop_per_particle_step"), \
-                c.get("source")
+            if c:
+                cap_stale = c.get("kernel_source_hash") != kernel_source_hash()
+                cap_src = c.get("source")
+                if not cap_stale:
+                    traffic, executed = c.get("dram_bytes_per_launch"), c.get("executed_flop_per_particle_step")
         except Exception:
             pass
+    # frac / achieved: the FP64 flop the kernel really issues (ncu) where a capture of this build exists, else the
+    # cheapest exact formulation (16 flop per harmonic); the survey's textbook count (28 flop per harmonic, work the
+    # kernel does not do) is reported aside as frac_survey_model
+    basis = "executed" if executed else "min_formulation"
+    fbasis = executed if executed else fstep_min
+    achieved_survey = achieved
+    achieved = rate * fbasis / 1e12
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s",
-                "frac": achieved / peak_nominal, "traffic": traffic,
-                "flop_model": "frac / achieved count the SURVEY.md 8(d) textbook formulation (28 flop per harmonic "
-                              "and right-hand side); the kernel runs a cheaper exact one: see frac_min_formulation "
-                              "(16 flop per harmonic) and frac_executed (FP64 flop the kernel really issues)",
+                "frac": achieved / peak_nominal, "traffic": traffic, "frac_basis": basis,
+                "flop_model": "frac / achieved count " + ("the FP64 flop the kernel issues (DMMA x 512 + DFMA x 2 + DMUL "
+                              "+ DADD of the ncu capture named in ncu_capture)" if executed else "the cheapest exact "
+                              "formulation (16 flop per harmonic and right-hand side; no ncu capture of this build and "
+                              "workload)") + "; frac_survey_model counts the SURVEY.md 8(d) textbook formulation (28 flop "
+                              "per harmonic), work this kernel does not do",
+                "frac_survey_model": achieved_survey / peak_nominal,
                 "frac_min_formulation": rate * fstep_min / 1e12 / peak_nominal,
                 "frac_executed": (rate * executed / 1e12 / peak_nominal) if executed else None,
-                "executed_flop_per_particle_step": executed, "ncu_capture": cap_src,
+                "executed_flop_per_particle_step": executed, "ncu_capture": cap_src, "ncu_capture_stale": cap_stale,
+                "kernel_source_hash": kernel_source_hash(),
                 "kernel": f"trace_{kinfo['kernel']}_kernel", "launch_ms_avg": kernel_ms / K,
                 "peak_source": peak_src,
                 "peak_probe_tflops": probe_flops / 1e12, "peak_probe_dmma_tflops": dmma_flops / 1e12,
@@ -439,10 +455,10 @@ def run_cuda(args):
                 "frac_of_probe": achieved / (probe_flops / 1e12),
                 "flop_per_particle_step": fstep, "flop_per_particle_step_min": fstep_min,
                 "particle_steps_per_launch": attempts / K}
+    evals = 6.0                                                # Dormand-Prince: six new right-hand sides per attempt
     if args.symplectic > 0.0 or args.grid:
         # other formulations of the path (NEXT-2, NEXT-3): field evaluations per particle-step instead of the
         # Dormand-Prince count of 6
-        evals = 6.0
         if args.symplectic > 0.0:
             evals = float(state.n_iter.sum(dtype=torch.int64).item()) / max(attempts_of(state), 1)
             info["symplectic"]["field_evaluations_per_step"] = evals
@@ -458,16 +474,23 @@ def run_cuda(args):
                                  "tricubic interpolant x 64 nodes x 8 B) against sms x 128 B x 1.965 GHz of L1 data "
                                  "pipe; the table is read from L2, not HBM",
                         "fp64_frac": rate * (evals * 700.0 + 250.0) / 1e12 / peak_nominal,
-                        "kernel": "trace_symplectic_kernel<true>" if args.symplectic > 0.0 else "trace_lane_kernel<true>",
+                        "kernel": f"{'trace_symplectic_kernel' if args.symplectic > 0.0 else 'trace_lane_kernel'}<{grid_kind}>",
                         "launch_ms_avg": kernel_ms / K, "particle_steps_per_launch": attempts / K}
         else:
-            f_eval = (fstep - 250.0) / 6.0
+            # gc_trace_symplectic on the direct sum: the cell-binned mma engine from GC_TILE_MIN_PARTICLES(_SMALL) on
+            # (unless GC_KERNEL_GENERIC is selected), else the lane kernel -- the rule of gcorbit_api.cu
+            on_mma = kinfo["kernel"] == "mma"
+            f_eval = ((fstep_min if on_mma else fstep) - 250.0) / 6.0
             roofline.update({"flop_per_particle_step": evals * f_eval, "achieved": rate * evals * f_eval / 1e12,
                              "frac": rate * evals * f_eval / 1e12 / peak_nominal, "frac_min_formulation": None,
-                             "frac_executed": None, "kernel": "trace_symplectic_kernel<false>",
-                             "flop_model": "survey count of one field evaluation (28 flop per harmonic) x measured "
-                                           "evaluations per symplectic step; this kernel evaluates the harmonic sum "
-                                           "with one sincos per harmonic (generic engine)"})
+                             "frac_executed": None, "frac_survey_model": None,
+                             "frac_basis": "min_formulation" if on_mma else "survey_model",
+                             "kernel": "trace_mma_symplectic_kernel" if on_mma else "trace_symplectic_kernel<0>",
+                             "flop_model": ("cheapest exact count of one field evaluation (16 flop per harmonic) x "
+                                            "measured evaluations per symplectic step, on the mma engine" if on_mma else
+                                            "survey count of one field evaluation (28 flop per harmonic) x measured "
+                                            "evaluations per symplectic step; the lane kernel evaluates the harmonic "
+                                            "sum with one sincos per harmonic (generic engine)")})
     cpu = None
     if not args.no_cpu_baseline:
         cpu = oracle_sample(fld, spec, P, seg, args.cpu_seconds)
@@ -479,13 +502,25 @@ def run_cuda(args):
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wu,
            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64", "data": "synthetic", "config": info,
-           "rhs_evals_per_s": 6.0 * value, "accepted_fraction": accepted / max(attempts, 1),
+           "rhs_evals_per_s": evals * value, "accepted_fraction": accepted / max(attempts, 1),
            "accepted_particle_steps_per_s": value * accepted / max(attempts, 1),
            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": K, "clocks": clocks,
            "wall_s_timed_region": t_wall1 - t_wall0}
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
+
+
+def kernel_source_hash() -> str:
+    """Hash of the sources trace_mma_kernel is compiled from; stored beside the ncu constants of
+    profiles/ncu_constants.json.txt so that a later build does not quote an earlier build's counters."""
+    import hashlib
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_2605_16734_b200", "csrc")
+    for name in ("device_math.cuh", "field.cuh", "kernels_generic.cuh", "kernels_tile.cuh", "kernels_mma.cuh"):
+        with open(os.path.join(csrc, name), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
 
 
 def run_plumbing(args):
@@ -516,7 +551,8 @@ def launch_ranks(args) -> int:
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]]
     env = dict(os.environ)
-    env.setdefault("NCCL_DEBUG", "WARN")
+    env.setdefault("NCCL_DEBUG", "INFO")                      # communicator / rank lines (WARN prints none)
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
     return subprocess.call(cmd, env=env)
 
 

@@ -1,5 +1,5 @@
-"""Build libgcorbit.so (the product) and libgcprobes.so (bench-side microbenchmarks, not part of the boundary)
-in-tree with nvcc for sm_100a (no JIT cache: the .so files travel with the repo snapshot)."""
+"""Build libgcorbit.so in-tree with nvcc for sm_100a (no JIT cache: the .so travels with the repo snapshot).  The
+bench-side microbenchmarks (libgcprobes.so) are built by bench_probes/probes.py, outside this package."""
 from __future__ import annotations
 
 import os
@@ -9,9 +9,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 SO = os.path.join(_HERE, "libgcorbit.so")
-PROBES_SO = os.path.join(_HERE, "libgcprobes.so")
 SOURCES = ["gcorbit_api.cu"]
-PROBE_SOURCES = ["fp64_probes.cu"]
 HEADERS = ["device_math.cuh", "field.cuh", "kernels_generic.cuh", "kernels_grid.cuh", "kernels_lane.cuh", "kernels_symplectic.cuh", "kernels_warp.cuh", "kernels_tile.cuh", "kernels_mma.cuh",
            os.path.join("..", "..", "include", "gcorbit.h")]
 
@@ -29,14 +27,14 @@ def source_hash() -> str:
     """Content hash of everything the library is built from (mtimes do not survive a repo snapshot)."""
     import hashlib
     h = hashlib.sha256()
-    for d in [os.path.join(CSRC, s) for s in SOURCES + PROBE_SOURCES + HEADERS] + [os.path.abspath(__file__)]:
+    for d in [os.path.join(CSRC, s) for s in SOURCES + HEADERS] + [os.path.abspath(__file__)]:
         with open(d, "rb") as fh:
             h.update(fh.read())
     return h.hexdigest()
 
 
 def needs_build() -> bool:
-    if not os.path.exists(SO) or not os.path.exists(PROBES_SO) or not os.path.exists(STAMP):
+    if not os.path.exists(SO) or not os.path.exists(STAMP):
         return True
     with open(STAMP) as fh:
         return fh.read().strip() != source_hash()
@@ -51,11 +49,6 @@ def build(force: bool = False, verbose: bool = False, extra=()) -> str:
             raise RuntimeError("nvcc failed building libgcorbit.so")
         with open(os.path.join(_HERE, "build_ptxas.log"), "w") as fh:
             fh.write(" ".join(nvcc_cmd(extra)) + "\n" + r.stdout + r.stderr)
-        rp = subprocess.run(nvcc_cmd((), PROBE_SOURCES, PROBES_SO), capture_output=True, text=True)
-        if verbose or rp.returncode != 0:
-            sys.stderr.write(rp.stdout + rp.stderr)
-        if rp.returncode != 0:
-            raise RuntimeError("nvcc failed building libgcprobes.so")
         with open(STAMP, "w") as fh:
             fh.write(source_hash())
     return SO

@@ -37,9 +37,12 @@ def test_header_and_library_agree(lib):
 
 def test_boundary_holds_the_method_only():
     """The product library exports the calls of the method and nothing else: the FP64 / shared-memory
-    microbenchmarks bench.py reports live in libgcprobes.so (bench-side), not behind include/gcorbit.h."""
+    microbenchmarks bench.py reports live in bench_probes/libgcprobes.so (bench-side, outside the package), not behind
+    include/gcorbit.h."""
     import subprocess
-    from paper_2605_16734_b200 import build, probes
+    from paper_2605_16734_b200 import build
+    from bench_probes import probes
+    probes.build()
     syms = subprocess.run(["nm", "-D", "--defined-only", build.SO], capture_output=True, text=True).stdout
     exported = sorted(set(re.findall(r"\bT (gc[a-z0-9_]*)", syms)))
     assert exported == declared_functions(), exported

@@ -68,6 +68,9 @@ def test_loss_fraction_and_loss_times_against_the_oracle_ensemble(config):
         p = ks_2samp(lt_g, lt_o).pvalue
         info[name] = dict(kernel=GF.kernel_info(P.n)["kernel"], loss_fraction=f_g, ks_p=float(p),
                           axis_fraction=float((st == 2).mean()), status_equal=float((st == st_o).mean()))
+        # the SAME particles on the SAME field and integrator: the paired comparison is the sharp one (the two-sample
+        # Monte Carlo bound below would let 2.5 % of the ensemble change sides) -- measured 100 %
+        assert (st == st_o).mean() >= 0.98, (name, float((st == st_o).mean()))
         assert abs(f_g - f_o) <= se, (name, f_g, f_o, se)
         assert p > 0.01, (name, p)
         assert set(np.unique(st)) <= {0, 1, 2}              # no particle ends in a state the config cannot produce
@@ -125,7 +128,15 @@ def test_interpolant_ensembles_reproduce_the_direct_sum_loss_statistics(config, 
     (101 x 128 x 128 nodes, either reading) against the DIRECT-SUM oracle ensemble -- a different field representation
     (interpolation error ~1e-6 of B), so single orbits differ after a few bounce times, but the ensemble loss fraction
     must agree within the Monte Carlo standard error and the loss times pass the KS test, as between two codes
-    (PAPER.md:68,72 "two codes report identical loss fractions")."""
+    (PAPER.md:68,72 "two codes report identical loss fractions").
+
+    What this does NOT show: at N = 2048 the Monte Carlo bound is +-0.02, so the test has no power against a bias of a
+    few 1e-3.  The full-size run (profiles/r2_full_runs.md: config 3, 10^6 particles to 2e-2 s) gives 0.1988 on the
+    Hermite 101 x 128 x 128 interpolant against 0.1946 on the direct sum, about 7 standard errors at that size: that
+    grid at rtol 1e-8 does NOT meet north_star's loss-fraction criterion on the target configuration, and its speed is
+    quoted as that of a reduced-accuracy field (README).  The sharper statement this test can
+    make at its size is the paired one: at 1e-3 s at most 3 % of the same particles end differently (measured
+    0.1-1.5 %)."""
     from scipy.stats import ks_2samp
     from paper_2605_16734_b200 import gcorbit as G
     st_o, t_o, s_o = _golden(config)
@@ -142,6 +153,7 @@ def test_interpolant_ensembles_reproduce_the_direct_sum_loss_statistics(config, 
     _record("interpolant_loss_statistics", config=config, kind=kind, oracle_loss_fraction=f_o, loss_fraction=f_g,
             bound=se, ks_p=float(p), status_equal=float((st == st_o).mean()), attempts=attempts,
             accepted_fraction=float(g.n_acc.sum().item()) / attempts)
+    assert (st == st_o).mean() >= 0.97, float((st == st_o).mean())
     assert abs(f_g - f_o) <= se, (f_g, f_o, se)
     assert p > 0.01, p
     assert set(np.unique(st)) <= {0, 1, 2}
@@ -177,5 +189,6 @@ def test_symplectic_ensembles_reproduce_the_dormand_prince_loss_statistics(confi
             loss_fraction=f_g, bound=se, ks_p=float(p), status_equal=float((st == st_o).mean()),
             iterations_per_step=float(r.n_iter.sum().item()) / max(float(r.n_steps.sum().item()), 1.0))
     assert set(np.unique(st)) <= {0, 1, 2}
+    assert (st == st_o).mean() >= 0.97, float((st == st_o).mean())   # paired: measured 98.5-98.9 %
     assert abs(f_g - f_o) <= se, (f_g, f_o, se)
     assert p > 0.01, p
